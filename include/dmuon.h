@@ -1,0 +1,161 @@
+/*
+ * dmuon.h -- C ABI of libdmuon: the single-GPU Muon optimizer step of DMuon (arxiv/paper_2606_27153)
+ * for NVIDIA B200 (sm_100a).
+ *
+ * The path (Eq. 1; Eq. 2; Gram form PAPER.md:170; Algorithm 1 l.12-15, PAPER.md:232-238;
+ * conventions the paper does not print are the readings N1..N15 of DESIGN.md):
+ *
+ *     M' = mu M + G ;  U = bf16( G + mu M' )                         Nesterov momentum + the bf16 cast
+ *     X0 = U / (||U||_F + 1e-7)        (transposed first when rows > cols)
+ *     k times:  A = X X^T ;  B = b A + c A A ;  X <- a X + B X       Newton-Schulz quintic, Gram form
+ *     W' = W - lr ( sqrt(max(1, rows/cols)) X_k + wd W )             Eq. 1 with shape scale + decoupled decay
+ *
+ * Every step runs in hand-written CUDA kernels (tcgen05/TMEM/TMA grouped GEMMs, vectorised elementwise
+ * kernels).  There is no CPU fallback: on a machine without an sm_100 device every compute entry point
+ * returns DMUON_ERR_UNSUPPORTED_DEVICE.
+ *
+ * Conventions for all entry points
+ *   - matrices: bfloat16, row-major, contiguous (leading dimension == cols), base pointer 16-byte aligned,
+ *     rows >= 1, cols >= 1.  DEVICE pointers unless the function name ends in _host.
+ *   - `shapes`: HOST array of count*2 int32 = {rows, cols} per matrix.  Pointer arrays are HOST arrays.
+ *     All host arrays are copied before the call returns.
+ *   - ownership: the caller owns every tensor.  `grads` are never written.  `params`, `momenta` (and `ptrs` of
+ *     dmuon_ns_batched) are updated in place.  Two entries of one call must not alias or overlap (undefined).
+ *   - asynchrony: work is enqueued on `stream` (a cudaStream_t) and the call returns without synchronising,
+ *     EXCEPT the first call for a shape set not seen before, which builds a plan, allocates workspace and
+ *     autotunes tile configurations on scratch buffers (never on caller data) and synchronises the device.
+ *   - errors: return value 0 = DMUON_OK, negative = error; dmuon_last_error() gives a message for the calling
+ *     thread's last failure.  Nothing throws or aborts across this boundary.  Non-finite inputs propagate.
+ *   - count == 0 is a valid no-op.  Not thread-safe: serialise calls from several host threads.
+ */
+#ifndef DMUON_H_
+#define DMUON_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define DMUON_API __attribute__((visibility("default")))
+#else
+#define DMUON_API
+#endif
+
+#define DMUON_OK 0
+#define DMUON_ERR_INVALID_ARG (-1)        /* null pointer, count < 0, dimension <= 0, steps < 0, misaligned pointer, bad option */
+#define DMUON_ERR_UNSUPPORTED_DEVICE (-2) /* current device is not compute capability 10.x, or no device */
+#define DMUON_ERR_OOM (-3)                /* workspace allocation failed, or a caller workspace is too small */
+#define DMUON_ERR_CUDA (-4)               /* a CUDA runtime / driver call failed */
+#define DMUON_ERR_INTERNAL (-5)
+
+/* A cudaStream_t, spelled without including CUDA headers. */
+typedef struct CUstream_st* dmuon_stream_t;
+
+/*
+ * Batched Newton-Schulz orthogonalisation (Eq. 2 in the Gram form of :170, batched by shape as in :180).
+ *   ptrs    HOST array[count] of DEVICE pointers; matrix i is shapes[2i] x shapes[2i+1] bf16 and is OVERWRITTEN in
+ *           place by NS_steps( X / (||X||_F + 1e-7) ), rounded to bf16, in the input's own orientation.
+ *   steps   number of NS steps k >= 0 (0 = normalisation only).
+ *   coeffs  HOST, exactly 3 floats {a, b, c} used at every step; NULL = {3.4445, -4.7750, 2.0315}.
+ */
+DMUON_API int dmuon_ns_batched(void* const* ptrs, const int32_t* shapes, int32_t count, int32_t steps,
+                               const float* coeffs, dmuon_stream_t stream);
+
+/* Same with a per-step schedule: coeffs is HOST [steps][3] (e.g. Polar Express; values are the caller's). */
+DMUON_API int dmuon_ns_batched_sched(void* const* ptrs, const int32_t* shapes, int32_t count, int32_t steps,
+                                     const float* coeffs, dmuon_stream_t stream);
+
+/*
+ * One Muon optimizer step over `count` 2-D parameters (Eq. 1; Alg. 1 l.12-15).
+ *   params   HOST array[count] of DEVICE pointers to W (bf16), updated in place.
+ *   grads    HOST array[count] of DEVICE pointers to G (bf16), read only.
+ *   momenta  HOST array[count] of DEVICE pointers to M (bf16), updated in place to mu M + G.
+ *   lr, mu, wd  learning rate, momentum, decoupled weight decay.
+ * Uses the NS step count and coefficients set through dmuon_set_option ("steps", "coeffs"; defaults 5 and the
+ * standard quintic).
+ */
+DMUON_API int dmuon_muon_step(void* const* params, const void* const* grads, void* const* momenta,
+                              const int32_t* shapes, int32_t count, float lr, float mu, float wd,
+                              dmuon_stream_t stream);
+
+/*
+ * The same step for tensors that live in HOST memory (pinned memory gives asynchronous copies): copies W, G, M of
+ * every matrix to device staging buffers owned by the library, runs dmuon_muon_step there, and copies W and M
+ * back; all on `stream`.  The caller synchronises `stream` before reading the results.
+ */
+DMUON_API int dmuon_muon_step_host(void* const* params_host, const void* const* grads_host,
+                                   void* const* momenta_host, const int32_t* shapes, int32_t count, float lr,
+                                   float mu, float wd, dmuon_stream_t stream);
+
+/* Plan + allocate + autotune for a shape set ahead of time (what the first dmuon_muon_step would do). */
+DMUON_API int dmuon_warmup(const int32_t* shapes, int32_t count, dmuon_stream_t stream);
+
+/* Bytes of device workspace a step over this shape set needs (0 on bad arguments). */
+DMUON_API size_t dmuon_workspace_bytes(const int32_t* shapes, int32_t count);
+
+/* Hand the library a caller-owned DEVICE workspace (256-byte aligned) to use instead of its own allocation;
+ * (NULL, 0) returns to library-owned workspace.  Drops all cached plans. */
+DMUON_API int dmuon_set_workspace(void* dev_ptr, size_t bytes);
+
+/*
+ * Options (string key/value).  Keys:
+ *   "steps"       NS steps of dmuon_muon_step (default "5")
+ *   "coeffs"      "a,b,c" used by dmuon_muon_step (default "3.4445,-4.7750,2.0315")
+ *   "mode"        "tc"  = fp16 operands on tcgen05 tensor cores, fp32 accumulation in TMEM (default; PAPER.md:262 runs NS in fp16);
+ *                 "fp32_check" = fp32 operands, plain SIMT kernels: the <= 1e-4 check mode, small shapes only
+ *   "autotune"    "1"/"0": pick each bucket's tile configuration by on-device measurement (default "1")
+ *   "cache_path"  file for the persistent tuning cache ("" disables; default $DMUON_CACHE or ~/.cache/dmuon/tune.txt)
+ *   "profile"     "1"/"0": record CUDA events around every kernel launch (read with dmuon_profile_read)
+ * Returns DMUON_ERR_INVALID_ARG for an unknown key or unparsable value.
+ */
+DMUON_API int dmuon_set_option(const char* key, const char* value);
+
+/* Thread's last error message ("" if none).  The pointer stays valid until the thread's next failing call. */
+DMUON_API const char* dmuon_last_error(void);
+
+/*
+ * With option profile=1: synchronises the recorded events and writes a JSON object
+ *   {"kernels": {"<name>": {"launches": L, "ms": total}, ...}, "launches": total}
+ * accumulated since the last dmuon_profile_reset into buf (NUL terminated, truncated to len).  Returns the number
+ * of bytes needed (excluding the NUL), or a negative error.
+ */
+DMUON_API int dmuon_profile_read(char* buf, size_t len);
+DMUON_API int dmuon_profile_reset(void);
+
+/*
+ * Building block of the NS iteration, exposed for tests and benchmarks: ONE grouped launch over `count`
+ * same-shape problems on fp16 row-major DEVICE matrices whose dimensions are multiples of 128.
+ *   op 0 (SYRK, step a3):  C[m x m] = alpha * X X^T                X = in0[i] is m x k;  in1 ignored
+ *   op 1 (SQ,   step a4):  C[m x m] = alpha * A A + beta * A       A = in0[i] is m x m, symmetric;  in1 ignored
+ *   op 2 (BX,   step a5):  C[m x n] = alpha * B X + beta * X       B = in0[i] is m x m;  X = in1[i] is m x n
+ * For op 0 `n` is k (the contraction length); for op 1 it is ignored.  Symmetric ops compute upper-triangular
+ * tiles only and mirror them.  in0/in1/out are HOST arrays[count] of DEVICE pointers; out must not alias an input.
+ * variant: -1 = the tuned/default tile configuration, >= 0 selects configuration `variant`.
+ */
+DMUON_API int dmuon_ns_gemm(int32_t op, const void* const* in0, const void* const* in1, void* const* out,
+                            int32_t m, int32_t n, int32_t count, float alpha, float beta, int32_t variant,
+                            dmuon_stream_t stream);
+
+/* Number of tile-configuration variants dmuon_ns_gemm accepts for `op`. */
+DMUON_API int dmuon_ns_gemm_variants(int32_t op);
+
+/*
+ * Test hook: copies the Newton-Schulz result O = NS_k(X0) of matrix `index` of the MOST RECENT dmuon_muon_step /
+ * dmuon_ns_batched call out of the library's workspace, before any rounding to bf16, as fp32 into out_dev
+ * (DEVICE, rows*cols floats, the matrix's stored orientation).  Valid until the next call that uses the workspace.
+ */
+DMUON_API int dmuon_read_ns_output(int32_t index, float* out_dev, dmuon_stream_t stream);
+
+/* Free every plan, workspace, staging buffer and event; the library can be used again afterwards. */
+DMUON_API void dmuon_shutdown(void);
+
+/* Library version string. */
+DMUON_API const char* dmuon_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DMUON_H_ */

@@ -1,0 +1,216 @@
+"""Thin ctypes binding over libdmuon.so (include/dmuon.h).  Argument marshalling only: every step of the path
+runs in the library's CUDA kernels.  There is no fallback: if the library is missing, loading raises."""
+from __future__ import annotations
+
+import ctypes
+import json
+import os
+from typing import Iterable, List, Optional, Sequence
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libdmuon.so")
+
+OK = 0
+ERR_INVALID_ARG = -1
+ERR_UNSUPPORTED_DEVICE = -2
+ERR_OOM = -3
+ERR_CUDA = -4
+ERR_INTERNAL = -5
+
+OP_SYRK, OP_SQ, OP_BX = 0, 1, 2
+
+#: every symbol include/dmuon.h declares
+SYMBOLS = ("dmuon_ns_batched", "dmuon_ns_batched_sched", "dmuon_muon_step", "dmuon_muon_step_host", "dmuon_warmup",
+           "dmuon_workspace_bytes", "dmuon_set_workspace", "dmuon_set_option", "dmuon_last_error",
+           "dmuon_profile_read", "dmuon_profile_reset", "dmuon_ns_gemm", "dmuon_ns_gemm_variants", "dmuon_read_ns_output", "dmuon_shutdown",
+           "dmuon_version")
+
+
+class DmuonError(RuntimeError):
+    def __init__(self, code: int, message: str):
+        super().__init__(f"libdmuon error {code}: {message}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Load libdmuon.so (built by paper_2606_27153_b200.build).  Fails loudly if it is not there."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2606_27153_b200.build` "
+                              "(there is no CPU or PyTorch fallback for the Muon step)")
+        L = ctypes.CDLL(LIB_PATH)
+        vp, i32, f32 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_float
+        pp = ctypes.POINTER(ctypes.c_void_p)
+        pi = ctypes.POINTER(ctypes.c_int32)
+        pf = ctypes.POINTER(ctypes.c_float)
+        L.dmuon_ns_batched.argtypes = [pp, pi, i32, i32, pf, vp]
+        L.dmuon_ns_batched_sched.argtypes = [pp, pi, i32, i32, pf, vp]
+        L.dmuon_muon_step.argtypes = [pp, pp, pp, pi, i32, f32, f32, f32, vp]
+        L.dmuon_muon_step_host.argtypes = [pp, pp, pp, pi, i32, f32, f32, f32, vp]
+        L.dmuon_warmup.argtypes = [pi, i32, vp]
+        L.dmuon_workspace_bytes.argtypes = [pi, i32]
+        L.dmuon_workspace_bytes.restype = ctypes.c_size_t
+        L.dmuon_set_workspace.argtypes = [vp, ctypes.c_size_t]
+        L.dmuon_set_option.argtypes = [ctypes.c_char_p, ctypes.c_char_p]
+        L.dmuon_last_error.restype = ctypes.c_char_p
+        L.dmuon_profile_read.argtypes = [ctypes.c_char_p, ctypes.c_size_t]
+        L.dmuon_ns_gemm.argtypes = [i32, pp, pp, pp, i32, i32, i32, f32, f32, i32, vp]
+        L.dmuon_ns_gemm_variants.argtypes = [i32]
+        L.dmuon_read_ns_output.argtypes = [i32, vp, vp]
+        L.dmuon_shutdown.restype = None
+        L.dmuon_version.restype = ctypes.c_char_p
+        for name in SYMBOLS:
+            fn = getattr(L, name)
+            if fn.restype is ctypes.c_int and name not in ("dmuon_shutdown",):
+                fn.restype = ctypes.c_int
+        _lib = L
+    return _lib
+
+
+def _check(rc: int) -> None:
+    if rc != OK:
+        raise DmuonError(rc, lib().dmuon_last_error().decode())
+
+
+def _stream(stream) -> ctypes.c_void_p:
+    if stream is None:
+        stream = torch.cuda.current_stream().cuda_stream if torch.cuda.is_available() else 0
+    elif isinstance(stream, torch.cuda.Stream):
+        stream = stream.cuda_stream
+    return ctypes.c_void_p(int(stream))
+
+
+def _ptr_array(tensors: Sequence[torch.Tensor]):
+    return (ctypes.c_void_p * len(tensors))(*[t.data_ptr() for t in tensors])
+
+
+def _shape_array(shapes: Iterable[Sequence[int]]):
+    flat: List[int] = []
+    for s in shapes:
+        flat += [int(s[0]), int(s[1])]
+    return (ctypes.c_int32 * len(flat))(*flat), len(flat) // 2
+
+
+def _check_mats(tensors: Sequence[torch.Tensor], device_type: str, what: str) -> None:
+    for i, t in enumerate(tensors):
+        if t.dim() != 2 or t.dtype != torch.bfloat16 or not t.is_contiguous() or t.device.type != device_type:
+            raise ValueError(f"{what}[{i}] must be a contiguous 2-D bfloat16 {device_type} tensor")
+
+
+# ---------------------------------------------------------------- entry points (names follow include/dmuon.h)
+
+def version() -> str:
+    return lib().dmuon_version().decode()
+
+
+def last_error() -> str:
+    return lib().dmuon_last_error().decode()
+
+
+def set_option(key: str, value) -> None:
+    _check(lib().dmuon_set_option(key.encode(), str(value).encode()))
+
+
+def ns_batched(tensors: Sequence[torch.Tensor], steps: int = 5, coeffs: Optional[Sequence[float]] = None, stream=None) -> None:
+    """dmuon_ns_batched: each tensor is overwritten by NS_steps(X / (||X||_F + 1e-7))."""
+    _check_mats(tensors, "cuda", "tensors")
+    shp, n = _shape_array([t.shape for t in tensors])
+    co = (ctypes.c_float * 3)(*coeffs) if coeffs is not None else None
+    _check(lib().dmuon_ns_batched(_ptr_array(tensors), shp, n, int(steps), co, _stream(stream)))
+
+
+def ns_batched_sched(tensors: Sequence[torch.Tensor], coeffs: Sequence[Sequence[float]], stream=None) -> None:
+    """dmuon_ns_batched_sched: one (a, b, c) per step."""
+    _check_mats(tensors, "cuda", "tensors")
+    shp, n = _shape_array([t.shape for t in tensors])
+    flat = [float(v) for row in coeffs for v in row]
+    co = (ctypes.c_float * len(flat))(*flat)
+    _check(lib().dmuon_ns_batched_sched(_ptr_array(tensors), shp, n, len(coeffs), co, _stream(stream)))
+
+
+def muon_step(params: Sequence[torch.Tensor], grads: Sequence[torch.Tensor], momenta: Sequence[torch.Tensor],
+              lr: float, mu: float, wd: float, stream=None) -> None:
+    """dmuon_muon_step: params and momenta updated in place; grads read only."""
+    if not (len(params) == len(grads) == len(momenta)):
+        raise ValueError("params, grads, momenta must have one length")
+    for name, ts in (("params", params), ("grads", grads), ("momenta", momenta)):
+        _check_mats(ts, "cuda", name)
+    for p, g, m in zip(params, grads, momenta):
+        if p.shape != g.shape or p.shape != m.shape:
+            raise ValueError("param / grad / momentum shapes differ")
+    shp, n = _shape_array([t.shape for t in params])
+    _check(lib().dmuon_muon_step(_ptr_array(params), _ptr_array(grads), _ptr_array(momenta), shp, n, float(lr),
+                                 float(mu), float(wd), _stream(stream)))
+
+
+def muon_step_host(params: Sequence[torch.Tensor], grads: Sequence[torch.Tensor], momenta: Sequence[torch.Tensor],
+                   lr: float, mu: float, wd: float, stream=None) -> None:
+    """dmuon_muon_step_host: the same step for HOST tensors (pinned for asynchronous copies)."""
+    for name, ts in (("params", params), ("grads", grads), ("momenta", momenta)):
+        _check_mats(ts, "cpu", name)
+    shp, n = _shape_array([t.shape for t in params])
+    _check(lib().dmuon_muon_step_host(_ptr_array(params), _ptr_array(grads), _ptr_array(momenta), shp, n, float(lr),
+                                      float(mu), float(wd), _stream(stream)))
+
+
+def warmup(shapes: Sequence[Sequence[int]], stream=None) -> None:
+    shp, n = _shape_array(shapes)
+    _check(lib().dmuon_warmup(shp, n, _stream(stream)))
+
+
+def workspace_bytes(shapes: Sequence[Sequence[int]]) -> int:
+    shp, n = _shape_array(shapes)
+    return int(lib().dmuon_workspace_bytes(shp, n))
+
+
+def set_workspace(buf: Optional[torch.Tensor]) -> None:
+    if buf is None:
+        _check(lib().dmuon_set_workspace(None, 0))
+    else:
+        _check(lib().dmuon_set_workspace(ctypes.c_void_p(buf.data_ptr()), buf.numel() * buf.element_size()))
+
+
+def profile_reset() -> None:
+    _check(lib().dmuon_profile_reset())
+
+
+def profile_read() -> dict:
+    buf = ctypes.create_string_buffer(1 << 16)
+    rc = lib().dmuon_profile_read(buf, len(buf))
+    if rc < 0:
+        _check(rc)
+    return json.loads(buf.value.decode())
+
+
+def ns_gemm(op: int, in0: Sequence[torch.Tensor], in1: Optional[Sequence[torch.Tensor]], out: Sequence[torch.Tensor],
+            alpha: float, beta: float, variant: int = -1, stream=None) -> None:
+    """dmuon_ns_gemm: one grouped launch of an NS product on fp16 matrices (dims multiples of 128)."""
+    for ts in (in0, in1 or [], out):
+        for t in ts:
+            if t.dtype != torch.float16 or not t.is_contiguous() or t.device.type != "cuda" or t.dim() != 2:
+                raise ValueError("ns_gemm takes contiguous 2-D float16 cuda tensors")
+    m = in0[0].shape[0]
+    n = in0[0].shape[1] if op == OP_SYRK else (out[0].shape[1] if op == OP_BX else m)
+    _check(lib().dmuon_ns_gemm(op, _ptr_array(in0), _ptr_array(in1) if in1 else None, _ptr_array(out), m, n, len(in0),
+                               float(alpha), float(beta), int(variant), _stream(stream)))
+
+
+def read_ns_output(index: int, shape: Sequence[int], stream=None) -> torch.Tensor:
+    """dmuon_read_ns_output: the unrounded NS result of matrix `index` of the last call, as an fp32 cuda tensor."""
+    out = torch.empty(tuple(shape), dtype=torch.float32, device="cuda")
+    _check(lib().dmuon_read_ns_output(int(index), ctypes.c_void_p(out.data_ptr()), _stream(stream)))
+    return out
+
+
+def ns_gemm_variants(op: int) -> int:
+    return int(lib().dmuon_ns_gemm_variants(op))
+
+
+def shutdown() -> None:
+    lib().dmuon_shutdown()

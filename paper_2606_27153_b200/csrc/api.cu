@@ -1,0 +1,430 @@
+// C ABI of libdmuon (include/dmuon.h): argument validation, options, error strings, profiling events, and the
+// enqueue order of the Muon step:  momentum+Nesterov+cast+sumsq -> norms -> normalise/orient/cast -> k x (SYRK, SQ, BX)
+// per shape bucket -> apply.   (Eq. 1, Eq. 2, Alg. 1 l.12-15.)
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <map>
+
+#include "planner.h"
+
+namespace dmuon {
+
+namespace {
+
+thread_local char g_err[512] = "";
+Options g_opt;
+Plan* g_last_plan = nullptr;     // plan of the most recent step / ns call (for dmuon_read_ns_output)
+void* g_ext_ws = nullptr;
+size_t g_ext_ws_bytes = 0;
+
+// ---------------------------------------------------------------- profiling
+struct ProfRec {
+  const char* name;
+  cudaEvent_t e0, e1;
+};
+std::vector<ProfRec> g_prof_open;                 // recorded, not yet folded
+std::vector<cudaEvent_t> g_event_pool;
+std::map<std::string, std::pair<long long, double>> g_prof_acc;   // name -> (launches, ms)
+long long g_launches = 0;
+
+cudaEvent_t take_event() {
+  if (!g_event_pool.empty()) {
+    cudaEvent_t e = g_event_pool.back();
+    g_event_pool.pop_back();
+    return e;
+  }
+  cudaEvent_t e = nullptr;
+  cudaEventCreate(&e);
+  return e;
+}
+
+int fold_profile() {
+  for (ProfRec& r : g_prof_open) {
+    if (cudaEventSynchronize(r.e1) != cudaSuccess) { cudaGetLastError(); set_error("profile: event sync failed"); return DMUON_ERR_CUDA; }
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, r.e0, r.e1);
+    auto& acc = g_prof_acc[r.name];
+    acc.first += 1;
+    acc.second += ms;
+    g_event_pool.push_back(r.e0);
+    g_event_pool.push_back(r.e1);
+  }
+  g_prof_open.clear();
+  return DMUON_OK;
+}
+
+int validate(const void* const* a, const void* const* b, const void* const* c, const int32_t* shapes, int32_t count,
+             const char* fn) {
+  if (count < 0) { set_error("%s: count < 0", fn); return DMUON_ERR_INVALID_ARG; }
+  if (count == 0) return DMUON_OK;
+  if (!a || !shapes) { set_error("%s: null argument", fn); return DMUON_ERR_INVALID_ARG; }
+  for (int i = 0; i < count; ++i) {
+    if (shapes[2 * i] <= 0 || shapes[2 * i + 1] <= 0) {
+      set_error("%s: matrix %d has non-positive dimension %d x %d", fn, i, shapes[2 * i], shapes[2 * i + 1]);
+      return DMUON_ERR_INVALID_ARG;
+    }
+    const void* ptrs[3] = {a[i], b ? b[i] : a[i], c ? c[i] : a[i]};
+    for (const void* p : ptrs) {
+      if (!p) { set_error("%s: matrix %d has a null pointer", fn, i); return DMUON_ERR_INVALID_ARG; }
+      if (reinterpret_cast<uintptr_t>(p) & 15) { set_error("%s: matrix %d pointer %p is not 16-byte aligned", fn, i, p); return DMUON_ERR_INVALID_ARG; }
+    }
+  }
+  return DMUON_OK;
+}
+
+// Patch the per-call pointers into the plan's records and upload them if anything changed.
+int bind_pointers(Plan& plan, void* const* w, const void* const* g, void* const* m, int steps, cudaStream_t stream) {
+  const int count = static_cast<int>(plan.mats.size());
+  bool dirty = plan.o_parity != (steps & 1);
+  for (int i = 0; i < count; ++i) {
+    MatRec& r = plan.h_recs[i];
+    void* gi = g ? const_cast<void*>(g[i]) : nullptr;
+    void* mi = m ? m[i] : nullptr;
+    if (r.W != w[i] || r.G != gi || r.M != mi) dirty = true;
+    r.W = w[i];
+    r.G = gi;
+    r.M = mi;
+    const MatrixInfo& info = plan.mats[i];
+    r.O = plan.ws + ((steps & 1) ? info.off_p : info.off_q);   // X0 in Q; each step swaps buffers
+  }
+  plan.o_parity = steps & 1;
+  if (dirty && count > 0)
+    DMUON_CUDA_CHECK(cudaMemcpyAsync(plan.d_recs, plan.h_recs.data(), sizeof(MatRec) * count, cudaMemcpyHostToDevice, stream));
+  return DMUON_OK;
+}
+
+int muon_step_device(void* const* params, const void* const* grads, void* const* momenta, const int32_t* shapes,
+                     int32_t count, float lr, float mu, float wd, cudaStream_t stream, Plan** plan_out) {
+  Plan* plan = nullptr;
+  int rc = get_plan(shapes, count, g_opt, g_ext_ws, g_ext_ws_bytes, stream, &plan);
+  if (rc) return rc;
+  if (plan_out) *plan_out = plan;
+  g_last_plan = plan;
+  if ((rc = bind_pointers(*plan, params, grads, momenta, g_opt.steps, stream))) return rc;
+  const ElemTables& T = plan->tables;
+  if ((rc = launch_momentum(T, mu, stream))) return rc;
+  if ((rc = launch_finalize_norms(T, g_opt.eps, stream))) return rc;
+  if ((rc = launch_normalize(T, /*from_user=*/false, plan->fp32, stream))) return rc;
+  if ((rc = run_ns_steps(*plan, g_opt.steps, g_opt.coeffs, false, stream))) return rc;
+  if ((rc = launch_apply(T, lr, wd, plan->fp32, stream))) return rc;
+  return DMUON_OK;
+}
+
+int ns_batched_impl(void* const* ptrs, const int32_t* shapes, int32_t count, int32_t steps, const float* coeffs,
+                    bool per_step, cudaStream_t stream) {
+  static const float kDefault[3] = {3.4445f, -4.7750f, 2.0315f};
+  if (steps < 0) { set_error("dmuon_ns_batched: steps < 0"); return DMUON_ERR_INVALID_ARG; }
+  int rc = validate(reinterpret_cast<const void* const*>(ptrs), nullptr, nullptr, shapes, count, "dmuon_ns_batched");
+  if (rc || count == 0) return rc;
+  if (!coeffs) {
+    if (per_step && steps > 0) { set_error("dmuon_ns_batched_sched: coeffs is null"); return DMUON_ERR_INVALID_ARG; }
+    coeffs = kDefault;
+    per_step = false;
+  }
+  Plan* plan = nullptr;
+  if ((rc = get_plan(shapes, count, g_opt, g_ext_ws, g_ext_ws_bytes, stream, &plan))) return rc;
+  g_last_plan = plan;
+  if ((rc = bind_pointers(*plan, ptrs, nullptr, nullptr, steps, stream))) return rc;
+  const ElemTables& T = plan->tables;
+  if ((rc = launch_sumsq(T, stream))) return rc;
+  if ((rc = launch_finalize_norms(T, g_opt.eps, stream))) return rc;
+  if ((rc = launch_normalize(T, /*from_user=*/true, plan->fp32, stream))) return rc;
+  if ((rc = run_ns_steps(*plan, steps, coeffs, per_step, stream))) return rc;
+  if ((rc = launch_store_ns(T, plan->fp32, stream))) return rc;
+  return DMUON_OK;
+}
+
+// ---- dmuon_ns_gemm table cache (one entry: the last argument set)
+struct GemmCall {
+  std::vector<const void*> in0, in1;
+  std::vector<void*> out;
+  int op = -1, m = 0, n = 0, variant = -2;
+  GemmProblem* d_probs = nullptr;
+  TileUnit* d_units = nullptr;
+  int units = 0;
+} g_gemm_call;
+
+}  // namespace
+
+void set_error(const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof g_err, fmt, ap);
+  va_end(ap);
+}
+
+void prof_begin(const char* name, cudaStream_t s) {
+  ++g_launches;
+  if (!g_opt.profile) return;
+  ProfRec r{name, take_event(), take_event()};
+  cudaEventRecord(r.e0, s);
+  g_prof_open.push_back(r);
+}
+
+void prof_end(cudaStream_t s) {
+  if (!g_opt.profile || g_prof_open.empty()) return;
+  cudaEventRecord(g_prof_open.back().e1, s);
+}
+
+}  // namespace dmuon
+
+using namespace dmuon;
+
+extern "C" {
+
+DMUON_API const char* dmuon_version(void) { return "libdmuon 0.1 (sm_100a)"; }
+
+DMUON_API const char* dmuon_last_error(void) { return g_err; }
+
+DMUON_API int dmuon_set_option(const char* key, const char* value) {
+  if (!key || !value) { set_error("dmuon_set_option: null argument"); return DMUON_ERR_INVALID_ARG; }
+  const std::string k(key), v(value);
+  auto as_bool = [&](bool* out) {
+    if (v == "1" || v == "true" || v == "on") { *out = true; return true; }
+    if (v == "0" || v == "false" || v == "off") { *out = false; return true; }
+    return false;
+  };
+  if (k == "steps") {
+    char* end = nullptr;
+    long s = strtol(value, &end, 10);
+    if (end == value || *end || s < 0 || s > 64) { set_error("option steps: bad value '%s'", value); return DMUON_ERR_INVALID_ARG; }
+    g_opt.steps = static_cast<int>(s);
+    return DMUON_OK;
+  }
+  if (k == "coeffs") {
+    float a, b, c;
+    char tail;
+    if (sscanf(value, " %f , %f , %f %c", &a, &b, &c, &tail) != 3) { set_error("option coeffs: expected 'a,b,c', got '%s'", value); return DMUON_ERR_INVALID_ARG; }
+    g_opt.coeffs[0] = a; g_opt.coeffs[1] = b; g_opt.coeffs[2] = c;
+    return DMUON_OK;
+  }
+  if (k == "mode") {
+    if (v == "tc") g_opt.fp32_check = false;
+    else if (v == "fp32_check") g_opt.fp32_check = true;
+    else { set_error("option mode: expected 'tc' or 'fp32_check', got '%s'", value); return DMUON_ERR_INVALID_ARG; }
+    return DMUON_OK;
+  }
+  if (k == "autotune") { if (as_bool(&g_opt.autotune)) return DMUON_OK; set_error("option autotune: bad value '%s'", value); return DMUON_ERR_INVALID_ARG; }
+  if (k == "profile") { if (as_bool(&g_opt.profile)) return DMUON_OK; set_error("option profile: bad value '%s'", value); return DMUON_ERR_INVALID_ARG; }
+  if (k == "cache_path") { g_opt.cache_path = v; g_opt.cache_path_set = true; return DMUON_OK; }
+  set_error("dmuon_set_option: unknown key '%s'", key);
+  return DMUON_ERR_INVALID_ARG;
+}
+
+DMUON_API int dmuon_ns_batched(void* const* ptrs, const int32_t* shapes, int32_t count, int32_t steps,
+                               const float* coeffs, dmuon_stream_t stream) {
+  return ns_batched_impl(ptrs, shapes, count, steps, coeffs, false, reinterpret_cast<cudaStream_t>(stream));
+}
+
+DMUON_API int dmuon_ns_batched_sched(void* const* ptrs, const int32_t* shapes, int32_t count, int32_t steps,
+                                     const float* coeffs, dmuon_stream_t stream) {
+  return ns_batched_impl(ptrs, shapes, count, steps, coeffs, true, reinterpret_cast<cudaStream_t>(stream));
+}
+
+DMUON_API int dmuon_muon_step(void* const* params, const void* const* grads, void* const* momenta,
+                              const int32_t* shapes, int32_t count, float lr, float mu, float wd,
+                              dmuon_stream_t stream) {
+  int rc = validate(reinterpret_cast<const void* const*>(params), grads, reinterpret_cast<const void* const*>(momenta),
+                    shapes, count, "dmuon_muon_step");
+  if (rc || count == 0) return rc;
+  if (!grads || !momenta) { set_error("dmuon_muon_step: null argument"); return DMUON_ERR_INVALID_ARG; }
+  return muon_step_device(params, grads, momenta, shapes, count, lr, mu, wd, reinterpret_cast<cudaStream_t>(stream), nullptr);
+}
+
+DMUON_API int dmuon_muon_step_host(void* const* params_host, const void* const* grads_host, void* const* momenta_host,
+                                   const int32_t* shapes, int32_t count, float lr, float mu, float wd,
+                                   dmuon_stream_t stream_) {
+  cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
+  if (count < 0) { set_error("dmuon_muon_step_host: count < 0"); return DMUON_ERR_INVALID_ARG; }
+  if (count == 0) return DMUON_OK;
+  if (!params_host || !grads_host || !momenta_host || !shapes) { set_error("dmuon_muon_step_host: null argument"); return DMUON_ERR_INVALID_ARG; }
+  for (int i = 0; i < count; ++i) {
+    if (shapes[2 * i] <= 0 || shapes[2 * i + 1] <= 0) { set_error("dmuon_muon_step_host: bad shape of matrix %d", i); return DMUON_ERR_INVALID_ARG; }
+    if (!params_host[i] || !grads_host[i] || !momenta_host[i]) { set_error("dmuon_muon_step_host: matrix %d has a null pointer", i); return DMUON_ERR_INVALID_ARG; }
+  }
+  Plan* plan = nullptr;
+  int rc = get_plan(shapes, count, g_opt, g_ext_ws, g_ext_ws_bytes, stream, &plan);
+  if (rc) return rc;
+  if (!plan->stage) {
+    size_t off = 0;
+    plan->stage_off.resize(count);
+    for (int i = 0; i < count; ++i) {
+      plan->stage_off[i] = off;
+      off += (static_cast<size_t>(shapes[2 * i]) * shapes[2 * i + 1] * 2 + 255) / 256 * 256;
+    }
+    plan->stage_third = off;
+    void* p = nullptr;
+    cudaError_t e = cudaMalloc(&p, 3 * off);
+    if (e != cudaSuccess) { cudaGetLastError(); set_error("staging allocation of %zu bytes failed", 3 * off); return DMUON_ERR_OOM; }
+    plan->d_allocs.push_back(p);
+    plan->stage = static_cast<uint8_t*>(p);
+  }
+  std::vector<void*> w(count), m(count);
+  std::vector<const void*> g(count);
+  {
+    ProfScope ps("h2d_copies", stream);
+    for (int i = 0; i < count; ++i) {
+      const size_t bytes = static_cast<size_t>(shapes[2 * i]) * shapes[2 * i + 1] * 2;
+      w[i] = plan->stage + plan->stage_off[i];
+      g[i] = plan->stage + plan->stage_third + plan->stage_off[i];
+      m[i] = plan->stage + 2 * plan->stage_third + plan->stage_off[i];
+      DMUON_CUDA_CHECK(cudaMemcpyAsync(w[i], params_host[i], bytes, cudaMemcpyHostToDevice, stream));
+      DMUON_CUDA_CHECK(cudaMemcpyAsync(const_cast<void*>(g[i]), grads_host[i], bytes, cudaMemcpyHostToDevice, stream));
+      DMUON_CUDA_CHECK(cudaMemcpyAsync(m[i], momenta_host[i], bytes, cudaMemcpyHostToDevice, stream));
+    }
+  }
+  if ((rc = muon_step_device(w.data(), g.data(), m.data(), shapes, count, lr, mu, wd, stream, nullptr))) return rc;
+  {
+    ProfScope ps("d2h_copies", stream);
+    for (int i = 0; i < count; ++i) {
+      const size_t bytes = static_cast<size_t>(shapes[2 * i]) * shapes[2 * i + 1] * 2;
+      DMUON_CUDA_CHECK(cudaMemcpyAsync(params_host[i], w[i], bytes, cudaMemcpyDeviceToHost, stream));
+      DMUON_CUDA_CHECK(cudaMemcpyAsync(momenta_host[i], m[i], bytes, cudaMemcpyDeviceToHost, stream));
+    }
+  }
+  return DMUON_OK;
+}
+
+DMUON_API int dmuon_warmup(const int32_t* shapes, int32_t count, dmuon_stream_t stream) {
+  if (count < 0 || (count > 0 && !shapes)) { set_error("dmuon_warmup: bad arguments"); return DMUON_ERR_INVALID_ARG; }
+  for (int i = 0; i < count; ++i)
+    if (shapes[2 * i] <= 0 || shapes[2 * i + 1] <= 0) { set_error("dmuon_warmup: bad shape of matrix %d", i); return DMUON_ERR_INVALID_ARG; }
+  if (count == 0) return DMUON_OK;
+  Plan* plan = nullptr;
+  return get_plan(shapes, count, g_opt, g_ext_ws, g_ext_ws_bytes, reinterpret_cast<cudaStream_t>(stream), &plan);
+}
+
+DMUON_API size_t dmuon_workspace_bytes(const int32_t* shapes, int32_t count) {
+  if (count <= 0 || !shapes) return 0;
+  for (int i = 0; i < count; ++i)
+    if (shapes[2 * i] <= 0 || shapes[2 * i + 1] <= 0) return 0;
+  return plan_workspace_bytes(shapes, count, g_opt.fp32_check);
+}
+
+DMUON_API int dmuon_set_workspace(void* dev_ptr, size_t bytes) {
+  if ((dev_ptr == nullptr) != (bytes == 0)) { set_error("dmuon_set_workspace: pointer and size must both be set or both be zero"); return DMUON_ERR_INVALID_ARG; }
+  if (reinterpret_cast<uintptr_t>(dev_ptr) & 255) { set_error("dmuon_set_workspace: pointer must be 256-byte aligned"); return DMUON_ERR_INVALID_ARG; }
+  cudaDeviceSynchronize();
+  cudaGetLastError();
+  drop_plans();
+  g_last_plan = nullptr;
+  g_ext_ws = dev_ptr;
+  g_ext_ws_bytes = bytes;
+  return DMUON_OK;
+}
+
+DMUON_API int dmuon_read_ns_output(int32_t index, float* out_dev, dmuon_stream_t stream) {
+  if (!g_last_plan) { set_error("dmuon_read_ns_output: no step has run"); return DMUON_ERR_INVALID_ARG; }
+  Plan& p = *g_last_plan;
+  if (index < 0 || index >= static_cast<int>(p.mats.size()) || !out_dev) { set_error("dmuon_read_ns_output: bad index or null output"); return DMUON_ERR_INVALID_ARG; }
+  const MatrixInfo& mi = p.mats[index];
+  return launch_export(p.h_recs[index].O, out_dev, mi.rows, mi.cols, mi.n_pad, mi.transposed, p.fp32,
+                       reinterpret_cast<cudaStream_t>(stream));
+}
+
+DMUON_API int dmuon_profile_reset(void) {
+  int rc = fold_profile();
+  g_prof_acc.clear();
+  g_launches = 0;
+  return rc;
+}
+
+DMUON_API int dmuon_profile_read(char* buf, size_t len) {
+  int rc = fold_profile();
+  if (rc) return rc;
+  std::string s = "{\"kernels\": {";
+  bool first = true;
+  for (auto& kv : g_prof_acc) {
+    char item[256];
+    snprintf(item, sizeof item, "%s\"%s\": {\"launches\": %lld, \"ms\": %.6f}", first ? "" : ", ", kv.first.c_str(),
+             kv.second.first, kv.second.second);
+    s += item;
+    first = false;
+  }
+  char tail[64];
+  snprintf(tail, sizeof tail, "}, \"launches\": %lld}", g_launches);
+  s += tail;
+  if (buf && len > 0) {
+    const size_t n = s.size() < len - 1 ? s.size() : len - 1;
+    memcpy(buf, s.data(), n);
+    buf[n] = 0;
+  }
+  return static_cast<int>(s.size());
+}
+
+DMUON_API int dmuon_ns_gemm_variants(int32_t op) { return (op == OP_BX) ? kNumVariants : (op == OP_SYRK || op == OP_SQ) ? 2 : 0; }
+
+DMUON_API int dmuon_ns_gemm(int32_t op, const void* const* in0, const void* const* in1, void* const* out, int32_t m,
+                            int32_t n, int32_t count, float alpha, float beta, int32_t variant, dmuon_stream_t stream_) {
+  cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
+  if (op < 0 || op > 2) { set_error("dmuon_ns_gemm: bad op %d", op); return DMUON_ERR_INVALID_ARG; }
+  if (count < 0 || (count > 0 && (!in0 || !out || (op == OP_BX && !in1)))) { set_error("dmuon_ns_gemm: null argument"); return DMUON_ERR_INVALID_ARG; }
+  if (op == OP_SQ) n = m;
+  if (m <= 0 || n <= 0 || m % kBlk || n % kBlk) { set_error("dmuon_ns_gemm: m and n must be positive multiples of 128 (got %d, %d)", m, n); return DMUON_ERR_INVALID_ARG; }
+  if (variant < -1 || variant >= kNumVariants) { set_error("dmuon_ns_gemm: bad variant %d", variant); return DMUON_ERR_INVALID_ARG; }
+  if (count == 0) return DMUON_OK;
+  int rc = check_device();
+  if (rc) return rc;
+  GemmCall& gc = g_gemm_call;
+  bool same = gc.op == op && gc.m == m && gc.n == n && gc.variant == variant && gc.in0.size() == static_cast<size_t>(count);
+  for (int i = 0; same && i < count; ++i)
+    same = gc.in0[i] == in0[i] && gc.out[i] == out[i] && (op != OP_BX || gc.in1[i] == in1[i]);
+  if (!same) {
+    if (gc.d_probs) cudaFree(gc.d_probs);
+    if (gc.d_units) cudaFree(gc.d_units);
+    gc = GemmCall();
+    std::vector<GemmProblem> probs(count);
+    for (int i = 0; i < count; ++i) {
+      if (!in0[i] || !out[i] || (op == OP_BX && !in1[i])) { set_error("dmuon_ns_gemm: problem %d has a null pointer", i); return DMUON_ERR_INVALID_ARG; }
+      if (op == OP_SYRK) rc = fill_problem(probs[i], OP_SYRK, in0[i], m, n, in0[i], m, n, nullptr, out[i], m);
+      else if (op == OP_SQ) rc = fill_problem(probs[i], OP_SQ, in0[i], m, m, in0[i], m, m, in0[i], out[i], m);
+      else rc = fill_problem(probs[i], OP_BX, in0[i], m, m, in1[i], m, n, in1[i], out[i], n);
+      if (rc) return rc;
+    }
+    std::vector<TileUnit> units = make_units(static_cast<GemmOp>(op), m / kBlk, n / kBlk, variant_config(variant < 0 ? 0 : variant));
+    DMUON_CUDA_CHECK(cudaMalloc(&gc.d_probs, probs.size() * sizeof(GemmProblem)));
+    DMUON_CUDA_CHECK(cudaMalloc(&gc.d_units, units.size() * sizeof(TileUnit)));
+    DMUON_CUDA_CHECK(cudaMemcpy(gc.d_probs, probs.data(), probs.size() * sizeof(GemmProblem), cudaMemcpyHostToDevice));
+    DMUON_CUDA_CHECK(cudaMemcpy(gc.d_units, units.data(), units.size() * sizeof(TileUnit), cudaMemcpyHostToDevice));
+    gc.units = static_cast<int>(units.size());
+    gc.op = op; gc.m = m; gc.n = n; gc.variant = variant;
+    gc.in0.assign(in0, in0 + count);
+    gc.out.assign(out, out + count);
+    if (op == OP_BX) gc.in1.assign(in1, in1 + count);
+  }
+  int dev = 0, sms = 148;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  GemmLaunch L;
+  L.op = static_cast<GemmOp>(op);
+  L.problems = gc.d_probs;
+  L.units = gc.d_units;
+  L.units_per_problem = gc.units;
+  L.num_problems = count;
+  L.k_blocks = (op == OP_SYRK ? n : m) / kBlkK;
+  L.alpha = alpha;
+  L.beta = beta;
+  L.grid = sms;
+  static const char* kNames[3] = {"ns_syrk_xxt", "ns_sq_poly", "ns_bx_update"};
+  ProfScope ps(kNames[op], stream);
+  return launch_ns_gemm(L, stream);
+}
+
+DMUON_API void dmuon_shutdown(void) {
+  cudaDeviceSynchronize();
+  cudaGetLastError();
+  fold_profile();
+  drop_plans();
+  g_last_plan = nullptr;
+  if (g_gemm_call.d_probs) cudaFree(g_gemm_call.d_probs);
+  if (g_gemm_call.d_units) cudaFree(g_gemm_call.d_units);
+  g_gemm_call = GemmCall();
+  for (cudaEvent_t e : g_event_pool) cudaEventDestroy(e);
+  g_event_pool.clear();
+  g_prof_acc.clear();
+  g_launches = 0;
+}
+
+}  // extern "C"

@@ -1,0 +1,445 @@
+// Host-side planner: buckets, workspace layout, TMA descriptors, grouped-launch tables, autotune + persistent cache.
+// See planner.h.  (PAPER.md:180 batching by shape; PAPER.md:184 autotuner and persistent kernel cache.)
+#include "planner.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <fstream>
+#include <sstream>
+#include <sys/stat.h>
+
+namespace dmuon {
+
+namespace {
+
+std::vector<std::unique_ptr<Plan>> g_plans;
+std::map<std::string, int> g_tune_cache;     // "op m_pad n_pad count" -> variant
+bool g_tune_loaded = false;
+std::string g_tune_loaded_path;
+
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+inline int pad128(int v) { return (v + kBlk - 1) / kBlk * kBlk; }
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn g_encode = nullptr;
+
+int load_encode() {
+  if (g_encode) return DMUON_OK;
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  cudaError_t e = cudaGetDriverEntryPointByVersion("cuTensorMapEncodeTiled", &fn, 12000, cudaEnableDefault, &qres);
+  if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess || !fn) {
+    set_error("cuTensorMapEncodeTiled is not available from the driver (%s)", cudaGetErrorString(e));
+    return DMUON_ERR_CUDA;
+  }
+  g_encode = reinterpret_cast<EncodeTiledFn>(fn);
+  return DMUON_OK;
+}
+
+template <typename T>
+int dev_alloc(Plan& p, T** out, size_t count) {
+  void* ptr = nullptr;
+  cudaError_t e = cudaMalloc(&ptr, std::max<size_t>(count, 1) * sizeof(T));
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    set_error("cudaMalloc of %zu bytes failed: %s", count * sizeof(T), cudaGetErrorString(e));
+    return DMUON_ERR_OOM;
+  }
+  p.d_allocs.push_back(ptr);
+  *out = static_cast<T*>(ptr);
+  return DMUON_OK;
+}
+
+template <typename T>
+int upload(Plan& p, T** out, const std::vector<T>& host) {
+  int rc = dev_alloc(p, out, host.size());
+  if (rc) return rc;
+  if (!host.empty()) DMUON_CUDA_CHECK(cudaMemcpy(*out, host.data(), host.size() * sizeof(T), cudaMemcpyHostToDevice));
+  return DMUON_OK;
+}
+
+void describe(const int32_t* shapes, int count, std::vector<MatrixInfo>& mats, size_t es, size_t* ws_bytes) {
+  mats.resize(count);
+  size_t off = 0;
+  for (int i = 0; i < count; ++i) {
+    MatrixInfo& mi = mats[i];
+    mi.rows = shapes[2 * i];
+    mi.cols = shapes[2 * i + 1];
+    mi.transposed = mi.rows > mi.cols;            // work in the smaller Gram dimension
+    mi.m = std::min(mi.rows, mi.cols);
+    mi.n = std::max(mi.rows, mi.cols);
+    mi.m_pad = pad128(mi.m);
+    mi.n_pad = pad128(mi.n);
+    mi.bucket = -1;
+    const size_t xb = align_up(static_cast<size_t>(mi.m_pad) * mi.n_pad * es, 1024);
+    const size_t ab = align_up(static_cast<size_t>(mi.m_pad) * mi.m_pad * es, 1024);
+    mi.off_p = off; off += xb;
+    mi.off_q = off; off += xb;
+    mi.off_a = off; off += ab;
+    mi.off_b = off; off += ab;
+  }
+  *ws_bytes = off;
+}
+
+std::string resolve_cache_path(const Options& opt) {
+  if (opt.cache_path_set) return opt.cache_path;
+  if (const char* e = getenv("DMUON_CACHE")) return e;
+  if (const char* h = getenv("HOME")) return std::string(h) + "/.cache/dmuon/tune.txt";
+  return "";
+}
+
+void load_tune_cache(const std::string& path) {
+  if (g_tune_loaded && g_tune_loaded_path == path) return;
+  g_tune_cache.clear();
+  g_tune_loaded = true;
+  g_tune_loaded_path = path;
+  if (path.empty()) return;
+  std::ifstream in(path);
+  std::string line;
+  while (std::getline(in, line)) {
+    std::istringstream ss(line);
+    std::string tag;
+    int op, m, n, cnt, variant;
+    if (ss >> tag >> op >> m >> n >> cnt >> variant && tag == "v1" && variant >= 0 && variant < kNumVariants) {
+      char key[96];
+      snprintf(key, sizeof key, "%d %d %d %d", op, m, n, cnt);
+      g_tune_cache[key] = variant;
+    }
+  }
+}
+
+void save_tune_cache(const std::string& path) {
+  if (path.empty()) return;
+  const size_t slash = path.find_last_of('/');
+  if (slash != std::string::npos) {
+    std::string dir = path.substr(0, slash);
+    for (size_t i = 1; i <= dir.size(); ++i)
+      if (i == dir.size() || dir[i] == '/') mkdir(dir.substr(0, i).c_str(), 0755);
+  }
+  std::ofstream out(path, std::ios::trunc);
+  for (auto& kv : g_tune_cache) out << "v1 " << kv.first << " " << kv.second << "\n";
+}
+
+int bucket_launch(const Plan& plan, const BucketPlan& b, GemmOp op, int parity, float alpha, float beta,
+                  cudaStream_t stream, const TileUnit* units_override = nullptr, int upp_override = 0) {
+  GemmLaunch L;
+  L.op = op;
+  L.problems = op == OP_SYRK ? b.syrk[parity] : op == OP_SQ ? b.sq : b.bx[parity];
+  L.units = units_override ? units_override : b.units[op];
+  L.units_per_problem = units_override ? upp_override : b.units_per_problem[op];
+  L.num_problems = static_cast<int>(b.mats.size());
+  L.k_blocks = (op == OP_SYRK ? b.n_pad : b.m_pad) / kBlkK;
+  L.alpha = alpha;
+  L.beta = beta;
+  L.grid = plan.sm_count;
+  return launch_ns_gemm(L, stream);
+}
+
+// Time each variant of each op of a bucket on the plan's own (scratch) workspace and keep the fastest.
+int autotune_bucket(Plan& plan, BucketPlan& b, const Options& opt, cudaStream_t stream) {
+  const std::string path = resolve_cache_path(opt);
+  load_tune_cache(path);
+  bool dirty = false;
+  for (int op = 0; op < 3; ++op) {
+    char key[96];
+    snprintf(key, sizeof key, "%d %d %d %d", op, b.m_pad, b.n_pad, static_cast<int>(b.mats.size()));
+    auto it = g_tune_cache.find(key);
+    int best = 0;
+    if (it != g_tune_cache.end()) {
+      best = it->second;
+    } else if (opt.autotune) {
+      cudaEvent_t e0, e1;
+      DMUON_CUDA_CHECK(cudaEventCreate(&e0));
+      DMUON_CUDA_CHECK(cudaEventCreate(&e1));
+      float best_ms = 1e30f;
+      for (int v = 0; v < kNumVariants; ++v) {
+        const TileConfig cfg = variant_config(v);
+        if (op != OP_BX && cfg.order != 0) continue;   // symmetric ops have one ordering
+        std::vector<TileUnit> hu = make_units(static_cast<GemmOp>(op), b.m_pad / kBlk, b.n_pad / kBlk, cfg);
+        TileUnit* du = nullptr;
+        DMUON_CUDA_CHECK(cudaMalloc(&du, hu.size() * sizeof(TileUnit)));
+        DMUON_CUDA_CHECK(cudaMemcpy(du, hu.data(), hu.size() * sizeof(TileUnit), cudaMemcpyHostToDevice));
+        int rc = DMUON_OK;
+        float ms = 1e30f;
+        for (int rep = 0; rep < 3 && rc == DMUON_OK; ++rep) {   // rep 0 warms up
+          cudaEventRecord(e0, stream);
+          rc = bucket_launch(plan, b, static_cast<GemmOp>(op), 0, 1.f, 0.f, stream, du, static_cast<int>(hu.size()));
+          cudaEventRecord(e1, stream);
+          if (cudaEventSynchronize(e1) != cudaSuccess) rc = DMUON_ERR_CUDA;
+          float t = 0.f;
+          cudaEventElapsedTime(&t, e0, e1);
+          if (rep > 0) ms = std::min(ms, t);
+        }
+        cudaFree(du);
+        if (rc) { cudaEventDestroy(e0); cudaEventDestroy(e1); set_error("autotune launch failed"); return rc; }
+        if (ms < best_ms) { best_ms = ms; best = v; }
+      }
+      cudaEventDestroy(e0);
+      cudaEventDestroy(e1);
+      g_tune_cache[key] = best;
+      dirty = true;
+    }
+    b.variant[op] = best;
+  }
+  if (dirty) save_tune_cache(path);
+  return DMUON_OK;
+}
+
+}  // namespace
+
+int fill_problem(GemmProblem& g, GemmOp op, const void* a_mat, uint64_t a_rows, uint64_t a_cols, const void* b_mat,
+                 uint64_t b_rows, uint64_t b_cols, const void* d, void* c, int ldc) {
+  memset(&g, 0, sizeof g);
+  int rc = encode_tmap_2d(&g.tmA, a_mat, a_rows, a_cols, kBlkK, kBlk);
+  if (rc) return rc;
+  if (op == OP_BX) rc = encode_tmap_2d(&g.tmB, b_mat, b_rows, b_cols, 64, kBlkK);   // MN-major: 64 (n) x 64 (k) boxes
+  else rc = encode_tmap_2d(&g.tmB, b_mat, b_rows, b_cols, kBlkK, kBlk);
+  if (rc) return rc;
+  g.D = static_cast<const __half*>(d);
+  g.C = static_cast<__half*>(c);
+  g.ldc = ldc;
+  return DMUON_OK;
+}
+
+Plan::~Plan() {
+  for (void* p : d_allocs) cudaFree(p);
+}
+
+TileConfig variant_config(int variant) {
+  TileConfig c;
+  c.width = (variant & 1) ? 1 : 2;
+  c.order = (variant >> 1) & 1;
+  return c;
+}
+
+std::vector<TileUnit> make_units(GemmOp op, int mb, int nb, const TileConfig& cfg) {
+  std::vector<TileUnit> u;
+  auto push = [&](int i, int j, int w) { u.push_back(TileUnit{static_cast<int16_t>(i), static_cast<int16_t>(j), static_cast<int16_t>(w), 0}); };
+  if (op == OP_BX) {
+    if (cfg.order == 0) {
+      for (int j = 0; j < nb; j += cfg.width)
+        for (int i = 0; i < mb; ++i) push(i, j, std::min(cfg.width, nb - j));
+    } else {
+      for (int i = 0; i < mb; ++i)
+        for (int j = 0; j < nb; j += cfg.width) push(i, j, std::min(cfg.width, nb - j));
+    }
+  } else {
+    // upper-triangular blocks only (PAPER.md:182 computes one triangle and reconstructs the other in the epilogue)
+    for (int i = 0; i < mb; ++i)
+      for (int j = i; j < mb; j += cfg.width) push(i, j, std::min(cfg.width, mb - j));
+  }
+  return u;
+}
+
+int encode_tmap_2d(CUtensorMap* out, const void* base, uint64_t rows, uint64_t cols, uint32_t box_cols,
+                   uint32_t box_rows) {
+  int rc = load_encode();
+  if (rc) return rc;
+  const cuuint64_t gdim[2] = {cols, rows};
+  const cuuint64_t gstride[1] = {cols * sizeof(__half)};
+  const cuuint32_t box[2] = {box_cols, box_rows};
+  const cuuint32_t estr[2] = {1, 1};
+  CUresult r = g_encode(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, const_cast<void*>(base), gdim, gstride, box, estr,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    set_error("cuTensorMapEncodeTiled failed (%d) for %llu x %llu, box %u x %u, base %p", static_cast<int>(r),
+              static_cast<unsigned long long>(rows), static_cast<unsigned long long>(cols), box_rows, box_cols, base);
+    return DMUON_ERR_CUDA;
+  }
+  return DMUON_OK;
+}
+
+int check_device() {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    set_error("no CUDA device: %s", cudaGetErrorString(e));
+    return DMUON_ERR_UNSUPPORTED_DEVICE;
+  }
+  int major = 0;
+  e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+  if (e != cudaSuccess || major != 10) {
+    cudaGetLastError();
+    set_error("libdmuon needs an sm_100 (B200) device; found compute capability major %d", major);
+    return DMUON_ERR_UNSUPPORTED_DEVICE;
+  }
+  return DMUON_OK;
+}
+
+size_t plan_workspace_bytes(const int32_t* shapes, int count, bool fp32) {
+  std::vector<MatrixInfo> mats;
+  size_t bytes = 0;
+  describe(shapes, count, mats, fp32 ? 4 : 2, &bytes);
+  return bytes;
+}
+
+void drop_plans() { g_plans.clear(); }
+
+int get_plan(const int32_t* shapes, int count, const Options& opt, void* ext_ws, size_t ext_bytes, cudaStream_t stream,
+             Plan** out) {
+  for (auto& up : g_plans) {
+    Plan& p = *up;
+    if (p.fp32 == opt.fp32_check && p.shapes.size() == static_cast<size_t>(2 * count) &&
+        (count == 0 || memcmp(p.shapes.data(), shapes, sizeof(int32_t) * 2 * count) == 0)) {
+      *out = &p;
+      return DMUON_OK;
+    }
+  }
+  int rc = check_device();
+  if (rc) return rc;
+
+  std::unique_ptr<Plan> up(new Plan);
+  Plan& p = *up;
+  p.shapes.assign(shapes, shapes + 2 * count);
+  p.fp32 = opt.fp32_check;
+  const size_t es = p.fp32 ? 4 : 2;
+  describe(shapes, count, p.mats, es, &p.ws_bytes);
+  int dev = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&p.sm_count, cudaDevAttrMultiProcessorCount, dev);
+
+  // ---- workspace
+  if (ext_ws) {
+    if (ext_bytes < p.ws_bytes) {
+      set_error("caller workspace of %zu bytes is smaller than the %zu bytes this shape set needs", ext_bytes, p.ws_bytes);
+      return DMUON_ERR_OOM;
+    }
+    p.ws = static_cast<uint8_t*>(ext_ws);
+  } else {
+    rc = dev_alloc(p, &p.ws, p.ws_bytes);
+    if (rc) return rc;
+    p.ws_owned = true;
+  }
+
+  // scratch contents for the autotuner (tensor-core mode) / zeros (check mode)
+  if (!p.fp32) { if ((rc = launch_fill_scratch(p.ws, p.ws_bytes, stream))) return rc; }
+  else DMUON_CUDA_CHECK(cudaMemsetAsync(p.ws, 0, p.ws_bytes, stream));
+
+  // ---- buckets by padded oriented shape
+  std::map<std::pair<int, int>, int> bucket_of;
+  for (int i = 0; i < count; ++i) {
+    MatrixInfo& mi = p.mats[i];
+    auto key = std::make_pair(mi.m_pad, mi.n_pad);
+    auto it = bucket_of.find(key);
+    if (it == bucket_of.end()) {
+      it = bucket_of.emplace(key, static_cast<int>(p.buckets.size())).first;
+      p.buckets.emplace_back();
+      p.buckets.back().m_pad = mi.m_pad;
+      p.buckets.back().n_pad = mi.n_pad;
+    }
+    mi.bucket = it->second;
+    p.buckets[it->second].mats.push_back(i);
+  }
+
+  // ---- elementwise tables
+  std::vector<int64_t> flat_prefix(count + 1, 0), tile_prefix(count + 1, 0), ptile_prefix(count + 1, 0);
+  p.h_recs.resize(count);
+  for (int i = 0; i < count; ++i) {
+    const MatrixInfo& mi = p.mats[i];
+    const int64_t elems = static_cast<int64_t>(mi.rows) * mi.cols;
+    flat_prefix[i + 1] = flat_prefix[i] + (elems + kFlatChunk - 1) / kFlatChunk;
+    tile_prefix[i + 1] = tile_prefix[i] + static_cast<int64_t>((mi.rows + kTile - 1) / kTile) * ((mi.cols + kTile - 1) / kTile);
+    ptile_prefix[i + 1] = ptile_prefix[i] + static_cast<int64_t>(mi.m_pad / kTile) * (mi.n_pad / kTile);
+    MatRec& r = p.h_recs[i];
+    memset(&r, 0, sizeof r);
+    r.U = p.ws + mi.off_p;
+    r.X0 = p.ws + mi.off_q;
+    r.O = nullptr;
+    r.rows = mi.rows; r.cols = mi.cols;
+    r.m_pad = mi.m_pad; r.n_pad = mi.n_pad;
+    r.transposed = mi.transposed ? 1 : 0;
+    r.scale = static_cast<float>(std::sqrt(std::max(1.0, static_cast<double>(mi.rows) / mi.cols)));   // reading N4
+    r.flat_chunk0 = flat_prefix[i]; r.tile0 = tile_prefix[i]; r.ptile0 = ptile_prefix[i];
+  }
+  if ((rc = dev_alloc(p, &p.d_recs, count))) return rc;
+  if ((rc = upload(p, &p.d_flat_prefix, flat_prefix))) return rc;
+  if ((rc = upload(p, &p.d_tile_prefix, tile_prefix))) return rc;
+  if ((rc = upload(p, &p.d_ptile_prefix, ptile_prefix))) return rc;
+  if ((rc = dev_alloc(p, &p.d_partials, static_cast<size_t>(flat_prefix[count])))) return rc;
+  if ((rc = dev_alloc(p, &p.d_inv_norm, count))) return rc;
+  p.tables.recs = p.d_recs;
+  p.tables.flat_prefix = p.d_flat_prefix;
+  p.tables.tile_prefix = p.d_tile_prefix;
+  p.tables.ptile_prefix = p.d_ptile_prefix;
+  p.tables.count = count;
+  p.tables.flat_chunks = flat_prefix[count];
+  p.tables.tiles = tile_prefix[count];
+  p.tables.ptiles = ptile_prefix[count];
+  p.tables.partials = p.d_partials;
+  p.tables.inv_norm = p.d_inv_norm;
+
+  // ---- grouped GEMM tables (tensor-core mode only)
+  if (!p.fp32) {
+    for (BucketPlan& b : p.buckets) {
+      const size_t nprob = b.mats.size();
+      std::vector<GemmProblem> syrk[2], sq(nprob), bx[2];
+      for (int s = 0; s < 2; ++s) { syrk[s].resize(nprob); bx[s].resize(nprob); }
+      for (size_t k = 0; k < nprob; ++k) {
+        const MatrixInfo& mi = p.mats[b.mats[k]];
+        void* X[2] = {p.ws + mi.off_q, p.ws + mi.off_p};     // parity 0: X in Q, parity 1: X in P
+        void* A = p.ws + mi.off_a;
+        void* B = p.ws + mi.off_b;
+        const uint64_t m = mi.m_pad, n = mi.n_pad;
+        for (int s = 0; s < 2; ++s) {
+          if ((rc = fill_problem(syrk[s][k], OP_SYRK, X[s], m, n, X[s], m, n, nullptr, A, mi.m_pad))) return rc;
+          if ((rc = fill_problem(bx[s][k], OP_BX, B, m, m, X[s], m, n, X[s], X[1 - s], mi.n_pad))) return rc;
+        }
+        if ((rc = fill_problem(sq[k], OP_SQ, A, m, m, A, m, m, A, B, mi.m_pad))) return rc;
+      }
+      for (int s = 0; s < 2; ++s) {
+        if ((rc = upload(p, &b.syrk[s], syrk[s]))) return rc;
+        if ((rc = upload(p, &b.bx[s], bx[s]))) return rc;
+      }
+      if ((rc = upload(p, &b.sq, sq))) return rc;
+      // tile configuration: tuned (cache or measurement) or default variant 0
+      if ((rc = autotune_bucket(p, b, opt, stream))) return rc;
+      for (int op = 0; op < 3; ++op) {
+        std::vector<TileUnit> hu = make_units(static_cast<GemmOp>(op), b.m_pad / kBlk, b.n_pad / kBlk, variant_config(b.variant[op]));
+        b.units_per_problem[op] = static_cast<int>(hu.size());
+        if ((rc = upload(p, &b.units[op], hu))) return rc;
+      }
+    }
+  }
+  DMUON_CUDA_CHECK(cudaDeviceSynchronize());
+  g_plans.push_back(std::move(up));
+  *out = g_plans.back().get();
+  return DMUON_OK;
+}
+
+int run_ns_steps(Plan& plan, int steps, const float* coeffs, bool per_step, cudaStream_t stream) {
+  static const char* kNames[3] = {"ns_syrk_xxt", "ns_sq_poly", "ns_bx_update"};
+  for (BucketPlan& b : plan.buckets) {
+    for (int s = 0; s < steps; ++s) {
+      const float* q = coeffs + (per_step ? 3 * s : 0);
+      const float a = q[0], bb = q[1], c = q[2];
+      const int parity = s & 1;                 // step 0 reads Q (parity 0) and writes P
+      if (!plan.fp32) {
+        int rc;
+        { ProfScope ps(kNames[0], stream); if ((rc = bucket_launch(plan, b, OP_SYRK, parity, 1.f, 0.f, stream))) return rc; }
+        { ProfScope ps(kNames[1], stream); if ((rc = bucket_launch(plan, b, OP_SQ, 0, c, bb, stream))) return rc; }
+        { ProfScope ps(kNames[2], stream); if ((rc = bucket_launch(plan, b, OP_BX, parity, 1.f, a, stream))) return rc; }
+      } else {
+        for (int idx : b.mats) {
+          const MatrixInfo& mi = plan.mats[idx];
+          float* X[2] = {reinterpret_cast<float*>(plan.ws + mi.off_q), reinterpret_cast<float*>(plan.ws + mi.off_p)};
+          float* A = reinterpret_cast<float*>(plan.ws + mi.off_a);
+          float* B = reinterpret_cast<float*>(plan.ws + mi.off_b);
+          int rc;
+          if ((rc = launch_check_gemm(OP_SYRK, X[parity], nullptr, A, mi.m_pad, mi.n_pad, 1.f, 0.f, stream))) return rc;
+          if ((rc = launch_check_gemm(OP_SQ, A, nullptr, B, mi.m_pad, mi.m_pad, c, bb, stream))) return rc;
+          if ((rc = launch_check_gemm(OP_BX, B, X[parity], X[1 - parity], mi.m_pad, mi.n_pad, 1.f, a, stream))) return rc;
+        }
+      }
+    }
+  }
+  return DMUON_OK;
+}
+
+}  // namespace dmuon

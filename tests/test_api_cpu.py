@@ -1,0 +1,118 @@
+"""CPU-side checks: the C-ABI library loads and exports every symbol include/dmuon.h declares, argument
+validation and options behave as the header says, and the host logic (shape sets, workspace sizing) is right.
+No compute call needs a GPU here."""
+import ctypes
+import os
+import re
+
+import pytest
+import torch
+
+import paper_2606_27153_b200 as dm
+from paper_2606_27153_b200 import binding, synth
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "dmuon.h")).read()
+    return sorted(set(re.findall(r"DMUON_API\s+[\w\s\*]+?\b(dmuon_\w+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol():
+    names = declared_symbols()
+    assert len(names) >= 15
+    assert sorted(binding.SYMBOLS) == names, "binding.SYMBOLS must list exactly what the header declares"
+    L = ctypes.CDLL(binding.LIB_PATH)
+    for n in names:
+        assert hasattr(L, n), f"{n} not exported by libdmuon.so"
+    assert "sm_100a" in dm.version()
+
+
+def test_options_validation():
+    dm.set_option("steps", 5)
+    dm.set_option("coeffs", "3.4445,-4.7750,2.0315")
+    dm.set_option("autotune", "1")
+    dm.set_option("profile", "0")
+    for key, val in (("steps", "-1"), ("steps", "abc"), ("coeffs", "1,2"), ("mode", "bogus"), ("nope", "1"),
+                     ("autotune", "maybe")):
+        with pytest.raises(dm.DmuonError) as ei:
+            dm.set_option(key, val)
+        assert ei.value.code == binding.ERR_INVALID_ARG
+        assert binding.last_error() != ""
+    dm.set_option("mode", "tc")
+
+
+def test_invalid_arguments_rejected_before_any_device_work():
+    L = binding.lib()
+    shapes = (ctypes.c_int32 * 2)(128, 0)
+    ptrs = (ctypes.c_void_p * 1)(0x1000)
+    assert L.dmuon_ns_batched(ptrs, shapes, 1, 5, None, None) == binding.ERR_INVALID_ARG     # cols = 0
+    shapes = (ctypes.c_int32 * 2)(128, 128)
+    assert L.dmuon_ns_batched(ptrs, shapes, -1, 5, None, None) == binding.ERR_INVALID_ARG    # count < 0
+    assert L.dmuon_ns_batched(ptrs, shapes, 1, -2, None, None) == binding.ERR_INVALID_ARG    # steps < 0
+    assert L.dmuon_ns_batched(None, shapes, 1, 5, None, None) == binding.ERR_INVALID_ARG     # null array
+    bad = (ctypes.c_void_p * 1)(0x1002)
+    assert L.dmuon_ns_batched(bad, shapes, 1, 5, None, None) == binding.ERR_INVALID_ARG      # misaligned
+    null = (ctypes.c_void_p * 1)(None)
+    assert L.dmuon_muon_step(ptrs, null, ptrs, shapes, 1, 0.02, 0.95, 0.01, None) == binding.ERR_INVALID_ARG
+    assert L.dmuon_ns_batched(ptrs, shapes, 0, 5, None, None) == binding.OK                   # count == 0: no-op
+    assert L.dmuon_muon_step(None, None, None, None, 0, 0.02, 0.95, 0.01, None) == binding.OK
+    assert L.dmuon_ns_gemm(7, ptrs, None, ptrs, 128, 128, 1, 1.0, 0.0, -1, None) == binding.ERR_INVALID_ARG
+    assert L.dmuon_ns_gemm(0, ptrs, None, ptrs, 100, 128, 1, 1.0, 0.0, -1, None) == binding.ERR_INVALID_ARG
+    assert L.dmuon_set_workspace(ctypes.c_void_p(0x1000), 0) == binding.ERR_INVALID_ARG
+    assert L.dmuon_read_ns_output(0, None, None) == binding.ERR_INVALID_ARG
+
+
+@pytest.mark.skipif(torch.cuda.is_available(), reason="only meaningful on a box without a GPU")
+def test_no_cpu_fallback():
+    """Without an sm_100 device the product path must fail loudly, not compute somewhere else."""
+    with pytest.raises(dm.DmuonError) as ei:
+        dm.warmup([(128, 512)])
+    assert ei.value.code == binding.ERR_UNSUPPORTED_DEVICE
+    x = torch.zeros((128, 512), dtype=torch.bfloat16)
+    with pytest.raises(ValueError):
+        dm.ns_batched([x])            # host tensor handed to the device entry point
+
+
+def test_workspace_bytes_formula():
+    dm.set_option("mode", "tc")
+    # one 4096 x 14336 matrix: two X buffers + A + B in fp16
+    want = 2 * 4096 * 14336 * 2 + 2 * 4096 * 4096 * 2
+    assert dm.workspace_bytes([(4096, 14336)]) == want
+    assert dm.workspace_bytes([(14336, 4096)]) == want                # tall: same oriented shape
+    # ragged: padded to multiples of 128
+    assert dm.workspace_bytes([(100, 260)]) == 2 * 128 * 384 * 2 + 2 * 128 * 128 * 2
+    assert dm.workspace_bytes([]) == 0
+    assert dm.workspace_bytes([(0, 5)]) == 0
+    dm.set_option("mode", "fp32_check")
+    assert dm.workspace_bytes([(4096, 14336)]) == 2 * want
+    dm.set_option("mode", "tc")
+
+
+def test_config_shape_sets_match_baseline():
+    c2, c3, c4 = synth.config_shapes(2), synth.config_shapes(3), synth.config_shapes(4)
+    assert (len(c2), len(c3), len(c4)) == (72, 168, 224)
+    elems = lambda s: sum(r * c for r, c in s)
+    assert abs(elems(c2) / 1e6 - 84.9) < 0.1
+    assert abs(elems(c3) / 1e6 - 357.8) < 0.1
+    assert abs(elems(c4) / 1e6 - 6979.3) < 0.1
+    assert synth.config_shapes(1) == [(128, 512)] * 8
+    sq = dict(synth.sweep_shapes())
+    assert sq[(256, 256)] == 65536 and sq[(8192, 8192)] == 64
+
+
+def test_synthetic_gradient_statistics():
+    """configs[1] recipe: N(0, 1e-3^2) noise + rank-8 component carrying 10x the noise energy."""
+    g = synth.gradient((768, 3072), 1234).to(torch.float64)
+    energy = (g ** 2).sum().item()
+    noise = 768 * 3072 * 1e-6
+    assert 7.0 < energy / noise < 16.0
+    sv = torch.linalg.svdvals(g)
+    assert sv[7] / sv[8] > 3.0               # 8 spikes stand out of the bulk
+    a = synth.gradient((64, 64), 5)
+    b = synth.gradient((64, 64), 5)
+    assert torch.equal(a, b)                 # seeded
+    assert not torch.equal(a, synth.gradient((64, 64), 6))
+    w = synth.weight((512, 512), 9).float()
+    assert abs(w.std().item() - 0.02) < 2e-3

@@ -1,0 +1,81 @@
+"""The three tcgen05 NS products (dmuon_ns_gemm) against a plain fp32 matmul of the same fp16 inputs.
+This checks the kernel family (TMA/UMMA descriptors, triangular scheduling, mirrored stores, epilogues) in
+isolation; parity of the whole path against the fp64 oracle is in test_parity_gpu.py."""
+import pytest
+import torch
+
+import paper_2606_27153_b200 as dm
+from paper_2606_27153_b200.binding import OP_BX, OP_SQ, OP_SYRK
+
+pytestmark = pytest.mark.gpu
+
+
+def _rand(shape, seed, scale):
+    g = torch.Generator(device="cuda")
+    g.manual_seed(seed)
+    return (torch.randn(shape, generator=g, device="cuda", dtype=torch.float32) * scale).to(torch.float16)
+
+
+def _rel(a, b):
+    return (torch.linalg.norm(a.double() - b.double()) / torch.linalg.norm(b.double())).item()
+
+
+SHAPES = [(128, 128, 1), (128, 512, 3), (256, 256, 2), (384, 640, 2), (768, 3072, 2), (896, 896, 3), (1024, 4096, 1),
+          (2048, 1408 + 128, 2)]
+
+
+@pytest.mark.parametrize("m,k,count", SHAPES)
+@pytest.mark.parametrize("variant", [0, 1])
+def test_syrk(m, k, count, variant):
+    X = [_rand((m, k), 10 + i, k ** -0.5) for i in range(count)]
+    C = [torch.full((m, m), float("nan"), device="cuda", dtype=torch.float16) for _ in range(count)]
+    dm.ns_gemm(OP_SYRK, X, None, C, alpha=0.75, beta=0.0, variant=variant)
+    torch.cuda.synchronize()
+    for x, c in zip(X, C):
+        ref = 0.75 * (x.float() @ x.float().t())
+        assert torch.isfinite(c).all()
+        assert _rel(c, ref) < 1e-3
+        assert torch.equal(c, c.t())          # mirrored store: bitwise symmetric
+
+
+@pytest.mark.parametrize("m,count", [(128, 1), (256, 3), (384, 2), (896, 2), (1024, 2), (4096, 1)])
+@pytest.mark.parametrize("variant", [0, 1])
+def test_sq(m, count, variant):
+    A = []
+    for i in range(count):
+        x = _rand((m, 2 * m), 20 + i, (2 * m) ** -0.5)
+        a = (x.float() @ x.float().t()).to(torch.float16)
+        A.append(torch.triu(a) + torch.triu(a, 1).t())      # exactly symmetric fp16
+    C = [torch.full((m, m), float("nan"), device="cuda", dtype=torch.float16) for _ in range(count)]
+    dm.ns_gemm(OP_SQ, A, None, C, alpha=2.0315, beta=-4.775, variant=variant)
+    torch.cuda.synchronize()
+    for a, c in zip(A, C):
+        ref = 2.0315 * (a.float() @ a.float()) - 4.775 * a.float()
+        assert torch.isfinite(c).all()
+        assert _rel(c, ref) < 1e-3
+        assert torch.equal(c, c.t())
+
+
+@pytest.mark.parametrize("m,n,count", SHAPES)
+@pytest.mark.parametrize("variant", [0, 1, 2, 3])
+def test_bx(m, n, count, variant):
+    B = [_rand((m, m), 30 + i, m ** -0.5) for i in range(count)]       # not symmetric on purpose: catches a transposed operand
+    X = [_rand((m, n), 40 + i, 1.0) for i in range(count)]
+    C = [torch.full((m, n), float("nan"), device="cuda", dtype=torch.float16) for _ in range(count)]
+    dm.ns_gemm(OP_BX, B, X, C, alpha=1.0, beta=3.4445, variant=variant)
+    torch.cuda.synchronize()
+    for b, x, c in zip(B, X, C):
+        ref = b.float() @ x.float() + 3.4445 * x.float()
+        assert torch.isfinite(c).all()
+        assert _rel(c, ref) < 1e-3
+
+
+def test_many_problems_more_units_than_sms():
+    """Persistent loop + double-buffered TMEM across many work units per CTA."""
+    m, k, count = 256, 384, 200
+    X = [_rand((m, k), 100 + i, k ** -0.5) for i in range(count)]
+    C = [torch.empty((m, m), device="cuda", dtype=torch.float16) for _ in range(count)]
+    dm.ns_gemm(OP_SYRK, X, None, C, alpha=1.0, beta=0.0)
+    torch.cuda.synchronize()
+    for i in (0, 1, 57, 148, 199):
+        assert _rel(C[i], X[i].float() @ X[i].float().t()) < 1e-3

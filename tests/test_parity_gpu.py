@@ -1,0 +1,278 @@
+"""Parity of the CUDA path (through the C ABI) against the fp64 oracle on the same seeded bf16 inputs.
+
+Bars (BASELINE.json north_star): relative Frobenius error of O = NS_5(.) <= 1e-2 on the tensor-core path
+(16-bit operands, fp32 accumulation) and <= 1e-4 in the fp32-operand check mode.  M' is compared elementwise
+(<= 1 bf16 ulp: fp32 vs fp64 arithmetic before the same rounding), W' by the criterion of DESIGN.md
+("error no worse than the output rounding plus 1 % of the update").
+"""
+import functools
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_2606_27153_b200 as dm
+from paper_2606_27153_b200 import synth
+from helpers import LR, LR_F, MU, MU_F, TOL_CHECK, TOL_TC, WD, WD_F, bf16_ulp, rel_fro, to64
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(autouse=True)
+def _reset_options():
+    dm.set_option("mode", "tc")
+    dm.set_option("steps", 5)
+    dm.set_option("coeffs", "3.4445,-4.7750,2.0315")
+    yield
+    dm.set_option("mode", "tc")
+    dm.set_option("steps", 5)
+
+
+@functools.lru_cache(maxsize=None)
+def oracle_muon(config: int, index: int, random_momentum: bool):
+    """Oracle Muon step for matrix `index` of a config (inputs regenerated on the GPU with the same seed and read back)."""
+    _, W, G, M = synth.muon_inputs(config, "cuda", random_momentum, indices=[index])
+    return oracle.muon_step(to64(W[0]), to64(G[0]), to64(M[0]), LR_F, MU_F, WD_F, momentum_fp32=True)
+
+
+def check_muon_matrix(idx, shape, W0, Wg, Mg, Og, orc, tol):
+    """Wg, Mg: GPU results (bf16 tensors); Og: unrounded GPU O (fp32); W0: W before the step (float64)."""
+    e_o = rel_fro(to64(Og), orc["O"])
+    assert e_o <= tol, f"matrix {idx} {shape}: O rel err {e_o:.3e} > {tol}"
+    # M': a quantised value; both sides form it in binary32 with one fused rounding (reading N16) -> identical bits
+    m_orc = oracle.round_bf16(orc["M_new"])
+    assert np.array_equal(to64(Mg), m_orc), f"matrix {idx}: M' differs ({(to64(Mg) != m_orc).mean():.2e} of elements)"
+    # W': no worse than the output rounding plus 1 % of the update (2 % slack on the rounding term: the two
+    # roundings are different random draws of the same distribution)
+    w_orc = orc["W_new"]
+    r = np.linalg.norm(oracle.round_bf16(w_orc) - w_orc)
+    upd = np.linalg.norm(w_orc - W0)
+    err = np.linalg.norm(to64(Wg) - w_orc)
+    assert err <= 1.02 * r + tol * upd, f"matrix {idx}: W' err {err:.3e} > {1.02 * r + tol * upd:.3e}"
+    return e_o
+
+
+# ------------------------------------------------------------------------------------------------ configs[0]
+
+@pytest.mark.parametrize("mode,tol", [("tc", TOL_TC), ("fp32_check", TOL_CHECK)])
+def test_config1_ns_batched(mode, tol):
+    dm.set_option("mode", mode)
+    shapes, Xs = synth.ns_inputs("cuda")
+    X64 = [to64(x) for x in Xs]
+    dm.ns_batched(Xs, steps=5)
+    torch.cuda.synchronize()
+    worst = 0.0
+    for i, (x64, xg) in enumerate(zip(X64, Xs)):
+        o = oracle.ns(x64)
+        og = dm.binding.read_ns_output(i, shapes[i])
+        e = rel_fro(to64(og), o)
+        worst = max(worst, e)
+        assert e <= tol, f"matrix {i}: O rel err {e:.3e}"
+        # the in-place bf16 result is the RNE of the unrounded one
+        assert torch.equal(xg, og.to(torch.bfloat16))
+        assert rel_fro(to64(xg), o) <= max(tol, 3e-3)          # bf16 output rounding floor ~1.7e-3
+    print(f"config1 {mode}: worst rel err {worst:.3e}")
+
+
+# ------------------------------------------------------------------------------------------------ configs[1]
+
+def _run_muon_config(config, random_momentum, mode, check_indices, tol):
+    dm.set_option("mode", mode)
+    shapes, W, G, M = synth.muon_inputs(config, "cuda", random_momentum)
+    W0 = {i: to64(W[i]) for i in check_indices}
+    G0 = [g.clone() for g in G]
+    dm.muon_step(W, G, M, LR, MU, WD)
+    torch.cuda.synchronize()
+    worst = 0.0
+    for i in check_indices:
+        og = dm.binding.read_ns_output(i, shapes[i])
+        orc = oracle_muon(config, i, random_momentum)
+        worst = max(worst, check_muon_matrix(i, shapes[i], W0[i], W[i], M[i], og, orc, tol))
+    for g, g0 in zip(G, G0):
+        assert torch.equal(g, g0), "grads must never be written"
+    print(f"config{config} {mode} momentum={random_momentum}: worst O rel err {worst:.3e} over {len(check_indices)} matrices")
+
+
+def test_config2_muon_step_all_matrices():
+    _run_muon_config(2, False, "tc", list(range(72)), TOL_TC)
+
+
+def test_config2_muon_step_check_mode_first_layer():
+    _run_muon_config(2, False, "fp32_check", list(range(6)), TOL_CHECK)
+
+
+def test_config2_with_momentum_state():
+    _run_muon_config(2, True, "tc", [0, 4, 5, 66, 70, 71], TOL_TC)
+
+
+# ------------------------------------------------------------------------------------------------ configs[2]
+
+def test_config3_full_launch_sampled_layers():
+    """All 168 matrices go through the GPU in the configuration bench.py would time; the oracle checks one full
+    layer (7 matrices, every distinct shape incl. the tall 4864x896 and the 128-row k/v) plus the last matrix."""
+    _run_muon_config(3, True, "tc", [0, 1, 2, 3, 4, 5, 6, 167], TOL_TC)
+
+
+# ------------------------------------------------------------------------------------------------ configs[3]
+
+@pytest.mark.slow
+def test_config4_full_size_sampled():
+    """Llama-3-8B-shaped set at full size (42 GB resident).  Oracle on the k (1024x4096) matrix of layer 0 and 31;
+    for the large shapes: O's singular values inside the quintic's band and agreement with the fp32 check mode."""
+    dm.set_option("mode", "tc")
+    shapes, W, G, M = synth.muon_inputs(4, "cuda", False)
+    idx = [1, 218]
+    W0 = {i: to64(W[i]) for i in idx}
+    keep = {i: (W[i].clone(), G[i].clone(), M[i].clone()) for i in (0, 6)}
+    dm.muon_step(W, G, M, LR, MU, WD)
+    torch.cuda.synchronize()
+    for i in idx:
+        og = dm.binding.read_ns_output(i, shapes[i])
+        check_muon_matrix(i, shapes[i], W0[i], W[i], M[i], og, oracle_muon(4, i, False), TOL_TC)
+    big = {}
+    for i in (0, 4, 6):       # q (4096^2), gate (14336x4096, tall), down (4096x14336)
+        og = dm.binding.read_ns_output(i, shapes[i])
+        sv = torch.linalg.svdvals(og if og.shape[0] <= og.shape[1] else og.t().contiguous())
+        assert sv.max().item() <= 1.2024 + 2e-2
+        # inputs have a rank-8 spike over a noise floor: the floor's normalised sigmas are far above 1.5e-3
+        assert sv.min().item() >= 0.6818 - 2e-2
+        big[i] = og
+    del W, G, M
+    torch.cuda.empty_cache()
+    dm.shutdown()
+    dm.set_option("mode", "fp32_check")
+    for i in (0, 6):
+        w, g, m = keep[i]
+        dm.muon_step([w], [g], [m], LR, MU, WD)
+        torch.cuda.synchronize()
+        oc = dm.binding.read_ns_output(0, shapes[i])
+        e = (torch.linalg.norm(big[i].double() - oc.double()) / torch.linalg.norm(oc.double())).item()
+        assert e <= TOL_TC, f"matrix {i}: tc vs fp32 check mode {e:.3e}"
+    dm.shutdown()
+
+
+# ------------------------------------------------------------------------------------------------ edge cases
+
+RAGGED = [(100, 260), (130, 70), (1, 64), (64, 1), (200, 200), (37, 91), (8, 8), (257, 129), (128, 128), (3, 1000)]
+
+
+@pytest.mark.parametrize("mode,tol", [("tc", TOL_TC), ("fp32_check", TOL_CHECK)])
+def test_ragged_and_degenerate_shapes(mode, tol):
+    dm.set_option("mode", mode)
+    Xs = [synth.iid_normal(s, 7000 + i, "cuda", std=0.3) for i, s in enumerate(RAGGED)]
+    X64 = [to64(x) for x in Xs]
+    dm.ns_batched(Xs, steps=5)
+    torch.cuda.synchronize()
+    for i, s in enumerate(RAGGED):
+        og = dm.binding.read_ns_output(i, s)
+        e = rel_fro(to64(og), oracle.ns(X64[i]))
+        assert e <= tol, f"{s}: rel err {e:.3e}"
+
+
+def test_zero_matrix_steps0_count0_and_schedule():
+    z = torch.zeros((128, 256), dtype=torch.bfloat16, device="cuda")
+    x = synth.iid_normal((96, 160), 7100, "cuda")
+    x64 = to64(x)
+    dm.ns_batched([z, x.clone()], steps=5)
+    torch.cuda.synchronize()
+    assert torch.count_nonzero(z).item() == 0                       # reading N14: zero in, zero out, no NaN
+    # steps = 0: normalisation only
+    y = x.clone()
+    dm.ns_batched([y], steps=0)
+    torch.cuda.synchronize()
+    assert rel_fro(to64(dm.binding.read_ns_output(0, (96, 160))), oracle.ns(x64, steps=0)) < 1e-3
+    # count = 0
+    dm.ns_batched([], steps=5)
+    dm.muon_step([], [], [], LR, MU, WD)
+    # per-step schedule (NEXT-1 entry) == oracle with the same schedule
+    sched = [[3.0, -3.5, 1.2], [2.5, -2.0, 0.6], [1.5, -0.5, 0.0]]
+    y = x.clone()
+    dm.ns_batched_sched([y], sched)
+    torch.cuda.synchronize()
+    assert rel_fro(to64(dm.binding.read_ns_output(0, (96, 160))), oracle.ns(x64, steps=3, coeffs=np.array(sched))) <= TOL_TC
+
+
+def test_zero_gradient_muon_step():
+    w = synth.weight((256, 128), 7200, "cuda")
+    w0 = to64(w)
+    g = torch.zeros_like(w)
+    m = torch.zeros_like(w)
+    dm.muon_step([w], [g], [m], LR, MU, WD)
+    torch.cuda.synchronize()
+    want = oracle.round_bf16(w0 - LR_F * WD_F * w0)
+    assert np.abs(to64(w) - want).max() <= bf16_ulp(want).max()
+    assert torch.count_nonzero(m).item() == 0
+
+
+def test_two_steps_state_carried():
+    """Two consecutive steps; the oracle restarts each step from the GPU's bf16 state (DESIGN.md parity rules)."""
+    shapes, W, G, M = synth.muon_inputs(2, "cuda", False, indices=[0, 4, 5])
+    for step in range(2):
+        W0 = [to64(w) for w in W]
+        M0 = [to64(m) for m in M]
+        dm.muon_step(W, G, M, LR, MU, WD)
+        torch.cuda.synchronize()
+        for i in range(3):
+            orc = oracle.muon_step(W0[i], to64(G[i]), M0[i], LR_F, MU_F, WD_F, momentum_fp32=True)
+            og = dm.binding.read_ns_output(i, shapes[i])
+            check_muon_matrix(i, shapes[i], W0[i], W[i], M[i], og, orc, TOL_TC)
+
+
+def test_deterministic_and_host_entry_and_caller_workspace():
+    shapes, W, G, M = synth.muon_inputs(2, "cuda", True, indices=[0, 4, 5, 6])
+    Wa, Ma = [w.clone() for w in W], [m.clone() for m in M]
+    Wb, Mb = [w.clone() for w in W], [m.clone() for m in M]
+    dm.muon_step(Wa, G, Ma, LR, MU, WD)
+    dm.muon_step(Wb, G, Mb, LR, MU, WD)
+    torch.cuda.synchronize()
+    for a, b in zip(Wa + Ma, Wb + Mb):
+        assert torch.equal(a, b), "two runs on the same inputs must agree bitwise"
+    # host entry point: same bits as the device entry point
+    Wh = [w.cpu().pin_memory() for w in W]
+    Gh = [g.cpu().pin_memory() for g in G]
+    Mh = [m.cpu().pin_memory() for m in M]
+    dm.muon_step_host(Wh, Gh, Mh, LR, MU, WD)
+    torch.cuda.synchronize()
+    for a, h in zip(Wa + Ma, Wh + Mh):
+        assert torch.equal(a.cpu(), h)
+    # caller-owned workspace
+    need = dm.workspace_bytes(shapes)
+    assert need > 0
+    ws = torch.empty(need, dtype=torch.uint8, device="cuda")
+    dm.set_workspace(ws)
+    Wc, Mc = [w.clone() for w in W], [m.clone() for m in M]
+    dm.muon_step(Wc, G, Mc, LR, MU, WD)
+    torch.cuda.synchronize()
+    for a, c in zip(Wa + Ma, Wc + Mc):
+        assert torch.equal(a, c)
+    dm.set_workspace(None)
+    small = torch.empty(1024, dtype=torch.uint8, device="cuda")
+    dm.set_workspace(small)
+    with pytest.raises(dm.DmuonError) as ei:
+        dm.muon_step([w.clone() for w in W], G, [m.clone() for m in M], LR, MU, WD)
+    assert ei.value.code == dm.binding.ERR_OOM
+    dm.set_workspace(None)
+
+
+def test_profile_counts_launches():
+    dm.set_option("profile", 1)
+    dm.profile_reset()
+    shapes, W, G, M = synth.muon_inputs(2, "cuda", False, indices=[0, 4, 5])
+    dm.muon_step(W, G, M, LR, MU, WD)
+    prof = dm.profile_read()
+    dm.set_option("profile", 0)
+    k = prof["kernels"]
+    # 2 buckets (768x768, 768x3072) x 5 steps x 3 products, + momentum, norms, normalise, apply
+    assert k["ns_syrk_xxt"]["launches"] == 10 and k["ns_sq_poly"]["launches"] == 10 and k["ns_bx_update"]["launches"] == 10
+    assert k["momentum_nesterov_sumsq"]["launches"] == 1 and k["apply_update"]["launches"] == 1
+    assert prof["launches"] == 34
+    assert all(v["ms"] > 0 for v in k.values())
+
+
+def test_misaligned_pointer_rejected():
+    buf = torch.zeros(128 * 128 + 8, dtype=torch.bfloat16, device="cuda")
+    x = buf[1:1 + 128 * 128].view(128, 128)        # 2-byte offset: not 16-byte aligned
+    with pytest.raises(dm.DmuonError) as ei:
+        dm.ns_batched([x], steps=5)
+    assert ei.value.code == dm.binding.ERR_INVALID_ARG
