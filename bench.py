@@ -1,0 +1,374 @@
+#!/usr/bin/env python
+"""bench.py -- the Muon optimizer step of DMuon (arxiv/paper_2606_27153) on B200, one JSON line.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (momentum+Nesterov+cast+norm, 5 Newton-Schulz steps of three grouped
+GEMMs per shape bucket, apply) over one synthetic matrix set.  Default workload: BASELINE.json configs[3], the
+Llama-3-8B-shaped set (224 matrices, 6.98 G elements, bf16 W/G/M resident in HBM), the configuration the metric
+is quoted on.  `value` = dense-equivalent NS TFLOP/s of the whole step (BASELINE.json: "counting the full dense
+FLOPs") = sum over matrices of 5 (4 m^2 n + 2 m^3) divided by the step time, aggregated over ranks.
+The path does not shard (north_star: one GPU, no collectives): --gpus N runs N independent replicas ("replicas
+only"), timed as the max over ranks.
+--impl reference times the fp64 CPU oracle (oracle/) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+import torch
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "Muon step NS throughput, dense-equivalent FLOPs (BASELINE: Muon step ms & NS TFLOP/s, % of B200 bf16 peak)"
+UNIT = "TFLOP/s"
+LR, MU, WD = 0.02, 0.95, 0.01
+NS_STEPS = 5
+WORKLOADS = {1: "config1: tiny NS batch 8 x (128x512)", 2: "config2: GPT-2-small-shaped, 72 matrices",
+             3: "config3: Qwen-0.5B-style, 168 matrices", 4: "config4: Llama-3-8B-shaped, 224 matrices, 6.98 G elements"}
+
+
+# ------------------------------------------------------------------------------------------------ accounting
+def oriented(shape):
+    r, c = shape
+    return min(r, c), max(r, c)
+
+
+def dense_flops(shapes, steps=NS_STEPS):
+    """Metric FLOPs: 5 (4 m^2 n + 2 m^3) per matrix."""
+    return sum(steps * (4 * m * m * n + 2 * m ** 3) for m, n in map(oriented, shapes))
+
+
+def executed_flops(shapes, steps=NS_STEPS):
+    """FLOPs the symmetric kernels execute on 128-blocks: upper-triangular share (T+1)/(2T) of the two symmetric products."""
+    tot = 0.0
+    for m, n in map(oriented, shapes):
+        t = -(-m // 128)
+        tot += steps * ((t + 1) / (2 * t) * (2 * m * m * n + 2 * m ** 3) + 2 * m * m * n)
+    return tot
+
+
+def kernel_work(shapes, steps=NS_STEPS):
+    """Algorithmic work per step of each kernel family: FLOPs (dense-equivalent) or bytes."""
+    el = sum(r * c for r, c in shapes)
+    mn = [oriented(s) for s in shapes]
+    return {
+        "ns_syrk_xxt": ("flop", steps * sum(2 * m * m * n for m, n in mn)),
+        "ns_sq_poly": ("flop", steps * sum(2 * m ** 3 for m, n in mn)),
+        "ns_bx_update": ("flop", steps * sum(2 * m * m * n for m, n in mn)),
+        "momentum_nesterov_sumsq": ("byte", 8 * el),       # read G, M; write M', U          (a1 + a2)
+        "normalize_orient_cast": ("byte", 4 * el),         # read U; write X0
+        "apply_update": ("byte", 6 * el),                  # read O, W; write W'             (a6)
+    }
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        p = json.load(open(path))
+        return {"hbm_gbs": p["hbm_gbs"], "tflops_burst": p["bf16_tflops"],
+                "tflops_sustained": p.get("bf16_tflops_sustained", p["bf16_tflops"]), "source": "measured"}
+    # fallback stated in /opt/skills/guides/B200_PROFILING.md
+    return {"hbm_gbs": 6650.0, "tflops_burst": 1590.0, "tflops_sustained": 1400.0, "source": "fallback"}
+
+
+# ------------------------------------------------------------------------------------------------ clocks
+class ClockSampler:
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.gpu = gpu_index
+        self.proc = None
+        self.path = None
+
+    def start(self):
+        try:
+            f = tempfile.NamedTemporaryFile("w", suffix=".csv", delete=False)
+            self.path = f.name
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"], stdout=f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if not self.proc:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        rows = []
+        for line in open(self.path):
+            parts = [p.strip() for p in line.split(",")]
+            if len(parts) >= 9:
+                try:
+                    rows.append((float(parts[1]), float(parts[2]), float(parts[3]), parts[5], parts[6], parts[7], parts[8]))
+                except ValueError:
+                    pass
+        os.unlink(self.path)
+        if rows:
+            pmax = max(r[2] for r in rows)
+            load = [r for r in rows if r[2] >= 0.6 * pmax] or rows
+            out["sm_mhz"] = statistics.median(r[0] for r in load)
+            out["sm_max_mhz"] = rows[0][1]
+            out["power_w_max"] = pmax
+            out["samples"] = len(load)
+            names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+            for k, name in enumerate(names):
+                if any(r[3 + k].lower().startswith("active") for r in load):
+                    out["reasons"].append(name)
+        return out
+
+
+# ------------------------------------------------------------------------------------------------ oracle arm
+def oracle_sample(config: int, max_seconds: float = 30.0):
+    """Time the fp64 oracle, as it stands, on a bounded sample of the workload: whole Muon steps of single matrices,
+    smallest distinct shapes first, until ~max_seconds are used.  Returns (dense TFLOP/s, description, cores, seconds)."""
+    import oracle
+    from paper_2606_27153_b200 import synth
+    shapes = synth.config_shapes(config)
+    distinct = sorted(set(shapes), key=lambda s: dense_flops([s]))
+    oracle.ns(torch.zeros(8, 8).double().numpy())          # build + load outside the timed region
+    done, flops, secs = [], 0.0, 0.0
+    for s in distinct:
+        est = dense_flops([s]) / 2.5e10                     # ~25 GFLOP/s plain loops: skip what cannot fit the budget
+        if done and secs + est > max_seconds:
+            break
+        i = shapes.index(s)
+        _, W, G, M = synth.muon_inputs(config, "cpu", False, indices=[i]) if config != 1 else (None, *([synth.ns_inputs("cpu")[1][:1]] * 3))
+        w, g, m = (t[0].to(torch.float64).numpy() for t in (W, G, M))
+        t0 = time.perf_counter()
+        oracle.muon_step(w, g, m, LR, MU, WD, momentum_fp32=True)
+        secs += time.perf_counter() - t0
+        flops += dense_flops([s])
+        done.append(f"{s[0]}x{s[1]}")
+        if secs > max_seconds:
+            break
+    desc = f"one full Muon step (5 NS steps, fp64, dense) of one matrix each of shape {', '.join(done)} from {WORKLOADS[config].split(':')[0]}"
+    return flops / secs / 1e12, desc, oracle.num_threads(), secs
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores; each step is one bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    budget = max(5.0, 60.0 / max(1, args.steps + args.warmup))
+    vals, secs, desc, cores = [], [], "", 0
+    for it in range(args.warmup + args.steps):
+        v, desc, cores, s = oracle_sample(args.config, budget)
+        if it >= args.warmup:
+            vals.append(v)
+            secs.append(s)
+    value = statistics.mean(vals)
+    shapes = __import__("paper_2606_27153_b200.synth", fromlist=["config_shapes"]).config_shapes(args.config)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dense_flops(shapes) / (value * 1e12), "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": WORKLOADS[args.config], "note": "ms_per_step extrapolated from the sample by FLOPs"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
+                         "seconds_per_sample": statistics.mean(secs)},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------------ our arm
+def run_ours(args):
+    import paper_2606_27153_b200 as dm
+    from paper_2606_27153_b200 import synth
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a B200: the Muon step has no CPU path (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist_mod.init_process_group("nccl", device_id=torch.device("cuda", local))
+        dist = dist_mod
+
+    def barrier():
+        if dist:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x: float) -> float:
+        if not dist:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return t.item()
+
+    cfg = args.config
+    shapes = synth.config_shapes(cfg)
+    peaks = load_peaks()
+    dm.set_option("mode", "tc")
+    dm.set_option("steps", NS_STEPS)
+    dm.set_option("profile", 1)
+    t_setup = time.perf_counter()
+    if cfg == 1:
+        _, W = synth.ns_inputs("cuda")
+        G = M = None
+    else:
+        _, W, G, M = synth.muon_inputs(cfg, "cuda", False)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        if cfg == 1:
+            dm.ns_batched(W, steps=NS_STEPS)
+        else:
+            dm.muon_step(W, G, M, LR, MU, WD)
+
+    step()                                    # first call: plan + workspace + autotune (reported, not timed)
+    torch.cuda.synchronize()
+    plan_s = time.perf_counter() - t_setup
+    for _ in range(max(0, args.warmup - 1)):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    dm.profile_reset()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(stream)
+    barrier()
+    ms = max_over_ranks(e0.elapsed_time(e1)) / args.steps
+    prof = dm.profile_read()
+    clocks = sampler.stop() if rank == 0 else {}
+
+    dflops, xflops = dense_flops(shapes), executed_flops(shapes)
+    value = world * dflops / (ms * 1e-3) / 1e12
+
+    # per-kernel rooflines from the library's own CUDA events (recorded on the launching stream, in the timed region)
+    work = kernel_work(shapes)
+    kernels = {}
+    for name, rec in prof["kernels"].items():
+        per_step_ms = rec["ms"] / args.steps
+        entry = {"launches_per_step": rec["launches"] / args.steps, "ms_per_step": per_step_ms, "share": per_step_ms / ms}
+        if name in work and per_step_ms > 0:
+            kind, amount = work[name]
+            if kind == "flop":
+                ach = amount / (per_step_ms * 1e-3) / 1e12
+                entry.update({"bound": "tensor", "achieved": ach, "unit": "TFLOP/s", "frac": ach / peaks["tflops_sustained"],
+                              "frac_of_burst": ach / peaks["tflops_burst"], "frac_of_nominal_2250": ach / 2250.0})
+            else:
+                ach = amount / (per_step_ms * 1e-3) / 1e9
+                entry.update({"bound": "hbm", "achieved": ach, "unit": "GB/s", "frac": ach / peaks["hbm_gbs"]})
+        kernels[name] = entry
+    dom = max((k for k in kernels if k in work and work[k][0] == "flop"), key=lambda k: kernels[k]["ms_per_step"], default=None)
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "roofline_traffic.json")
+    if dom and os.path.exists(tpath):
+        traffic = json.load(open(tpath)).get(f"config{cfg}", {}).get(dom)
+    roofline = None
+    if dom:
+        k = kernels[dom]
+        roofline = {"kernel": dom, "bound": "tensor", "achieved": k["achieved"], "peak": peaks["tflops_sustained"],
+                    "unit": "TFLOP/s", "frac": k["frac"], "traffic": traffic,
+                    "peak_kind": f"{peaks['source']} bf16 cuBLAS, sustained (kernel timed inside a long step); "
+                                 f"burst {peaks['tflops_burst']}, nominal 2250",
+                    "flops_counted": "algorithmic dense: 2 m^2 n per matrix per launch (no symmetry in this product)"}
+
+    # ---- end to end through the C ABI with HOST buffers (copies inside the timed region)
+    e2e = None
+    if cfg != 1 and not args.no_e2e:
+        try:
+            pinned = True
+            host = []
+            for ts in (W, G, M):
+                hs = []
+                for t in ts:
+                    try:
+                        h = torch.empty(t.shape, dtype=t.dtype, pin_memory=pinned)
+                    except RuntimeError:
+                        pinned = False
+                        h = torch.empty(t.shape, dtype=t.dtype)
+                    h.copy_(t)
+                    hs.append(h)
+                host.append(hs)
+            Wh, Gh, Mh = host
+            del W, G, M
+            torch.cuda.empty_cache()
+            n_e2e = max(1, min(args.steps, 3))
+            dm.muon_step_host(Wh, Gh, Mh, LR, MU, WD)         # warm-up: allocates the staging buffers
+            barrier()
+            e0.record(stream)
+            for _ in range(n_e2e):
+                dm.muon_step_host(Wh, Gh, Mh, LR, MU, WD)
+            e1.record(stream)
+            barrier()
+            ms_e2e = max_over_ranks(e0.elapsed_time(e1)) / n_e2e
+            elb = 2 * sum(r * c for r, c in shapes)
+            e2e = {"value": world * dflops / (ms_e2e * 1e-3) / 1e12, "unit": UNIT, "ms_per_step": ms_e2e,
+                   "h2d_bytes_per_step": 3 * elb, "d2h_bytes_per_step": 2 * elb, "steps": n_e2e,
+                   "host_memory": "pinned" if pinned else "pageable", "api": "dmuon_muon_step_host"}
+        except Exception as ex:  # an e2e failure must not hide the device-resident number
+            e2e = {"value": None, "unit": UNIT, "error": str(ex)[:200]}
+
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        v, desc, cores, secs = oracle_sample(cfg, 20.0)
+        cpu_baseline = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc, "seconds": secs}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f16",
+            "data": "synthetic",
+            "config": {"workload": WORKLOADS[cfg], "ns_steps": NS_STEPS, "coeffs": [3.4445, -4.7750, 2.0315], "lr": LR,
+                       "mu": MU, "wd": WD, "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "l2": "inputs (W, G, M + workspace, tens of GB) exceed the 126 MB L2; no flush needed",
+                       "arithmetic": "bf16 in/out, fp16 operands on tcgen05 with fp32 TMEM accumulation, fp32 elementwise"},
+            "muon_step_ms": ms, "ns_tflops_dense_equiv": value / world, "ns_tflops_executed": xflops / (ms * 1e-3) / 1e12,
+            "pct_of_bf16_peak": {"dense_equiv_of_measured_sustained": 100 * value / world / peaks["tflops_sustained"],
+                                 "dense_equiv_of_measured_burst": 100 * value / world / peaks["tflops_burst"],
+                                 "dense_equiv_of_nominal_2250": 100 * value / world / 2250.0,
+                                 "executed_of_measured_sustained": 100 * xflops / (ms * 1e-3) / 1e12 / peaks["tflops_sustained"]},
+            "roofline": roofline, "kernels": kernels, "cpu_baseline": cpu_baseline, "e2e": e2e,
+            "gpu_launches": prof["launches"], "clocks": clocks, "plan_autotune_seconds": plan_s,
+            "paper_context": "DMuon reports 6.85x-163x optimizer-step and 1.48x-3.01x end-to-end speedups on 8-256 A800 "
+                             "(PAPER.md:5, :274) and ~2x on one GPU (:329): other hardware, context only",
+        }
+        print(json.dumps(line))
+    if dist:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
