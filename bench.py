@@ -247,10 +247,12 @@ def run_ours(args):
         sampler.start()
     dm.profile_reset()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.nvtx.range_push("dmuon_timed")     # lets `ncu --nvtx --nvtx-include dmuon_timed/` profile timed launches only
     e0.record(stream)
     for _ in range(args.steps):
         step()
     e1.record(stream)
+    torch.cuda.nvtx.range_pop()
     barrier()
     ms = max_over_ranks(e0.elapsed_time(e1)) / args.steps
     prof = dm.profile_read()

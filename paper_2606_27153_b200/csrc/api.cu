@@ -354,7 +354,7 @@ DMUON_API int dmuon_profile_read(char* buf, size_t len) {
   return static_cast<int>(s.size());
 }
 
-DMUON_API int dmuon_ns_gemm_variants(int32_t op) { return (op == OP_BX) ? kNumVariants : (op == OP_SYRK || op == OP_SQ) ? 2 : 0; }
+DMUON_API int dmuon_ns_gemm_variants(int32_t op) { return (op >= OP_SYRK && op <= OP_BX) ? kNumVariants : 0; }
 
 DMUON_API int dmuon_ns_gemm(int32_t op, const void* const* in0, const void* const* in1, void* const* out, int32_t m,
                             int32_t n, int32_t count, float alpha, float beta, int32_t variant, dmuon_stream_t stream_) {
@@ -363,7 +363,7 @@ DMUON_API int dmuon_ns_gemm(int32_t op, const void* const* in0, const void* cons
   if (count < 0 || (count > 0 && (!in0 || !out || (op == OP_BX && !in1)))) { set_error("dmuon_ns_gemm: null argument"); return DMUON_ERR_INVALID_ARG; }
   if (op == OP_SQ) n = m;
   if (m <= 0 || n <= 0 || m % kBlk || n % kBlk) { set_error("dmuon_ns_gemm: m and n must be positive multiples of 128 (got %d, %d)", m, n); return DMUON_ERR_INVALID_ARG; }
-  if (variant < -1 || variant >= kNumVariants) { set_error("dmuon_ns_gemm: bad variant %d", variant); return DMUON_ERR_INVALID_ARG; }
+  if (variant < -1 || (variant >= 0 && !variant_valid(static_cast<GemmOp>(op), variant))) { set_error("dmuon_ns_gemm: variant %d is not defined for op %d", variant, op); return DMUON_ERR_INVALID_ARG; }
   if (count == 0) return DMUON_OK;
   int rc = check_device();
   if (rc) return rc;
@@ -404,6 +404,9 @@ DMUON_API int dmuon_ns_gemm(int32_t op, const void* const* in0, const void* cons
   L.units_per_problem = gc.units;
   L.num_problems = count;
   L.k_blocks = (op == OP_SYRK ? n : m) / kBlkK;
+  L.m_blocks = m / kBlk;
+  L.n_blocks = (op == OP_BX ? n : m) / kBlk;
+  L.pair = variant_config(variant < 0 ? 0 : variant).pair;
   L.alpha = alpha;
   L.beta = beta;
   L.grid = sms;

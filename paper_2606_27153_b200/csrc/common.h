@@ -26,8 +26,9 @@ void set_error(const char* fmt, ...);
   } while (0)
 
 // ---------------------------------------------------------------- GEMM family (gemm_sm100.cu)
-// Tile geometry: output tiles are built from 128 x 128 blocks; a work unit is one block row of 1 or 2 blocks
-// (UMMA 128 x 128 or 128 x 256), the contraction advances 64 elements per pipeline stage.
+// Tile geometry: output tiles are built from 128 x 128 blocks.  A work unit of the single-CTA tiling is one block row
+// of 1 or 2 blocks (UMMA 128 x 128 or 128 x 256); a work unit of the CTA-pair tiling is 2 x 2 blocks (UMMA 256 x 256
+// over two SMs).  The contraction advances 64 elements per pipeline stage.
 constexpr int kBlk = 128;     // block edge (UMMA_M)
 constexpr int kBlkK = 64;     // K elements per stage = one 128-byte swizzle row of fp16
 
@@ -44,7 +45,8 @@ struct alignas(128) GemmProblem {
 };
 static_assert(sizeof(GemmProblem) == 384, "GemmProblem layout");
 
-// One work unit of a problem: block row, first block column, number of blocks (1 or 2).
+// One work unit of a problem.  Single-CTA tiling: block row, first block column, number of blocks (1 or 2), in
+// 128-blocks.  CTA-pair tiling: m_blk, n_blk index 256 x 256 units (width unused).
 struct TileUnit {
   int16_t m_blk, n_blk, width, flags;
 };
@@ -56,6 +58,8 @@ struct GemmLaunch {
   int units_per_problem;
   int num_problems;
   int k_blocks;                 // K / 64
+  int m_blocks, n_blocks;       // extent of the output in 128-blocks
+  bool pair;                    // CTA-pair (cta_group::2) tiling
   float alpha, beta;
   int grid;                     // CTAs (<= #SM)
 };

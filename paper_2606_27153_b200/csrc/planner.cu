@@ -126,7 +126,9 @@ void save_tune_cache(const std::string& path) {
 }
 
 int bucket_launch(const Plan& plan, const BucketPlan& b, GemmOp op, int parity, float alpha, float beta,
-                  cudaStream_t stream, const TileUnit* units_override = nullptr, int upp_override = 0) {
+                  cudaStream_t stream, const TileUnit* units_override = nullptr, int upp_override = 0,
+                  int variant_override = -1) {
+  const bool pair = variant_config(variant_override >= 0 ? variant_override : b.variant[op]).pair;
   GemmLaunch L;
   L.op = op;
   L.problems = op == OP_SYRK ? b.syrk[parity] : op == OP_SQ ? b.sq : b.bx[parity];
@@ -134,6 +136,9 @@ int bucket_launch(const Plan& plan, const BucketPlan& b, GemmOp op, int parity, 
   L.units_per_problem = units_override ? upp_override : b.units_per_problem[op];
   L.num_problems = static_cast<int>(b.mats.size());
   L.k_blocks = (op == OP_SYRK ? b.n_pad : b.m_pad) / kBlkK;
+  L.m_blocks = b.m_pad / kBlk;
+  L.n_blocks = (op == OP_BX ? b.n_pad : b.m_pad) / kBlk;
+  L.pair = pair;
   L.alpha = alpha;
   L.beta = beta;
   L.grid = plan.sm_count;
@@ -158,8 +163,8 @@ int autotune_bucket(Plan& plan, BucketPlan& b, const Options& opt, cudaStream_t 
       DMUON_CUDA_CHECK(cudaEventCreate(&e1));
       float best_ms = 1e30f;
       for (int v = 0; v < kNumVariants; ++v) {
+        if (!variant_valid(static_cast<GemmOp>(op), v)) continue;
         const TileConfig cfg = variant_config(v);
-        if (op != OP_BX && cfg.order != 0) continue;   // symmetric ops have one ordering
         std::vector<TileUnit> hu = make_units(static_cast<GemmOp>(op), b.m_pad / kBlk, b.n_pad / kBlk, cfg);
         TileUnit* du = nullptr;
         DMUON_CUDA_CHECK(cudaMalloc(&du, hu.size() * sizeof(TileUnit)));
@@ -168,7 +173,7 @@ int autotune_bucket(Plan& plan, BucketPlan& b, const Options& opt, cudaStream_t 
         float ms = 1e30f;
         for (int rep = 0; rep < 3 && rc == DMUON_OK; ++rep) {   // rep 0 warms up
           cudaEventRecord(e0, stream);
-          rc = bucket_launch(plan, b, static_cast<GemmOp>(op), 0, 1.f, 0.f, stream, du, static_cast<int>(hu.size()));
+          rc = bucket_launch(plan, b, static_cast<GemmOp>(op), 0, 1.f, 0.f, stream, du, static_cast<int>(hu.size()), v);
           cudaEventRecord(e1, stream);
           if (cudaEventSynchronize(e1) != cudaSuccess) rc = DMUON_ERR_CUDA;
           float t = 0.f;
@@ -212,14 +217,35 @@ Plan::~Plan() {
 
 TileConfig variant_config(int variant) {
   TileConfig c;
-  c.width = (variant & 1) ? 1 : 2;
-  c.order = (variant >> 1) & 1;
+  if (variant >= 4) {
+    c.pair = true;
+    c.order = variant & 1;
+  } else {
+    c.width = (variant & 1) ? 1 : 2;
+    c.order = (variant >> 1) & 1;
+  }
   return c;
+}
+
+bool variant_valid(GemmOp op, int variant) {
+  if (variant < 0 || variant >= kNumVariants) return false;
+  return op == OP_BX || variant_config(variant).order == 0;   // symmetric ops have one ordering
 }
 
 std::vector<TileUnit> make_units(GemmOp op, int mb, int nb, const TileConfig& cfg) {
   std::vector<TileUnit> u;
   auto push = [&](int i, int j, int w) { u.push_back(TileUnit{static_cast<int16_t>(i), static_cast<int16_t>(j), static_cast<int16_t>(w), 0}); };
+  if (cfg.pair) {
+    // 256 x 256 units; an odd block count leaves a half-empty last unit (operands zero-filled, stores skipped)
+    const int MB = (mb + 1) / 2, NB = (nb + 1) / 2;
+    if (op == OP_BX) {
+      if (cfg.order == 0) { for (int j = 0; j < NB; ++j) for (int i = 0; i < MB; ++i) push(i, j, 2); }
+      else                { for (int i = 0; i < MB; ++i) for (int j = 0; j < NB; ++j) push(i, j, 2); }
+    } else {
+      for (int i = 0; i < MB; ++i) for (int j = i; j < MB; ++j) push(i, j, 2);
+    }
+    return u;
+  }
   if (op == OP_BX) {
     if (cfg.order == 0) {
       for (int j = 0; j < nb; j += cfg.width)

@@ -33,10 +33,14 @@ struct MatrixInfo {
 
 // Tile configuration of one op of one bucket ("variant" of dmuon_ns_gemm).
 struct TileConfig {
-  int width = 2;         // blocks per work unit: 2 -> UMMA N = 256, 1 -> N = 128
+  bool pair = false;     // CTA-pair tiling: 256 x 256 units on two SMs (cta_group::2)
+  int width = 2;         // single-CTA tiling, blocks per work unit: 2 -> UMMA N = 256, 1 -> N = 128
   int order = 0;         // 0: panel-major (all block rows of one column panel first), 1: row-major
 };
-constexpr int kNumVariants = 4;
+// Variants 0..3: single CTA, (width, order) = (2,0), (1,0), (2,1), (1,1); 4, 5: CTA pair, order 0, 1.
+// The symmetric ops have one ordering: their variants are 0, 1 (single CTA) and 4 (pair).
+constexpr int kNumVariants = 6;
+bool variant_valid(GemmOp op, int variant);
 TileConfig variant_config(int variant);
 
 struct BucketPlan {

@@ -25,7 +25,7 @@ SHAPES = [(128, 128, 1), (128, 512, 3), (256, 256, 2), (384, 640, 2), (768, 3072
 
 
 @pytest.mark.parametrize("m,k,count", SHAPES)
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 4])      # single CTA N=256 / N=128, CTA pair 256 x 256
 def test_syrk(m, k, count, variant):
     X = [_rand((m, k), 10 + i, k ** -0.5) for i in range(count)]
     C = [torch.full((m, m), float("nan"), device="cuda", dtype=torch.float16) for _ in range(count)]
@@ -39,7 +39,7 @@ def test_syrk(m, k, count, variant):
 
 
 @pytest.mark.parametrize("m,count", [(128, 1), (256, 3), (384, 2), (896, 2), (1024, 2), (4096, 1)])
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 4])
 def test_sq(m, count, variant):
     A = []
     for i in range(count):
@@ -57,7 +57,7 @@ def test_sq(m, count, variant):
 
 
 @pytest.mark.parametrize("m,n,count", SHAPES)
-@pytest.mark.parametrize("variant", [0, 1, 2, 3])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5])
 def test_bx(m, n, count, variant):
     B = [_rand((m, m), 30 + i, m ** -0.5) for i in range(count)]       # not symmetric on purpose: catches a transposed operand
     X = [_rand((m, n), 40 + i, 1.0) for i in range(count)]
@@ -70,12 +70,22 @@ def test_bx(m, n, count, variant):
         assert _rel(c, ref) < 1e-3
 
 
-def test_many_problems_more_units_than_sms():
-    """Persistent loop + double-buffered TMEM across many work units per CTA."""
+@pytest.mark.parametrize("variant", [0, 4])
+def test_many_problems_more_units_than_sms(variant):
+    """Persistent loop + double-buffered TMEM across many work units per CTA (or CTA pair)."""
     m, k, count = 256, 384, 200
     X = [_rand((m, k), 100 + i, k ** -0.5) for i in range(count)]
     C = [torch.empty((m, m), device="cuda", dtype=torch.float16) for _ in range(count)]
-    dm.ns_gemm(OP_SYRK, X, None, C, alpha=1.0, beta=0.0)
+    dm.ns_gemm(OP_SYRK, X, None, C, alpha=1.0, beta=0.0, variant=variant)
     torch.cuda.synchronize()
     for i in (0, 1, 57, 148, 199):
         assert _rel(C[i], X[i].float() @ X[i].float().t()) < 1e-3
+
+
+def test_variant_table():
+    assert dm.binding.ns_gemm_variants(OP_BX) == 6
+    x = _rand((128, 128), 1, 1.0)
+    c = torch.empty_like(x)
+    for bad in (2, 3, 5, 6):           # symmetric ops have one ordering; 6 is out of range
+        with pytest.raises(dm.DmuonError):
+            dm.ns_gemm(OP_SYRK, [x], None, [c], alpha=1.0, beta=0.0, variant=bad)
