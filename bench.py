@@ -142,7 +142,7 @@ def oracle_sample(config: int, max_seconds: float = 30.0):
     oracle.ns(torch.zeros(8, 8).double().numpy())          # build + load outside the timed region
     done, flops, secs = [], 0.0, 0.0
     for s in distinct:
-        est = dense_flops([s]) / 2.5e10                     # ~25 GFLOP/s plain loops: skip what cannot fit the budget
+        est = dense_flops([s]) / 7e10                       # ~70 GFLOP/s plain loops on 16 cores: skip what cannot fit the budget
         if done and secs + est > max_seconds:
             break
         i = shapes.index(s)
@@ -218,6 +218,11 @@ def run_ours(args):
 
     cfg = args.config
     shapes = synth.config_shapes(cfg)
+    indices = None
+    if args.layers > 0 and cfg != 1:          # profiling aid: the first L layers of the set (NOT a bench line)
+        per_layer = {2: 6, 3: 7, 4: 7}[cfg]
+        indices = list(range(min(len(shapes), per_layer * args.layers)))
+        shapes = shapes[:len(indices)]
     peaks = load_peaks()
     dm.set_option("mode", "tc")
     dm.set_option("steps", NS_STEPS)
@@ -227,7 +232,7 @@ def run_ours(args):
         _, W = synth.ns_inputs("cuda")
         G = M = None
     else:
-        _, W, G, M = synth.muon_inputs(cfg, "cuda", False)
+        _, W, G, M = synth.muon_inputs(cfg, "cuda", False, indices=indices)
     stream = torch.cuda.current_stream()
 
     def step():
@@ -329,7 +334,7 @@ def run_ours(args):
 
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        v, desc, cores, secs = oracle_sample(cfg, 20.0)
+        v, desc, cores, secs = oracle_sample(cfg, 32.0)
         cpu_baseline = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc, "seconds": secs}
 
     if rank == 0:
@@ -337,7 +342,7 @@ def run_ours(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f16",
             "data": "synthetic",
-            "config": {"workload": WORKLOADS[cfg], "ns_steps": NS_STEPS, "coeffs": [3.4445, -4.7750, 2.0315], "lr": LR,
+            "config": {"workload": WORKLOADS[cfg] + (f" -- REDUCED to the first {args.layers} layers (profiling run, not a bench value)" if indices is not None else ""), "ns_steps": NS_STEPS, "coeffs": [3.4445, -4.7750, 2.0315], "lr": LR,
                        "mu": MU, "wd": WD, "parallelism": "replicas only" if world > 1 else "single GPU",
                        "l2": "inputs (W, G, M + workspace, tens of GB) exceed the 126 MB L2; no flush needed",
                        "arithmetic": "bf16 in/out, fp16 operands on tcgen05 with fp32 TMEM accumulation, fp32 elementwise"},
@@ -363,6 +368,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--layers", type=int, default=0, help="profiling aid: only the first L layers of the set (0 = all)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
