@@ -47,23 +47,47 @@ def dense_flops(shapes, steps=NS_STEPS):
     return sum(steps * (4 * m * m * n + 2 * m ** 3) for m, n in map(oriented, shapes))
 
 
-def executed_flops(shapes, steps=NS_STEPS):
-    """FLOPs the symmetric kernels execute on 128-blocks: upper-triangular share (T+1)/(2T) of the two symmetric products."""
-    tot = 0.0
+def pad128(v):
+    return -(-v // 128) * 128
+
+
+def launch_counts(shapes, plan):
+    """Per matrix (m, n, products): how many launches of each product family the library's block schedule
+    (dmuon_describe_plan) runs.  A block of length L: 1 SYRK, L polynomial products, 3 (L - 1) Gram-space products
+    (T = aG + BG, G' = aT + TB, R' = pB' + aR + B'R), 1 X update."""
+    blocks = {(b["m"], b["n"]): b["blocks"] for b in plan["buckets"]}
+    out = []
     for m, n in map(oriented, shapes):
+        part = blocks[(pad128(m), pad128(n))]
+        out.append((m, n, {"ns_syrk_xxt": len(part), "ns_sq_poly": sum(part), "ns_gram_mm": sum(3 * (L - 1) for L in part),
+                           "ns_bx_update": len(part)}))
+    return out
+
+
+def executed_flops(shapes, plan):
+    """FLOPs the kernels execute: every m x m result and X X^T is symmetric and only its upper-triangular 128-blocks
+    are computed, a share (T+1)/(2T) of the dense product; X updates are dense."""
+    tot = 0.0
+    for m, n, cnt in launch_counts(shapes, plan):
         t = -(-m // 128)
-        tot += steps * ((t + 1) / (2 * t) * (2 * m * m * n + 2 * m ** 3) + 2 * m * m * n)
+        sym = (t + 1) / (2 * t)
+        tot += sym * (cnt["ns_syrk_xxt"] * 2 * m * m * n + (cnt["ns_sq_poly"] + cnt["ns_gram_mm"]) * 2 * m ** 3)
+        tot += cnt["ns_bx_update"] * 2 * m * m * n
     return tot
 
 
-def kernel_work(shapes, steps=NS_STEPS):
-    """Algorithmic work per step of each kernel family: FLOPs (dense-equivalent) or bytes."""
+def kernel_work(shapes, plan):
+    """Algorithmic work per step of each kernel family: FLOPs or bytes.  For the symmetric
+    products the algorithmic FLOPs are those of the upper-triangular 128-blocks, (T+1)/(2T) of the dense 2 m^2 n or
+    2 m^3 (the rest of the result is a mirror, not arithmetic); the X update is dense."""
     el = sum(r * c for r, c in shapes)
-    mn = [oriented(s) for s in shapes]
+    lc = launch_counts(shapes, plan)
+    sym = lambda m: (-(-m // 128) + 1) / (2 * -(-m // 128))
     return {
-        "ns_syrk_xxt": ("flop", steps * sum(2 * m * m * n for m, n in mn)),
-        "ns_sq_poly": ("flop", steps * sum(2 * m ** 3 for m, n in mn)),
-        "ns_bx_update": ("flop", steps * sum(2 * m * m * n for m, n in mn)),
+        "ns_syrk_xxt": ("flop", sum(c["ns_syrk_xxt"] * sym(m) * 2 * m * m * n for m, n, c in lc)),
+        "ns_sq_poly": ("flop", sum(c["ns_sq_poly"] * sym(m) * 2 * m ** 3 for m, n, c in lc)),
+        "ns_gram_mm": ("flop", sum(c["ns_gram_mm"] * sym(m) * 2 * m ** 3 for m, n, c in lc)),
+        "ns_bx_update": ("flop", sum(c["ns_bx_update"] * 2 * m * m * n for m, n, c in lc)),
         "momentum_nesterov_sumsq": ("byte", 8 * el),       # read G, M; write M', U          (a1 + a2)
         "normalize_orient_cast": ("byte", 4 * el),         # read U; write X0
         "apply_update": ("byte", 6 * el),                  # read O, W; write W'             (a6)
@@ -263,11 +287,12 @@ def run_ours(args):
     prof = dm.profile_read()
     clocks = sampler.stop() if rank == 0 else {}
 
-    dflops, xflops = dense_flops(shapes), executed_flops(shapes)
+    plan_desc = dm.describe_plan(shapes, NS_STEPS)
+    dflops, xflops = dense_flops(shapes), executed_flops(shapes, plan_desc)
     value = world * dflops / (ms * 1e-3) / 1e12
 
     # per-kernel rooflines from the library's own CUDA events (recorded on the launching stream, in the timed region)
-    work = kernel_work(shapes)
+    work = kernel_work(shapes, plan_desc)
     kernels = {}
     for name, rec in prof["kernels"].items():
         per_step_ms = rec["ms"] / args.steps
@@ -294,7 +319,9 @@ def run_ours(args):
                     "unit": "TFLOP/s", "frac": k["frac"], "traffic": traffic,
                     "peak_kind": f"{peaks['source']} bf16 cuBLAS, sustained (kernel timed inside a long step); "
                                  f"burst {peaks['tflops_burst']}, nominal 2250",
-                    "flops_counted": "algorithmic dense: 2 m^2 n per matrix per launch (no symmetry in this product)"}
+                    "flops_counted": "algorithmic FLOPs of this family's launches: 2 m^2 n per matrix per X update (dense, no "
+                                     "symmetry); (T+1)/(2T) of 2 m^2 n or 2 m^3 per matrix for the symmetric products "
+                                     "(upper-triangular 128-blocks; the mirror is not arithmetic)"}
 
     # ---- end to end through the C ABI with HOST buffers (copies inside the timed region)
     e2e = None
@@ -343,7 +370,7 @@ def run_ours(args):
             "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f16",
             "data": "synthetic",
             "config": {"workload": WORKLOADS[cfg] + (f" -- REDUCED to the first {args.layers} layers (profiling run, not a bench value)" if indices is not None else ""), "ns_steps": NS_STEPS, "coeffs": [3.4445, -4.7750, 2.0315], "lr": LR,
-                       "mu": MU, "wd": WD, "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "mu": MU, "wd": WD, "schedule": plan_desc["buckets"], "parallelism": "replicas only" if world > 1 else "single GPU",
                        "l2": "inputs (W, G, M + workspace, tens of GB) exceed the 126 MB L2; no flush needed",
                        "arithmetic": "bf16 in/out, fp16 operands on tcgen05 with fp32 TMEM accumulation, fp32 elementwise"},
             "muon_step_ms": ms, "ns_tflops_dense_equiv": value / world, "ns_tflops_executed": xflops / (ms * 1e-3) / 1e12,

@@ -106,12 +106,35 @@ DMUON_API int dmuon_set_workspace(void* dev_ptr, size_t bytes);
  *   "coeffs"      "a,b,c" used by dmuon_muon_step (default "3.4445,-4.7750,2.0315")
  *   "mode"        "tc"  = fp16 operands on tcgen05 tensor cores, fp32 accumulation in TMEM (default; PAPER.md:262 runs NS in fp16);
  *                 "fp32_check" = fp32 operands, plain SIMT kernels: the <= 1e-4 check mode, small shapes only
+ *   "schedule"    "auto" = on wide buckets (n >= 1.5 m, m >= 256) run the k steps as Gram blocks: G = X X^T once per block,
+ *                 G_{i+1} = P_i G_i P_i in the m x m Gram space (Eq. 4), Q = prod P_i, one X <- Q X per
+ *                 block; blocks of 3 then 2 steps for k = 5 (restarts keep fp16 storage stable).  An exact
+ *                 reformulation of Eq. 2: same result up to rounding (default).
+ *                 "x" = the plain iteration X <- (a I + B) X at every step, on every bucket
  *   "autotune"    "1"/"0": pick each bucket's tile configuration by on-device measurement (default "1")
  *   "cache_path"  file for the persistent tuning cache ("" disables; default $DMUON_CACHE or ~/.cache/dmuon/tune.txt)
  *   "profile"     "1"/"0": record CUDA events around every kernel launch (read with dmuon_profile_read)
  * Returns DMUON_ERR_INVALID_ARG for an unknown key or unparsable value.
  */
 DMUON_API int dmuon_set_option(const char* key, const char* value);
+
+/*
+ * Describe how a shape set is executed: writes a JSON object
+ *   {"buckets": [{"m": m_pad, "n": n_pad, "count": matrices, "blocks": [3, 2], "variants": [syrk, sq, bx]}, ...]}
+ * for `steps` NS steps with the current options and default coefficients into buf (NUL terminated, truncated to
+ * len); builds the plan if needed (like dmuon_warmup).  Returns the bytes needed (excluding the NUL) or a negative error.
+ */
+DMUON_API int dmuon_describe_plan(const int32_t* shapes, int32_t count, int32_t steps, char* buf, size_t len,
+                                  dmuon_stream_t stream);
+
+/*
+ * Host-only (no device needed): the block schedule the library would use for ONE rows x cols matrix and `steps` NS
+ * steps under the current "schedule" option.  coeffs: HOST, 3 floats (per_step = 0), [steps][3] (per_step = 1) or
+ * NULL (defaults).  Writes up to `cap` block lengths into out (sum = steps) and returns the number of blocks, or a
+ * negative error.  A block of length 1 is the plain step; longer blocks run in the Gram space (see "schedule").
+ */
+DMUON_API int dmuon_block_schedule(int32_t rows, int32_t cols, int32_t steps, const float* coeffs, int32_t per_step,
+                                   int32_t* out, int32_t cap);
 
 /* Thread's last error message ("" if none).  The pointer stays valid until the thread's next failing call. */
 DMUON_API const char* dmuon_last_error(void);
@@ -140,6 +163,18 @@ DMUON_API int dmuon_profile_reset(void);
 DMUON_API int dmuon_ns_gemm(int32_t op, const void* const* in0, const void* const* in1, void* const* out,
                             int32_t m, int32_t n, int32_t count, float alpha, float beta, int32_t variant,
                             dmuon_stream_t stream);
+
+/*
+ * The symmetric m x m product of the Gram blocks (Eq. 4), for tests: ONE grouped launch of
+ *   C = alpha * A B^T + beta * D + beta2 * D2
+ * over `count` problems; every matrix is fp16 m x m row-major on the DEVICE, m a multiple of 128.  The RESULT is
+ * assumed symmetric (A, B commuting symmetric matrices): only upper-triangular tiles are computed and mirrored.
+ * d and/or d2 may be NULL (term absent; d2 requires d).  a/b/d/d2/out: HOST arrays[count] of DEVICE pointers; out
+ * must not alias an input.  variant as for dmuon_ns_gemm op 1.  Synchronises `stream` before returning (test entry).
+ */
+DMUON_API int dmuon_ns_sym_mm(const void* const* a, const void* const* b, const void* const* d, const void* const* d2,
+                              void* const* out, int32_t m, int32_t count, float alpha, float beta, float beta2,
+                              int32_t variant, dmuon_stream_t stream);
 
 /* Number of tile-configuration variants dmuon_ns_gemm accepts for `op`. */
 DMUON_API int dmuon_ns_gemm_variants(int32_t op);

@@ -25,7 +25,7 @@ OP_SYRK, OP_SQ, OP_BX = 0, 1, 2
 SYMBOLS = ("dmuon_ns_batched", "dmuon_ns_batched_sched", "dmuon_muon_step", "dmuon_muon_step_host", "dmuon_warmup",
            "dmuon_workspace_bytes", "dmuon_set_workspace", "dmuon_set_option", "dmuon_last_error",
            "dmuon_profile_read", "dmuon_profile_reset", "dmuon_ns_gemm", "dmuon_ns_gemm_variants", "dmuon_read_ns_output", "dmuon_shutdown",
-           "dmuon_version")
+           "dmuon_version", "dmuon_describe_plan", "dmuon_ns_sym_mm", "dmuon_block_schedule")
 
 
 class DmuonError(RuntimeError):
@@ -62,6 +62,9 @@ def lib() -> ctypes.CDLL:
         L.dmuon_profile_read.argtypes = [ctypes.c_char_p, ctypes.c_size_t]
         L.dmuon_ns_gemm.argtypes = [i32, pp, pp, pp, i32, i32, i32, f32, f32, i32, vp]
         L.dmuon_ns_gemm_variants.argtypes = [i32]
+        L.dmuon_ns_sym_mm.argtypes = [pp, pp, pp, pp, pp, i32, i32, f32, f32, f32, i32, vp]
+        L.dmuon_block_schedule.argtypes = [i32, i32, i32, pf, i32, pi, i32]
+        L.dmuon_describe_plan.argtypes = [pi, i32, i32, ctypes.c_char_p, ctypes.c_size_t, vp]
         L.dmuon_read_ns_output.argtypes = [i32, vp, vp]
         L.dmuon_shutdown.restype = None
         L.dmuon_version.restype = ctypes.c_char_p
@@ -199,6 +202,43 @@ def ns_gemm(op: int, in0: Sequence[torch.Tensor], in1: Optional[Sequence[torch.T
     n = in0[0].shape[1] if op == OP_SYRK else (out[0].shape[1] if op == OP_BX else m)
     _check(lib().dmuon_ns_gemm(op, _ptr_array(in0), _ptr_array(in1) if in1 else None, _ptr_array(out), m, n, len(in0),
                                float(alpha), float(beta), int(variant), _stream(stream)))
+
+
+def ns_sym_mm(a: Sequence[torch.Tensor], b: Sequence[torch.Tensor], d: Optional[Sequence[torch.Tensor]],
+              d2: Optional[Sequence[torch.Tensor]], out: Sequence[torch.Tensor], alpha: float, beta: float = 0.0,
+              beta2: float = 0.0, variant: int = -1, stream=None) -> None:
+    """dmuon_ns_sym_mm: out = alpha a b^T + beta d + beta2 d2 on fp16 m x m matrices (symmetric result)."""
+    for ts in (a, b, d or [], d2 or [], out):
+        for t in ts:
+            if t.dtype != torch.float16 or not t.is_contiguous() or t.device.type != "cuda" or t.dim() != 2:
+                raise ValueError("ns_sym_mm takes contiguous 2-D float16 cuda tensors")
+    _check(lib().dmuon_ns_sym_mm(_ptr_array(a), _ptr_array(b), _ptr_array(d) if d else None,
+                                 _ptr_array(d2) if d2 else None, _ptr_array(out), a[0].shape[0], len(a), float(alpha),
+                                 float(beta), float(beta2), int(variant), _stream(stream)))
+
+
+def block_schedule(shape: Sequence[int], steps: int = 5, coeffs: Optional[Sequence] = None) -> List[int]:
+    """dmuon_block_schedule (host only): block lengths for one matrix; coeffs = (a, b, c) or one triple per step."""
+    per_step, co = 0, None
+    if coeffs is not None:
+        per_step = int(len(coeffs) > 0 and hasattr(coeffs[0], "__len__"))
+        flat = [float(v) for row in coeffs for v in row] if per_step else [float(v) for v in coeffs]
+        co = (ctypes.c_float * len(flat))(*flat)
+    out = (ctypes.c_int32 * 64)()
+    rc = lib().dmuon_block_schedule(int(shape[0]), int(shape[1]), int(steps), co, per_step, out, 64)
+    if rc < 0:
+        _check(rc)
+    return [int(out[i]) for i in range(rc)]
+
+
+def describe_plan(shapes: Sequence[Sequence[int]], steps: int = 5, stream=None) -> dict:
+    """dmuon_describe_plan: buckets, block schedule and tile variants the library uses for this shape set."""
+    shp, n = _shape_array(shapes)
+    buf = ctypes.create_string_buffer(1 << 16)
+    rc = lib().dmuon_describe_plan(shp, n, int(steps), buf, len(buf), _stream(stream))
+    if rc < 0:
+        _check(rc)
+    return json.loads(buf.value.decode())
 
 
 def read_ns_output(index: int, shape: Sequence[int], stream=None) -> torch.Tensor:

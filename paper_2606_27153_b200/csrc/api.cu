@@ -75,9 +75,13 @@ int validate(const void* const* a, const void* const* b, const void* const* c, c
 }
 
 // Patch the per-call pointers into the plan's records and upload them if anything changed.
-int bind_pointers(Plan& plan, void* const* w, const void* const* g, void* const* m, int steps, cudaStream_t stream) {
+int bind_pointers(Plan& plan, void* const* w, const void* const* g, void* const* m, int steps, const float* coeffs,
+                  bool per_step, cudaStream_t stream) {
   const int count = static_cast<int>(plan.mats.size());
-  bool dirty = plan.o_parity != (steps & 1);
+  bool dirty = false;
+  std::vector<int> parity(plan.buckets.size());
+  for (size_t b = 0; b < plan.buckets.size(); ++b)
+    parity[b] = result_parity(plan, plan.buckets[b], steps, coeffs, per_step, g_opt);
   for (int i = 0; i < count; ++i) {
     MatRec& r = plan.h_recs[i];
     void* gi = g ? const_cast<void*>(g[i]) : nullptr;
@@ -87,9 +91,10 @@ int bind_pointers(Plan& plan, void* const* w, const void* const* g, void* const*
     r.G = gi;
     r.M = mi;
     const MatrixInfo& info = plan.mats[i];
-    r.O = plan.ws + ((steps & 1) ? info.off_p : info.off_q);   // X0 in Q; each step swaps buffers
+    const void* o = plan.ws + (parity[info.bucket] ? info.off_p : info.off_q);   // X0 in Q; each block swaps buffers
+    if (r.O != o) dirty = true;
+    r.O = o;
   }
-  plan.o_parity = steps & 1;
   if (dirty && count > 0)
     DMUON_CUDA_CHECK(cudaMemcpyAsync(plan.d_recs, plan.h_recs.data(), sizeof(MatRec) * count, cudaMemcpyHostToDevice, stream));
   return DMUON_OK;
@@ -102,12 +107,12 @@ int muon_step_device(void* const* params, const void* const* grads, void* const*
   if (rc) return rc;
   if (plan_out) *plan_out = plan;
   g_last_plan = plan;
-  if ((rc = bind_pointers(*plan, params, grads, momenta, g_opt.steps, stream))) return rc;
+  if ((rc = bind_pointers(*plan, params, grads, momenta, g_opt.steps, g_opt.coeffs, false, stream))) return rc;
   const ElemTables& T = plan->tables;
   if ((rc = launch_momentum(T, mu, stream))) return rc;
   if ((rc = launch_finalize_norms(T, g_opt.eps, stream))) return rc;
   if ((rc = launch_normalize(T, /*from_user=*/false, plan->fp32, stream))) return rc;
-  if ((rc = run_ns_steps(*plan, g_opt.steps, g_opt.coeffs, false, stream))) return rc;
+  if ((rc = run_ns_steps(*plan, g_opt.steps, g_opt.coeffs, false, g_opt, stream))) return rc;
   if ((rc = launch_apply(T, lr, wd, plan->fp32, stream))) return rc;
   return DMUON_OK;
 }
@@ -126,12 +131,12 @@ int ns_batched_impl(void* const* ptrs, const int32_t* shapes, int32_t count, int
   Plan* plan = nullptr;
   if ((rc = get_plan(shapes, count, g_opt, g_ext_ws, g_ext_ws_bytes, stream, &plan))) return rc;
   g_last_plan = plan;
-  if ((rc = bind_pointers(*plan, ptrs, nullptr, nullptr, steps, stream))) return rc;
+  if ((rc = bind_pointers(*plan, ptrs, nullptr, nullptr, steps, coeffs, per_step, stream))) return rc;
   const ElemTables& T = plan->tables;
   if ((rc = launch_sumsq(T, stream))) return rc;
   if ((rc = launch_finalize_norms(T, g_opt.eps, stream))) return rc;
   if ((rc = launch_normalize(T, /*from_user=*/true, plan->fp32, stream))) return rc;
-  if ((rc = run_ns_steps(*plan, steps, coeffs, per_step, stream))) return rc;
+  if ((rc = run_ns_steps(*plan, steps, coeffs, per_step, g_opt, stream))) return rc;
   if ((rc = launch_store_ns(T, plan->fp32, stream))) return rc;
   return DMUON_OK;
 }
@@ -208,6 +213,12 @@ DMUON_API int dmuon_set_option(const char* key, const char* value) {
   }
   if (k == "autotune") { if (as_bool(&g_opt.autotune)) return DMUON_OK; set_error("option autotune: bad value '%s'", value); return DMUON_ERR_INVALID_ARG; }
   if (k == "profile") { if (as_bool(&g_opt.profile)) return DMUON_OK; set_error("option profile: bad value '%s'", value); return DMUON_ERR_INVALID_ARG; }
+  if (k == "schedule") {
+    if (v == "auto") g_opt.gram_blocks = true;
+    else if (v == "x") g_opt.gram_blocks = false;
+    else { set_error("option schedule: expected 'auto' or 'x', got '%s'", value); return DMUON_ERR_INVALID_ARG; }
+    return DMUON_OK;
+  }
   if (k == "cache_path") { g_opt.cache_path = v; g_opt.cache_path_set = true; return DMUON_OK; }
   set_error("dmuon_set_option: unknown key '%s'", key);
   return DMUON_ERR_INVALID_ARG;
@@ -294,6 +305,53 @@ DMUON_API int dmuon_warmup(const int32_t* shapes, int32_t count, dmuon_stream_t 
   if (count == 0) return DMUON_OK;
   Plan* plan = nullptr;
   return get_plan(shapes, count, g_opt, g_ext_ws, g_ext_ws_bytes, reinterpret_cast<cudaStream_t>(stream), &plan);
+}
+
+DMUON_API int dmuon_block_schedule(int32_t rows, int32_t cols, int32_t steps, const float* coeffs, int32_t per_step,
+                                   int32_t* out, int32_t cap) {
+  if (rows <= 0 || cols <= 0 || steps < 0 || cap < 0 || (cap > 0 && !out) || (per_step && !coeffs && steps > 0)) {
+    set_error("dmuon_block_schedule: bad arguments");
+    return DMUON_ERR_INVALID_ARG;
+  }
+  const int m = rows < cols ? rows : cols, n = rows < cols ? cols : rows;
+  const int m_pad = (m + kBlk - 1) / kBlk * kBlk, n_pad = (n + kBlk - 1) / kBlk * kBlk;
+  const bool gram = g_opt.gram_blocks && gram_eligible(m_pad, n_pad, g_opt.fp32_check);
+  const Partition part = choose_partition(steps, coeffs ? coeffs : g_opt.coeffs, coeffs && per_step, gram);
+  for (size_t k = 0; k < part.size() && k < static_cast<size_t>(cap); ++k) out[k] = part[k];
+  return static_cast<int>(part.size());
+}
+
+DMUON_API int dmuon_describe_plan(const int32_t* shapes, int32_t count, int32_t steps, char* buf, size_t len,
+                                  dmuon_stream_t stream) {
+  if (count < 0 || steps < 0 || (count > 0 && !shapes)) { set_error("dmuon_describe_plan: bad arguments"); return DMUON_ERR_INVALID_ARG; }
+  for (int i = 0; i < count; ++i)
+    if (shapes[2 * i] <= 0 || shapes[2 * i + 1] <= 0) { set_error("dmuon_describe_plan: bad shape of matrix %d", i); return DMUON_ERR_INVALID_ARG; }
+  std::string s = "{\"buckets\": [";
+  if (count > 0) {
+    Plan* plan = nullptr;
+    int rc = get_plan(shapes, count, g_opt, g_ext_ws, g_ext_ws_bytes, reinterpret_cast<cudaStream_t>(stream), &plan);
+    if (rc) return rc;
+    bool first = true;
+    for (const BucketPlan& b : plan->buckets) {
+      const Partition part = plan->fp32 ? Partition(steps, 1)
+                                        : choose_partition(steps, g_opt.coeffs, false, b.gram && g_opt.gram_blocks);
+      char item[160];
+      snprintf(item, sizeof item, "%s{\"m\": %d, \"n\": %d, \"count\": %d, \"blocks\": [", first ? "" : ", ", b.m_pad,
+               b.n_pad, static_cast<int>(b.mats.size()));
+      s += item;
+      for (size_t k = 0; k < part.size(); ++k) s += (k ? ", " : "") + std::to_string(part[k]);
+      snprintf(item, sizeof item, "], \"variants\": [%d, %d, %d]}", b.variant[0], b.variant[1], b.variant[2]);
+      s += item;
+      first = false;
+    }
+  }
+  s += "]}";
+  if (buf && len > 0) {
+    const size_t n = s.size() < len - 1 ? s.size() : len - 1;
+    memcpy(buf, s.data(), n);
+    buf[n] = 0;
+  }
+  return static_cast<int>(s.size());
 }
 
 DMUON_API size_t dmuon_workspace_bytes(const int32_t* shapes, int32_t count) {
@@ -409,10 +467,64 @@ DMUON_API int dmuon_ns_gemm(int32_t op, const void* const* in0, const void* cons
   L.pair = variant_config(variant < 0 ? 0 : variant).pair;
   L.alpha = alpha;
   L.beta = beta;
+  L.beta2 = 0.f;
   L.grid = sms;
   static const char* kNames[3] = {"ns_syrk_xxt", "ns_sq_poly", "ns_bx_update"};
   ProfScope ps(kNames[op], stream);
   return launch_ns_gemm(L, stream);
+}
+
+DMUON_API int dmuon_ns_sym_mm(const void* const* a, const void* const* b, const void* const* d, const void* const* d2,
+                              void* const* out, int32_t m, int32_t count, float alpha, float beta, float beta2,
+                              int32_t variant, dmuon_stream_t stream_) {
+  cudaStream_t stream = reinterpret_cast<cudaStream_t>(stream_);
+  if (count < 0 || (count > 0 && (!a || !b || !out)) || (d2 && !d)) { set_error("dmuon_ns_sym_mm: null argument"); return DMUON_ERR_INVALID_ARG; }
+  if (m <= 0 || m % kBlk) { set_error("dmuon_ns_sym_mm: m must be a positive multiple of 128 (got %d)", m); return DMUON_ERR_INVALID_ARG; }
+  if (variant < -1 || (variant >= 0 && !variant_valid(OP_SQ, variant))) { set_error("dmuon_ns_sym_mm: variant %d is not defined", variant); return DMUON_ERR_INVALID_ARG; }
+  if (count == 0) return DMUON_OK;
+  int rc = check_device();
+  if (rc) return rc;
+  const GemmOp op = d2 ? OP_SQ2 : d ? OP_SQ : OP_SYRK;
+  std::vector<GemmProblem> probs(count);
+  for (int i = 0; i < count; ++i) {
+    if (!a[i] || !b[i] || !out[i] || (d && !d[i]) || (d2 && !d2[i])) { set_error("dmuon_ns_sym_mm: problem %d has a null pointer", i); return DMUON_ERR_INVALID_ARG; }
+    if ((rc = fill_problem(probs[i], op, a[i], m, m, b[i], m, m, d ? d[i] : nullptr, out[i], m, d2 ? d2[i] : nullptr))) return rc;
+  }
+  const TileConfig cfg = variant_config(variant < 0 ? 0 : variant);
+  std::vector<TileUnit> units = make_units(OP_SQ, m / kBlk, m / kBlk, cfg);
+  GemmProblem* d_probs = nullptr;
+  TileUnit* d_units = nullptr;
+  DMUON_CUDA_CHECK(cudaMalloc(&d_probs, probs.size() * sizeof(GemmProblem)));
+  DMUON_CUDA_CHECK(cudaMalloc(&d_units, units.size() * sizeof(TileUnit)));
+  DMUON_CUDA_CHECK(cudaMemcpy(d_probs, probs.data(), probs.size() * sizeof(GemmProblem), cudaMemcpyHostToDevice));
+  DMUON_CUDA_CHECK(cudaMemcpy(d_units, units.data(), units.size() * sizeof(TileUnit), cudaMemcpyHostToDevice));
+  int dev = 0, sms = 148;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  GemmLaunch L;
+  L.op = op;
+  L.problems = d_probs;
+  L.units = d_units;
+  L.units_per_problem = static_cast<int>(units.size());
+  L.num_problems = count;
+  L.k_blocks = m / kBlkK;
+  L.m_blocks = m / kBlk;
+  L.n_blocks = m / kBlk;
+  L.pair = cfg.pair;
+  L.alpha = alpha;
+  L.beta = beta;
+  L.beta2 = beta2;
+  L.grid = sms;
+  {
+    ProfScope ps("ns_gram_mm", stream);
+    rc = launch_ns_gemm(L, stream);
+  }
+  cudaError_t e = cudaStreamSynchronize(stream);
+  cudaFree(d_probs);
+  cudaFree(d_units);
+  if (rc) return rc;
+  if (e != cudaSuccess) { set_error("dmuon_ns_sym_mm: %s", cudaGetErrorString(e)); return DMUON_ERR_CUDA; }
+  return DMUON_OK;
 }
 
 DMUON_API void dmuon_shutdown(void) {

@@ -32,7 +32,12 @@ void set_error(const char* fmt, ...);
 constexpr int kBlk = 128;     // block edge (UMMA_M)
 constexpr int kBlkK = 64;     // K elements per stage = one 128-byte swizzle row of fp16
 
-enum GemmOp : int { OP_SYRK = 0, OP_SQ = 1, OP_BX = 2 };
+// OP_SYRK  C = alpha A B^T                      (symmetric result: upper blocks computed, mirrored)
+// OP_SQ    C = alpha A B^T + beta D             (symmetric result)
+// OP_BX    C = alpha A B   + beta D             (B operand MN-major; general result)
+// OP_SQ2   C = alpha A B^T + beta D + beta2 D2  (symmetric result; the product of the P_i of a Gram block)
+enum GemmOp : int { OP_SYRK = 0, OP_SQ = 1, OP_BX = 2, OP_SQ2 = 3 };
+constexpr int kNumOps = 4;
 
 // One problem of a grouped launch.  Lives in device memory; the tensor maps are read by the TMA unit.
 struct alignas(128) GemmProblem {
@@ -40,8 +45,9 @@ struct alignas(128) GemmProblem {
   CUtensorMap tmB;      // operand B: K-major box {64, 128} (SYRK, SQ) or MN-major box {64 (n), 64 (k)} (BX)
   const __half* D;      // addend matrix (SQ: A, BX: X), same leading dimension as C; null for SYRK
   __half* C;            // output
-  int32_t ldc;          // leading dimension of C and D, in elements
-  int32_t pad_[27];
+  const __half* D2;     // second addend (SQ2 only)
+  int32_t ldc;          // leading dimension of C, D and D2, in elements
+  int32_t pad_[25];
 };
 static_assert(sizeof(GemmProblem) == 384, "GemmProblem layout");
 
@@ -60,7 +66,7 @@ struct GemmLaunch {
   int k_blocks;                 // K / 64
   int m_blocks, n_blocks;       // extent of the output in 128-blocks
   bool pair;                    // CTA-pair (cta_group::2) tiling
-  float alpha, beta;
+  float alpha, beta, beta2;
   int grid;                     // CTAs (<= #SM)
 };
 int launch_ns_gemm(const GemmLaunch& L, cudaStream_t stream);

@@ -3,6 +3,8 @@
 //   OP_SYRK  C = alpha * X X^T                (PAPER.md:170 G = X X^T; symmetric kernel of PAPER.md:182)
 //   OP_SQ    C = alpha * A A + beta * A       (the polynomial in the Gram matrix; A A = A A^T)
 //   OP_BX    C = alpha * B X + beta * X       (X_{i+1} = P X_i with the a X term in the epilogue)
+//   OP_SQ2   C = alpha * A B + beta * D + beta2 * D2   (symmetric, two addends: the running product of the
+//                                              P_i = a_i I + B_i of a Gram block, Eq. 4)
 //
 // Two tilings of the same warp-specialised pipeline (warp 0 = TMA producer, warp 1 = tcgen05.mma issuer and TMEM
 // owner, warps 2..5 = epilogue: TMEM -> registers -> global):
@@ -60,22 +62,35 @@ template <bool kPair> constexpr int smem_bytes() {
 // One 32-column chunk of one accumulator row: v = 32 fp32 accumulators of row `grow`, columns [gcol, gcol + 32).
 template <int kOp>
 __device__ __forceinline__ void epilogue_chunk(const uint32_t (&v)[32], __half* __restrict__ C,
-                                               const __half* __restrict__ D, int64_t ldc, int64_t grow, int64_t gcol,
-                                               float alpha, float beta, bool mirror) {
+                                               const __half* __restrict__ D, const __half* __restrict__ D2,
+                                               int64_t ldc, int64_t grow, int64_t gcol, float alpha, float beta,
+                                               float beta2, bool mirror) {
   uint32_t o[16];
   if (kOp != OP_SYRK) {
     const uint4* dp = reinterpret_cast<const uint4*>(D + grow * ldc + gcol);
-    uint4 d4[4];
+    uint4 d4[4], e4[4] = {};
 #pragma unroll
     for (int g = 0; g < 4; ++g) d4[g] = __ldg(dp + g);
+    if (kOp == OP_SQ2) {
+      const uint4* ep = reinterpret_cast<const uint4*>(D2 + grow * ldc + gcol);
+#pragma unroll
+      for (int g = 0; g < 4; ++g) e4[g] = __ldg(ep + g);
+    }
 #pragma unroll
     for (int g = 0; g < 4; ++g) {
       const uint32_t dw[4] = {d4[g].x, d4[g].y, d4[g].z, d4[g].w};
+      const uint32_t ew[4] = {e4[g].x, e4[g].y, e4[g].z, e4[g].w};
 #pragma unroll
       for (int e = 0; e < 4; ++e) {
         const float2 df = __half22float2(*reinterpret_cast<const __half2*>(&dw[e]));
-        const float lo = fmaf(alpha, __uint_as_float(v[g * 8 + e * 2]), beta * df.x);
-        const float hi = fmaf(alpha, __uint_as_float(v[g * 8 + e * 2 + 1]), beta * df.y);
+        float ax = beta * df.x, ay = beta * df.y;
+        if (kOp == OP_SQ2) {
+          const float2 ef = __half22float2(*reinterpret_cast<const __half2*>(&ew[e]));
+          ax = fmaf(beta2, ef.x, ax);
+          ay = fmaf(beta2, ef.y, ay);
+        }
+        const float lo = fmaf(alpha, __uint_as_float(v[g * 8 + e * 2]), ax);
+        const float hi = fmaf(alpha, __uint_as_float(v[g * 8 + e * 2 + 1]), ay);
         o[g * 4 + e] = pack_half2(lo, hi);
       }
     }
@@ -105,7 +120,7 @@ __device__ __forceinline__ void epilogue_chunk(const uint32_t (&v)[32], __half* 
 template <int kOp, bool kPair>
 __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ probs, const TileUnit* __restrict__ units,
                                              int units_per_problem, int total_units, int k_blocks, int mb, int nb,
-                                             float alpha, float beta) {
+                                             float alpha, float beta, float beta2) {
   constexpr bool kSym = (kOp != OP_BX);
   constexpr bool kBMn = (kOp == OP_BX);
   constexpr int kCG = kPair ? 2 : 1;
@@ -237,6 +252,7 @@ __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ pro
       const GemmProblem* pr = probs + p;
       __half* __restrict__ C = pr->C;
       const __half* __restrict__ D = pr->D;
+      const __half* __restrict__ D2 = pr->D2;
       const int64_t ldc = pr->ldc;
       const int as = it & 1;
       const uint32_t aphase = (it >> 1) & 1;
@@ -254,7 +270,7 @@ __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ pro
           uint32_t v[32];
           tmem_ld_32x32(taddr + c * 32, v);
           tmem_wait_ld();
-          epilogue_chunk<kOp>(v, C, D, ldc, grow, static_cast<int64_t>(bj0) * kBlk + c * 32, alpha, beta, bj != bi);
+          epilogue_chunk<kOp>(v, C, D, D2, ldc, grow, static_cast<int64_t>(bj0) * kBlk + c * 32, alpha, beta, beta2, bj != bi);
         }
       }
       // accumulator fully read by this warp: hand it back to the MMA thread
@@ -275,8 +291,8 @@ __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ pro
 #define DMUON_GEMM_ENTRY(name, op, pair)                                                                        \
   __global__ void __launch_bounds__(kNumThreads, 1)                                                             \
   name(const GemmProblem* __restrict__ probs, const TileUnit* __restrict__ units, int units_per_problem,       \
-       int total_units, int k_blocks, int mb, int nb, float alpha, float beta) {                                \
-    ns_gemm_body<op, pair>(probs, units, units_per_problem, total_units, k_blocks, mb, nb, alpha, beta);        \
+       int total_units, int k_blocks, int mb, int nb, float alpha, float beta, float beta2) {                   \
+    ns_gemm_body<op, pair>(probs, units, units_per_problem, total_units, k_blocks, mb, nb, alpha, beta, beta2); \
   }
 DMUON_GEMM_ENTRY(ns_syrk_xxt_kernel, OP_SYRK, false)
 DMUON_GEMM_ENTRY(ns_sq_poly_kernel, OP_SQ, false)
@@ -284,9 +300,11 @@ DMUON_GEMM_ENTRY(ns_bx_update_kernel, OP_BX, false)
 DMUON_GEMM_ENTRY(ns_syrk_xxt_pair_kernel, OP_SYRK, true)
 DMUON_GEMM_ENTRY(ns_sq_poly_pair_kernel, OP_SQ, true)
 DMUON_GEMM_ENTRY(ns_bx_update_pair_kernel, OP_BX, true)
+DMUON_GEMM_ENTRY(ns_gram_acc_kernel, OP_SQ2, false)
+DMUON_GEMM_ENTRY(ns_gram_acc_pair_kernel, OP_SQ2, true)
 #undef DMUON_GEMM_ENTRY
 
-typedef void (*GemmKernel)(const GemmProblem*, const TileUnit*, int, int, int, int, int, float, float);
+typedef void (*GemmKernel)(const GemmProblem*, const TileUnit*, int, int, int, int, int, float, float, float);
 
 template <bool kPair>
 int launch_op(GemmKernel kern, bool* configured, const GemmLaunch& L, cudaStream_t stream) {
@@ -312,7 +330,7 @@ int launch_op(GemmKernel kern, bool* configured, const GemmLaunch& L, cudaStream
   cfg.attrs = attr;
   cfg.numAttrs = 1;
   DMUON_CUDA_CHECK(cudaLaunchKernelEx(&cfg, kern, L.problems, L.units, L.units_per_problem, total, L.k_blocks,
-                                      L.m_blocks, L.n_blocks, L.alpha, L.beta));
+                                      L.m_blocks, L.n_blocks, L.alpha, L.beta, L.beta2));
   return DMUON_OK;
 }
 
@@ -321,14 +339,15 @@ int launch_op(GemmKernel kern, bool* configured, const GemmLaunch& L, cudaStream
 int gemm_smem_bytes() { return smem_bytes<false>() > smem_bytes<true>() ? smem_bytes<false>() : smem_bytes<true>(); }
 
 int launch_ns_gemm(const GemmLaunch& L, cudaStream_t stream) {
-  static bool configured[6] = {false, false, false, false, false, false};
-  if (L.op < OP_SYRK || L.op > OP_BX) {
+  static bool configured[2 * kNumOps] = {};
+  if (L.op < OP_SYRK || L.op >= kNumOps) {
     set_error("launch_ns_gemm: bad op %d", static_cast<int>(L.op));
     return DMUON_ERR_INVALID_ARG;
   }
-  static const GemmKernel kSingle[3] = {ns_syrk_xxt_kernel, ns_sq_poly_kernel, ns_bx_update_kernel};
-  static const GemmKernel kPairK[3] = {ns_syrk_xxt_pair_kernel, ns_sq_poly_pair_kernel, ns_bx_update_pair_kernel};
-  if (L.pair) return launch_op<true>(kPairK[L.op], &configured[3 + L.op], L, stream);
+  static const GemmKernel kSingle[kNumOps] = {ns_syrk_xxt_kernel, ns_sq_poly_kernel, ns_bx_update_kernel, ns_gram_acc_kernel};
+  static const GemmKernel kPairK[kNumOps] = {ns_syrk_xxt_pair_kernel, ns_sq_poly_pair_kernel, ns_bx_update_pair_kernel,
+                                             ns_gram_acc_pair_kernel};
+  if (L.pair) return launch_op<true>(kPairK[L.op], &configured[kNumOps + L.op], L, stream);
   return launch_op<false>(kSingle[L.op], &configured[L.op], L, stream);
 }
 

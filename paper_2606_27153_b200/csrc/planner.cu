@@ -13,6 +13,10 @@
 
 namespace dmuon {
 
+// Gram blocks replace 2 (L - 1) of the m x n products of L steps by 4 (L - 1) m x m products: worth it when the matrix
+// is wide.  Tiny Gram matrices (one block) stay on the plain iteration (latency-bound either way).
+bool gram_eligible(int m_pad, int n_pad, bool fp32) { return !fp32 && m_pad >= 2 * kBlk && 2 * n_pad >= 3 * m_pad; }
+
 namespace {
 
 std::vector<std::unique_ptr<Plan>> g_plans;
@@ -78,10 +82,13 @@ void describe(const int32_t* shapes, int count, std::vector<MatrixInfo>& mats, s
     mi.bucket = -1;
     const size_t xb = align_up(static_cast<size_t>(mi.m_pad) * mi.n_pad * es, 1024);
     const size_t ab = align_up(static_cast<size_t>(mi.m_pad) * mi.m_pad * es, 1024);
+    mi.gram = gram_eligible(mi.m_pad, mi.n_pad, es == 4);
     mi.off_p = off; off += xb;
     mi.off_q = off; off += xb;
-    mi.off_a = off; off += ab;
-    mi.off_b = off; off += ab;
+    for (int k = 0; k < 5; ++k) {
+      mi.off_sq[k] = off;
+      if (k < 2 || mi.gram) off += ab;
+    }
   }
   *ws_bytes = off;
 }
@@ -125,15 +132,18 @@ void save_tune_cache(const std::string& path) {
   for (auto& kv : g_tune_cache) out << "v1 " << kv.first << " " << kv.second << "\n";
 }
 
-int bucket_launch(const Plan& plan, const BucketPlan& b, GemmOp op, int parity, float alpha, float beta,
-                  cudaStream_t stream, const TileUnit* units_override = nullptr, int upp_override = 0,
+inline int tiling_op(GemmOp op) { return op == OP_SQ2 ? OP_SQ : op; }   // SQ2 shares SQ's units and variant
+
+int bucket_launch(const Plan& plan, const BucketPlan& b, GemmOp op, const GemmProblem* probs, float alpha, float beta,
+                  float beta2, cudaStream_t stream, const TileUnit* units_override = nullptr, int upp_override = 0,
                   int variant_override = -1) {
-  const bool pair = variant_config(variant_override >= 0 ? variant_override : b.variant[op]).pair;
+  const int top = tiling_op(op);
+  const bool pair = variant_config(variant_override >= 0 ? variant_override : b.variant[top]).pair;
   GemmLaunch L;
   L.op = op;
-  L.problems = op == OP_SYRK ? b.syrk[parity] : op == OP_SQ ? b.sq : b.bx[parity];
-  L.units = units_override ? units_override : b.units[op];
-  L.units_per_problem = units_override ? upp_override : b.units_per_problem[op];
+  L.problems = probs;
+  L.units = units_override ? units_override : b.units[top];
+  L.units_per_problem = units_override ? upp_override : b.units_per_problem[top];
   L.num_problems = static_cast<int>(b.mats.size());
   L.k_blocks = (op == OP_SYRK ? b.n_pad : b.m_pad) / kBlkK;
   L.m_blocks = b.m_pad / kBlk;
@@ -141,6 +151,7 @@ int bucket_launch(const Plan& plan, const BucketPlan& b, GemmOp op, int parity, 
   L.pair = pair;
   L.alpha = alpha;
   L.beta = beta;
+  L.beta2 = beta2;
   L.grid = plan.sm_count;
   return launch_ns_gemm(L, stream);
 }
@@ -173,7 +184,7 @@ int autotune_bucket(Plan& plan, BucketPlan& b, const Options& opt, cudaStream_t 
         float ms = 1e30f;
         for (int rep = 0; rep < 3 && rc == DMUON_OK; ++rep) {   // rep 0 warms up
           cudaEventRecord(e0, stream);
-          rc = bucket_launch(plan, b, static_cast<GemmOp>(op), 0, 1.f, 0.f, stream, du, static_cast<int>(hu.size()), v);
+          rc = bucket_launch(plan, b, static_cast<GemmOp>(op), b.tune_probs[op], 1.f, 0.f, 0.f, stream, du, static_cast<int>(hu.size()), v);
           cudaEventRecord(e1, stream);
           if (cudaEventSynchronize(e1) != cudaSuccess) rc = DMUON_ERR_CUDA;
           float t = 0.f;
@@ -198,7 +209,7 @@ int autotune_bucket(Plan& plan, BucketPlan& b, const Options& opt, cudaStream_t 
 }  // namespace
 
 int fill_problem(GemmProblem& g, GemmOp op, const void* a_mat, uint64_t a_rows, uint64_t a_cols, const void* b_mat,
-                 uint64_t b_rows, uint64_t b_cols, const void* d, void* c, int ldc) {
+                 uint64_t b_rows, uint64_t b_cols, const void* d, void* c, int ldc, const void* d2) {
   memset(&g, 0, sizeof g);
   int rc = encode_tmap_2d(&g.tmA, a_mat, a_rows, a_cols, kBlkK, kBlk);
   if (rc) return rc;
@@ -207,6 +218,7 @@ int fill_problem(GemmProblem& g, GemmOp op, const void* a_mat, uint64_t a_rows, 
   if (rc) return rc;
   g.D = static_cast<const __half*>(d);
   g.C = static_cast<__half*>(c);
+  g.D2 = static_cast<const __half*>(d2);
   g.ldc = ldc;
   return DMUON_OK;
 }
@@ -401,29 +413,27 @@ int get_plan(const int32_t* shapes, int count, const Options& opt, void* ext_ws,
   p.tables.partials = p.d_partials;
   p.tables.inv_norm = p.d_inv_norm;
 
-  // ---- grouped GEMM tables (tensor-core mode only)
+  // ---- grouped GEMM tables (tensor-core mode only): scratch problems for the autotuner, tile units per op.  The
+  //      launch programs of the NS steps are built on first use (build_program), they depend on the step count.
   if (!p.fp32) {
     for (BucketPlan& b : p.buckets) {
       const size_t nprob = b.mats.size();
-      std::vector<GemmProblem> syrk[2], sq(nprob), bx[2];
-      for (int s = 0; s < 2; ++s) { syrk[s].resize(nprob); bx[s].resize(nprob); }
+      b.gram = p.mats[b.mats[0]].gram;
+      std::vector<GemmProblem> tp[3];
+      for (int op = 0; op < 3; ++op) tp[op].resize(nprob);
       for (size_t k = 0; k < nprob; ++k) {
         const MatrixInfo& mi = p.mats[b.mats[k]];
-        void* X[2] = {p.ws + mi.off_q, p.ws + mi.off_p};     // parity 0: X in Q, parity 1: X in P
-        void* A = p.ws + mi.off_a;
-        void* B = p.ws + mi.off_b;
+        void* XQ = p.ws + mi.off_q;
+        void* XP = p.ws + mi.off_p;
+        void* A = p.ws + mi.off_sq[0];
+        void* B = p.ws + mi.off_sq[1];
         const uint64_t m = mi.m_pad, n = mi.n_pad;
-        for (int s = 0; s < 2; ++s) {
-          if ((rc = fill_problem(syrk[s][k], OP_SYRK, X[s], m, n, X[s], m, n, nullptr, A, mi.m_pad))) return rc;
-          if ((rc = fill_problem(bx[s][k], OP_BX, B, m, m, X[s], m, n, X[s], X[1 - s], mi.n_pad))) return rc;
-        }
-        if ((rc = fill_problem(sq[k], OP_SQ, A, m, m, A, m, m, A, B, mi.m_pad))) return rc;
+        if ((rc = fill_problem(tp[OP_SYRK][k], OP_SYRK, XQ, m, n, XQ, m, n, nullptr, A, mi.m_pad))) return rc;
+        if ((rc = fill_problem(tp[OP_SQ][k], OP_SQ, A, m, m, A, m, m, A, B, mi.m_pad))) return rc;
+        if ((rc = fill_problem(tp[OP_BX][k], OP_BX, B, m, m, XQ, m, n, XQ, XP, mi.n_pad))) return rc;
       }
-      for (int s = 0; s < 2; ++s) {
-        if ((rc = upload(p, &b.syrk[s], syrk[s]))) return rc;
-        if ((rc = upload(p, &b.bx[s], bx[s]))) return rc;
-      }
-      if ((rc = upload(p, &b.sq, sq))) return rc;
+      for (int op = 0; op < 3; ++op)
+        if ((rc = upload(p, &b.tune_probs[op], tp[op]))) return rc;
       // tile configuration: tuned (cache or measurement) or default variant 0
       if ((rc = autotune_bucket(p, b, opt, stream))) return rc;
       for (int op = 0; op < 3; ++op) {
@@ -439,24 +449,155 @@ int get_plan(const int32_t* shapes, int count, const Options& opt, void* ext_ws,
   return DMUON_OK;
 }
 
-int run_ns_steps(Plan& plan, int steps, const float* coeffs, bool per_step, cudaStream_t stream) {
-  static const char* kNames[3] = {"ns_syrk_xxt", "ns_sq_poly", "ns_bx_update"};
+std::string partition_key(const Partition& part) {
+  std::string k;
+  for (int L : part) k += static_cast<char>('0' + L);
+  return k;
+}
+
+// Block lengths for `steps` NS steps.  A 3-block is taken only as the FIRST block: there ||X||_F = 1 bounds ||G||, so
+// the fp16 rounding of G is small in absolute terms; later blocks are 2-blocks (measured).
+// A block is shortened until the error gain of its Gram recurrence, prod a_j^2 over all but its last step, is <= 200
+// (the default a = 3.4445 gives 11.9 for a 2-block and 140.8 for a 3-block).
+Partition choose_partition(int steps, const float* coeffs, bool per_step, bool gram) {
+  Partition part;
+  int s = 0;
+  while (s < steps) {
+    const int rem = steps - s;
+    int L = 1;
+    if (gram) {
+      L = (part.empty() && rem >= 3 && rem != 4) ? 3 : (rem >= 2 ? 2 : 1);
+      while (L > 1) {
+        double gain = 1.0;
+        for (int j = s; j < s + L - 1; ++j) {
+          const double a = coeffs[per_step ? 3 * j : 0];
+          gain *= a * a;
+        }
+        if (gain <= 200.0) break;   // also false for NaN
+        --L;
+      }
+    }
+    part.push_back(L);
+    s += L;
+  }
+  return part;
+}
+
+int result_parity(const Plan& plan, const BucketPlan& b, int steps, const float* coeffs, bool per_step, const Options& opt) {
+  if (plan.fp32) return steps & 1;
+  return static_cast<int>(choose_partition(steps, coeffs, per_step, b.gram && opt.gram_blocks).size()) & 1;
+}
+
+namespace {
+
+// Build the launch list of one bucket for a partition of the steps into blocks.  m x m buffers: 0 = G, 1/2 = B and B'
+// (alternating), 3 = T, 4 = R.
+int build_program(Plan& p, BucketPlan& b, const Partition& part, NsProgram& prog) {
+  const size_t nprob = b.mats.size();
+  const int kb_n = b.n_pad / kBlkK, kb_m = b.m_pad / kBlkK, nb_m = b.m_pad / kBlk, nb_n = b.n_pad / kBlk;
+  int rc;
+  auto emit = [&](GemmOp op, CoefKind ck, int s0, int s1, const char* name, int a_buf, int b_buf, int d_buf, int d2_buf,
+                  int c_buf, int xsrc) -> int {
+    // buffer ids: 0..4 = m x m buffers; 10 / 11 = X in Q / P
+    std::vector<GemmProblem> hp(nprob);
+    for (size_t k = 0; k < nprob; ++k) {
+      const MatrixInfo& mi = p.mats[b.mats[k]];
+      auto buf = [&](int id) -> void* {
+        if (id < 0) return nullptr;
+        if (id >= 10) return p.ws + (id == 10 ? mi.off_q : mi.off_p);
+        return p.ws + mi.off_sq[id];
+      };
+      const uint64_t m = mi.m_pad, n = mi.n_pad;
+      if (op == OP_SYRK) rc = fill_problem(hp[k], op, buf(xsrc), m, n, buf(xsrc), m, n, nullptr, buf(c_buf), mi.m_pad);
+      else if (op == OP_BX) rc = fill_problem(hp[k], op, buf(a_buf), m, m, buf(xsrc), m, n, buf(xsrc), buf(c_buf), mi.n_pad);
+      else rc = fill_problem(hp[k], op, buf(a_buf), m, m, buf(b_buf), m, m, buf(d_buf), buf(c_buf), mi.m_pad, buf(d2_buf));
+      if (rc) return rc;
+    }
+    NsLaunch L;
+    L.op = op; L.ck = ck; L.s0 = s0; L.s1 = s1; L.name = name;
+    L.k_blocks = op == OP_SYRK ? kb_n : kb_m;
+    L.n_blocks = op == OP_BX ? nb_n : nb_m;
+    if ((rc = upload(p, &L.probs, hp))) return rc;
+    prog.launches.push_back(L);
+    return DMUON_OK;
+  };
+  int s = 0, par = 0;   // X0 is in Q (parity 0)
+  for (int L : part) {
+    if (L > 1 && !b.gram) { set_error("internal: Gram block on a bucket without Gram buffers"); return DMUON_ERR_INVALID_ARG; }
+    if (L > 3) { set_error("internal: Gram block longer than 3"); return DMUON_ERR_INVALID_ARG; }
+    const int xs = 10 + par, xd = 10 + (1 - par);
+    int g = 0, bc = 1, bn = 2, t = 3, r = 1;     // R_0 = B_0 (alias)
+    if ((rc = emit(OP_SYRK, CK_ONE, s, s, "ns_syrk_xxt", -1, -1, -1, -1, g, xs))) return rc;            // G = X X^T
+    if ((rc = emit(OP_SQ, CK_POLY, s, s, "ns_sq_poly", g, g, g, -1, bc, -1))) return rc;                // B = b G + c G G
+    for (int i = 1; i < L; ++i) {
+      const int st = s + i;
+      if ((rc = emit(OP_SQ, CK_A, st - 1, st - 1, "ns_gram_mm", bc, g, g, -1, t, -1))) return rc;       // T = a G + B G
+      if ((rc = emit(OP_SQ, CK_A, st - 1, st - 1, "ns_gram_mm", t, bc, t, -1, g, -1))) return rc;       // G' = a T + T B
+      if ((rc = emit(OP_SQ, CK_POLY, st, st, "ns_sq_poly", g, g, g, -1, bn, -1))) return rc;            // B' = b G' + c G' G'
+      const int rn = (i == 1) ? 4 : t;            // free buffer: R (i = 1), then T (not needed after G')
+      if ((rc = emit(OP_SQ2, CK_RACC, s, st, "ns_gram_mm", bn, r, bn, r, rn, -1))) return rc;            // R' = (prod a) B' + a R + B' R
+      r = rn;
+      const int tmp = bc; bc = bn; bn = tmp;
+    }
+    if ((rc = emit(OP_BX, CK_APOW, s, s + L - 1, "ns_bx_update", r, -1, -1, -1, xd, xs))) return rc;     // X' = (prod a) X + R X
+    s += L;
+    par ^= 1;
+    ++prog.x_updates;
+  }
+  return DMUON_OK;
+}
+
+void launch_coefs(const NsLaunch& L, const float* coeffs, bool per_step, float* alpha, float* beta, float* beta2) {
+  auto co = [&](int step, int which) { return coeffs[(per_step ? 3 * step : 0) + which]; };
+  *alpha = 1.f; *beta = 0.f; *beta2 = 0.f;
+  double prod = 1.0;
+  switch (L.ck) {
+    case CK_ONE: break;
+    case CK_POLY: *alpha = co(L.s1, 2); *beta = co(L.s1, 1); break;
+    case CK_A: *beta = co(L.s1, 0); break;
+    case CK_RACC:
+      for (int j = L.s0; j < L.s1; ++j) prod *= co(j, 0);
+      *beta = static_cast<float>(prod);
+      *beta2 = co(L.s1, 0);
+      break;
+    case CK_APOW:
+      for (int j = L.s0; j <= L.s1; ++j) prod *= co(j, 0);
+      *beta = static_cast<float>(prod);
+      break;
+  }
+}
+
+}  // namespace
+
+int run_ns_steps(Plan& plan, int steps, const float* coeffs, bool per_step, const Options& opt, cudaStream_t stream) {
   for (BucketPlan& b : plan.buckets) {
-    for (int s = 0; s < steps; ++s) {
-      const float* q = coeffs + (per_step ? 3 * s : 0);
-      const float a = q[0], bb = q[1], c = q[2];
-      const int parity = s & 1;                 // step 0 reads Q (parity 0) and writes P
-      if (!plan.fp32) {
-        int rc;
-        { ProfScope ps(kNames[0], stream); if ((rc = bucket_launch(plan, b, OP_SYRK, parity, 1.f, 0.f, stream))) return rc; }
-        { ProfScope ps(kNames[1], stream); if ((rc = bucket_launch(plan, b, OP_SQ, 0, c, bb, stream))) return rc; }
-        { ProfScope ps(kNames[2], stream); if ((rc = bucket_launch(plan, b, OP_BX, parity, 1.f, a, stream))) return rc; }
-      } else {
+    if (!plan.fp32) {
+      const Partition part = choose_partition(steps, coeffs, per_step, b.gram && opt.gram_blocks);
+      const std::string key = partition_key(part);
+      auto it = b.programs.find(key);
+      if (it == b.programs.end()) {
+        NsProgram prog;
+        int rc = build_program(plan, b, part, prog);
+        if (rc) return rc;
+        it = b.programs.emplace(key, std::move(prog)).first;
+      }
+      for (const NsLaunch& L : it->second.launches) {
+        float alpha, beta, beta2;
+        launch_coefs(L, coeffs, per_step, &alpha, &beta, &beta2);
+        ProfScope ps(L.name, stream);
+        int rc = bucket_launch(plan, b, L.op, L.probs, alpha, beta, beta2, stream);
+        if (rc) return rc;
+      }
+    } else {
+      for (int s = 0; s < steps; ++s) {
+        const float* q = coeffs + (per_step ? 3 * s : 0);
+        const float a = q[0], bb = q[1], c = q[2];
+        const int parity = s & 1;                 // step 0 reads Q (parity 0) and writes P
         for (int idx : b.mats) {
           const MatrixInfo& mi = plan.mats[idx];
           float* X[2] = {reinterpret_cast<float*>(plan.ws + mi.off_q), reinterpret_cast<float*>(plan.ws + mi.off_p)};
-          float* A = reinterpret_cast<float*>(plan.ws + mi.off_a);
-          float* B = reinterpret_cast<float*>(plan.ws + mi.off_b);
+          float* A = reinterpret_cast<float*>(plan.ws + mi.off_sq[0]);
+          float* B = reinterpret_cast<float*>(plan.ws + mi.off_sq[1]);
           int rc;
           if ((rc = launch_check_gemm(OP_SYRK, X[parity], nullptr, A, mi.m_pad, mi.n_pad, 1.f, 0.f, stream))) return rc;
           if ((rc = launch_check_gemm(OP_SQ, A, nullptr, B, mi.m_pad, mi.m_pad, c, bb, stream))) return rc;

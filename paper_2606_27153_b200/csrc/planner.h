@@ -20,6 +20,7 @@ struct Options {
   std::string cache_path;       // resolved lazily
   bool cache_path_set = false;
   float eps = 1e-7f;
+  bool gram_blocks = true;      // schedule "auto": Gram blocks (Eq. 4) on wide buckets; false = plain X iteration
 };
 
 struct MatrixInfo {
@@ -28,7 +29,9 @@ struct MatrixInfo {
   int m_pad, n_pad;      // padded to multiples of 128
   bool transposed;
   int bucket;
-  size_t off_p, off_q, off_a, off_b;   // byte offsets into the workspace
+  size_t off_p, off_q;   // byte offsets into the workspace: the two m_pad x n_pad X buffers
+  size_t off_sq[5];      // m_pad x m_pad buffers: G, B, and (Gram-block buckets only) B', T, R
+  bool gram;             // bucket eligible for Gram blocks (wide enough that they save work)
 };
 
 // Tile configuration of one op of one bucket ("variant" of dmuon_ns_gemm).
@@ -43,16 +46,46 @@ constexpr int kNumVariants = 6;
 bool variant_valid(GemmOp op, int variant);
 TileConfig variant_config(int variant);
 
+// How the k NS steps of a bucket are executed: a list of blocks whose lengths sum to k.  A block of length 1 is the
+// plain step X <- (a I + B) X.  A block of length L > 1 forms G once from X, advances it in the m x m Gram space
+// (G_{i+1} = P_i G_i P_i, Eq. 4), accumulates Q = P_{s+L-1} ... P_s and touches X once: X <- Q X.
+// Blocks are restarts: G is always recomputed from X at the start of a block, which is what keeps fp16 storage stable
+// (DESIGN.md section 6).
+typedef std::vector<int> Partition;
+Partition choose_partition(int steps, const float* coeffs, bool per_step, bool gram);
+bool gram_eligible(int m_pad, int n_pad, bool fp32);
+
+// How a launch's (alpha, beta, beta2) follow from the per-step coefficients (a_i, b_i, c_i).
+enum CoefKind : int {
+  CK_ONE = 0,    // alpha = 1                                            SYRK: G = X X^T
+  CK_POLY,       // alpha = c_s1, beta = b_s1                            B = b G + c G G
+  CK_A,          // alpha = 1, beta = a_s1                               T = a G + B G ; G' = a T + T B
+  CK_RACC,       // alpha = 1, beta = prod a_[s0, s1), beta2 = a_s1      R' = (prod a) B' + a R + B' R
+  CK_APOW        // alpha = 1, beta = prod a_[s0, s1]                    X' = (prod a) X + R X
+};
+struct NsLaunch {
+  GemmOp op;
+  CoefKind ck;
+  int s0, s1;                  // step indices the coefficients come from
+  GemmProblem* probs;          // device, one per matrix of the bucket
+  int k_blocks, n_blocks;
+  const char* name;            // profiling family
+};
+struct NsProgram {
+  std::vector<NsLaunch> launches;
+  int x_updates = 0;           // how many times X switched buffers (result parity)
+};
+
 struct BucketPlan {
   int m_pad = 0, n_pad = 0;
+  bool gram = false;
   std::vector<int> mats;               // matrix indices
-  // device tables
-  GemmProblem* syrk[2] = {nullptr, nullptr};   // [src parity]: 0 = X in Q, 1 = X in P
-  GemmProblem* sq = nullptr;
-  GemmProblem* bx[2] = {nullptr, nullptr};     // [src parity]: 0 = Q -> P, 1 = P -> Q
-  TileUnit* units[3] = {nullptr, nullptr, nullptr};   // per op
+  std::map<std::string, NsProgram> programs;   // by partition signature, e.g. "32"
+  TileUnit* units[3] = {nullptr, nullptr, nullptr};   // per tiling op (SYRK, SQ / SQ2, BX)
   int units_per_problem[3] = {0, 0, 0};
   int variant[3] = {0, 0, 0};
+  // scratch problem tables for the autotuner
+  GemmProblem* tune_probs[3] = {nullptr, nullptr, nullptr};
 };
 
 struct Plan {
@@ -69,7 +102,7 @@ struct Plan {
   int64_t *d_flat_prefix = nullptr, *d_tile_prefix = nullptr, *d_ptile_prefix = nullptr;
   float *d_partials = nullptr, *d_inv_norm = nullptr;
   ElemTables tables{};
-  int o_parity = -1;                   // which buffer rec.O points at (steps & 1), -1 = unset
+  std::string bound_key;               // schedule signature rec.O was last bound for
   // staging for the _host entry point
   uint8_t* stage = nullptr;            // W | G | M device copies
   std::vector<size_t> stage_off;       // per matrix offset of W; G at +stage_third, M at +2*stage_third
@@ -85,15 +118,18 @@ int get_plan(const int32_t* shapes, int count, const Options& opt, void* ext_ws,
              Plan** out);
 void drop_plans();
 
-// Enqueue k NS steps over every bucket of the plan; X0 is in buffer Q; result ends in P if steps is odd, else Q.
-int run_ns_steps(Plan& plan, int steps, const float* coeffs, bool per_step, cudaStream_t stream);
+// Enqueue k NS steps over every bucket of the plan; X0 is in buffer Q.  result_parity(...) tells where a bucket's
+// result ends (0 = Q, 1 = P) for the same arguments.
+int run_ns_steps(Plan& plan, int steps, const float* coeffs, bool per_step, const Options& opt, cudaStream_t stream);
+int result_parity(const Plan& plan, const BucketPlan& b, int steps, const float* coeffs, bool per_step, const Options& opt);
+std::string partition_key(const Partition& p);
 
 // Build tile units for an op.
 std::vector<TileUnit> make_units(GemmOp op, int m_blocks, int n_blocks, const TileConfig& cfg);
 int encode_tmap_2d(CUtensorMap* out, const void* base, uint64_t rows, uint64_t cols, uint32_t box_cols,
                    uint32_t box_rows);
 int fill_problem(GemmProblem& g, GemmOp op, const void* a_mat, uint64_t a_rows, uint64_t a_cols, const void* b_mat,
-                 uint64_t b_rows, uint64_t b_cols, const void* d, void* c, int ldc);
+                 uint64_t b_rows, uint64_t b_cols, const void* d, void* c, int ldc, const void* d2 = nullptr);
 int check_device();
 
 }  // namespace dmuon

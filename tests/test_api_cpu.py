@@ -35,7 +35,7 @@ def test_options_validation():
     dm.set_option("autotune", "1")
     dm.set_option("profile", "0")
     for key, val in (("steps", "-1"), ("steps", "abc"), ("coeffs", "1,2"), ("mode", "bogus"), ("nope", "1"),
-                     ("autotune", "maybe")):
+                     ("autotune", "maybe"), ("schedule", "gram")):
         with pytest.raises(dm.DmuonError) as ei:
             dm.set_option(key, val)
         assert ei.value.code == binding.ERR_INVALID_ARG
@@ -77,17 +77,51 @@ def test_no_cpu_fallback():
 
 def test_workspace_bytes_formula():
     dm.set_option("mode", "tc")
-    # one 4096 x 14336 matrix: two X buffers + A + B in fp16
-    want = 2 * 4096 * 14336 * 2 + 2 * 4096 * 4096 * 2
+    # one 4096 x 14336 matrix: two X buffers + five m x m buffers (G, B, B', T, R of the Gram blocks) in fp16
+    want = 2 * 4096 * 14336 * 2 + 5 * 4096 * 4096 * 2
     assert dm.workspace_bytes([(4096, 14336)]) == want
     assert dm.workspace_bytes([(14336, 4096)]) == want                # tall: same oriented shape
+    # square: plain iteration, two X buffers + A + B
+    assert dm.workspace_bytes([(4096, 4096)]) == 4 * 4096 * 4096 * 2
     # ragged: padded to multiples of 128
     assert dm.workspace_bytes([(100, 260)]) == 2 * 128 * 384 * 2 + 2 * 128 * 128 * 2
     assert dm.workspace_bytes([]) == 0
     assert dm.workspace_bytes([(0, 5)]) == 0
     dm.set_option("mode", "fp32_check")
-    assert dm.workspace_bytes([(4096, 14336)]) == 2 * want
+    assert dm.workspace_bytes([(4096, 14336)]) == 2 * (2 * 4096 * 14336 * 2 + 2 * 4096 * 4096 * 2)
     dm.set_option("mode", "tc")
+
+
+def test_block_schedule_host_logic():
+    """Gram blocks (Eq. 4, PAPER.md:172) only on wide buckets; a 3-block only first; lengths sum to the step count;
+    blocks shrink when the recurrence's error gain prod a^2 exceeds 200."""
+    dm.set_option("mode", "tc")
+    dm.set_option("schedule", "auto")
+    for shape in ((4096, 14336), (14336, 4096), (1024, 4096), (768, 3072), (896, 4864), (2048, 3072)):
+        assert dm.block_schedule(shape, 5) == [3, 2]
+        for k in range(0, 12):
+            part = dm.block_schedule(shape, k)
+            assert sum(part) == k and all(1 <= L <= 3 for L in part)
+            assert all(L <= 2 for L in part[1:]), "a 3-block may only come first"
+        assert dm.block_schedule(shape, 4) == [2, 2]
+    for shape in ((4096, 4096), (896, 896), (128, 896), (128, 512), (1000, 1400), (1, 64), (37, 91)):
+        assert dm.block_schedule(shape, 5) == [1] * 5              # square-ish or a single-block Gram matrix
+    # large a: shorter blocks.  a = 4: a^4 = 256 > 200 forbids the 3-block; a = 15: a^2 = 225 forbids any block
+    assert dm.block_schedule((1024, 4096), 5, (4.0, -5.0, 2.0)) == [2, 2, 1]
+    assert dm.block_schedule((1024, 4096), 5, (15.0, -5.0, 2.0)) == [1] * 5
+    sched = [(8.0, -20.0, 14.0), (4.0, -3.0, 0.5), (3.9, -2.9, 0.5), (3.3, -2.4, 0.4), (2.3, -1.7, 0.4)]
+    assert dm.block_schedule((1024, 4096), 5, sched) == [2, 2, 1]  # 64 * 16 > 200 -> 2-block; then 3.9^2 -> 2-block
+    dm.set_option("schedule", "x")
+    assert dm.block_schedule((1024, 4096), 5) == [1] * 5
+    dm.set_option("schedule", "auto")
+    dm.set_option("mode", "fp32_check")
+    assert dm.block_schedule((1024, 4096), 5) == [1] * 5           # the check mode is always the plain iteration
+    dm.set_option("mode", "tc")
+    L = binding.lib()
+    out = (ctypes.c_int32 * 4)()
+    assert L.dmuon_block_schedule(0, 5, 5, None, 0, out, 4) == binding.ERR_INVALID_ARG
+    assert L.dmuon_block_schedule(8, 8, -1, None, 0, out, 4) == binding.ERR_INVALID_ARG
+    assert L.dmuon_block_schedule(8, 8, 5, None, 1, out, 4) == binding.ERR_INVALID_ARG   # per-step without coeffs
 
 
 def test_config_shape_sets_match_baseline():

@@ -56,6 +56,43 @@ def test_sq(m, count, variant):
         assert torch.equal(c, c.t())
 
 
+def _commuting_pair(m, seed):
+    """Two exactly symmetric fp16 matrices that are polynomials of one Gram matrix (so their product is symmetric up
+    to the fp16 rounding of the factors), as in a Gram block: G and B = b G + c G G."""
+    x = _rand((m, 2 * m), seed, (2 * m) ** -0.5).double()
+    g = x @ x.t()
+    b = -4.775 * g + 2.0315 * (g @ g)
+    sym16 = lambda t: (torch.triu(t) + torch.triu(t, 1).t()).to(torch.float16)
+    return sym16(g), sym16(b)
+
+
+@pytest.mark.parametrize("m,count", [(128, 2), (256, 3), (384, 2), (896, 2), (1024, 1), (2048, 1)])
+@pytest.mark.parametrize("variant", [0, 1, 4])
+def test_sym_mm(m, count, variant):
+    """dmuon_ns_sym_mm: the Gram-block products T = a G + B G (one addend) and R' = p B' + a R + B' R (two addends)."""
+    pairs = [_commuting_pair(m, 50 + i) for i in range(count)]
+    G = [p[0] for p in pairs]
+    B = [p[1] for p in pairs]
+    nan = lambda: [torch.full((m, m), float("nan"), device="cuda", dtype=torch.float16) for _ in range(count)]
+    T, R, S = nan(), nan(), nan()
+    dm.ns_sym_mm(B, G, G, None, T, alpha=1.0, beta=3.4445, variant=variant)
+    dm.ns_sym_mm(B, G, B, G, R, alpha=0.5, beta=3.4445, beta2=-1.25, variant=variant)
+    dm.ns_sym_mm(B, G, None, None, S, alpha=2.0, variant=variant)
+    torch.cuda.synchronize()
+    for g, b, t, r, s_ in zip(G, B, T, R, S):
+        bg = b.double() @ g.double()
+        for got, ref in ((t, 3.4445 * g.double() + bg), (r, 0.5 * bg + 3.4445 * b.double() - 1.25 * g.double()),
+                         (s_, 2.0 * bg)):
+            assert torch.isfinite(got).all()
+            # the reference product is symmetric only up to the rounding of the factors; compare on the upper triangle
+            assert _rel(torch.triu(got), torch.triu(ref)) < 2e-3
+            # off-diagonal 128-blocks are mirrored (bitwise symmetric); diagonal blocks are computed in full
+            blk = torch.arange(m, device="cuda") // 128
+            off = blk[:, None] != blk[None, :]
+            assert torch.equal(got[off], got.t()[off])
+            assert _rel(got, got.t()) < 2e-3
+
+
 @pytest.mark.parametrize("m,n,count", SHAPES)
 @pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5])
 def test_bx(m, n, count, variant):

@@ -24,9 +24,11 @@ def _reset_options():
     dm.set_option("mode", "tc")
     dm.set_option("steps", 5)
     dm.set_option("coeffs", "3.4445,-4.7750,2.0315")
+    dm.set_option("schedule", "auto")
     yield
     dm.set_option("mode", "tc")
     dm.set_option("steps", 5)
+    dm.set_option("schedule", "auto")
 
 
 @functools.lru_cache(maxsize=None)
@@ -104,6 +106,50 @@ def test_config2_muon_step_check_mode_first_layer():
 
 def test_config2_with_momentum_state():
     _run_muon_config(2, True, "tc", [0, 4, 5, 66, 70, 71], TOL_TC)
+
+
+def test_config2_plain_iteration_schedule():
+    """schedule=x: the wide buckets (3072x768, 768x3072) take the plain X iteration instead of Gram blocks."""
+    dm.set_option("schedule", "x")
+    _run_muon_config(2, True, "tc", [0, 4, 5, 70, 71], TOL_TC)
+
+
+def test_config2_schedule_reported():
+    plan = dm.describe_plan(synth.config_shapes(2), steps=5)
+    blocks = {(b["m"], b["n"]): b["blocks"] for b in plan["buckets"]}
+    assert blocks == {(768, 768): [1, 1, 1, 1, 1], (768, 3072): [3, 2]}
+    assert sum(b["count"] for b in plan["buckets"]) == 72
+
+
+@pytest.mark.parametrize("steps", [1, 2, 3, 4, 5, 6, 7])
+def test_gram_blocks_every_step_count(steps):
+    """Wide matrices (Gram-block buckets, incl. a tall and a ragged one) against the oracle for every block
+    partition: [1], [2], [3], [2,2], [3,2], [3,2,1], [3,2,2] (Eq. 4 PAPER.md:172 is an exact reformulation of Eq. 2)."""
+    shapes = [(256, 1024), (1024, 256), (384, 640), (257, 1000), (512, 1536)]
+    Xs = [synth.gradient(s, 7300 + i, "cuda") if i % 2 == 0 else synth.iid_normal(s, 7300 + i, "cuda")
+          for i, s in enumerate(shapes)]
+    assert all(sum(dm.block_schedule(s, steps)) == steps for s in shapes)
+    assert dm.block_schedule(shapes[0], steps) != [1] * steps or steps == 1
+    X64 = [to64(x) for x in Xs]
+    dm.ns_batched(Xs, steps=steps)
+    torch.cuda.synchronize()
+    for i, s in enumerate(shapes):
+        e = rel_fro(to64(dm.binding.read_ns_output(i, s)), oracle.ns(X64[i], steps=steps))
+        assert e <= TOL_TC, f"steps={steps} {s}: rel err {e:.3e}"
+
+
+def test_gram_blocks_per_step_coefficients():
+    """dmuon_ns_batched_sched on a Gram-block bucket: P_i = a_i I + B_i with a different triple per step."""
+    sched = [[3.9, -6.0, 2.8], [3.6, -5.2, 2.3], [3.4445, -4.775, 2.0315], [3.0, -3.6, 1.3], [2.4, -2.2, 0.6]]
+    shapes = [(256, 1024), (640, 384)]
+    assert dm.block_schedule(shapes[0], 5, sched) == [3, 2]
+    Xs = [synth.gradient(s, 7400 + i, "cuda") for i, s in enumerate(shapes)]
+    X64 = [to64(x) for x in Xs]
+    dm.ns_batched_sched(Xs, sched)
+    torch.cuda.synchronize()
+    for i, s in enumerate(shapes):
+        e = rel_fro(to64(dm.binding.read_ns_output(i, s)), oracle.ns(X64[i], steps=5, coeffs=np.array(sched)))
+        assert e <= TOL_TC, f"{s}: rel err {e:.3e}"
 
 
 # ------------------------------------------------------------------------------------------------ configs[2]
@@ -274,10 +320,12 @@ def test_profile_counts_launches():
     prof = dm.profile_read()
     dm.set_option("profile", 0)
     k = prof["kernels"]
-    # 2 buckets (768x768, 768x3072) x 5 steps x 3 products, + momentum, norms, normalise, apply
-    assert k["ns_syrk_xxt"]["launches"] == 10 and k["ns_sq_poly"]["launches"] == 10 and k["ns_bx_update"]["launches"] == 10
+    # bucket 768x768: 5 plain steps x (SYRK, polynomial, X update); bucket 768x3072: blocks [3, 2] = 2 SYRK, 5 polynomial
+    # products, 3 (3 - 1) + 3 (2 - 1) = 9 Gram-space products, 2 X updates; + momentum, norms, normalise, apply
+    assert k["ns_syrk_xxt"]["launches"] == 7 and k["ns_sq_poly"]["launches"] == 10 and k["ns_bx_update"]["launches"] == 7
+    assert k["ns_gram_mm"]["launches"] == 9
     assert k["momentum_nesterov_sumsq"]["launches"] == 1 and k["apply_update"]["launches"] == 1
-    assert prof["launches"] == 34
+    assert prof["launches"] == 37
     assert all(v["ms"] > 0 for v in k.values())
 
 
