@@ -188,7 +188,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    budget = max(5.0, 60.0 / max(1, args.steps + args.warmup))
+    budget = args.sample_seconds if args.sample_seconds > 0 else max(5.0, 60.0 / max(1, args.steps + args.warmup))
     vals, secs, desc, cores = [], [], "", 0
     for it in range(args.warmup + args.steps):
         v, desc, cores, s = oracle_sample(args.config, budget)
@@ -211,6 +211,20 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------------------------ our arm
+def reduce_max(x: float, dist, device) -> float:
+    """Max over ranks of a per-rank device time (the path does not shard: N replicas, the slowest one counts)."""
+    if not dist:
+        return x
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return t.item()
+
+
+def whole_job_value(world: int, flops_per_replica: float, ms: float) -> float:
+    """TFLOP/s of the whole job: every rank ran one replica of the step in `ms` (max over ranks)."""
+    return world * flops_per_replica / (ms * 1e-3) / 1e12
+
+
 def run_ours(args):
     import paper_2606_27153_b200 as dm
     from paper_2606_27153_b200 import synth
@@ -234,11 +248,7 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     def max_over_ranks(x: float) -> float:
-        if not dist:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return t.item()
+        return reduce_max(x, dist, "cuda")
 
     cfg = args.config
     shapes = synth.config_shapes(cfg)
@@ -289,7 +299,7 @@ def run_ours(args):
 
     plan_desc = dm.describe_plan(shapes, NS_STEPS)
     dflops, xflops = dense_flops(shapes), executed_flops(shapes, plan_desc)
-    value = world * dflops / (ms * 1e-3) / 1e12
+    value = whole_job_value(world, dflops, ms)
 
     # per-kernel rooflines from the library's own CUDA events (recorded on the launching stream, in the timed region)
     work = kernel_work(shapes, plan_desc)
@@ -396,6 +406,7 @@ def main():
     ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--layers", type=int, default=0, help="profiling aid: only the first L layers of the set (0 = all)")
+    ap.add_argument("--sample-seconds", type=float, default=0.0, help="--impl reference: CPU seconds per step (0 = auto)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
