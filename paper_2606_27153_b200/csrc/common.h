@@ -102,8 +102,13 @@ struct ElemTables {
   const int64_t* flat_prefix;  // device [count + 1] chunk prefix
   const int64_t* tile_prefix;  // device [count + 1] stored-orientation tile prefix
   const int64_t* ptile_prefix; // device [count + 1] padded oriented tile prefix
+  // Fast paths of the normalise / apply passes (fp16 workspace only).  A matrix is on exactly one path; the other
+  // paths' prefix arrays give it zero work items.
+  const int64_t* fa_prefix;    // path A: not transposed, rows and cols multiples of 128 (workspace layout == stored
+                               //         layout): flat 8192-element chunks
+  const int64_t* fb_prefix;    // path B: transposed, rows and cols multiples of 128: 64 x 64 tiles, 16-bit transpose
   int count;
-  int64_t flat_chunks, tiles, ptiles;
+  int64_t flat_chunks, tiles, ptiles, fa_chunks, fb_tiles;
   float* partials;             // device [flat_chunks] per-chunk sum of squares
   float* inv_norm;             // device [count] 1 / (||U||_F + eps)
 };

@@ -29,6 +29,13 @@ __device__ __forceinline__ float bf16_bits_to_float(uint32_t b) { return __uint_
 __device__ __forceinline__ uint32_t float_to_bf16_bits(float f) {
   return static_cast<uint32_t>(__bfloat16_as_ushort(__float2bfloat16_rn(f)));
 }
+__device__ __forceinline__ float2 bf16x2_to_float2(uint32_t w) {
+  return make_float2(__uint_as_float(w << 16), __uint_as_float(w & 0xFFFF0000u));
+}
+__device__ __forceinline__ uint32_t float2_to_bf16x2(float2 f) {
+  const __nv_bfloat162 b = __floats2bfloat162_rn(f.x, f.y);     // .x in the low half
+  return *reinterpret_cast<const uint32_t*>(&b);
+}
 __device__ __forceinline__ void unpack8(const uint4& v, float (&f)[8]) {
   const uint32_t w[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
@@ -74,6 +81,8 @@ __global__ void __launch_bounds__(kThreads) flat_kernel(const MatRec* __restrict
     const int64_t start = (chunk - __ldg(prefix + mat)) * kFlatChunk;
     const int64_t end = min(start + static_cast<int64_t>(kFlatChunk), elems);
     float acc = 0.f;
+    float2 acc2 = make_float2(0.f, 0.f);
+    const float2 mu2 = make_float2(mu, mu);
     if (kMomentum) {
       const uint16_t* __restrict__ G = static_cast<const uint16_t*>(rec.G);
       uint16_t* __restrict__ M = static_cast<uint16_t*>(rec.M);
@@ -91,18 +100,23 @@ __global__ void __launch_bounds__(kThreads) flat_kernel(const MatRec* __restrict
       for (int it = 0; it < kIter; ++it) {
         const int64_t i = start + (static_cast<int64_t>(it) * kThreads + threadIdx.x) * 8;
         if (i + 8 <= end) {
-          float g[8], m[8], mn[8], u[8];
-          unpack8(g4[it], g);
-          unpack8(m4[it], m);
+          // two elements per instruction: fma.rn.f32x2 and cvt.rn.bf16x2.f32 (same roundings as the scalar forms)
+          const uint32_t gw[4] = {g4[it].x, g4[it].y, g4[it].z, g4[it].w};
+          const uint32_t mw[4] = {m4[it].x, m4[it].y, m4[it].z, m4[it].w};
+          uint32_t mo[4], uo[4];
 #pragma unroll
-          for (int e = 0; e < 8; ++e) {
-            mn[e] = fmaf(mu, m[e], g[e]);            // M' = mu M + G
-            const float uf = fmaf(mu, mn[e], g[e]);  // U  = G + mu M'   (from the unrounded M')
-            u[e] = bf16_bits_to_float(float_to_bf16_bits(uf));
-            acc = fmaf(u[e], u[e], acc);
+          for (int e = 0; e < 4; ++e) {
+            const float2 gf = bf16x2_to_float2(gw[e]);
+            const float2 mf = bf16x2_to_float2(mw[e]);
+            const float2 mn = __ffma2_rn(mu2, mf, gf);            // M' = mu M + G
+            const float2 uf = __ffma2_rn(mu2, mn, gf);            // U  = G + mu M'   (from the unrounded M')
+            mo[e] = float2_to_bf16x2(mn);
+            uo[e] = float2_to_bf16x2(uf);
+            const float2 ur = bf16x2_to_float2(uo[e]);            // the rounded U is what the norm is taken of
+            acc2 = __ffma2_rn(ur, ur, acc2);
           }
-          *reinterpret_cast<uint4*>(M + i) = pack8_bf16(mn);
-          *reinterpret_cast<uint4*>(U + i) = pack8_bf16(u);
+          *reinterpret_cast<uint4*>(M + i) = make_uint4(mo[0], mo[1], mo[2], mo[3]);
+          *reinterpret_cast<uint4*>(U + i) = make_uint4(uo[0], uo[1], uo[2], uo[3]);
         } else {
           for (int64_t j = i; j < end; ++j) {       // ragged tail of the matrix
             const float g = bf16_bits_to_float(G[j]), m = bf16_bits_to_float(M[j]);
@@ -127,10 +141,12 @@ __global__ void __launch_bounds__(kThreads) flat_kernel(const MatRec* __restrict
       for (int it = 0; it < kIter; ++it) {
         const int64_t i = start + (static_cast<int64_t>(it) * kThreads + threadIdx.x) * 8;
         if (i + 8 <= end) {
-          float x[8];
-          unpack8(x4[it], x);
+          const uint32_t xw[4] = {x4[it].x, x4[it].y, x4[it].z, x4[it].w};
 #pragma unroll
-          for (int e = 0; e < 8; ++e) acc = fmaf(x[e], x[e], acc);
+          for (int e = 0; e < 4; ++e) {
+            const float2 xf = bf16x2_to_float2(xw[e]);
+            acc2 = __ffma2_rn(xf, xf, acc2);
+          }
         } else {
           for (int64_t j = i; j < end; ++j) {
             const float x = bf16_bits_to_float(X[j]);
@@ -139,7 +155,7 @@ __global__ void __launch_bounds__(kThreads) flat_kernel(const MatRec* __restrict
         }
       }
     }
-    const float total = block_sum(acc, red);
+    const float total = block_sum(acc + (acc2.x + acc2.y), red);
     if (threadIdx.x == 0) partials[chunk] = total;
   }
 }
@@ -337,6 +353,192 @@ __global__ void __launch_bounds__(kThreads) apply_kernel(const MatRec* __restric
   }
 }
 
+// ---------------------------------------------------------------------------------------------- fast paths
+// Path A (matrix not transposed, rows and cols multiples of 128, fp16 workspace): the workspace buffer has the stored
+// layout, so normalise and apply are flat streaming passes: 4 x 16-byte loads per thread in flight, two elements per
+// arithmetic instruction (f32x2), one 16-byte store per 8 elements.
+__device__ __forceinline__ uint32_t float2_to_half2_bits(float2 f) {
+  const __half2 h = __float22half2_rn(f);
+  return *reinterpret_cast<const uint32_t*>(&h);
+}
+__device__ __forceinline__ float2 half2_bits_to_float2(uint32_t w) {
+  return __half22float2(*reinterpret_cast<const __half2*>(&w));
+}
+// one 32-bit word (two elements) of the update  W' = W - (lr scale O + lr wd W), rounded once to bf16
+__device__ __forceinline__ uint32_t apply_word(uint32_t w_bits, uint32_t o_bits, float2 so2, float2 lrwd2) {
+  const float2 w = bf16x2_to_float2(w_bits);
+  const float2 o = half2_bits_to_float2(o_bits);
+  const float2 t = __ffma2_rn(so2, o, __fmul2_rn(lrwd2, w));
+  return float2_to_bf16x2(__ffma2_rn(make_float2(-1.f, -1.f), t, w));      // w - t, one rounding
+}
+
+template <bool kFromUser>
+__global__ void __launch_bounds__(kThreads) normalize_flat_kernel(const MatRec* __restrict__ recs,
+                                                                  const int64_t* __restrict__ prefix, int count,
+                                                                  int64_t total_chunks,
+                                                                  const float* __restrict__ inv_norm) {
+  constexpr int kIter = kFlatChunk / (kThreads * 8);
+  for (int64_t chunk = blockIdx.x; chunk < total_chunks; chunk += gridDim.x) {
+    const int mat = find_matrix(prefix, count, chunk);
+    const MatRec& rec = recs[mat];
+    const int64_t start = (chunk - __ldg(prefix + mat)) * kFlatChunk;
+    const uint16_t* __restrict__ src = static_cast<const uint16_t*>(kFromUser ? rec.W : rec.U) + start;
+    uint16_t* __restrict__ dst = static_cast<uint16_t*>(rec.X0) + start;
+    const float inv = __ldg(inv_norm + mat);
+    const float2 inv2 = make_float2(inv, inv);
+    uint4 v[kIter];
+#pragma unroll
+    for (int it = 0; it < kIter; ++it) v[it] = __ldcs(reinterpret_cast<const uint4*>(src + (it * kThreads + threadIdx.x) * 8));
+#pragma unroll
+    for (int it = 0; it < kIter; ++it) {
+      const uint32_t w[4] = {v[it].x, v[it].y, v[it].z, v[it].w};
+      uint32_t o[4];
+#pragma unroll
+      for (int e = 0; e < 4; ++e) o[e] = float2_to_half2_bits(__fmul2_rn(bf16x2_to_float2(w[e]), inv2));
+      *reinterpret_cast<uint4*>(dst + (it * kThreads + threadIdx.x) * 8) = make_uint4(o[0], o[1], o[2], o[3]);
+    }
+  }
+}
+
+template <bool kApply>
+__global__ void __launch_bounds__(kThreads) apply_flat_kernel(const MatRec* __restrict__ recs,
+                                                              const int64_t* __restrict__ prefix, int count,
+                                                              int64_t total_chunks, float lr, float wd) {
+  constexpr int kIter = kFlatChunk / (kThreads * 8);
+  for (int64_t chunk = blockIdx.x; chunk < total_chunks; chunk += gridDim.x) {
+    const int mat = find_matrix(prefix, count, chunk);
+    const MatRec& rec = recs[mat];
+    const int64_t start = (chunk - __ldg(prefix + mat)) * kFlatChunk;
+    const uint16_t* __restrict__ O = static_cast<const uint16_t*>(rec.O) + start;
+    uint16_t* __restrict__ W = static_cast<uint16_t*>(rec.W) + start;
+    const float so = lr * rec.scale, lrwd = lr * wd;
+    const float2 so2 = make_float2(so, so), lrwd2 = make_float2(lrwd, lrwd);
+    uint4 o4[kIter], w4[kIter];
+#pragma unroll
+    for (int it = 0; it < kIter; ++it) {
+      const int off = (it * kThreads + threadIdx.x) * 8;
+      o4[it] = __ldcs(reinterpret_cast<const uint4*>(O + off));
+      if (kApply) w4[it] = __ldcs(reinterpret_cast<const uint4*>(W + off));
+    }
+#pragma unroll
+    for (int it = 0; it < kIter; ++it) {
+      const uint32_t ow[4] = {o4[it].x, o4[it].y, o4[it].z, o4[it].w};
+      const uint32_t ww[4] = {w4[it].x, w4[it].y, w4[it].z, w4[it].w};
+      uint32_t r[4];
+#pragma unroll
+      for (int e = 0; e < 4; ++e)
+        r[e] = kApply ? apply_word(ww[e], ow[e], so2, lrwd2) : float2_to_bf16x2(half2_bits_to_float2(ow[e]));
+      *reinterpret_cast<uint4*>(W + (it * kThreads + threadIdx.x) * 8) = make_uint4(r[0], r[1], r[2], r[3]);
+    }
+  }
+}
+
+// Path B (matrix transposed, rows and cols multiples of 128, fp16 workspace): 64 x 64 tiles transposed as raw 16-bit
+// elements.  Thread (a, b) = (tid / 8, tid % 8) loads the source rows 2a, 2a+1, columns 8b .. 8b+7 (two 16-byte
+// loads), pairs the two rows column by column with PRMT into 32-bit words (src[2a][c], src[2a+1][c]) and stores word
+// a of transposed row c; then thread (c', k') reads 16 bytes = transposed row c', elements 8k' .. 8k'+7.  The 16-byte
+// chunks of a transposed row (128 B) are XOR-swizzled with (c & 7) ^ (c >> 3) so that both the word stores and the
+// 16-byte loads are free of bank conflicts.
+__device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {
+  uint32_t r;
+  asm("prmt.b32 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(sel));
+  return r;
+}
+__device__ __forceinline__ void transpose_tile16(const uint16_t* __restrict__ src, int64_t ld, uint32_t* tile,
+                                                 uint4 (&out)[2]) {
+  const int a = threadIdx.x >> 3, b = threadIdx.x & 7;
+  const uint4 r0 = __ldcs(reinterpret_cast<const uint4*>(src + static_cast<int64_t>(2 * a) * ld + 8 * b));
+  const uint4 r1 = __ldcs(reinterpret_cast<const uint4*>(src + static_cast<int64_t>(2 * a + 1) * ld + 8 * b));
+  const uint32_t w0[4] = {r0.x, r0.y, r0.z, r0.w}, w1[4] = {r1.x, r1.y, r1.z, r1.w};
+  __syncthreads();                                   // the previous tile has been read out
+#pragma unroll
+  for (int w = 0; w < 4; ++w) {
+#pragma unroll
+    for (int odd = 0; odd < 2; ++odd) {
+      const int c = 8 * b + 2 * w + odd;             // transposed row = source column
+      const int chunk = (a >> 2) ^ (c & 7) ^ (c >> 3);
+      tile[c * 32 + chunk * 4 + (a & 3)] = prmt(w0[w], w1[w], odd ? 0x7632u : 0x5410u);
+    }
+  }
+  __syncthreads();
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    const int c = a + 32 * h, k = b;
+    const int chunk = k ^ (c & 7) ^ ((c >> 3) & 7);
+    out[h] = *reinterpret_cast<const uint4*>(tile + c * 32 + chunk * 4);
+  }
+}
+
+template <bool kFromUser>
+__global__ void __launch_bounds__(kThreads) normalize_tr_kernel(const MatRec* __restrict__ recs,
+                                                                const int64_t* __restrict__ prefix, int count,
+                                                                int64_t total_tiles, const float* __restrict__ inv_norm) {
+  __shared__ __align__(16) uint32_t tile[kTile * 32];
+  for (int64_t t = blockIdx.x; t < total_tiles; t += gridDim.x) {
+    const int mat = find_matrix(prefix, count, t);
+    const MatRec& rec = recs[mat];
+    const int64_t local = t - __ldg(prefix + mat);
+    const int tiles_c = rec.cols / kTile;
+    const int tR = static_cast<int>(local / tiles_c), tC = static_cast<int>(local % tiles_c);
+    const uint16_t* __restrict__ src = static_cast<const uint16_t*>(kFromUser ? rec.W : rec.U);
+    uint16_t* __restrict__ dst = static_cast<uint16_t*>(rec.X0);
+    const float inv = __ldg(inv_norm + mat);
+    const float2 inv2 = make_float2(inv, inv);
+    uint4 v[2];
+    transpose_tile16(src + static_cast<int64_t>(tR) * kTile * rec.cols + tC * kTile, rec.cols, tile, v);
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const uint32_t w[4] = {v[h].x, v[h].y, v[h].z, v[h].w};
+      uint32_t o[4];
+#pragma unroll
+      for (int e = 0; e < 4; ++e) o[e] = float2_to_half2_bits(__fmul2_rn(bf16x2_to_float2(w[e]), inv2));
+      // X0[i][j] = src[j][i]: oriented row = stored column, leading dimension n_pad (= rows)
+      const int64_t i = tC * kTile + (threadIdx.x >> 3) + 32 * h, j = tR * kTile + (threadIdx.x & 7) * 8;
+      *reinterpret_cast<uint4*>(dst + i * rec.n_pad + j) = make_uint4(o[0], o[1], o[2], o[3]);
+    }
+  }
+}
+
+template <bool kApply>
+__global__ void __launch_bounds__(kThreads) apply_tr_kernel(const MatRec* __restrict__ recs,
+                                                            const int64_t* __restrict__ prefix, int count,
+                                                            int64_t total_tiles, float lr, float wd) {
+  __shared__ __align__(16) uint32_t tile[kTile * 32];
+  for (int64_t t = blockIdx.x; t < total_tiles; t += gridDim.x) {
+    const int mat = find_matrix(prefix, count, t);
+    const MatRec& rec = recs[mat];
+    const int64_t local = t - __ldg(prefix + mat);
+    const int tiles_c = rec.cols / kTile;
+    const int tR = static_cast<int>(local / tiles_c), tC = static_cast<int>(local % tiles_c);
+    const uint16_t* __restrict__ O = static_cast<const uint16_t*>(rec.O);
+    uint16_t* __restrict__ W = static_cast<uint16_t*>(rec.W);
+    const float so = lr * rec.scale, lrwd = lr * wd;
+    const float2 so2 = make_float2(so, so), lrwd2 = make_float2(lrwd, lrwd);
+    // O(R, C) = Obuf[C][R]: the source tile is Obuf rows tC*64.., columns tR*64.. (leading dimension n_pad = rows)
+    uint4 w4[2];
+    if (kApply) {
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        const int64_t R = tR * kTile + (threadIdx.x >> 3) + 32 * h, C = tC * kTile + (threadIdx.x & 7) * 8;
+        w4[h] = __ldcs(reinterpret_cast<const uint4*>(W + R * rec.cols + C));
+      }
+    }
+    uint4 v[2];
+    transpose_tile16(O + static_cast<int64_t>(tC) * kTile * rec.n_pad + tR * kTile, rec.n_pad, tile, v);
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const uint32_t ow[4] = {v[h].x, v[h].y, v[h].z, v[h].w};
+      const uint32_t ww[4] = {w4[h].x, w4[h].y, w4[h].z, w4[h].w};
+      uint32_t r[4];
+#pragma unroll
+      for (int e = 0; e < 4; ++e)
+        r[e] = kApply ? apply_word(ww[e], ow[e], so2, lrwd2) : float2_to_bf16x2(half2_bits_to_float2(ow[e]));
+      const int64_t R = tR * kTile + (threadIdx.x >> 3) + 32 * h, C = tC * kTile + (threadIdx.x & 7) * 8;
+      *reinterpret_cast<uint4*>(W + R * rec.cols + C) = make_uint4(r[0], r[1], r[2], r[3]);
+    }
+  }
+}
+
 // Pseudo-random fp16 values in (-0.025, 0.025) for the autotuner's scratch operands (all-zero operands would draw
 // far less power than real data and skew the comparison between tile configurations).
 __global__ void fill_scratch_kernel(uint32_t* __restrict__ p, size_t words) {
@@ -419,6 +621,20 @@ int launch_finalize_norms(const ElemTables& T, float eps, cudaStream_t s) {
 }
 
 int launch_normalize(const ElemTables& T, bool from_user, bool fp32_internal, cudaStream_t s) {
+  if (T.ptiles + T.fa_chunks + T.fb_tiles == 0) return DMUON_OK;
+  if (T.fa_chunks > 0) {
+    ProfScope ps("normalize_orient_cast", s);
+    const int g = grid_for(T.fa_chunks, 8);
+    if (from_user) normalize_flat_kernel<true><<<g, kThreads, 0, s>>>(T.recs, T.fa_prefix, T.count, T.fa_chunks, T.inv_norm);
+    else normalize_flat_kernel<false><<<g, kThreads, 0, s>>>(T.recs, T.fa_prefix, T.count, T.fa_chunks, T.inv_norm);
+  }
+  if (T.fb_tiles > 0) {
+    ProfScope ps("normalize_orient_cast", s);
+    const int g = grid_for(T.fb_tiles, 8);
+    if (from_user) normalize_tr_kernel<true><<<g, kThreads, 0, s>>>(T.recs, T.fb_prefix, T.count, T.fb_tiles, T.inv_norm);
+    else normalize_tr_kernel<false><<<g, kThreads, 0, s>>>(T.recs, T.fb_prefix, T.count, T.fb_tiles, T.inv_norm);
+  }
+  DMUON_CUDA_CHECK(cudaGetLastError());
   if (T.ptiles == 0) return DMUON_OK;
   ProfScope ps("normalize_orient_cast", s);
   const int grid = grid_for(T.ptiles, 16);
@@ -432,6 +648,16 @@ int launch_normalize(const ElemTables& T, bool from_user, bool fp32_internal, cu
 }
 
 int launch_apply(const ElemTables& T, float lr, float wd, bool fp32_internal, cudaStream_t s) {
+  if (T.tiles + T.fa_chunks + T.fb_tiles == 0) return DMUON_OK;
+  if (T.fa_chunks > 0) {
+    ProfScope ps("apply_update", s);
+    apply_flat_kernel<true><<<grid_for(T.fa_chunks, 8), kThreads, 0, s>>>(T.recs, T.fa_prefix, T.count, T.fa_chunks, lr, wd);
+  }
+  if (T.fb_tiles > 0) {
+    ProfScope ps("apply_update", s);
+    apply_tr_kernel<true><<<grid_for(T.fb_tiles, 8), kThreads, 0, s>>>(T.recs, T.fb_prefix, T.count, T.fb_tiles, lr, wd);
+  }
+  DMUON_CUDA_CHECK(cudaGetLastError());
   if (T.tiles == 0) return DMUON_OK;
   ProfScope ps("apply_update", s);
   const int grid = grid_for(T.tiles, 16);
@@ -442,6 +668,16 @@ int launch_apply(const ElemTables& T, float lr, float wd, bool fp32_internal, cu
 }
 
 int launch_store_ns(const ElemTables& T, bool fp32_internal, cudaStream_t s) {
+  if (T.tiles + T.fa_chunks + T.fb_tiles == 0) return DMUON_OK;
+  if (T.fa_chunks > 0) {
+    ProfScope ps("store_ns_output", s);
+    apply_flat_kernel<false><<<grid_for(T.fa_chunks, 8), kThreads, 0, s>>>(T.recs, T.fa_prefix, T.count, T.fa_chunks, 0.f, 0.f);
+  }
+  if (T.fb_tiles > 0) {
+    ProfScope ps("store_ns_output", s);
+    apply_tr_kernel<false><<<grid_for(T.fb_tiles, 8), kThreads, 0, s>>>(T.recs, T.fb_prefix, T.count, T.fb_tiles, 0.f, 0.f);
+  }
+  DMUON_CUDA_CHECK(cudaGetLastError());
   if (T.tiles == 0) return DMUON_OK;
   ProfScope ps("store_ns_output", s);
   const int grid = grid_for(T.tiles, 16);

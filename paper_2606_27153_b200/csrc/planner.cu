@@ -378,13 +378,20 @@ int get_plan(const int32_t* shapes, int count, const Options& opt, void* ext_ws,
 
   // ---- elementwise tables
   std::vector<int64_t> flat_prefix(count + 1, 0), tile_prefix(count + 1, 0), ptile_prefix(count + 1, 0);
+  std::vector<int64_t> fa_prefix(count + 1, 0), fb_prefix(count + 1, 0);
   p.h_recs.resize(count);
   for (int i = 0; i < count; ++i) {
     const MatrixInfo& mi = p.mats[i];
     const int64_t elems = static_cast<int64_t>(mi.rows) * mi.cols;
     flat_prefix[i + 1] = flat_prefix[i] + (elems + kFlatChunk - 1) / kFlatChunk;
-    tile_prefix[i + 1] = tile_prefix[i] + static_cast<int64_t>((mi.rows + kTile - 1) / kTile) * ((mi.cols + kTile - 1) / kTile);
-    ptile_prefix[i + 1] = ptile_prefix[i] + static_cast<int64_t>(mi.m_pad / kTile) * (mi.n_pad / kTile);
+    // normalise / apply path of this matrix: A (flat), B (16-bit tile transpose) or the generic tiles
+    const bool aligned = !p.fp32 && mi.rows % kBlk == 0 && mi.cols % kBlk == 0;
+    const bool path_a = aligned && !mi.transposed, path_b = aligned && mi.transposed;
+    fa_prefix[i + 1] = fa_prefix[i] + (path_a ? elems / kFlatChunk : 0);
+    fb_prefix[i + 1] = fb_prefix[i] + (path_b ? static_cast<int64_t>(mi.rows / kTile) * (mi.cols / kTile) : 0);
+    const bool generic = !path_a && !path_b;
+    tile_prefix[i + 1] = tile_prefix[i] + (generic ? static_cast<int64_t>((mi.rows + kTile - 1) / kTile) * ((mi.cols + kTile - 1) / kTile) : 0);
+    ptile_prefix[i + 1] = ptile_prefix[i] + (generic ? static_cast<int64_t>(mi.m_pad / kTile) * (mi.n_pad / kTile) : 0);
     MatRec& r = p.h_recs[i];
     memset(&r, 0, sizeof r);
     r.U = p.ws + mi.off_p;
@@ -400,6 +407,8 @@ int get_plan(const int32_t* shapes, int count, const Options& opt, void* ext_ws,
   if ((rc = upload(p, &p.d_flat_prefix, flat_prefix))) return rc;
   if ((rc = upload(p, &p.d_tile_prefix, tile_prefix))) return rc;
   if ((rc = upload(p, &p.d_ptile_prefix, ptile_prefix))) return rc;
+  if ((rc = upload(p, &p.d_fa_prefix, fa_prefix))) return rc;
+  if ((rc = upload(p, &p.d_fb_prefix, fb_prefix))) return rc;
   if ((rc = dev_alloc(p, &p.d_partials, static_cast<size_t>(flat_prefix[count])))) return rc;
   if ((rc = dev_alloc(p, &p.d_inv_norm, count))) return rc;
   p.tables.recs = p.d_recs;
@@ -410,6 +419,10 @@ int get_plan(const int32_t* shapes, int count, const Options& opt, void* ext_ws,
   p.tables.flat_chunks = flat_prefix[count];
   p.tables.tiles = tile_prefix[count];
   p.tables.ptiles = ptile_prefix[count];
+  p.tables.fa_prefix = p.d_fa_prefix;
+  p.tables.fb_prefix = p.d_fb_prefix;
+  p.tables.fa_chunks = fa_prefix[count];
+  p.tables.fb_tiles = fb_prefix[count];
   p.tables.partials = p.d_partials;
   p.tables.inv_norm = p.d_inv_norm;
 

@@ -99,7 +99,8 @@ struct Plan {
   // elementwise tables
   std::vector<MatRec> h_recs;          // host mirror (pointers patched per call)
   MatRec* d_recs = nullptr;
-  int64_t *d_flat_prefix = nullptr, *d_tile_prefix = nullptr, *d_ptile_prefix = nullptr;
+  int64_t *d_flat_prefix = nullptr, *d_tile_prefix = nullptr, *d_ptile_prefix = nullptr, *d_fa_prefix = nullptr,
+          *d_fb_prefix = nullptr;
   float *d_partials = nullptr, *d_inv_norm = nullptr;
   ElemTables tables{};
   std::string bound_key;               // schedule signature rec.O was last bound for

@@ -324,8 +324,10 @@ def test_profile_counts_launches():
     # products, 3 (3 - 1) + 3 (2 - 1) = 9 Gram-space products, 2 X updates; + momentum, norms, normalise, apply
     assert k["ns_syrk_xxt"]["launches"] == 7 and k["ns_sq_poly"]["launches"] == 10 and k["ns_bx_update"]["launches"] == 7
     assert k["ns_gram_mm"]["launches"] == 9
-    assert k["momentum_nesterov_sumsq"]["launches"] == 1 and k["apply_update"]["launches"] == 1
-    assert prof["launches"] == 37
+    # normalise and apply: one flat launch (768x768, 768x3072) + one transposing launch (3072x768) each
+    assert k["momentum_nesterov_sumsq"]["launches"] == 1 and k["apply_update"]["launches"] == 2
+    assert k["normalize_orient_cast"]["launches"] == 2
+    assert prof["launches"] == 39
     assert all(v["ms"] > 0 for v in k.values())
 
 
