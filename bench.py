@@ -301,37 +301,57 @@ def run_ours(args):
     dflops, xflops = dense_flops(shapes), executed_flops(shapes, plan_desc)
     value = whole_job_value(world, dflops, ms)
 
-    # per-kernel rooflines from the library's own CUDA events (recorded on the launching stream, in the timed region)
+    # per-kernel rooflines from the library's own CUDA events (recorded on the launching stream, in the timed region).
+    # The library names GEMM launches family[m x n] per shape bucket; `kernels` aggregates per family, `launch_types`
+    # keeps the buckets apart, and `roofline` is the launch type that takes the most time.
     work = kernel_work(shapes, plan_desc)
-    kernels = {}
-    for name, rec in prof["kernels"].items():
-        per_step_ms = rec["ms"] / args.steps
-        entry = {"launches_per_step": rec["launches"] / args.steps, "ms_per_step": per_step_ms, "share": per_step_ms / ms}
-        if name in work and per_step_ms > 0:
-            kind, amount = work[name]
+
+    def entry(ms_tot, launches, kind, amount):
+        per_step_ms = ms_tot / args.steps
+        e = {"launches_per_step": launches / args.steps, "ms_per_step": per_step_ms, "share": per_step_ms / ms}
+        if kind and per_step_ms > 0:
             if kind == "flop":
                 ach = amount / (per_step_ms * 1e-3) / 1e12
-                entry.update({"bound": "tensor", "achieved": ach, "unit": "TFLOP/s", "frac": ach / peaks["tflops_sustained"],
-                              "frac_of_burst": ach / peaks["tflops_burst"], "frac_of_nominal_2250": ach / 2250.0})
+                e.update({"bound": "tensor", "achieved": ach, "unit": "TFLOP/s", "frac": ach / peaks["tflops_sustained"],
+                          "frac_of_burst": ach / peaks["tflops_burst"], "frac_of_nominal_2250": ach / 2250.0})
             else:
                 ach = amount / (per_step_ms * 1e-3) / 1e9
-                entry.update({"bound": "hbm", "achieved": ach, "unit": "GB/s", "frac": ach / peaks["hbm_gbs"]})
-        kernels[name] = entry
-    dom = max((k for k in kernels if k in work and work[k][0] == "flop"), key=lambda k: kernels[k]["ms_per_step"], default=None)
+                e.update({"bound": "hbm", "achieved": ach, "unit": "GB/s", "frac": ach / peaks["hbm_gbs"]})
+        return e
+
+    fam = {}
+    for name, rec in prof["kernels"].items():
+        f = fam.setdefault(name.split("[")[0], {"ms": 0.0, "launches": 0})
+        f["ms"] += rec["ms"]
+        f["launches"] += rec["launches"]
+    kernels = {f: entry(v["ms"], v["launches"], *work.get(f, (None, 0))) for f, v in fam.items()}
+    launch_types = {}
+    for name, rec in prof["kernels"].items():
+        if "[" not in name:
+            continue
+        f, dims = name[:-1].split("[")
+        bm, bn = (int(v) for v in dims.split("x"))
+        sub = [sh for sh in shapes if (pad128(min(sh)), pad128(max(sh))) == (bm, bn)]
+        launch_types[name] = entry(rec["ms"], rec["launches"], *kernel_work(sub, plan_desc)[f])
+        launch_types[name]["matrices_per_launch"] = len(sub)
+    dom = max(launch_types, key=lambda k: launch_types[k]["ms_per_step"], default=None)
     traffic = None
     tpath = os.path.join(ROOT, "profiles", "roofline_traffic.json")
     if dom and os.path.exists(tpath):
         traffic = json.load(open(tpath)).get(f"config{cfg}", {}).get(dom)
     roofline = None
     if dom:
-        k = kernels[dom]
+        k = launch_types[dom]
         roofline = {"kernel": dom, "bound": "tensor", "achieved": k["achieved"], "peak": peaks["tflops_sustained"],
                     "unit": "TFLOP/s", "frac": k["frac"], "traffic": traffic,
+                    "launches_per_step": k["launches_per_step"], "matrices_per_launch": k["matrices_per_launch"],
                     "peak_kind": f"{peaks['source']} bf16 cuBLAS, sustained (kernel timed inside a long step); "
                                  f"burst {peaks['tflops_burst']}, nominal 2250",
-                    "flops_counted": "algorithmic FLOPs of this family's launches: 2 m^2 n per matrix per X update (dense, no "
+                    "flops_counted": "algorithmic FLOPs per launch: 2 m^2 n per matrix for an X update (dense, no "
                                      "symmetry); (T+1)/(2T) of 2 m^2 n or 2 m^3 per matrix for the symmetric products "
-                                     "(upper-triangular 128-blocks; the mirror is not arithmetic)"}
+                                     "(upper-triangular 128-blocks; the mirror is not arithmetic)",
+                    "traffic_unit": "bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum, ncu --set full; "
+                                    "profiles/roofline_traffic.json)"}
 
     # ---- end to end through the C ABI with HOST buffers (copies inside the timed region)
     e2e = None
@@ -388,7 +408,7 @@ def run_ours(args):
                                  "dense_equiv_of_measured_burst": 100 * value / world / peaks["tflops_burst"],
                                  "dense_equiv_of_nominal_2250": 100 * value / world / 2250.0,
                                  "executed_of_measured_sustained": 100 * xflops / (ms * 1e-3) / 1e12 / peaks["tflops_sustained"]},
-            "roofline": roofline, "kernels": kernels, "cpu_baseline": cpu_baseline, "e2e": e2e,
+            "roofline": roofline, "kernels": kernels, "launch_types": launch_types, "cpu_baseline": cpu_baseline, "e2e": e2e,
             "gpu_launches": prof["launches"], "clocks": clocks, "plan_autotune_seconds": plan_s,
             "paper_context": "DMuon reports 6.85x-163x optimizer-step and 1.48x-3.01x end-to-end speedups on 8-256 A800 "
                              "(PAPER.md:5, :274) and ~2x on one GPU (:329): other hardware, context only",
@@ -396,6 +416,94 @@ def run_ours(args):
         print(json.dumps(line))
     if dist:
         dist.destroy_process_group()
+
+
+def run_sweep(args):
+    """BASELINE.json configs[4]: the NS kernel alone (dmuon_ns_batched, 5 steps) over a shape sweep, one JSON line per
+    shape with dense-equivalent and executed TFLOP/s.  Not the bench line: a per-shape table for profiles/."""
+    import paper_2606_27153_b200 as dm
+    from paper_2606_27153_b200 import synth
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --sweep needs a B200")
+    torch.cuda.set_device(0)
+    dm.set_option("mode", "tc")
+    cap = 16384                      # bounds plan-building time (TMA descriptors per matrix); said in the output
+    for (r, c), batch in synth.sweep_shapes():
+        b = min(batch, cap)
+        g = torch.Generator(device="cuda")
+        g.manual_seed(5000 + r + c)
+        big = torch.randn((b, r, c), generator=g, device="cuda", dtype=torch.float32).to(torch.bfloat16)
+        Xs = [big[i] for i in range(b)]
+        shapes = [(r, c)] * b
+        t0 = time.perf_counter()
+        dm.ns_batched(Xs, steps=NS_STEPS)      # plan + autotune
+        torch.cuda.synchronize()
+        plan_s = time.perf_counter() - t0
+        plan = dm.describe_plan(shapes, NS_STEPS)
+        reps = 3
+        for _ in range(2):
+            dm.ns_batched(Xs, steps=NS_STEPS)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(reps):
+            dm.ns_batched(Xs, steps=NS_STEPS)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / reps
+        print(json.dumps({"sweep": True, "shape": [r, c], "batch": b, "batch_in_config": batch, "ms": ms,
+                          "tflops_dense_equiv": dense_flops(shapes) / ms / 1e9,
+                          "tflops_executed": executed_flops(shapes, plan) / ms / 1e9,
+                          "blocks": plan["buckets"][0]["blocks"], "variants": plan["buckets"][0]["variants"],
+                          "plan_seconds": plan_s, "includes": "norm + normalise + 5 NS steps + bf16 store"}), flush=True)
+        del Xs, big
+        dm.shutdown()
+        torch.cuda.empty_cache()
+
+
+def run_power_probe(args):
+    """Sustained throughput of the grouped X-update and SYRK kernels (dmuon_ns_gemm, CTA-pair tiling, 8 matrices of
+    4096 x 14336) against operand bit patterns: random fp16, low mantissa bits cleared, constant, zeros.  Shows how
+    much of the 1 kW cap is operand toggling.  One JSON line per (pattern, kernel)."""
+    import paper_2606_27153_b200 as dm
+    from paper_2606_27153_b200.binding import OP_BX, OP_SYRK
+    torch.cuda.set_device(0)
+    m, n, cnt = 4096, 14336, 8
+
+    def clear_low(x, bits):
+        return (x.view(torch.int16) & ~((1 << bits) - 1)).view(torch.float16)
+
+    for kind in ("random", "low3_cleared", "low6_cleared", "constant", "zeros", "random"):
+        g = torch.Generator(device="cuda")
+        g.manual_seed(1)
+        B = [(torch.randn((m, m), generator=g, device="cuda") * 0.02).half() for _ in range(cnt)]
+        X = [(torch.randn((m, n), generator=g, device="cuda") * 1e-2).half() for _ in range(cnt)]
+        if kind == "zeros":
+            B, X = [torch.zeros_like(t) for t in B], [torch.zeros_like(t) for t in X]
+        elif kind == "constant":
+            B, X = [torch.full_like(t, 0.01) for t in B], [torch.full_like(t, 0.01) for t in X]
+        elif kind.startswith("low"):
+            k = int(kind[3])
+            B, X = [clear_low(t, k) for t in B], [clear_low(t, k) for t in X]
+        C = [torch.empty((m, n), device="cuda", dtype=torch.float16) for _ in range(cnt)]
+        A = [torch.empty((m, m), device="cuda", dtype=torch.float16) for _ in range(cnt)]
+        for op, name, reps in ((OP_BX, "ns_bx_update_pair", 80), (OP_SYRK, "ns_syrk_xxt_pair", 150)):
+            call = (lambda: dm.ns_gemm(OP_BX, B, X, C, 1.0, 3.4445, variant=5)) if op == OP_BX else \
+                   (lambda: dm.ns_gemm(OP_SYRK, X, None, A, 1.0, 0.0, variant=4))
+            for _ in range(3):
+                call()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record()
+            for _ in range(reps):
+                call()
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / reps
+            flops = cnt * 2 * m * m * n * (1.0 if op == OP_BX else 136 * 4 / 1024)   # SYRK: 136 of 256 pair units
+            print(json.dumps({"probe": "power", "operands": kind, "kernel": name, "ms": ms, "seconds_timed": ms * reps / 1e3,
+                              "tflops_executed": flops / ms / 1e9}), flush=True)
+        del B, X, C, A
 
 
 def main():
@@ -409,8 +517,14 @@ def main():
     ap.add_argument("--sample-seconds", type=float, default=0.0, help="--impl reference: CPU seconds per step (0 = auto)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--power-probe", action="store_true", help="kernel throughput vs operand bit patterns (power cap)")
+    ap.add_argument("--sweep", action="store_true", help="configs[4]: NS-only shape sweep, one JSON line per shape")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.sweep:
+        run_sweep(args)
+    elif args.power_probe:
+        run_power_probe(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

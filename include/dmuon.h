@@ -84,7 +84,11 @@ DMUON_API int dmuon_muon_step(void* const* params, const void* const* grads, voi
 /*
  * The same step for tensors that live in HOST memory (pinned memory gives asynchronous copies): copies W, G, M of
  * every matrix to device staging buffers owned by the library, runs dmuon_muon_step there, and copies W and M
- * back; all on `stream`.  The caller synchronises `stream` before reading the results.
+ * back.  The matrix list is processed in up to 8 groups of whole repetitions of its shape pattern (layers), so that
+ * the host->device copies of one group, the step of the previous one and the device->host copies of the one before
+ * overlap (two library-owned copy streams, both PCIe directions busy).  All work is ordered after what `stream`
+ * held at the call and `stream` waits for all of it: the caller synchronises `stream` before reading the results.
+ * Host buffers should be pinned (pageable memory makes the copies synchronous).
  */
 DMUON_API int dmuon_muon_step_host(void* const* params_host, const void* const* grads_host,
                                    void* const* momenta_host, const int32_t* shapes, int32_t count, float lr,

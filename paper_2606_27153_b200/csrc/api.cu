@@ -21,7 +21,7 @@ size_t g_ext_ws_bytes = 0;
 
 // ---------------------------------------------------------------- profiling
 struct ProfRec {
-  const char* name;
+  std::string name;
   cudaEvent_t e0, e1;
 };
 std::vector<ProfRec> g_prof_open;                 // recorded, not yet folded
@@ -141,6 +141,27 @@ int ns_batched_impl(void* const* ptrs, const int32_t* shapes, int32_t count, int
   return DMUON_OK;
 }
 
+// ---- state of dmuon_muon_step_host: device staging of W | G | M, copy streams, events (one shape set at a time)
+struct HostCtx {
+  std::vector<int32_t> shapes;
+  uint8_t* stage = nullptr;
+  std::vector<size_t> off;      // per matrix offset of W; G at + third, M at + 2 * third
+  size_t third = 0;
+  int group = 0;                // matrices per group
+  cudaStream_t s_in = nullptr, s_out = nullptr;
+  std::vector<cudaEvent_t> ev;  // [2 g] copy-in done, [2 g + 1] step done, then start / end
+  int release() {
+    if (stage || s_in) cudaDeviceSynchronize();
+    if (stage) cudaFree(stage);
+    if (s_in) cudaStreamDestroy(s_in);
+    if (s_out) cudaStreamDestroy(s_out);
+    for (cudaEvent_t e : ev) cudaEventDestroy(e);
+    cudaGetLastError();
+    *this = HostCtx();
+    return DMUON_OK;
+  }
+} g_host;
+
 // ---- dmuon_ns_gemm table cache (one entry: the last argument set)
 struct GemmCall {
   std::vector<const void*> in0, in1;
@@ -244,6 +265,10 @@ DMUON_API int dmuon_muon_step(void* const* params, const void* const* grads, voi
   return muon_step_device(params, grads, momenta, shapes, count, lr, mu, wd, reinterpret_cast<cudaStream_t>(stream), nullptr);
 }
 
+// Host-buffer entry: the matrix list is cut into groups of whole periods of its shape pattern (a transformer's layers),
+// so that every group has the same shape list and shares one plan and one workspace.  Group g's host->device copies
+// (copy-in stream), the step of group g-1 (caller's stream) and the device->host copies of group g-2 (copy-out stream)
+// overlap; PCIe carries both directions at once.
 DMUON_API int dmuon_muon_step_host(void* const* params_host, const void* const* grads_host, void* const* momenta_host,
                                    const int32_t* shapes, int32_t count, float lr, float mu, float wd,
                                    dmuon_stream_t stream_) {
@@ -255,46 +280,74 @@ DMUON_API int dmuon_muon_step_host(void* const* params_host, const void* const* 
     if (shapes[2 * i] <= 0 || shapes[2 * i + 1] <= 0) { set_error("dmuon_muon_step_host: bad shape of matrix %d", i); return DMUON_ERR_INVALID_ARG; }
     if (!params_host[i] || !grads_host[i] || !momenta_host[i]) { set_error("dmuon_muon_step_host: matrix %d has a null pointer", i); return DMUON_ERR_INVALID_ARG; }
   }
-  Plan* plan = nullptr;
-  int rc = get_plan(shapes, count, g_opt, g_ext_ws, g_ext_ws_bytes, stream, &plan);
+  int rc = check_device();
   if (rc) return rc;
-  if (!plan->stage) {
+  HostCtx& hc = g_host;
+  if (hc.shapes.size() != static_cast<size_t>(2 * count) || memcmp(hc.shapes.data(), shapes, sizeof(int32_t) * 2 * count) != 0) {
+    if ((rc = hc.release())) return rc;
+    hc.shapes.assign(shapes, shapes + 2 * count);
+    // smallest period of the shape pattern, then the smallest number of periods per group that gives <= 8 groups
+    int period = count;
+    for (int p = 1; p < count; ++p) {
+      if (count % p) continue;
+      bool ok = true;
+      for (int k = p; k < count && ok; ++k) ok = shapes[2 * k] == shapes[2 * (k - p)] && shapes[2 * k + 1] == shapes[2 * (k - p) + 1];
+      if (ok) { period = p; break; }
+    }
+    const int periods = count / period;
+    int per_group = periods;
+    for (int d = 1; d <= periods; ++d)
+      if (periods % d == 0 && periods / d <= 8) { per_group = d; break; }
+    hc.group = per_group * period;
     size_t off = 0;
-    plan->stage_off.resize(count);
+    hc.off.resize(count);
     for (int i = 0; i < count; ++i) {
-      plan->stage_off[i] = off;
+      hc.off[i] = off;
       off += (static_cast<size_t>(shapes[2 * i]) * shapes[2 * i + 1] * 2 + 255) / 256 * 256;
     }
-    plan->stage_third = off;
+    hc.third = off;
     void* p = nullptr;
     cudaError_t e = cudaMalloc(&p, 3 * off);
-    if (e != cudaSuccess) { cudaGetLastError(); set_error("staging allocation of %zu bytes failed", 3 * off); return DMUON_ERR_OOM; }
-    plan->d_allocs.push_back(p);
-    plan->stage = static_cast<uint8_t*>(p);
+    if (e != cudaSuccess) { cudaGetLastError(); hc.shapes.clear(); set_error("staging allocation of %zu bytes failed", 3 * off); return DMUON_ERR_OOM; }
+    hc.stage = static_cast<uint8_t*>(p);
+    DMUON_CUDA_CHECK(cudaStreamCreateWithFlags(&hc.s_in, cudaStreamNonBlocking));
+    DMUON_CUDA_CHECK(cudaStreamCreateWithFlags(&hc.s_out, cudaStreamNonBlocking));
+    const int groups = count / hc.group;
+    hc.ev.resize(2 * groups + 2);
+    for (cudaEvent_t& ev : hc.ev) DMUON_CUDA_CHECK(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
   }
+  const int groups = count / hc.group;
+  cudaEvent_t ev_start = hc.ev[2 * groups], ev_end = hc.ev[2 * groups + 1];
+  DMUON_CUDA_CHECK(cudaEventRecord(ev_start, stream));            // copies start after the caller's earlier work
+  DMUON_CUDA_CHECK(cudaStreamWaitEvent(hc.s_in, ev_start, 0));
   std::vector<void*> w(count), m(count);
   std::vector<const void*> g(count);
-  {
-    ProfScope ps("h2d_copies", stream);
-    for (int i = 0; i < count; ++i) {
-      const size_t bytes = static_cast<size_t>(shapes[2 * i]) * shapes[2 * i + 1] * 2;
-      w[i] = plan->stage + plan->stage_off[i];
-      g[i] = plan->stage + plan->stage_third + plan->stage_off[i];
-      m[i] = plan->stage + 2 * plan->stage_third + plan->stage_off[i];
-      DMUON_CUDA_CHECK(cudaMemcpyAsync(w[i], params_host[i], bytes, cudaMemcpyHostToDevice, stream));
-      DMUON_CUDA_CHECK(cudaMemcpyAsync(const_cast<void*>(g[i]), grads_host[i], bytes, cudaMemcpyHostToDevice, stream));
-      DMUON_CUDA_CHECK(cudaMemcpyAsync(m[i], momenta_host[i], bytes, cudaMemcpyHostToDevice, stream));
+  auto bytes_of = [&](int i) { return static_cast<size_t>(shapes[2 * i]) * shapes[2 * i + 1] * 2; };
+  for (int i = 0; i < count; ++i) {
+    w[i] = hc.stage + hc.off[i];
+    g[i] = hc.stage + hc.third + hc.off[i];
+    m[i] = hc.stage + 2 * hc.third + hc.off[i];
+  }
+  g_launches += 5 * count;                                         // 3 H2D + 2 D2H copies per matrix
+  for (int gi = 0; gi < groups; ++gi) {
+    const int b = gi * hc.group, e = b + hc.group;
+    for (int i = b; i < e; ++i) {
+      DMUON_CUDA_CHECK(cudaMemcpyAsync(w[i], params_host[i], bytes_of(i), cudaMemcpyHostToDevice, hc.s_in));
+      DMUON_CUDA_CHECK(cudaMemcpyAsync(const_cast<void*>(g[i]), grads_host[i], bytes_of(i), cudaMemcpyHostToDevice, hc.s_in));
+      DMUON_CUDA_CHECK(cudaMemcpyAsync(m[i], momenta_host[i], bytes_of(i), cudaMemcpyHostToDevice, hc.s_in));
+    }
+    DMUON_CUDA_CHECK(cudaEventRecord(hc.ev[2 * gi], hc.s_in));
+    DMUON_CUDA_CHECK(cudaStreamWaitEvent(stream, hc.ev[2 * gi], 0));
+    if ((rc = muon_step_device(w.data() + b, g.data() + b, m.data() + b, shapes + 2 * b, hc.group, lr, mu, wd, stream, nullptr))) return rc;
+    DMUON_CUDA_CHECK(cudaEventRecord(hc.ev[2 * gi + 1], stream));
+    DMUON_CUDA_CHECK(cudaStreamWaitEvent(hc.s_out, hc.ev[2 * gi + 1], 0));
+    for (int i = b; i < e; ++i) {
+      DMUON_CUDA_CHECK(cudaMemcpyAsync(params_host[i], w[i], bytes_of(i), cudaMemcpyDeviceToHost, hc.s_out));
+      DMUON_CUDA_CHECK(cudaMemcpyAsync(momenta_host[i], m[i], bytes_of(i), cudaMemcpyDeviceToHost, hc.s_out));
     }
   }
-  if ((rc = muon_step_device(w.data(), g.data(), m.data(), shapes, count, lr, mu, wd, stream, nullptr))) return rc;
-  {
-    ProfScope ps("d2h_copies", stream);
-    for (int i = 0; i < count; ++i) {
-      const size_t bytes = static_cast<size_t>(shapes[2 * i]) * shapes[2 * i + 1] * 2;
-      DMUON_CUDA_CHECK(cudaMemcpyAsync(params_host[i], w[i], bytes, cudaMemcpyDeviceToHost, stream));
-      DMUON_CUDA_CHECK(cudaMemcpyAsync(momenta_host[i], m[i], bytes, cudaMemcpyDeviceToHost, stream));
-    }
-  }
+  DMUON_CUDA_CHECK(cudaEventRecord(ev_end, hc.s_out));
+  DMUON_CUDA_CHECK(cudaStreamWaitEvent(stream, ev_end, 0));      // the caller's stream sees the results
   return DMUON_OK;
 }
 
@@ -531,6 +584,7 @@ DMUON_API void dmuon_shutdown(void) {
   cudaDeviceSynchronize();
   cudaGetLastError();
   fold_profile();
+  g_host.release();
   drop_plans();
   g_last_plan = nullptr;
   if (g_gemm_call.d_probs) cudaFree(g_gemm_call.d_probs);

@@ -527,7 +527,8 @@ int build_program(Plan& p, BucketPlan& b, const Partition& part, NsProgram& prog
       if (rc) return rc;
     }
     NsLaunch L;
-    L.op = op; L.ck = ck; L.s0 = s0; L.s1 = s1; L.name = name;
+    L.op = op; L.ck = ck; L.s0 = s0; L.s1 = s1;
+    L.name = std::string(name) + "[" + std::to_string(b.m_pad) + "x" + std::to_string(b.n_pad) + "]";
     L.k_blocks = op == OP_SYRK ? kb_n : kb_m;
     L.n_blocks = op == OP_BX ? nb_n : nb_m;
     if ((rc = upload(p, &L.probs, hp))) return rc;
@@ -597,7 +598,7 @@ int run_ns_steps(Plan& plan, int steps, const float* coeffs, bool per_step, cons
       for (const NsLaunch& L : it->second.launches) {
         float alpha, beta, beta2;
         launch_coefs(L, coeffs, per_step, &alpha, &beta, &beta2);
-        ProfScope ps(L.name, stream);
+        ProfScope ps(L.name.c_str(), stream);
         int rc = bucket_launch(plan, b, L.op, L.probs, alpha, beta, beta2, stream);
         if (rc) return rc;
       }

@@ -69,7 +69,7 @@ struct NsLaunch {
   int s0, s1;                  // step indices the coefficients come from
   GemmProblem* probs;          // device, one per matrix of the bucket
   int k_blocks, n_blocks;
-  const char* name;            // profiling family
+  std::string name;            // profiling name: family[m_pad x n_pad]
 };
 struct NsProgram {
   std::vector<NsLaunch> launches;
@@ -104,10 +104,6 @@ struct Plan {
   float *d_partials = nullptr, *d_inv_norm = nullptr;
   ElemTables tables{};
   std::string bound_key;               // schedule signature rec.O was last bound for
-  // staging for the _host entry point
-  uint8_t* stage = nullptr;            // W | G | M device copies
-  std::vector<size_t> stage_off;       // per matrix offset of W; G at +stage_third, M at +2*stage_third
-  size_t stage_third = 0;
   std::vector<void*> d_allocs;         // everything to cudaFree
   int sm_count = 148;
   ~Plan();

@@ -319,7 +319,12 @@ def test_profile_counts_launches():
     dm.muon_step(W, G, M, LR, MU, WD)
     prof = dm.profile_read()
     dm.set_option("profile", 0)
-    k = prof["kernels"]
+    k = {}
+    for name, rec in prof["kernels"].items():          # GEMM launches are named family[m x n] per shape bucket
+        f = k.setdefault(name.split("[")[0], {"launches": 0, "ms": 0.0})
+        f["launches"] += rec["launches"]
+        f["ms"] += rec["ms"]
+    assert prof["kernels"]["ns_bx_update[768x3072]"]["launches"] == 2 and prof["kernels"]["ns_bx_update[768x768]"]["launches"] == 5
     # bucket 768x768: 5 plain steps x (SYRK, polynomial, X update); bucket 768x3072: blocks [3, 2] = 2 SYRK, 5 polynomial
     # products, 3 (3 - 1) + 3 (2 - 1) = 9 Gram-space products, 2 X updates; + momentum, norms, normalise, apply
     assert k["ns_syrk_xxt"]["launches"] == 7 and k["ns_sq_poly"]["launches"] == 10 and k["ns_bx_update"]["launches"] == 7
