@@ -261,6 +261,8 @@ def run_ours(args):
     dm.set_option("mode", "tc")
     dm.set_option("steps", NS_STEPS)
     dm.set_option("profile", 1)
+    if args.variants:
+        dm.set_option("variants", args.variants)
     t_setup = time.perf_counter()
     if cfg == 1:
         _, W = synth.ns_inputs("cuda")
@@ -515,6 +517,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--layers", type=int, default=0, help="profiling aid: only the first L layers of the set (0 = all)")
     ap.add_argument("--sample-seconds", type=float, default=0.0, help="--impl reference: CPU seconds per step (0 = auto)")
+    ap.add_argument("--variants", default="", help="tuning aid: force tile configurations 'syrk,sq,bx' (-1 = tuned)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--power-probe", action="store_true", help="kernel throughput vs operand bit patterns (power cap)")

@@ -240,6 +240,14 @@ DMUON_API int dmuon_set_option(const char* key, const char* value) {
     else { set_error("option schedule: expected 'auto' or 'x', got '%s'", value); return DMUON_ERR_INVALID_ARG; }
     return DMUON_OK;
   }
+  if (k == "variants") {
+    int a, b, c;
+    char tail;
+    if (sscanf(value, " %d , %d , %d %c", &a, &b, &c, &tail) != 3 || a < -1 || b < -1 || c < -1 || a >= kNumVariants ||
+        b >= kNumVariants || c >= kNumVariants) { set_error("option variants: expected 'syrk,sq,bx' in -1..%d, got '%s'", kNumVariants - 1, value); return DMUON_ERR_INVALID_ARG; }
+    g_opt.force_variant[0] = a; g_opt.force_variant[1] = b; g_opt.force_variant[2] = c;
+    return DMUON_OK;
+  }
   if (k == "cache_path") { g_opt.cache_path = v; g_opt.cache_path_set = true; return DMUON_OK; }
   set_error("dmuon_set_option: unknown key '%s'", key);
   return DMUON_ERR_INVALID_ARG;

@@ -166,7 +166,9 @@ int autotune_bucket(Plan& plan, BucketPlan& b, const Options& opt, cudaStream_t 
     snprintf(key, sizeof key, "%d %d %d %d", op, b.m_pad, b.n_pad, static_cast<int>(b.mats.size()));
     auto it = g_tune_cache.find(key);
     int best = 0;
-    if (it != g_tune_cache.end()) {
+    if (opt.force_variant[op] >= 0 && variant_valid(static_cast<GemmOp>(op), opt.force_variant[op])) {
+      best = opt.force_variant[op];
+    } else if (it != g_tune_cache.end()) {
       best = it->second;
     } else if (opt.autotune) {
       cudaEvent_t e0, e1;

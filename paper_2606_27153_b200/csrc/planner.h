@@ -20,6 +20,7 @@ struct Options {
   std::string cache_path;       // resolved lazily
   bool cache_path_set = false;
   float eps = 1e-7f;
+  int force_variant[3] = {-1, -1, -1};   // per tiling op (SYRK, SQ, BX): -1 = tuned, else this tile configuration
   bool gram_blocks = true;      // schedule "auto": Gram blocks (Eq. 4) on wide buckets; false = plain X iteration
 };
 
