@@ -82,6 +82,17 @@ DMUON_API int dmuon_muon_step(void* const* params, const void* const* grads, voi
                               dmuon_stream_t stream);
 
 /*
+ * The Muon step with fp32 master weights ("the orthogonalized update is cast to fp32 and applied to the
+ * fp32 master weights, and then cast back to the parameter's working dtype").  As dmuon_muon_step, but the update
+ *     master' = master - lr * (sqrt(max(1, rows/cols)) * O + wd * master)       (fp32, one expression)
+ * is applied to masters[i] (DEVICE fp32, row-major, contiguous, 32-byte aligned, updated in place) and params[i] (bf16)
+ * is OVERWRITTEN with the round-to-nearest-even bf16 of the new master; its previous contents are not read.
+ */
+DMUON_API int dmuon_muon_step_master(void* const* params, void* const* masters, const void* const* grads,
+                                     void* const* momenta, const int32_t* shapes, int32_t count, float lr, float mu,
+                                     float wd, dmuon_stream_t stream);
+
+/*
  * The same step for tensors that live in HOST memory (pinned memory gives asynchronous copies): copies W, G, M of
  * every matrix to device staging buffers owned by the library, runs dmuon_muon_step there, and copies W and M
  * back.  The matrix list is processed in up to 8 groups of whole repetitions of its shape pattern (layers), so that

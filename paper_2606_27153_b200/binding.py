@@ -25,7 +25,7 @@ OP_SYRK, OP_SQ, OP_BX = 0, 1, 2
 SYMBOLS = ("dmuon_ns_batched", "dmuon_ns_batched_sched", "dmuon_muon_step", "dmuon_muon_step_host", "dmuon_warmup",
            "dmuon_workspace_bytes", "dmuon_set_workspace", "dmuon_set_option", "dmuon_last_error",
            "dmuon_profile_read", "dmuon_profile_reset", "dmuon_ns_gemm", "dmuon_ns_gemm_variants", "dmuon_read_ns_output", "dmuon_shutdown",
-           "dmuon_version", "dmuon_describe_plan", "dmuon_ns_sym_mm", "dmuon_block_schedule")
+           "dmuon_version", "dmuon_describe_plan", "dmuon_ns_sym_mm", "dmuon_block_schedule", "dmuon_muon_step_master")
 
 
 class DmuonError(RuntimeError):
@@ -52,6 +52,7 @@ def lib() -> ctypes.CDLL:
         L.dmuon_ns_batched.argtypes = [pp, pi, i32, i32, pf, vp]
         L.dmuon_ns_batched_sched.argtypes = [pp, pi, i32, i32, pf, vp]
         L.dmuon_muon_step.argtypes = [pp, pp, pp, pi, i32, f32, f32, f32, vp]
+        L.dmuon_muon_step_master.argtypes = [pp, pp, pp, pp, pi, i32, f32, f32, f32, vp]
         L.dmuon_muon_step_host.argtypes = [pp, pp, pp, pi, i32, f32, f32, f32, vp]
         L.dmuon_warmup.argtypes = [pi, i32, vp]
         L.dmuon_workspace_bytes.argtypes = [pi, i32]
@@ -150,6 +151,21 @@ def muon_step(params: Sequence[torch.Tensor], grads: Sequence[torch.Tensor], mom
     shp, n = _shape_array([t.shape for t in params])
     _check(lib().dmuon_muon_step(_ptr_array(params), _ptr_array(grads), _ptr_array(momenta), shp, n, float(lr),
                                  float(mu), float(wd), _stream(stream)))
+
+
+def muon_step_master(params: Sequence[torch.Tensor], masters: Sequence[torch.Tensor], grads: Sequence[torch.Tensor],
+                     momenta: Sequence[torch.Tensor], lr: float, mu: float, wd: float, stream=None) -> None:
+    """dmuon_muon_step_master: fp32 masters and momenta updated in place, params overwritten with bf16(master)."""
+    if not (len(params) == len(masters) == len(grads) == len(momenta)):
+        raise ValueError("params, masters, grads, momenta must have one length")
+    for name, ts in (("params", params), ("grads", grads), ("momenta", momenta)):
+        _check_mats(ts, "cuda", name)
+    for i, (p, w) in enumerate(zip(params, masters)):
+        if w.dtype != torch.float32 or not w.is_contiguous() or w.device.type != "cuda" or w.shape != p.shape:
+            raise ValueError(f"masters[{i}] must be a contiguous float32 cuda tensor of the parameter's shape")
+    shp, n = _shape_array([t.shape for t in params])
+    _check(lib().dmuon_muon_step_master(_ptr_array(params), _ptr_array(masters), _ptr_array(grads), _ptr_array(momenta),
+                                        shp, n, float(lr), float(mu), float(wd), _stream(stream)))
 
 
 def muon_step_host(params: Sequence[torch.Tensor], grads: Sequence[torch.Tensor], momenta: Sequence[torch.Tensor],

@@ -76,7 +76,7 @@ int validate(const void* const* a, const void* const* b, const void* const* c, c
 
 // Patch the per-call pointers into the plan's records and upload them if anything changed.
 int bind_pointers(Plan& plan, void* const* w, const void* const* g, void* const* m, int steps, const float* coeffs,
-                  bool per_step, cudaStream_t stream) {
+                  bool per_step, cudaStream_t stream, void* const* masters = nullptr) {
   const int count = static_cast<int>(plan.mats.size());
   bool dirty = false;
   std::vector<int> parity(plan.buckets.size());
@@ -86,7 +86,9 @@ int bind_pointers(Plan& plan, void* const* w, const void* const* g, void* const*
     MatRec& r = plan.h_recs[i];
     void* gi = g ? const_cast<void*>(g[i]) : nullptr;
     void* mi = m ? m[i] : nullptr;
-    if (r.W != w[i] || r.G != gi || r.M != mi) dirty = true;
+    float* w32 = masters ? static_cast<float*>(masters[i]) : nullptr;
+    if (r.W != w[i] || r.G != gi || r.M != mi || r.W32 != w32) dirty = true;
+    r.W32 = w32;
     r.W = w[i];
     r.G = gi;
     r.M = mi;
@@ -101,13 +103,14 @@ int bind_pointers(Plan& plan, void* const* w, const void* const* g, void* const*
 }
 
 int muon_step_device(void* const* params, const void* const* grads, void* const* momenta, const int32_t* shapes,
-                     int32_t count, float lr, float mu, float wd, cudaStream_t stream, Plan** plan_out) {
+                     int32_t count, float lr, float mu, float wd, cudaStream_t stream, Plan** plan_out,
+                     void* const* masters = nullptr) {
   Plan* plan = nullptr;
   int rc = get_plan(shapes, count, g_opt, g_ext_ws, g_ext_ws_bytes, stream, &plan);
   if (rc) return rc;
   if (plan_out) *plan_out = plan;
   g_last_plan = plan;
-  if ((rc = bind_pointers(*plan, params, grads, momenta, g_opt.steps, g_opt.coeffs, false, stream))) return rc;
+  if ((rc = bind_pointers(*plan, params, grads, momenta, g_opt.steps, g_opt.coeffs, false, stream, masters))) return rc;
   const ElemTables& T = plan->tables;
   if ((rc = launch_momentum(T, mu, stream))) return rc;
   if ((rc = launch_finalize_norms(T, g_opt.eps, stream))) return rc;
@@ -271,6 +274,20 @@ DMUON_API int dmuon_muon_step(void* const* params, const void* const* grads, voi
   if (rc || count == 0) return rc;
   if (!grads || !momenta) { set_error("dmuon_muon_step: null argument"); return DMUON_ERR_INVALID_ARG; }
   return muon_step_device(params, grads, momenta, shapes, count, lr, mu, wd, reinterpret_cast<cudaStream_t>(stream), nullptr);
+}
+
+DMUON_API int dmuon_muon_step_master(void* const* params, void* const* masters, const void* const* grads,
+                                     void* const* momenta, const int32_t* shapes, int32_t count, float lr, float mu,
+                                     float wd, dmuon_stream_t stream) {
+  int rc = validate(reinterpret_cast<const void* const*>(params), grads, reinterpret_cast<const void* const*>(momenta),
+                    shapes, count, "dmuon_muon_step_master");
+  if (rc || count == 0) return rc;
+  if (!grads || !momenta || !masters) { set_error("dmuon_muon_step_master: null argument"); return DMUON_ERR_INVALID_ARG; }
+  for (int i = 0; i < count; ++i) {
+    if (!masters[i]) { set_error("dmuon_muon_step_master: matrix %d has a null master pointer", i); return DMUON_ERR_INVALID_ARG; }
+    if (reinterpret_cast<uintptr_t>(masters[i]) & 31) { set_error("dmuon_muon_step_master: master %d (%p) is not 32-byte aligned", i, masters[i]); return DMUON_ERR_INVALID_ARG; }
+  }
+  return muon_step_device(params, grads, momenta, shapes, count, lr, mu, wd, reinterpret_cast<cudaStream_t>(stream), nullptr, masters);
 }
 
 // Host-buffer entry: the matrix list is cut into groups of whole periods of its shape pattern (a transformer's layers),

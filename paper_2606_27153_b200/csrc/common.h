@@ -82,6 +82,7 @@ struct MatRec {
   void* W;              // bf16 parameter (muon) / in-out matrix (ns)
   const void* G;        // bf16 gradient (muon)
   void* M;              // bf16 momentum (muon)
+  float* W32;           // fp32 master copy of W (dmuon_muon_step_master) or null
   void* U;              // bf16 staging of U, rows*cols, stored orientation (muon); unused (ns)
   void* X0;             // internal buffer receiving the normalised, oriented, padded X0 (fp16 or fp32)
   const void* O;        // internal buffer holding NS_k(X0), oriented + padded

@@ -328,7 +328,16 @@ __global__ void __launch_bounds__(kThreads) apply_kernel(const MatRec* __restric
         Load8<T>::run(O + static_cast<int64_t>(R) * rec.n_pad + C, o);
       }
       uint16_t* wp = W + static_cast<int64_t>(R) * rec.cols + C;
-      if (vec_ok && C + 8 <= rec.cols) {
+      if (kApply && rec.W32 != nullptr) {
+        // fp32 master weights: the update is applied to the master, W is its bf16 rounding
+        float* mp = rec.W32 + static_cast<int64_t>(R) * rec.cols + C;
+        for (int e = 0; e < 8 && C + e < rec.cols; ++e) {
+          const float w0 = mp[e];
+          const float w1 = w0 - fmaf(s_o, o[e], lr * wd * w0);
+          mp[e] = w1;
+          wp[e] = static_cast<uint16_t>(float_to_bf16_bits(w1));
+        }
+      } else if (vec_ok && C + 8 <= rec.cols) {
         float w[8];
         if (kApply) {
           unpack8(*reinterpret_cast<const uint4*>(wp), w);
@@ -370,6 +379,25 @@ __device__ __forceinline__ uint32_t apply_word(uint32_t w_bits, uint32_t o_bits,
   const float2 o = half2_bits_to_float2(o_bits);
   const float2 t = __ffma2_rn(so2, o, __fmul2_rn(lrwd2, w));
   return float2_to_bf16x2(__ffma2_rn(make_float2(-1.f, -1.f), t, w));      // w - t, one rounding
+}
+
+// 8 consecutive elements with fp32 master weights: the update is applied to the master in fp32, the
+// bf16 parameter is the rounding of the new master.  o4: 8 fp16 values of O; mp: 8 floats of the master (32-byte aligned).
+__device__ __forceinline__ uint4 apply8_master(float* __restrict__ mp, const uint4& o4, float2 so2, float2 lrwd2) {
+  const float4 m0 = *reinterpret_cast<const float4*>(mp), m1 = *reinterpret_cast<const float4*>(mp + 4);
+  const float2 w[4] = {make_float2(m0.x, m0.y), make_float2(m0.z, m0.w), make_float2(m1.x, m1.y), make_float2(m1.z, m1.w)};
+  const uint32_t ow[4] = {o4.x, o4.y, o4.z, o4.w};
+  float2 n[4];
+  uint32_t r[4];
+#pragma unroll
+  for (int e = 0; e < 4; ++e) {
+    const float2 t = __ffma2_rn(so2, half2_bits_to_float2(ow[e]), __fmul2_rn(lrwd2, w[e]));
+    n[e] = __ffma2_rn(make_float2(-1.f, -1.f), t, w[e]);
+    r[e] = float2_to_bf16x2(n[e]);
+  }
+  *reinterpret_cast<float4*>(mp) = make_float4(n[0].x, n[0].y, n[1].x, n[1].y);
+  *reinterpret_cast<float4*>(mp + 4) = make_float4(n[2].x, n[2].y, n[3].x, n[3].y);
+  return make_uint4(r[0], r[1], r[2], r[3]);
 }
 
 template <bool kFromUser>
@@ -414,6 +442,17 @@ __global__ void __launch_bounds__(kThreads) apply_flat_kernel(const MatRec* __re
     const float so = lr * rec.scale, lrwd = lr * wd;
     const float2 so2 = make_float2(so, so), lrwd2 = make_float2(lrwd, lrwd);
     uint4 o4[kIter], w4[kIter];
+    if (kApply && rec.W32 != nullptr) {
+      float* __restrict__ M32 = rec.W32 + start;
+#pragma unroll
+      for (int it = 0; it < kIter; ++it) o4[it] = __ldcs(reinterpret_cast<const uint4*>(O + (it * kThreads + threadIdx.x) * 8));
+#pragma unroll
+      for (int it = 0; it < kIter; ++it) {
+        const int off = (it * kThreads + threadIdx.x) * 8;
+        *reinterpret_cast<uint4*>(W + off) = apply8_master(M32 + off, o4[it], so2, lrwd2);
+      }
+      continue;
+    }
 #pragma unroll
     for (int it = 0; it < kIter; ++it) {
       const int off = (it * kThreads + threadIdx.x) * 8;
@@ -516,7 +555,8 @@ __global__ void __launch_bounds__(kThreads) apply_tr_kernel(const MatRec* __rest
     const float2 so2 = make_float2(so, so), lrwd2 = make_float2(lrwd, lrwd);
     // O(R, C) = Obuf[C][R]: the source tile is Obuf rows tC*64.., columns tR*64.. (leading dimension n_pad = rows)
     uint4 w4[2];
-    if (kApply) {
+    const bool master = kApply && rec.W32 != nullptr;
+    if (kApply && !master) {
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
         const int64_t R = tR * kTile + (threadIdx.x >> 3) + 32 * h, C = tC * kTile + (threadIdx.x & 7) * 8;
@@ -527,13 +567,17 @@ __global__ void __launch_bounds__(kThreads) apply_tr_kernel(const MatRec* __rest
     transpose_tile16(O + static_cast<int64_t>(tC) * kTile * rec.n_pad + tR * kTile, rec.n_pad, tile, v);
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
+      const int64_t R = tR * kTile + (threadIdx.x >> 3) + 32 * h, C = tC * kTile + (threadIdx.x & 7) * 8;
+      if (master) {
+        *reinterpret_cast<uint4*>(W + R * rec.cols + C) = apply8_master(rec.W32 + R * rec.cols + C, v[h], so2, lrwd2);
+        continue;
+      }
       const uint32_t ow[4] = {v[h].x, v[h].y, v[h].z, v[h].w};
       const uint32_t ww[4] = {w4[h].x, w4[h].y, w4[h].z, w4[h].w};
       uint32_t r[4];
 #pragma unroll
       for (int e = 0; e < 4; ++e)
         r[e] = kApply ? apply_word(ww[e], ow[e], so2, lrwd2) : float2_to_bf16x2(half2_bits_to_float2(ow[e]));
-      const int64_t R = tR * kTile + (threadIdx.x >> 3) + 32 * h, C = tC * kTile + (threadIdx.x & 7) * 8;
       *reinterpret_cast<uint4*>(W + R * rec.cols + C) = make_uint4(r[0], r[1], r[2], r[3]);
     }
   }

@@ -62,6 +62,8 @@ def test_invalid_arguments_rejected_before_any_device_work():
     assert L.dmuon_ns_gemm(0, ptrs, None, ptrs, 100, 128, 1, 1.0, 0.0, -1, None) == binding.ERR_INVALID_ARG
     assert L.dmuon_set_workspace(ctypes.c_void_p(0x1000), 0) == binding.ERR_INVALID_ARG
     assert L.dmuon_read_ns_output(0, None, None) == binding.ERR_INVALID_ARG
+    assert L.dmuon_muon_step_master(ptrs, None, ptrs, ptrs, shapes, 1, 0.02, 0.95, 0.01, None) == binding.ERR_INVALID_ARG
+    assert L.dmuon_muon_step_master(None, None, None, None, None, 0, 0.02, 0.95, 0.01, None) == binding.OK
 
 
 @pytest.mark.skipif(torch.cuda.is_available(), reason="only meaningful on a box without a GPU")

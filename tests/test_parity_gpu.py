@@ -262,6 +262,45 @@ def test_zero_gradient_muon_step():
     assert torch.count_nonzero(m).item() == 0
 
 
+def test_master_weights_step():
+    """dmuon_muon_step_master: the update lands in the fp32 master; the bf16 parameter is its rounding.
+    Covers the flat, the transposing and the generic (ragged) apply paths.  With a master the UPDATE itself is
+    checked to the NS tolerance, which bf16 weights cannot show (their rounding swamps a 1-5 ulp update)."""
+    shapes = [(768, 768), (3072, 768), (768, 3072), (100, 260), (130, 70)]
+    G = [synth.gradient(s, 7500 + i, "cuda") for i, s in enumerate(shapes)]
+    M = [synth.gradient(s, 7600 + i, "cuda") for i, s in enumerate(shapes)]
+    W32 = []
+    for i, s in enumerate(shapes):
+        g = torch.Generator(device="cuda")
+        g.manual_seed(7700 + i)
+        W32.append((torch.randn(s, generator=g, device="cuda", dtype=torch.float32) * 0.02).contiguous())   # not bf16-representable
+    W = [torch.full(s, float("nan"), dtype=torch.bfloat16, device="cuda") for s in shapes]   # must be overwritten, never read
+    W0 = [to64(w) for w in W32]
+    M0 = [to64(m) for m in M]
+    dm.muon_step_master(W, W32, G, M, LR, MU, WD)
+    torch.cuda.synchronize()
+    for i, s in enumerate(shapes):
+        orc = oracle.muon_step(W0[i], to64(G[i]), M0[i], LR_F, MU_F, WD_F, momentum_fp32=True)
+        assert torch.equal(W[i], W32[i].to(torch.bfloat16)), f"{s}: bf16 parameter is not the rounding of the master"
+        assert np.array_equal(to64(M[i]), oracle.round_bf16(orc["M_new"])), f"{s}: M' differs"
+        upd_orc = orc["W_new"] - W0[i]
+        upd_gpu = to64(W32[i]) - W0[i]
+        e = np.linalg.norm(upd_gpu - upd_orc) / np.linalg.norm(upd_orc)
+        # fp32 rounding of a weight of size 0.02 is ~1e-9, the update per element ~1e-4..1e-3: negligible next to TOL_TC
+        assert e <= TOL_TC + 1e-4, f"{s}: relative error of the applied update {e:.3e}"
+    with pytest.raises(dm.DmuonError):                                  # misaligned master
+        buf = torch.zeros(128 * 128 + 4, dtype=torch.float32, device="cuda")
+        dm.binding._check(dm.binding.lib().dmuon_muon_step_master(
+            dm.binding._ptr_array([W[0][:128, :128].contiguous()]), dm.binding._ptr_array([buf[1:1 + 128 * 128]]),
+            dm.binding._ptr_array([G[0][:128, :128].contiguous()]), dm.binding._ptr_array([M[0][:128, :128].contiguous()]),
+            dm.binding._shape_array([(128, 128)])[0], 1, 0.02, 0.95, 0.01, None))
+    # a following plain step on the same shapes must not touch the masters (the binding is per call)
+    keep = [w.clone() for w in W32]
+    dm.muon_step(W, G, M, LR, MU, WD)
+    torch.cuda.synchronize()
+    assert all(torch.equal(a, b) for a, b in zip(keep, W32))
+
+
 def test_two_steps_state_carried():
     """Two consecutive steps; the oracle restarts each step from the GPU's bf16 state (DESIGN.md parity rules)."""
     shapes, W, G, M = synth.muon_inputs(2, "cuda", False, indices=[0, 4, 5])
