@@ -116,7 +116,7 @@ int muon_step_device(void* const* params, const void* const* grads, void* const*
   if ((rc = launch_finalize_norms(T, g_opt.eps, stream))) return rc;
   if ((rc = launch_normalize(T, /*from_user=*/false, plan->fp32, stream))) return rc;
   if ((rc = run_ns_steps(*plan, g_opt.steps, g_opt.coeffs, false, g_opt, stream))) return rc;
-  if ((rc = launch_apply(T, lr, wd, plan->fp32, stream))) return rc;
+  if ((rc = launch_apply(T, lr, wd, plan->fp32, masters != nullptr, stream))) return rc;
   return DMUON_OK;
 }
 

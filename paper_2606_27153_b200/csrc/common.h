@@ -119,7 +119,7 @@ int launch_momentum(const ElemTables& T, float mu, cudaStream_t s);          // 
 int launch_sumsq(const ElemTables& T, cudaStream_t s);                       // a2 alone (ns_batched)
 int launch_finalize_norms(const ElemTables& T, float eps, cudaStream_t s);
 int launch_normalize(const ElemTables& T, bool from_user, bool fp32_internal, cudaStream_t s);
-int launch_apply(const ElemTables& T, float lr, float wd, bool fp32_internal, cudaStream_t s);   // a6
+int launch_apply(const ElemTables& T, float lr, float wd, bool fp32_internal, bool master, cudaStream_t s);   // a6
 int launch_store_ns(const ElemTables& T, bool fp32_internal, cudaStream_t s);                    // ns_batched output
 
 int launch_export(const void* O, float* out, int rows, int cols, int n_pad, bool transposed, bool fp32_internal,

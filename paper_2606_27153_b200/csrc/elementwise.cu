@@ -428,7 +428,7 @@ __global__ void __launch_bounds__(kThreads) normalize_flat_kernel(const MatRec* 
   }
 }
 
-template <bool kApply>
+template <bool kApply, bool kMaster>
 __global__ void __launch_bounds__(kThreads) apply_flat_kernel(const MatRec* __restrict__ recs,
                                                               const int64_t* __restrict__ prefix, int count,
                                                               int64_t total_chunks, float lr, float wd) {
@@ -442,7 +442,7 @@ __global__ void __launch_bounds__(kThreads) apply_flat_kernel(const MatRec* __re
     const float so = lr * rec.scale, lrwd = lr * wd;
     const float2 so2 = make_float2(so, so), lrwd2 = make_float2(lrwd, lrwd);
     uint4 o4[kIter], w4[kIter];
-    if (kApply && rec.W32 != nullptr) {
+    if (kMaster) {
       float* __restrict__ M32 = rec.W32 + start;
 #pragma unroll
       for (int it = 0; it < kIter; ++it) o4[it] = __ldcs(reinterpret_cast<const uint4*>(O + (it * kThreads + threadIdx.x) * 8));
@@ -538,7 +538,7 @@ __global__ void __launch_bounds__(kThreads) normalize_tr_kernel(const MatRec* __
   }
 }
 
-template <bool kApply>
+template <bool kApply, bool kMaster>
 __global__ void __launch_bounds__(kThreads) apply_tr_kernel(const MatRec* __restrict__ recs,
                                                             const int64_t* __restrict__ prefix, int count,
                                                             int64_t total_tiles, float lr, float wd) {
@@ -555,7 +555,7 @@ __global__ void __launch_bounds__(kThreads) apply_tr_kernel(const MatRec* __rest
     const float2 so2 = make_float2(so, so), lrwd2 = make_float2(lrwd, lrwd);
     // O(R, C) = Obuf[C][R]: the source tile is Obuf rows tC*64.., columns tR*64.. (leading dimension n_pad = rows)
     uint4 w4[2];
-    const bool master = kApply && rec.W32 != nullptr;
+    constexpr bool master = kMaster;
     if (kApply && !master) {
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
@@ -691,15 +691,17 @@ int launch_normalize(const ElemTables& T, bool from_user, bool fp32_internal, cu
   return DMUON_OK;
 }
 
-int launch_apply(const ElemTables& T, float lr, float wd, bool fp32_internal, cudaStream_t s) {
+int launch_apply(const ElemTables& T, float lr, float wd, bool fp32_internal, bool master, cudaStream_t s) {
   if (T.tiles + T.fa_chunks + T.fb_tiles == 0) return DMUON_OK;
   if (T.fa_chunks > 0) {
     ProfScope ps("apply_update", s);
-    apply_flat_kernel<true><<<grid_for(T.fa_chunks, 8), kThreads, 0, s>>>(T.recs, T.fa_prefix, T.count, T.fa_chunks, lr, wd);
+    if (master) apply_flat_kernel<true, true><<<grid_for(T.fa_chunks, 8), kThreads, 0, s>>>(T.recs, T.fa_prefix, T.count, T.fa_chunks, lr, wd);
+    else apply_flat_kernel<true, false><<<grid_for(T.fa_chunks, 8), kThreads, 0, s>>>(T.recs, T.fa_prefix, T.count, T.fa_chunks, lr, wd);
   }
   if (T.fb_tiles > 0) {
     ProfScope ps("apply_update", s);
-    apply_tr_kernel<true><<<grid_for(T.fb_tiles, 8), kThreads, 0, s>>>(T.recs, T.fb_prefix, T.count, T.fb_tiles, lr, wd);
+    if (master) apply_tr_kernel<true, true><<<grid_for(T.fb_tiles, 8), kThreads, 0, s>>>(T.recs, T.fb_prefix, T.count, T.fb_tiles, lr, wd);
+    else apply_tr_kernel<true, false><<<grid_for(T.fb_tiles, 8), kThreads, 0, s>>>(T.recs, T.fb_prefix, T.count, T.fb_tiles, lr, wd);
   }
   DMUON_CUDA_CHECK(cudaGetLastError());
   if (T.tiles == 0) return DMUON_OK;
@@ -715,11 +717,11 @@ int launch_store_ns(const ElemTables& T, bool fp32_internal, cudaStream_t s) {
   if (T.tiles + T.fa_chunks + T.fb_tiles == 0) return DMUON_OK;
   if (T.fa_chunks > 0) {
     ProfScope ps("store_ns_output", s);
-    apply_flat_kernel<false><<<grid_for(T.fa_chunks, 8), kThreads, 0, s>>>(T.recs, T.fa_prefix, T.count, T.fa_chunks, 0.f, 0.f);
+    apply_flat_kernel<false, false><<<grid_for(T.fa_chunks, 8), kThreads, 0, s>>>(T.recs, T.fa_prefix, T.count, T.fa_chunks, 0.f, 0.f);
   }
   if (T.fb_tiles > 0) {
     ProfScope ps("store_ns_output", s);
-    apply_tr_kernel<false><<<grid_for(T.fb_tiles, 8), kThreads, 0, s>>>(T.recs, T.fb_prefix, T.count, T.fb_tiles, 0.f, 0.f);
+    apply_tr_kernel<false, false><<<grid_for(T.fb_tiles, 8), kThreads, 0, s>>>(T.recs, T.fb_prefix, T.count, T.fb_tiles, 0.f, 0.f);
   }
   DMUON_CUDA_CHECK(cudaGetLastError());
   if (T.tiles == 0) return DMUON_OK;
