@@ -484,6 +484,31 @@ def run_sweep(args):
         del Xs, big
         dm.shutdown()
         torch.cuda.empty_cache()
+    # PAPER.md:188 (Fig. 7): per-matrix NS time against the number of same-shape matrices advanced together
+    for (r, c) in ((1024, 1024), (2048, 22016)):
+        base = None
+        for b in (1, 2, 4, 8, 16, 32):
+            g = torch.Generator(device="cuda")
+            g.manual_seed(5100 + b)
+            big = torch.randn((b, r, c), generator=g, device="cuda", dtype=torch.float32).to(torch.bfloat16)
+            Xs = [big[i] for i in range(b)]
+            for _ in range(3):
+                dm.ns_batched(Xs, steps=NS_STEPS)
+            reps = 20 if r == 1024 else 5
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record()
+            for _ in range(reps):
+                dm.ns_batched(Xs, steps=NS_STEPS)
+            e1.record()
+            torch.cuda.synchronize()
+            per = e0.elapsed_time(e1) / reps / b
+            base = base or per
+            print(json.dumps({"sweep": "batching", "shape": [r, c], "batch": b, "ms_per_matrix": per,
+                              "speedup_vs_batch1": base / per}), flush=True)
+            del Xs, big
+            dm.shutdown()
+            torch.cuda.empty_cache()
 
 
 def run_power_probe(args):

@@ -172,6 +172,7 @@ def test_config4_full_size_sampled():
     idx = [1, 218]
     W0 = {i: to64(W[i]) for i in idx}
     keep = {i: (W[i].clone(), G[i].clone(), M[i].clone()) for i in (0, 6)}
+    pre = {i: (W[i].clone(), M[i].clone()) for i in (0, 4, 6)}
     dm.muon_step(W, G, M, LR, MU, WD)
     torch.cuda.synchronize()
     for i in idx:
@@ -195,6 +196,21 @@ def test_config4_full_size_sampled():
         assert d.mean().item() <= 1e-2 and d.max().item() <= 5e-2
         big[i] = og
         del u, s, sv
+        # elementwise at full size: M' against the oracle's momentum (steps = 0 skips its NS; M' does not depend on it),
+        # bit for bit; W' against the update formula applied to the kernel's own O (flat / transposing apply paths),
+        # within one bf16 ulp (one fp32 expression and one rounding on the GPU, fp64 here)
+        w_pre, m_pre = pre[i]
+        m_orc = oracle.muon_step(to64(w_pre), to64(G[i]), to64(m_pre), LR_F, MU_F, WD_F, steps=0, momentum_fp32=True)["M_new"]
+        assert np.array_equal(to64(M[i]), oracle.round_bf16(m_orc)), f"config4 matrix {i}: M' differs"
+        del m_orc
+        scale = max(1.0, shapes[i][0] / shapes[i][1]) ** 0.5
+        w64 = w_pre.double()
+        want = w64 - LR_F * (float(np.float32(scale)) * og.double() + WD_F * w64)
+        diff = (W[i].double() - want).abs()
+        ulp = torch.pow(2.0, torch.floor(torch.log2(want.abs().clamp_min(2.0 ** -126))) - 7)
+        assert (diff <= 1.001 * ulp).all(), f"config4 matrix {i}: W' off by more than one bf16 ulp"
+        assert (diff <= 0.501 * ulp).double().mean().item() > 0.999      # and correctly rounded almost everywhere
+        del w64, want, diff, ulp
     del W, G, M
     torch.cuda.empty_cache()
     dm.shutdown()
