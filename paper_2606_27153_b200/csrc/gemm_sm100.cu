@@ -59,27 +59,38 @@ template <bool kPair> constexpr int smem_bytes() {
 }
 
 // ------------------------------------------------------------------------------------------------ epilogue
+// Addend words of one 32-column chunk of one row: 64 bytes of D (and of D2 for OP_SQ2).  Loaded one chunk ahead of the
+// arithmetic (two register sets, alternating) so that their L2 latency overlaps the TMEM load and the stores of the
+// previous chunk: with short contractions (K <= 1024) the epilogue, not the mainloop, sets the pace.
+struct Addends {
+  uint4 d[4];
+  uint4 e[4];
+};
+template <int kOp>
+__device__ __forceinline__ void load_addends(Addends& a, const __half* __restrict__ D, const __half* __restrict__ D2,
+                                             int64_t ldc, int64_t grow, int64_t gcol) {
+  if (kOp == OP_SYRK) return;
+  const uint4* dp = reinterpret_cast<const uint4*>(D + grow * ldc + gcol);
+#pragma unroll
+  for (int g = 0; g < 4; ++g) a.d[g] = __ldg(dp + g);
+  if (kOp == OP_SQ2) {
+    const uint4* ep = reinterpret_cast<const uint4*>(D2 + grow * ldc + gcol);
+#pragma unroll
+    for (int g = 0; g < 4; ++g) a.e[g] = __ldg(ep + g);
+  }
+}
+
 // One 32-column chunk of one accumulator row: v = 32 fp32 accumulators of row `grow`, columns [gcol, gcol + 32).
 template <int kOp>
-__device__ __forceinline__ void epilogue_chunk(const uint32_t (&v)[32], __half* __restrict__ C,
-                                               const __half* __restrict__ D, const __half* __restrict__ D2,
+__device__ __forceinline__ void epilogue_chunk(const uint32_t (&v)[32], const Addends& a, __half* __restrict__ C,
                                                int64_t ldc, int64_t grow, int64_t gcol, float alpha, float beta,
                                                float beta2, bool mirror) {
   uint32_t o[16];
   if (kOp != OP_SYRK) {
-    const uint4* dp = reinterpret_cast<const uint4*>(D + grow * ldc + gcol);
-    uint4 d4[4], e4[4] = {};
-#pragma unroll
-    for (int g = 0; g < 4; ++g) d4[g] = __ldg(dp + g);
-    if (kOp == OP_SQ2) {
-      const uint4* ep = reinterpret_cast<const uint4*>(D2 + grow * ldc + gcol);
-#pragma unroll
-      for (int g = 0; g < 4; ++g) e4[g] = __ldg(ep + g);
-    }
 #pragma unroll
     for (int g = 0; g < 4; ++g) {
-      const uint32_t dw[4] = {d4[g].x, d4[g].y, d4[g].z, d4[g].w};
-      const uint32_t ew[4] = {e4[g].x, e4[g].y, e4[g].z, e4[g].w};
+      const uint32_t dw[4] = {a.d[g].x, a.d[g].y, a.d[g].z, a.d[g].w};
+      const uint32_t ew[4] = {a.e[g].x, a.e[g].y, a.e[g].z, a.e[g].w};
 #pragma unroll
       for (int e = 0; e < 4; ++e) {
         const float2 df = __half22float2(*reinterpret_cast<const __half2*>(&dw[e]));
@@ -171,6 +182,15 @@ __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ pro
         const GemmProblem* pr = probs + p;
         const uint64_t tmA = reinterpret_cast<uint64_t>(&pr->tmA);
         const uint64_t tmB = reinterpret_cast<uint64_t>(&pr->tmB);
+        // the next unit of this worker usually belongs to another matrix: fetch its descriptors ahead of use
+        const int un = u + num_workers;
+        if (un < total_units) {
+          const int pn = un / units_per_problem;
+          if (pn != p) {
+            tma_prefetch_desc(reinterpret_cast<uint64_t>(&probs[pn].tmA));
+            tma_prefetch_desc(reinterpret_cast<uint64_t>(&probs[pn].tmB));
+          }
+        }
         const int a_blk = kPair ? 2 * tu.m_blk + static_cast<int>(rank) : tu.m_blk;      // this CTA's 128 rows of A
         const int b_blk = kPair ? 2 * tu.n_blk + static_cast<int>(rank) : tu.n_blk;      // its first 128 columns of B
         const int w = kPair ? 1 : tu.width;
@@ -259,18 +279,31 @@ __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ pro
       const int bi = kPair ? 2 * tu.m_blk + static_cast<int>(rank) : tu.m_blk;      // row block of this CTA
       const int bj0 = kPair ? 2 * tu.n_blk : tu.n_blk;                               // first column block
       const int nbk = kPair ? 2 : tu.width;
+      const int64_t grow = static_cast<int64_t>(bi) * kBlk + row;
+      const int64_t gcol0 = static_cast<int64_t>(bj0) * kBlk;
+      // chunks (32 columns each) this warp stores: inside the matrix and, for symmetric results, not left of the
+      // diagonal block (those blocks are written by the mirror of another unit)
+      int c_lo = 0, c_hi = 0;
+      if (bi < mb) {
+        c_lo = (kSym && bi > bj0) ? (bi - bj0) * 4 : 0;
+        c_hi = (nb - bj0 < nbk ? nb - bj0 : nbk) * 4;
+      }
+      Addends a0 = {}, a1 = {};
+      if (c_lo < c_hi) load_addends<kOp>(a0, D, D2, ldc, grow, gcol0 + c_lo * 32);   // before the accumulator is ready
       mbar_wait(bar_tfull + 8 * as, aphase);
       tcgen05_fence_after();
       const uint32_t taddr = tmem_base + as * kAccCols + (static_cast<uint32_t>(q * 32) << 16);
-      const int64_t grow = static_cast<int64_t>(bi) * kBlk + row;
-      if (bi < mb) {
-        for (int c = 0; c < nbk * 4; ++c) {
-          const int bj = bj0 + (c >> 2);
-          if (bj >= nb || (kSym && bj < bi)) continue;     // outside the matrix / lower triangle (mirrored elsewhere)
-          uint32_t v[32];
-          tmem_ld_32x32(taddr + c * 32, v);
+      for (int c = c_lo; c < c_hi; c += 2) {
+        uint32_t v[32];
+        if (c + 1 < c_hi) load_addends<kOp>(a1, D, D2, ldc, grow, gcol0 + (c + 1) * 32);
+        tmem_ld_32x32(taddr + c * 32, v);
+        tmem_wait_ld();
+        epilogue_chunk<kOp>(v, a0, C, ldc, grow, gcol0 + c * 32, alpha, beta, beta2, bj0 + (c >> 2) != bi);
+        if (c + 1 < c_hi) {
+          if (c + 2 < c_hi) load_addends<kOp>(a0, D, D2, ldc, grow, gcol0 + (c + 2) * 32);
+          tmem_ld_32x32(taddr + (c + 1) * 32, v);
           tmem_wait_ld();
-          epilogue_chunk<kOp>(v, C, D, D2, ldc, grow, static_cast<int64_t>(bj0) * kBlk + c * 32, alpha, beta, beta2, bj != bi);
+          epilogue_chunk<kOp>(v, a1, C, ldc, grow, gcol0 + (c + 1) * 32, alpha, beta, beta2, bj0 + ((c + 1) >> 2) != bi);
         }
       }
       // accumulator fully read by this warp: hand it back to the MMA thread

@@ -208,9 +208,11 @@ def test_config4_full_size_sampled():
         want = w64 - LR_F * (float(np.float32(scale)) * og.double() + WD_F * w64)
         diff = (W[i].double() - want).abs()
         ulp = torch.pow(2.0, torch.floor(torch.log2(want.abs().clamp_min(2.0 ** -126))) - 7)
-        assert (diff <= 1.001 * ulp).all(), f"config4 matrix {i}: W' off by more than one bf16 ulp"
-        assert (diff <= 0.501 * ulp).double().mean().item() > 0.999      # and correctly rounded almost everywhere
-        del w64, want, diff, ulp
+        # fp32 evaluation error of the GPU expression (matters only where w and the update cancel to a tiny W')
+        slack = 2.0 ** -22 * (w64.abs() + LR_F * scale * og.double().abs())
+        assert (diff <= 1.001 * ulp + slack).all(), f"config4 matrix {i}: W' off by more than one bf16 ulp"
+        assert (diff <= 0.501 * ulp + slack).double().mean().item() > 0.999      # correctly rounded almost everywhere
+        del w64, want, diff, ulp, slack
     del W, G, M
     torch.cuda.empty_cache()
     dm.shutdown()
