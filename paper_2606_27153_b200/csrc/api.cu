@@ -543,6 +543,7 @@ DMUON_API int dmuon_ns_gemm(int32_t op, const void* const* in0, const void* cons
   L.m_blocks = m / kBlk;
   L.n_blocks = (op == OP_BX ? n : m) / kBlk;
   L.pair = variant_config(variant < 0 ? 0 : variant).pair;
+  L.quad = variant_config(variant < 0 ? 0 : variant).quad;
   L.alpha = alpha;
   L.beta = beta;
   L.beta2 = 0.f;
@@ -589,6 +590,7 @@ DMUON_API int dmuon_ns_sym_mm(const void* const* a, const void* const* b, const 
   L.m_blocks = m / kBlk;
   L.n_blocks = m / kBlk;
   L.pair = cfg.pair;
+  L.quad = cfg.quad;
   L.alpha = alpha;
   L.beta = beta;
   L.beta2 = beta2;

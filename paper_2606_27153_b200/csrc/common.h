@@ -52,7 +52,9 @@ struct alignas(128) GemmProblem {
 static_assert(sizeof(GemmProblem) == 384, "GemmProblem layout");
 
 // One work unit of a problem.  Single-CTA tiling: block row, first block column, number of blocks (1 or 2), in
-// 128-blocks.  CTA-pair tiling: m_blk, n_blk index 256 x 256 units (width unused).
+// 128-blocks.  CTA-pair tiling: m_blk, n_blk index 256 x 256 units (width unused).  CTA-quad tiling: two 256 x 256
+// units, (m_blk, n_blk) for pair 0 and (width, flags) for pair 1, sharing a block row or a block column (both equal:
+// pair 1 shadows pair 0 and stores nothing -- the odd unit left over).
 struct TileUnit {
   int16_t m_blk, n_blk, width, flags;
 };
@@ -66,6 +68,7 @@ struct GemmLaunch {
   int k_blocks;                 // K / 64
   int m_blocks, n_blocks;       // extent of the output in 128-blocks
   bool pair;                    // CTA-pair (cta_group::2) tiling
+  bool quad = false;            // CTA quad: two pairs sharing one operand panel by TMA multicast (units hold both)
   float alpha, beta, beta2;
   int grid;                     // CTAs (<= #SM)
 };

@@ -112,7 +112,7 @@ void load_tune_cache(const std::string& path) {
     std::istringstream ss(line);
     std::string tag;
     int op, m, n, cnt, variant;
-    if (ss >> tag >> op >> m >> n >> cnt >> variant && tag == "v1" && variant >= 0 && variant < kNumVariants) {
+    if (ss >> tag >> op >> m >> n >> cnt >> variant && tag == "v2" && variant >= 0 && variant < kNumVariants) {
       char key[96];
       snprintf(key, sizeof key, "%d %d %d %d", op, m, n, cnt);
       g_tune_cache[key] = variant;
@@ -129,7 +129,7 @@ void save_tune_cache(const std::string& path) {
       if (i == dir.size() || dir[i] == '/') mkdir(dir.substr(0, i).c_str(), 0755);
   }
   std::ofstream out(path, std::ios::trunc);
-  for (auto& kv : g_tune_cache) out << "v1 " << kv.first << " " << kv.second << "\n";
+  for (auto& kv : g_tune_cache) out << "v2 " << kv.first << " " << kv.second << "\n";
 }
 
 inline int tiling_op(GemmOp op) { return op == OP_SQ2 ? OP_SQ : op; }   // SQ2 shares SQ's units and variant
@@ -149,6 +149,7 @@ int bucket_launch(const Plan& plan, const BucketPlan& b, GemmOp op, const GemmPr
   L.m_blocks = b.m_pad / kBlk;
   L.n_blocks = (op == OP_BX ? b.n_pad : b.m_pad) / kBlk;
   L.pair = pair;
+  L.quad = variant_config(variant_override >= 0 ? variant_override : b.variant[top]).quad;
   L.alpha = alpha;
   L.beta = beta;
   L.beta2 = beta2;
@@ -178,6 +179,10 @@ int autotune_bucket(Plan& plan, BucketPlan& b, const Options& opt, cudaStream_t 
       for (int v = 0; v < kNumVariants; ++v) {
         if (!variant_valid(static_cast<GemmOp>(op), v)) continue;
         const TileConfig cfg = variant_config(v);
+        // The quad tiling measured slower than the pair tiling on every bucket tried (TMA multicast at cluster size 4
+        // saves no L2 traffic over concurrent unicast loads, and only 33 clusters of 4 are co-resident on 148 SMs): it
+        // stays available through option "variants" but is not a tuning candidate.
+        if (cfg.quad) continue;
         std::vector<TileUnit> hu = make_units(static_cast<GemmOp>(op), b.m_pad / kBlk, b.n_pad / kBlk, cfg);
         TileUnit* du = nullptr;
         DMUON_CUDA_CHECK(cudaMalloc(&du, hu.size() * sizeof(TileUnit)));
@@ -231,6 +236,12 @@ Plan::~Plan() {
 
 TileConfig variant_config(int variant) {
   TileConfig c;
+  if (variant == 6) {
+    c.pair = true;
+    c.quad = true;
+    c.order = 1;
+    return c;
+  }
   if (variant >= 4) {
     c.pair = true;
     c.order = variant & 1;
@@ -243,12 +254,31 @@ TileConfig variant_config(int variant) {
 
 bool variant_valid(GemmOp op, int variant) {
   if (variant < 0 || variant >= kNumVariants) return false;
+  if (variant == 6) return true;
   return op == OP_BX || variant_config(variant).order == 0;   // symmetric ops have one ordering
 }
 
 std::vector<TileUnit> make_units(GemmOp op, int mb, int nb, const TileConfig& cfg) {
   std::vector<TileUnit> u;
   auto push = [&](int i, int j, int w) { u.push_back(TileUnit{static_cast<int16_t>(i), static_cast<int16_t>(j), static_cast<int16_t>(w), 0}); };
+  if (cfg.quad) {
+    // two 256 x 256 units per entry, sharing a block row (pairs along a row) or a block column (leftovers of rows
+    // with an odd number of units, paired down the last column); a final odd unit is paired with itself
+    const int MB = (mb + 1) / 2, NB = (nb + 1) / 2;
+    auto quad = [&](int m0, int n0, int m1, int n1) {
+      u.push_back(TileUnit{static_cast<int16_t>(m0), static_cast<int16_t>(n0), static_cast<int16_t>(m1), static_cast<int16_t>(n1)});
+    };
+    const int ncols = op == OP_BX ? NB : MB;
+    std::vector<std::pair<int, int>> left;
+    for (int i = 0; i < MB; ++i) {
+      int j = op == OP_BX ? 0 : i;
+      for (; j + 1 < ncols; j += 2) quad(i, j, i, j + 1);
+      if (j < ncols) left.push_back({i, j});
+    }
+    for (size_t k = 0; k + 1 < left.size(); k += 2) quad(left[k].first, left[k].second, left[k + 1].first, left[k + 1].second);
+    if (left.size() % 2) quad(left.back().first, left.back().second, left.back().first, left.back().second);
+    return u;
+  }
   if (cfg.pair) {
     // 256 x 256 units; an odd block count leaves a half-empty last unit (operands zero-filled, stores skipped)
     const int MB = (mb + 1) / 2, NB = (nb + 1) / 2;

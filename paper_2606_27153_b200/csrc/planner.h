@@ -38,12 +38,13 @@ struct MatrixInfo {
 // Tile configuration of one op of one bucket ("variant" of dmuon_ns_gemm).
 struct TileConfig {
   bool pair = false;     // CTA-pair tiling: 256 x 256 units on two SMs (cta_group::2)
+  bool quad = false;     // CTA-quad tiling: two pair units per cluster of 4, shared operand panel multicast by TMA
   int width = 2;         // single-CTA tiling, blocks per work unit: 2 -> UMMA N = 256, 1 -> N = 128
   int order = 0;         // 0: panel-major (all block rows of one column panel first), 1: row-major
 };
 // Variants 0..3: single CTA, (width, order) = (2,0), (1,0), (2,1), (1,1); 4, 5: CTA pair, order 0, 1.
-// The symmetric ops have one ordering: their variants are 0, 1 (single CTA) and 4 (pair).
-constexpr int kNumVariants = 6;
+// 6: CTA quad.  The symmetric ops have one ordering: their variants are 0, 1 (single CTA), 4 (pair) and 6 (quad).
+constexpr int kNumVariants = 7;
 bool variant_valid(GemmOp op, int variant);
 TileConfig variant_config(int variant);
 

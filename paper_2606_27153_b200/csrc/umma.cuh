@@ -76,6 +76,27 @@ __device__ __forceinline__ void tma_load_2d_pair(uint32_t smem_dst, uint64_t tma
       ::"r"(smem_dst), "l"(tmap), "r"(c0), "r"(c1), "r"(bar)
       : "memory");
 }
+// Multicast form: the tile lands at the same CTA-relative offset in every CTA of `cta_mask` (cluster ranks), and each
+// destination CTA's mbarrier at the CTA-relative offset of `bar` receives the bytes that landed in that CTA.
+__device__ __forceinline__ void tma_load_2d_mcast(uint32_t smem_dst, uint64_t tmap, int c0, int c1, uint32_t bar,
+                                                  uint16_t cta_mask) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.multicast::cluster"
+      " [%0], [%1, {%2, %3}], [%4], %5;"
+      ::"r"(smem_dst), "l"(tmap), "r"(c0), "r"(c1), "r"(bar), "h"(cta_mask)
+      : "memory");
+}
+// CTA-pair multicast form: as above, but every destination CTA's bytes are signalled on the barrier of ITS pair's
+// leader (the even CTA): `bar` is this CTA's own barrier address with the pair bit (bit 24 of the cluster shared
+// window, the lowest bit of the CTA rank) cleared.
+__device__ __forceinline__ void tma_load_2d_pair_mcast(uint32_t smem_dst, uint64_t tmap, int c0, int c1, uint32_t bar,
+                                                       uint16_t cta_mask) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster"
+      " [%0], [%1, {%2, %3}], [%4], %5;"
+      ::"r"(smem_dst), "l"(tmap), "r"(c0), "r"(c1), "r"(bar & 0xFEFFFFFFu), "h"(cta_mask)
+      : "memory");
+}
 __device__ __forceinline__ void tma_prefetch_desc(uint64_t tmap) {
   asm volatile("prefetch.tensormap [%0];" ::"l"(tmap) : "memory");
 }
