@@ -263,6 +263,7 @@ def run_ours(args):
     dm.set_option("profile", 1)
     if args.variants:
         dm.set_option("variants", args.variants)
+    dm.set_option("overlap", args.overlap)
     t_setup = time.perf_counter()
     if cfg == 1:
         _, W = synth.ns_inputs("cuda")
@@ -361,6 +362,7 @@ def run_ours(args):
     hbm_alone = None
     if cfg != 1:
         dm.set_option("steps", 0)
+        dm.set_option("overlap", 0)           # one stream: the passes are timed one after the other
         for _ in range(2):
             step()
         torch.cuda.synchronize()
@@ -371,6 +373,7 @@ def run_ours(args):
         torch.cuda.synchronize()
         pa = dm.profile_read()["kernels"]
         dm.set_option("steps", NS_STEPS)
+        dm.set_option("overlap", args.overlap)
         hbm_alone = {}
         for name in ("momentum_nesterov_sumsq", "normalize_orient_cast", "apply_update"):
             if name in pa and pa[name]["ms"] > 0:
@@ -425,7 +428,8 @@ def run_ours(args):
             "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f16",
             "data": "synthetic",
             "config": {"workload": WORKLOADS[cfg] + (f" -- REDUCED to the first {args.layers} layers (profiling run, not a bench value)" if indices is not None else ""), "ns_steps": NS_STEPS, "coeffs": [3.4445, -4.7750, 2.0315], "lr": LR,
-                       "mu": MU, "wd": WD, "schedule": plan_desc["buckets"], "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "mu": MU, "wd": WD, "schedule": plan_desc["buckets"],
+                       "overlap": bool(args.overlap), "parallelism": "replicas only" if world > 1 else "single GPU",
                        "l2": "inputs (W, G, M + workspace, tens of GB) exceed the 126 MB L2; no flush needed",
                        "arithmetic": "bf16 in/out, fp16 operands on tcgen05 with fp32 TMEM accumulation, fp32 elementwise"},
             "muon_step_ms": ms, "ns_tflops_dense_equiv": value / world, "ns_tflops_executed": xflops / (ms * 1e-3) / 1e12,
@@ -565,6 +569,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--layers", type=int, default=0, help="profiling aid: only the first L layers of the set (0 = all)")
     ap.add_argument("--sample-seconds", type=float, default=0.0, help="--impl reference: CPU seconds per step (0 = auto)")
+    ap.add_argument("--overlap", type=int, default=0, choices=[0, 1], help="library option 'overlap' (side-stream schedule)")
     ap.add_argument("--variants", default="", help="tuning aid: force tile configurations 'syrk,sq,bx' (-1 = tuned)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -127,6 +127,9 @@ DMUON_API int dmuon_set_workspace(void* dev_ptr, size_t bytes);
  *                 reformulation of Eq. 2: same result up to rounding (default).
  *                 "x" = the plain iteration X <- (a I + B) X at every step, on every bucket
  *   "autotune"    "1"/"0": pick each bucket's tile configuration by on-device measurement (default "1")
+ *   "overlap"     "1"/"0": dmuon_muon_step on several shape buckets runs the HBM-bound passes (momentum, norm, normalise,
+ *                 apply) of one bucket on a library-owned side stream under the GEMMs of another; results are
+ *                 identical either way.  Measured gain on configs[3]: <= 1 % (the step is power-bound) (default "0")
  *   "variants"    "s,q,b": force the tile configuration (see dmuon_ns_gemm) of the SYRK, m x m and X-update products of
  *                 plans built from now on; -1 = measured / cached choice (default "-1,-1,-1")
  *   "cache_path"  file for the persistent tuning cache ("" disables; default $DMUON_CACHE or ~/.cache/dmuon/tune.txt)

@@ -111,12 +111,50 @@ int muon_step_device(void* const* params, const void* const* grads, void* const*
   if (plan_out) *plan_out = plan;
   g_last_plan = plan;
   if ((rc = bind_pointers(*plan, params, grads, momenta, g_opt.steps, g_opt.coeffs, false, stream, masters))) return rc;
-  const ElemTables& T = plan->tables;
-  if ((rc = launch_momentum(T, mu, stream))) return rc;
-  if ((rc = launch_finalize_norms(T, g_opt.eps, stream))) return rc;
-  if ((rc = launch_normalize(T, /*from_user=*/false, plan->fp32, stream))) return rc;
-  if ((rc = run_ns_steps(*plan, g_opt.steps, g_opt.coeffs, false, g_opt, stream))) return rc;
-  if ((rc = launch_apply(T, lr, wd, plan->fp32, masters != nullptr, stream))) return rc;
+  const bool master = masters != nullptr;
+  if (plan->parts.empty() || !g_opt.overlap) {
+    const ElemTables& T = plan->tables;
+    if ((rc = launch_momentum(T, mu, stream))) return rc;
+    if ((rc = launch_finalize_norms(T, g_opt.eps, stream))) return rc;
+    if ((rc = launch_normalize(T, /*from_user=*/false, plan->fp32, stream))) return rc;
+    if ((rc = run_ns_steps(*plan, g_opt.steps, g_opt.coeffs, false, g_opt, stream))) return rc;
+    if ((rc = launch_apply(T, lr, wd, plan->fp32, master, stream))) return rc;
+    return DMUON_OK;
+  }
+  // Several buckets: the HBM-bound passes of one bucket run on the plan's side stream under the GEMMs of another.
+  //   main:  prep(part 0) | NS(bucket 0) | NS(bucket 1) | ... | NS(last) | apply(last) | join
+  //   side:  prep(parts 1..)             | apply(part 0) after NS(bucket 0) | apply(part 1) after NS(bucket 1) | ...
+  // prep = momentum + norms + normalise.  Matrices of different buckets share no buffer, so only the fork/join and the
+  // per-bucket "ready" / "NS done" events order the two streams.
+  const int nb = static_cast<int>(plan->parts.size());
+  cudaStream_t side = plan->side;
+  cudaEvent_t ev_fork = plan->ev[2 * nb], ev_join = plan->ev[2 * nb + 1];
+  auto prep = [&](const ElemTables& T, cudaStream_t s) -> int {
+    int r;
+    if ((r = launch_momentum(T, mu, s))) return r;
+    if ((r = launch_finalize_norms(T, g_opt.eps, s))) return r;
+    return launch_normalize(T, /*from_user=*/false, false, s);
+  };
+  DMUON_CUDA_CHECK(cudaEventRecord(ev_fork, stream));            // after the pointer upload and the caller's earlier work
+  DMUON_CUDA_CHECK(cudaStreamWaitEvent(side, ev_fork, 0));
+  if ((rc = prep(plan->parts[0], stream))) return rc;
+  for (int k = 1; k < nb; ++k) {
+    if ((rc = prep(plan->parts[k], side))) return rc;
+    DMUON_CUDA_CHECK(cudaEventRecord(plan->ev[2 * k], side));   // bucket k's X0 is ready
+  }
+  for (int k = 0; k < nb; ++k) {
+    if (k > 0) DMUON_CUDA_CHECK(cudaStreamWaitEvent(stream, plan->ev[2 * k], 0));
+    if ((rc = run_ns_bucket(*plan, plan->order[k], g_opt.steps, g_opt.coeffs, false, g_opt, stream))) return rc;
+    if (k + 1 < nb) {
+      DMUON_CUDA_CHECK(cudaEventRecord(plan->ev[2 * k + 1], stream));                 // bucket k's O is ready
+      DMUON_CUDA_CHECK(cudaStreamWaitEvent(side, plan->ev[2 * k + 1], 0));
+      if ((rc = launch_apply(plan->parts[k], lr, wd, false, master, side))) return rc;
+    } else {
+      if ((rc = launch_apply(plan->parts[k], lr, wd, false, master, stream))) return rc;
+    }
+  }
+  DMUON_CUDA_CHECK(cudaEventRecord(ev_join, side));
+  DMUON_CUDA_CHECK(cudaStreamWaitEvent(stream, ev_join, 0));
   return DMUON_OK;
 }
 
@@ -251,6 +289,7 @@ DMUON_API int dmuon_set_option(const char* key, const char* value) {
     g_opt.force_variant[0] = a; g_opt.force_variant[1] = b; g_opt.force_variant[2] = c;
     return DMUON_OK;
   }
+  if (k == "overlap") { if (as_bool(&g_opt.overlap)) return DMUON_OK; set_error("option overlap: bad value '%s'", value); return DMUON_ERR_INVALID_ARG; }
   if (k == "cache_path") { g_opt.cache_path = v; g_opt.cache_path_set = true; return DMUON_OK; }
   set_error("dmuon_set_option: unknown key '%s'", key);
   return DMUON_ERR_INVALID_ARG;

@@ -167,6 +167,7 @@ __global__ void __launch_bounds__(kThreads) finalize_norms_kernel(const int64_t*
   __shared__ double red[kThreads];
   const int mat = blockIdx.x;
   const int64_t b = prefix[mat], e = prefix[mat + 1];
+  if (b == e) return;                     // matrix not in this launch's part (every member has at least one chunk)
   double acc = 0.0;
   for (int64_t i = b + threadIdx.x; i < e; i += kThreads) acc += static_cast<double>(partials[i]);
   red[threadIdx.x] = acc;

@@ -232,6 +232,8 @@ int fill_problem(GemmProblem& g, GemmOp op, const void* a_mat, uint64_t a_rows, 
 
 Plan::~Plan() {
   for (void* p : d_allocs) cudaFree(p);
+  for (cudaEvent_t e : ev) cudaEventDestroy(e);
+  if (side) cudaStreamDestroy(side);
 }
 
 TileConfig variant_config(int variant) {
@@ -408,22 +410,12 @@ int get_plan(const int32_t* shapes, int count, const Options& opt, void* ext_ws,
     p.buckets[it->second].mats.push_back(i);
   }
 
-  // ---- elementwise tables
-  std::vector<int64_t> flat_prefix(count + 1, 0), tile_prefix(count + 1, 0), ptile_prefix(count + 1, 0);
-  std::vector<int64_t> fa_prefix(count + 1, 0), fb_prefix(count + 1, 0);
+  // ---- elementwise tables.  One set over all matrices (`tables`) and, when there are several buckets, one set per
+  //      bucket (`parts`, in execution order) in which the matrices of the other buckets have no work items: the step
+  //      runs the elementwise passes of one bucket on a side stream under the GEMMs of another (api.cu).
   p.h_recs.resize(count);
   for (int i = 0; i < count; ++i) {
     const MatrixInfo& mi = p.mats[i];
-    const int64_t elems = static_cast<int64_t>(mi.rows) * mi.cols;
-    flat_prefix[i + 1] = flat_prefix[i] + (elems + kFlatChunk - 1) / kFlatChunk;
-    // normalise / apply path of this matrix: A (flat), B (16-bit tile transpose) or the generic tiles
-    const bool aligned = !p.fp32 && mi.rows % kBlk == 0 && mi.cols % kBlk == 0;
-    const bool path_a = aligned && !mi.transposed, path_b = aligned && mi.transposed;
-    fa_prefix[i + 1] = fa_prefix[i] + (path_a ? elems / kFlatChunk : 0);
-    fb_prefix[i + 1] = fb_prefix[i] + (path_b ? static_cast<int64_t>(mi.rows / kTile) * (mi.cols / kTile) : 0);
-    const bool generic = !path_a && !path_b;
-    tile_prefix[i + 1] = tile_prefix[i] + (generic ? static_cast<int64_t>((mi.rows + kTile - 1) / kTile) * ((mi.cols + kTile - 1) / kTile) : 0);
-    ptile_prefix[i + 1] = ptile_prefix[i] + (generic ? static_cast<int64_t>(mi.m_pad / kTile) * (mi.n_pad / kTile) : 0);
     MatRec& r = p.h_recs[i];
     memset(&r, 0, sizeof r);
     r.U = p.ws + mi.off_p;
@@ -433,30 +425,69 @@ int get_plan(const int32_t* shapes, int count, const Options& opt, void* ext_ws,
     r.m_pad = mi.m_pad; r.n_pad = mi.n_pad;
     r.transposed = mi.transposed ? 1 : 0;
     r.scale = static_cast<float>(std::sqrt(std::max(1.0, static_cast<double>(mi.rows) / mi.cols)));   // reading N4
-    r.flat_chunk0 = flat_prefix[i]; r.tile0 = tile_prefix[i]; r.ptile0 = ptile_prefix[i];
   }
   if ((rc = dev_alloc(p, &p.d_recs, count))) return rc;
-  if ((rc = upload(p, &p.d_flat_prefix, flat_prefix))) return rc;
-  if ((rc = upload(p, &p.d_tile_prefix, tile_prefix))) return rc;
-  if ((rc = upload(p, &p.d_ptile_prefix, ptile_prefix))) return rc;
-  if ((rc = upload(p, &p.d_fa_prefix, fa_prefix))) return rc;
-  if ((rc = upload(p, &p.d_fb_prefix, fb_prefix))) return rc;
-  if ((rc = dev_alloc(p, &p.d_partials, static_cast<size_t>(flat_prefix[count])))) return rc;
   if ((rc = dev_alloc(p, &p.d_inv_norm, count))) return rc;
-  p.tables.recs = p.d_recs;
-  p.tables.flat_prefix = p.d_flat_prefix;
-  p.tables.tile_prefix = p.d_tile_prefix;
-  p.tables.ptile_prefix = p.d_ptile_prefix;
-  p.tables.count = count;
-  p.tables.flat_chunks = flat_prefix[count];
-  p.tables.tiles = tile_prefix[count];
-  p.tables.ptiles = ptile_prefix[count];
-  p.tables.fa_prefix = p.d_fa_prefix;
-  p.tables.fb_prefix = p.d_fb_prefix;
-  p.tables.fa_chunks = fa_prefix[count];
-  p.tables.fb_tiles = fb_prefix[count];
-  p.tables.partials = p.d_partials;
-  p.tables.inv_norm = p.d_inv_norm;
+  auto build_tables = [&](int only_bucket, ElemTables* out) -> int {
+    std::vector<int64_t> flat_prefix(count + 1, 0), tile_prefix(count + 1, 0), ptile_prefix(count + 1, 0);
+    std::vector<int64_t> fa_prefix(count + 1, 0), fb_prefix(count + 1, 0);
+    for (int i = 0; i < count; ++i) {
+      const MatrixInfo& mi = p.mats[i];
+      const bool member = only_bucket < 0 || mi.bucket == only_bucket;
+      const int64_t elems = static_cast<int64_t>(mi.rows) * mi.cols;
+      // normalise / apply path of this matrix: A (flat), B (16-bit tile transpose) or the generic tiles
+      const bool aligned = !p.fp32 && mi.rows % kBlk == 0 && mi.cols % kBlk == 0;
+      const bool path_a = aligned && !mi.transposed, path_b = aligned && mi.transposed;
+      const bool generic = !path_a && !path_b;
+      flat_prefix[i + 1] = flat_prefix[i] + (member ? (elems + kFlatChunk - 1) / kFlatChunk : 0);
+      fa_prefix[i + 1] = fa_prefix[i] + (member && path_a ? elems / kFlatChunk : 0);
+      fb_prefix[i + 1] = fb_prefix[i] + (member && path_b ? static_cast<int64_t>(mi.rows / kTile) * (mi.cols / kTile) : 0);
+      tile_prefix[i + 1] = tile_prefix[i] + (member && generic ? static_cast<int64_t>((mi.rows + kTile - 1) / kTile) * ((mi.cols + kTile - 1) / kTile) : 0);
+      ptile_prefix[i + 1] = ptile_prefix[i] + (member && generic ? static_cast<int64_t>(mi.m_pad / kTile) * (mi.n_pad / kTile) : 0);
+    }
+    int64_t *d_flat = nullptr, *d_tile = nullptr, *d_ptile = nullptr, *d_fa = nullptr, *d_fb = nullptr;
+    float* d_partials = nullptr;
+    int r2;
+    if ((r2 = upload(p, &d_flat, flat_prefix))) return r2;
+    if ((r2 = upload(p, &d_tile, tile_prefix))) return r2;
+    if ((r2 = upload(p, &d_ptile, ptile_prefix))) return r2;
+    if ((r2 = upload(p, &d_fa, fa_prefix))) return r2;
+    if ((r2 = upload(p, &d_fb, fb_prefix))) return r2;
+    if ((r2 = dev_alloc(p, &d_partials, static_cast<size_t>(flat_prefix[count])))) return r2;
+    out->recs = p.d_recs;
+    out->flat_prefix = d_flat;
+    out->tile_prefix = d_tile;
+    out->ptile_prefix = d_ptile;
+    out->fa_prefix = d_fa;
+    out->fb_prefix = d_fb;
+    out->count = count;
+    out->flat_chunks = flat_prefix[count];
+    out->tiles = tile_prefix[count];
+    out->ptiles = ptile_prefix[count];
+    out->fa_chunks = fa_prefix[count];
+    out->fb_tiles = fb_prefix[count];
+    out->partials = d_partials;
+    out->inv_norm = p.d_inv_norm;
+    return DMUON_OK;
+  };
+  if ((rc = build_tables(-1, &p.tables))) return rc;
+  // execution order of the buckets: most NS work first, so that the largest elementwise passes that can be hidden
+  // (normalise of the later buckets, apply of the earlier ones) run under the longest GEMM phases
+  p.order.resize(p.buckets.size());
+  for (size_t b = 0; b < p.buckets.size(); ++b) p.order[b] = static_cast<int>(b);
+  auto cost = [&](int b) {
+    const BucketPlan& bp = p.buckets[b];
+    return static_cast<double>(bp.mats.size()) * bp.m_pad * bp.m_pad * (2.0 * bp.n_pad + bp.m_pad);
+  };
+  std::stable_sort(p.order.begin(), p.order.end(), [&](int a, int b) { return cost(a) > cost(b); });
+  if (!p.fp32 && p.buckets.size() > 1) {
+    p.parts.resize(p.buckets.size());
+    for (size_t k = 0; k < p.order.size(); ++k)
+      if ((rc = build_tables(p.order[k], &p.parts[k]))) return rc;
+    DMUON_CUDA_CHECK(cudaStreamCreateWithFlags(&p.side, cudaStreamNonBlocking));
+    p.ev.resize(2 * p.buckets.size() + 2);
+    for (cudaEvent_t& e : p.ev) DMUON_CUDA_CHECK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+  }
 
   // ---- grouped GEMM tables (tensor-core mode only): scratch problems for the autotuner, tile units per op.  The
   //      launch programs of the NS steps are built on first use (build_program), they depend on the step count.
@@ -616,7 +647,17 @@ void launch_coefs(const NsLaunch& L, const float* coeffs, bool per_step, float* 
 }  // namespace
 
 int run_ns_steps(Plan& plan, int steps, const float* coeffs, bool per_step, const Options& opt, cudaStream_t stream) {
-  for (BucketPlan& b : plan.buckets) {
+  for (int bi : plan.order) {
+    int rc = run_ns_bucket(plan, bi, steps, coeffs, per_step, opt, stream);
+    if (rc) return rc;
+  }
+  return DMUON_OK;
+}
+
+int run_ns_bucket(Plan& plan, int bucket, int steps, const float* coeffs, bool per_step, const Options& opt,
+                  cudaStream_t stream) {
+  {
+    BucketPlan& b = plan.buckets[bucket];
     if (!plan.fp32) {
       const Partition part = choose_partition(steps, coeffs, per_step, b.gram && opt.gram_blocks);
       const std::string key = partition_key(part);

@@ -21,6 +21,8 @@ struct Options {
   bool cache_path_set = false;
   float eps = 1e-7f;
   int force_variant[3] = {-1, -1, -1};   // per tiling op (SYRK, SQ, BX): -1 = tuned, else this tile configuration
+  bool overlap = false;         // run the elementwise passes of one bucket under the GEMMs of another (side stream);
+                                // measured <= 1 % on config 4 (the step is power-bound: hiding a pass saves no energy)
   bool gram_blocks = true;      // schedule "auto": Gram blocks (Eq. 4) on wide buckets; false = plain X iteration
 };
 
@@ -101,10 +103,12 @@ struct Plan {
   // elementwise tables
   std::vector<MatRec> h_recs;          // host mirror (pointers patched per call)
   MatRec* d_recs = nullptr;
-  int64_t *d_flat_prefix = nullptr, *d_tile_prefix = nullptr, *d_ptile_prefix = nullptr, *d_fa_prefix = nullptr,
-          *d_fb_prefix = nullptr;
-  float *d_partials = nullptr, *d_inv_norm = nullptr;
-  ElemTables tables{};
+  float* d_inv_norm = nullptr;
+  ElemTables tables{};                 // all matrices
+  std::vector<int> order;              // execution order of the buckets (most NS work first)
+  std::vector<ElemTables> parts;       // per bucket, in execution order (empty: one bucket or check mode)
+  cudaStream_t side = nullptr;         // side stream for the elementwise passes hidden under GEMMs
+  std::vector<cudaEvent_t> ev;         // fork / join events of the overlapped step
   std::string bound_key;               // schedule signature rec.O was last bound for
   std::vector<void*> d_allocs;         // everything to cudaFree
   int sm_count = 148;
@@ -120,6 +124,8 @@ void drop_plans();
 // Enqueue k NS steps over every bucket of the plan; X0 is in buffer Q.  result_parity(...) tells where a bucket's
 // result ends (0 = Q, 1 = P) for the same arguments.
 int run_ns_steps(Plan& plan, int steps, const float* coeffs, bool per_step, const Options& opt, cudaStream_t stream);
+int run_ns_bucket(Plan& plan, int bucket, int steps, const float* coeffs, bool per_step, const Options& opt,
+                  cudaStream_t stream);
 int result_parity(const Plan& plan, const BucketPlan& b, int steps, const float* coeffs, bool per_step, const Options& opt);
 std::string partition_key(const Partition& p);
 

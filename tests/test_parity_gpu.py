@@ -25,10 +25,12 @@ def _reset_options():
     dm.set_option("steps", 5)
     dm.set_option("coeffs", "3.4445,-4.7750,2.0315")
     dm.set_option("schedule", "auto")
+    dm.set_option("overlap", 0)
     yield
     dm.set_option("mode", "tc")
     dm.set_option("steps", 5)
     dm.set_option("schedule", "auto")
+    dm.set_option("overlap", 0)
 
 
 @functools.lru_cache(maxsize=None)
@@ -319,9 +321,11 @@ def test_master_weights_step():
     assert all(torch.equal(a, b) for a, b in zip(keep, W32))
 
 
-def test_step_is_cuda_graph_capturable():
+@pytest.mark.parametrize("overlap", [0, 1])
+def test_step_is_cuda_graph_capturable(overlap):
     """After the first call for a shape set (plan, autotune, pointer binding) a step only enqueues kernels on the
     caller's stream, so it can be captured into a CUDA graph; the replay equals the eager step bit for bit."""
+    dm.set_option("overlap", overlap)                      # 1: the library's side stream forks and joins inside the capture
     shapes, W, G, M = synth.muon_inputs(2, "cuda", True, indices=list(range(12)))
     W0, M0 = [w.clone() for w in W], [m.clone() for m in M]
     dm.muon_step(W, G, M, LR, MU, WD)                      # eager: builds the plan, binds these pointers
@@ -354,6 +358,20 @@ def test_step_is_cuda_graph_capturable():
     e1.record()
     torch.cuda.synchronize()
     print(f"2 layers of config 2: graph replay {t_graph:.3f} ms/step, eager {e0.elapsed_time(e1) / 10:.3f} ms/step")
+
+
+def test_overlap_off_equals_overlap_on():
+    """The side-stream schedule changes only when kernels run, never what they compute."""
+    res = []
+    for ov in (1, 0):
+        dm.set_option("overlap", ov)
+        shapes, W, G, M = synth.muon_inputs(3, "cuda", True, indices=list(range(14)))
+        for _ in range(2):
+            dm.muon_step(W, G, M, LR, MU, WD)
+        torch.cuda.synchronize()
+        res.append((W, M))
+    assert all(torch.equal(a, b) for a, b in zip(res[0][0], res[1][0]))
+    assert all(torch.equal(a, b) for a, b in zip(res[0][1], res[1][1]))
 
 
 def test_two_steps_state_carried():
