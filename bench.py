@@ -339,9 +339,12 @@ def run_ours(args):
         launch_types[name]["matrices_per_launch"] = len(sub)
     dom = max(launch_types, key=lambda k: launch_types[k]["ms_per_step"], default=None)
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "roofline_traffic.json")
+    tpath = os.path.join(ROOT, "profiles", "roofline_traffic.csv")
     if dom and os.path.exists(tpath):
-        traffic = json.load(open(tpath)).get(f"config{cfg}", {}).get(dom)
+        for row in open(tpath).read().splitlines()[1:]:
+            c, lt, nbytes = row.split(",")          # launch-type names hold no comma
+            if c == f"config{cfg}" and lt == dom:
+                traffic = int(nbytes)
     roofline = None
     if dom:
         k = launch_types[dom]
@@ -354,7 +357,7 @@ def run_ours(args):
                                      "symmetry); (T+1)/(2T) of 2 m^2 n or 2 m^3 per matrix for the symmetric products "
                                      "(upper-triangular 128-blocks; the mirror is not arithmetic)",
                     "traffic_unit": "bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum, ncu --set full; "
-                                    "profiles/roofline_traffic.json)"}
+                                    "profiles/roofline_traffic.csv)"}
 
     # ---- the HBM-bound kernels timed without the GEMM phase around them (steps = 0: momentum, norms, normalise,
     #      apply run back to back at the clocks a memory-bound phase gets); the in-step figures above inherit the
