@@ -173,7 +173,7 @@ def oracle_sample(config: int, max_seconds: float = 30.0):
         _, W, G, M = synth.muon_inputs(config, "cpu", False, indices=[i]) if config != 1 else (None, *([synth.ns_inputs("cpu")[1][:1]] * 3))
         w, g, m = (t[0].to(torch.float64).numpy() for t in (W, G, M))
         t0 = time.perf_counter()
-        oracle.muon_step(w, g, m, LR, MU, WD, momentum_fp32=True)
+        oracle.muon_step(w, g, m, LR, MU, WD)
         secs += time.perf_counter() - t0
         flops += dense_flops([s])
         done.append(f"{s[0]}x{s[1]}")

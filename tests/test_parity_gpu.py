@@ -1,9 +1,12 @@
-"""Parity of the CUDA path (through the C ABI) against the fp64 oracle on the same seeded bf16 inputs.
+"""Parity of the CUDA path (through the C ABI) against the PLAIN fp64 oracle on the same seeded bf16 inputs.
 
 Bars (BASELINE.json north_star): relative Frobenius error of O = NS_5(.) <= 1e-2 on the tensor-core path
 (16-bit operands, fp32 accumulation) and <= 1e-4 in the fp32-operand check mode.  M' is compared elementwise
-(<= 1 bf16 ulp: fp32 vs fp64 arithmetic before the same rounding), W' by the criterion of DESIGN.md
-("error no worse than the output rounding plus 1 % of the update").
+with the fp64 oracle's (<= 1 bf16 ulp: fp32 vs fp64 arithmetic before the same rounding; the share of elements
+that differ is printed), W' by the criterion of DESIGN.md ("error no worse than the output rounding plus 1 % of
+the update").  Every comparison is against oracle.muon_step(..., momentum_fp32=False), the definition
+north_star gives.  ADDITIONALLY M' is checked bit for bit against the oracle's binary32-momentum mode (reading
+N16, steps = 0 so no NS work is repeated): that check is extra, it replaces none of the fp64 ones.
 """
 import functools
 
@@ -37,16 +40,33 @@ def _reset_options():
 def oracle_muon(config: int, index: int, random_momentum: bool):
     """Oracle Muon step for matrix `index` of a config (inputs regenerated on the GPU with the same seed and read back)."""
     _, W, G, M = synth.muon_inputs(config, "cuda", random_momentum, indices=[index])
-    return oracle.muon_step(to64(W[0]), to64(G[0]), to64(M[0]), LR_F, MU_F, WD_F, momentum_fp32=True)
+    return oracle_both(to64(W[0]), to64(G[0]), to64(M[0]))
+
+
+def oracle_both(w, g, m):
+    """The plain fp64 oracle step, plus (key "M_n16") the stored M' of the binary32-momentum mode (N16)."""
+    orc = oracle.muon_step(w, g, m, LR_F, MU_F, WD_F)
+    orc["M_n16"] = oracle.muon_step(w, g, m, LR_F, MU_F, WD_F, steps=0, momentum_fp32=True)["M_new"]
+    return orc
+
+
+STATS = {"m_mismatch": []}     # share of M' elements that differ from RNE(fp64 M') (printed by the callers)
 
 
 def check_muon_matrix(idx, shape, W0, Wg, Mg, Og, orc, tol):
     """Wg, Mg: GPU results (bf16 tensors); Og: unrounded GPU O (fp32); W0: W before the step (float64)."""
     e_o = rel_fro(to64(Og), orc["O"])
     assert e_o <= tol, f"matrix {idx} {shape}: O rel err {e_o:.3e} > {tol}"
-    # M': a quantised value; both sides form it in binary32 with one fused rounding (reading N16) -> identical bits
-    m_orc = oracle.round_bf16(orc["M_new"])
-    assert np.array_equal(to64(Mg), m_orc), f"matrix {idx}: M' differs ({(to64(Mg) != m_orc).mean():.2e} of elements)"
+    # M' against the fp64 oracle: a quantised value, so fp32 (kernel) and fp64 (oracle) arithmetic before the same
+    # RNE rounding may land on neighbouring bf16 values where the exact value sits on a tie: <= 1 bf16 ulp elementwise
+    mg, m_orc = to64(Mg), oracle.round_bf16(orc["M_new"])
+    dm_ = np.abs(mg - m_orc)
+    assert (dm_ <= bf16_ulp(np.maximum(np.abs(mg), np.abs(m_orc)))).all(), f"matrix {idx}: M' off by more than 1 bf16 ulp"
+    STATS["m_mismatch"].append(float((dm_ != 0).mean()))
+    # additional check (reading N16): formed in binary32 with one fused rounding on both sides -> identical bits
+    if "M_n16" in orc:
+        m16 = oracle.round_bf16(orc["M_n16"])
+        assert np.array_equal(mg, m16), f"matrix {idx}: M' differs from the binary32 mode ({(mg != m16).mean():.2e} of elements)"
     # W': no worse than the output rounding plus 1 % of the update (2 % slack on the rounding term: the two
     # roundings are different random draws of the same distribution)
     w_orc = orc["W_new"]
@@ -95,7 +115,9 @@ def _run_muon_config(config, random_momentum, mode, check_indices, tol):
         worst = max(worst, check_muon_matrix(i, shapes[i], W0[i], W[i], M[i], og, orc, tol))
     for g, g0 in zip(G, G0):
         assert torch.equal(g, g0), "grads must never be written"
-    print(f"config{config} {mode} momentum={random_momentum}: worst O rel err {worst:.3e} over {len(check_indices)} matrices")
+    mm = STATS["m_mismatch"][-len(check_indices):]
+    print(f"config{config} {mode} momentum={random_momentum}: worst O rel err vs fp64 oracle {worst:.3e} over {len(check_indices)} matrices; "
+          f"M' elements differing from RNE(fp64 M') (all within 1 ulp): mean {np.mean(mm):.2e}, max {np.max(mm):.2e}")
 
 
 def test_config2_muon_step_all_matrices():
@@ -166,67 +188,32 @@ def test_config3_full_launch_sampled_layers():
 
 @pytest.mark.slow
 def test_config4_full_size_sampled():
-    """Llama-3-8B-shaped set at full size (42 GB resident).  Oracle on the k (1024x4096) matrix of layer 0 and 31;
-    for the large shapes, properties that hold at any size: O's singular values equal the quintic's scalar map of
-    U's, and the tensor-core O agrees with the fp32 check mode."""
+    """Llama-3-8B-shaped set at full size (42 GB resident), in the launch configuration bench.py times.  The plain
+    fp64 oracle runs a whole Muon step of one matrix of EVERY distinct shape: k (1024x4096, layers 0 and 31),
+    q (4096x4096), gate (14336x4096, tall) and down (4096x14336) -- the three shapes that carry 99 % of the FLOPs
+    (>= one matrix per distinct shape).  O, M' and W' are compared as on the small configs."""
+    import time
     dm.set_option("mode", "tc")
     shapes, W, G, M = synth.muon_inputs(4, "cuda", False)
-    idx = [1, 218]
-    W0 = {i: to64(W[i]) for i in idx}
-    keep = {i: (W[i].clone(), G[i].clone(), M[i].clone()) for i in (0, 6)}
-    pre = {i: (W[i].clone(), M[i].clone()) for i in (0, 4, 6)}
+    idx = [1, 218, 0, 4, 6]
+    pre = {i: (to64(W[i]), to64(G[i]), to64(M[i])) for i in idx}
     dm.muon_step(W, G, M, LR, MU, WD)
     torch.cuda.synchronize()
-    for i in idx:
-        og = dm.binding.read_ns_output(i, shapes[i])
-        check_muon_matrix(i, shapes[i], W0[i], W[i], M[i], og, oracle_muon(4, i, False), TOL_TC)
-    big = {}
-    a, b, c = 3.4445, -4.7750, 2.0315
-    for i in (0, 4, 6):       # q (4096^2), gate (14336x4096, tall), down (4096x14336)
-        og = dm.binding.read_ns_output(i, shapes[i])
-        sv = torch.linalg.svdvals(og.double()).sort().values
-        # NS acts on each singular value as p(s) = a s + b s^3 + c s^5 (Eq. 2 with X = U S V^T): the singular values of
-        # O are the sorted p^5(sigma_i(U) / ||U||_F).  M = 0, so U = bf16((1 + mu) G) formed here with torch ops.
-        u = torch.addcmul(G[i].float(), G[i].float(), torch.tensor(MU_F, device="cuda")).to(torch.bfloat16).double()
-        s = torch.linalg.svdvals(u) / torch.linalg.norm(u)
-        for _ in range(5):
-            s = a * s + b * s ** 3 + c * s ** 5
-        want = s.sort().values
-        assert sv.max().item() <= 1.2024 + 2e-2
-        d = (sv - want).abs()
-        print(f"config4 matrix {i} {shapes[i]}: singular values of O vs p^5(sigma(U)): mean |d| {d.mean().item():.2e}, max |d| {d.max().item():.2e}")
-        assert d.mean().item() <= 1e-2 and d.max().item() <= 5e-2
-        big[i] = og
-        del u, s, sv
-        # elementwise at full size: M' against the oracle's momentum (steps = 0 skips its NS; M' does not depend on it),
-        # bit for bit; W' against the update formula applied to the kernel's own O (flat / transposing apply paths),
-        # within one bf16 ulp (one fp32 expression and one rounding on the GPU, fp64 here)
-        w_pre, m_pre = pre[i]
-        m_orc = oracle.muon_step(to64(w_pre), to64(G[i]), to64(m_pre), LR_F, MU_F, WD_F, steps=0, momentum_fp32=True)["M_new"]
-        assert np.array_equal(to64(M[i]), oracle.round_bf16(m_orc)), f"config4 matrix {i}: M' differs"
-        del m_orc
-        scale = max(1.0, shapes[i][0] / shapes[i][1]) ** 0.5
-        w64 = w_pre.double()
-        want = w64 - LR_F * (float(np.float32(scale)) * og.double() + WD_F * w64)
-        diff = (W[i].double() - want).abs()
-        ulp = torch.pow(2.0, torch.floor(torch.log2(want.abs().clamp_min(2.0 ** -126))) - 7)
-        # fp32 evaluation error of the GPU expression (matters only where w and the update cancel to a tiny W')
-        slack = 2.0 ** -22 * (w64.abs() + LR_F * scale * og.double().abs())
-        assert (diff <= 1.001 * ulp + slack).all(), f"config4 matrix {i}: W' off by more than one bf16 ulp"
-        assert (diff <= 0.501 * ulp + slack).double().mean().item() > 0.999      # correctly rounded almost everywhere
-        del w64, want, diff, ulp, slack
+    got = {i: (W[i].clone(), M[i].clone(), dm.binding.read_ns_output(i, shapes[i]).cpu()) for i in idx}
+    plan = dm.describe_plan(shapes, steps=5)
     del W, G, M
     torch.cuda.empty_cache()
-    dm.shutdown()
-    dm.set_option("mode", "fp32_check")
-    for i in (0, 6):
-        w, g, m = keep[i]
-        dm.muon_step([w], [g], [m], LR, MU, WD)
-        torch.cuda.synchronize()
-        oc = dm.binding.read_ns_output(0, shapes[i])
-        e = (torch.linalg.norm(big[i].double() - oc.double()) / torch.linalg.norm(oc.double())).item()
-        assert e <= TOL_TC, f"matrix {i}: tc vs fp32 check mode {e:.3e}"
-    dm.shutdown()
+    for i in idx:
+        w0, g0, m0 = pre.pop(i)
+        t0 = time.perf_counter()
+        orc = oracle_both(w0, g0, m0)
+        secs = time.perf_counter() - t0
+        wg, mg, og = got.pop(i)
+        e = check_muon_matrix(i, shapes[i], w0, wg, mg, og, orc, TOL_TC)
+        print(f"config4 matrix {i} {shapes[i]}: O rel err vs fp64 oracle {e:.3e}; M' mismatch share {STATS['m_mismatch'][-1]:.2e} "
+              f"(oracle {secs:.0f} s on {oracle.num_threads()} threads)")
+        del orc, w0, g0, m0
+    print("config4 plan:", plan["buckets"])
 
 
 # ------------------------------------------------------------------------------------------------ edge cases
@@ -300,9 +287,11 @@ def test_master_weights_step():
     dm.muon_step_master(W, W32, G, M, LR, MU, WD)
     torch.cuda.synchronize()
     for i, s in enumerate(shapes):
-        orc = oracle.muon_step(W0[i], to64(G[i]), M0[i], LR_F, MU_F, WD_F, momentum_fp32=True)
+        orc = oracle_both(W0[i], to64(G[i]), M0[i])
         assert torch.equal(W[i], W32[i].to(torch.bfloat16)), f"{s}: bf16 parameter is not the rounding of the master"
-        assert np.array_equal(to64(M[i]), oracle.round_bf16(orc["M_new"])), f"{s}: M' differs"
+        assert np.array_equal(to64(M[i]), oracle.round_bf16(orc["M_n16"])), f"{s}: M' differs from the binary32 mode"
+        m_orc = oracle.round_bf16(orc["M_new"])
+        assert (np.abs(to64(M[i]) - m_orc) <= bf16_ulp(m_orc)).all(), f"{s}: M' off the fp64 oracle by more than 1 bf16 ulp"
         upd_orc = orc["W_new"] - W0[i]
         upd_gpu = to64(W32[i]) - W0[i]
         e = np.linalg.norm(upd_gpu - upd_orc) / np.linalg.norm(upd_orc)
@@ -383,7 +372,7 @@ def test_two_steps_state_carried():
         dm.muon_step(W, G, M, LR, MU, WD)
         torch.cuda.synchronize()
         for i in range(3):
-            orc = oracle.muon_step(W0[i], to64(G[i]), M0[i], LR_F, MU_F, WD_F, momentum_fp32=True)
+            orc = oracle_both(W0[i], to64(G[i]), M0[i])
             og = dm.binding.read_ns_output(i, shapes[i])
             check_muon_matrix(i, shapes[i], W0[i], W[i], M[i], og, orc, TOL_TC)
 
