@@ -3,14 +3,17 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--impl ours|reference]
 
-A "step" is one pass of the whole hot path (momentum+Nesterov+cast+norm, 5 Newton-Schulz steps of three grouped
-GEMMs per shape bucket, apply) over one synthetic matrix set.  Default workload: BASELINE.json configs[3], the
-Llama-3-8B-shaped set (224 matrices, 6.98 G elements, bf16 W/G/M resident in HBM), the configuration the metric
-is quoted on.  `value` = dense-equivalent NS TFLOP/s of the whole step (BASELINE.json: "counting the full dense
-FLOPs") = sum over matrices of 5 (4 m^2 n + 2 m^3) divided by the step time, aggregated over ranks.
-The path does not shard (north_star: one GPU, no collectives): --gpus N runs N independent replicas ("replicas
-only"), timed as the max over ranks.
+A "step" is one pass of the whole hot path (momentum+Nesterov+cast+norm, 5 Newton-Schulz steps of grouped GEMMs per
+shape bucket, the weight update applied in the last X-update epilogue) over one synthetic matrix set.  Default
+workload: BASELINE.json configs[3], the Llama-3-8B-shaped set (224 matrices, 6.98 G elements, bf16 W/G/M resident in
+HBM), the configuration the metric is quoted on.  `value` = dense-equivalent NS TFLOP/s of the whole step
+(BASELINE.json: "counting the full dense FLOPs") = sum over matrices of 5 (4 m^2 n + 2 m^3) divided by the step time,
+aggregated over ranks.  The timed loop runs with the library's per-launch profiling OFF; the per-kernel breakdown
+(`kernels`, `launch_types`, `roofline`) comes from a second pass of the same K steps with CUDA events around every
+launch.  The path does not shard (north_star: one GPU, no collectives): --gpus N runs N independent replicas
+("replicas only"), timed as the max over ranks.
 --impl reference times the fp64 CPU oracle (oracle/) on a bounded sample of the same workload.
+--sweep runs BASELINE.json configs[4] (NS-only shape sweep), one JSON line per shape.
 """
 from __future__ import annotations
 
@@ -34,6 +37,7 @@ LR, MU, WD = 0.02, 0.95, 0.01
 NS_STEPS = 5
 WORKLOADS = {1: "config1: tiny NS batch 8 x (128x512)", 2: "config2: GPT-2-small-shaped, 72 matrices",
              3: "config3: Qwen-0.5B-style, 168 matrices", 4: "config4: Llama-3-8B-shaped, 224 matrices, 6.98 G elements"}
+GEMM_X = ("ns_bx_update", "ns_bx_apply", "ns_bx_out", "ns_xb_update", "ns_xb_apply", "ns_xb_out")
 
 
 # ------------------------------------------------------------------------------------------------ accounting
@@ -51,16 +55,30 @@ def pad128(v):
     return -(-v // 128) * 128
 
 
+def bucket_key(shape):
+    """(m_pad, n_pad, kind) of the library's bucket for a stored shape: aligned matrices (rows, cols multiples of 128)
+    are held as stored -- "wide" (rows <= cols) or "tall" -- the others oriented and padded ("generic")."""
+    r, c = shape
+    m, n = oriented(shape)
+    aligned = r % 128 == 0 and c % 128 == 0
+    return pad128(m), pad128(n), ("generic" if not aligned else ("wide" if r <= c else "tall"))
+
+
 def launch_counts(shapes, plan):
     """Per matrix (m, n, products): how many launches of each product family the library's block schedule
-    (dmuon_describe_plan) runs.  A block of length L: 1 SYRK, L polynomial products, 3 (L - 1) Gram-space products
-    (T = aG + BG, G' = aT + TB, R' = pB' + aR + B'R), 1 X update."""
-    blocks = {(b["m"], b["n"]): b["blocks"] for b in plan["buckets"]}
+    (dmuon_describe_plan) runs.  A block of length L: 1 Gram product (SYRK), L polynomial products, 3 (L - 1)
+    Gram-space products (T = aG + BG, G' = aT + TB, R' = pB' + aR + B'R), 1 X update."""
+    blocks = {}
+    for b in plan["buckets"]:
+        blocks[(b["m"], b["n"], b.get("kind", "wide"))] = b["blocks"]
+        blocks.setdefault((b["m"], b["n"]), b["blocks"])          # plans described without a kind
     out = []
-    for m, n in map(oriented, shapes):
-        part = blocks[(pad128(m), pad128(n))]
-        out.append((m, n, {"ns_syrk_xxt": len(part), "ns_sq_poly": sum(part), "ns_gram_mm": sum(3 * (L - 1) for L in part),
-                           "ns_bx_update": len(part)}))
+    for s in shapes:
+        m, n = oriented(s)
+        key = bucket_key(s)
+        part = blocks.get(key) or blocks[key[:2]]
+        out.append((m, n, {"syrk": len(part), "ns_sq_poly": sum(part), "ns_gram_mm": sum(3 * (L - 1) for L in part),
+                           "xupd": len(part)}))
     return out
 
 
@@ -71,27 +89,47 @@ def executed_flops(shapes, plan):
     for m, n, cnt in launch_counts(shapes, plan):
         t = -(-m // 128)
         sym = (t + 1) / (2 * t)
-        tot += sym * (cnt["ns_syrk_xxt"] * 2 * m * m * n + (cnt["ns_sq_poly"] + cnt["ns_gram_mm"]) * 2 * m ** 3)
-        tot += cnt["ns_bx_update"] * 2 * m * m * n
+        tot += sym * (cnt["syrk"] * 2 * m * m * n + (cnt["ns_sq_poly"] + cnt["ns_gram_mm"]) * 2 * m ** 3)
+        tot += cnt["xupd"] * 2 * m * m * n
     return tot
 
 
-def kernel_work(shapes, plan):
-    """Algorithmic work per step of each kernel family: FLOPs or bytes.  For the symmetric
-    products the algorithmic FLOPs are those of the upper-triangular 128-blocks, (T+1)/(2T) of the dense 2 m^2 n or
-    2 m^3 (the rest of the result is a mirror, not arithmetic); the X update is dense."""
+def family_work(family, shapes, plan, x_share=1.0):
+    """Algorithmic work per step of one kernel family over `shapes`: ("flop" | "byte", amount).
+    For the symmetric products the algorithmic FLOPs are those of the upper-triangular 128-blocks, (T+1)/(2T) of the
+    dense 2 m^2 n or 2 m^3 (the rest of the result is a mirror, not arithmetic); the X update is dense.  The X updates
+    of a bucket run under two names (plain "_update", fused last "_apply" / "_out"): x_share = this name's share."""
     el = sum(r * c for r, c in shapes)
+    if family == "momentum_nesterov_sumsq":
+        return "byte", 8 * el                      # read G, M; write M', U          (a1 + a2)
+    if family == "sumsq":
+        return "byte", 2 * el
+    if family == "normalize_cast":
+        return "byte", 4 * el                      # read U; write X0
+    if family == "apply_update":
+        return "byte", 6 * el                      # read O, W; write W'             (a6, when not fused)
+    if family == "store_ns_output":
+        return "byte", 4 * el
     lc = launch_counts(shapes, plan)
     sym = lambda m: (-(-m // 128) + 1) / (2 * -(-m // 128))
-    return {
-        "ns_syrk_xxt": ("flop", sum(c["ns_syrk_xxt"] * sym(m) * 2 * m * m * n for m, n, c in lc)),
-        "ns_sq_poly": ("flop", sum(c["ns_sq_poly"] * sym(m) * 2 * m ** 3 for m, n, c in lc)),
-        "ns_gram_mm": ("flop", sum(c["ns_gram_mm"] * sym(m) * 2 * m ** 3 for m, n, c in lc)),
-        "ns_bx_update": ("flop", sum(c["ns_bx_update"] * 2 * m * m * n for m, n, c in lc)),
-        "momentum_nesterov_sumsq": ("byte", 8 * el),       # read G, M; write M', U          (a1 + a2)
-        "normalize_orient_cast": ("byte", 4 * el),         # read U; write X0
-        "apply_update": ("byte", 6 * el),                  # read O, W; write W'             (a6)
-    }
+    if family in ("ns_syrk_xxt", "ns_syrk_xtx"):
+        return "flop", sum(c["syrk"] * sym(m) * 2 * m * m * n for m, n, c in lc)
+    if family in ("ns_sq_poly", "ns_gram_mm"):
+        return "flop", sum(c[family] * sym(m) * 2 * m ** 3 for m, n, c in lc)
+    if family in GEMM_X:
+        return "flop", x_share * sum(c["xupd"] * 2 * m * m * n for m, n, c in lc)
+    return None, 0
+
+
+def launch_type_key(name):
+    """'family[R x C]' -> (m_pad, n_pad, tall?): GEMM launches are named by the bucket's stored shape."""
+    R, C = (int(v) for v in name[name.index("[") + 1:-1].split("x"))
+    return (min(R, C), max(R, C), R > C)
+
+
+def shapes_of_launch_type(name, shapes):
+    m_pad, n_pad, tall = launch_type_key(name)
+    return [s for s in shapes if bucket_key(s)[:2] == (m_pad, n_pad) and (bucket_key(s)[2] == "tall") == tall]
 
 
 def load_peaks():
@@ -102,6 +140,52 @@ def load_peaks():
                 "tflops_sustained": p.get("bf16_tflops_sustained", p["bf16_tflops"]), "source": "measured"}
     # fallback stated in /opt/skills/guides/B200_PROFILING.md
     return {"hbm_gbs": 6650.0, "tflops_burst": 1590.0, "tflops_sustained": 1400.0, "source": "fallback"}
+
+
+def profile_breakdown(prof, steps, ms, shapes, plan, peaks):
+    """(kernels per family, launch_types per family and bucket, dominant launch type) from the library's own CUDA events
+    (recorded on the launching stream) over `steps` steps of `ms` each."""
+    def entry(ms_tot, launches, kind, amount):
+        per_step_ms = ms_tot / steps
+        e = {"launches_per_step": launches / steps, "ms_per_step": per_step_ms, "share": per_step_ms / ms}
+        if kind and per_step_ms > 0:
+            if kind == "flop":
+                ach = amount / (per_step_ms * 1e-3) / 1e12
+                e.update({"bound": "tensor", "achieved": ach, "unit": "TFLOP/s", "frac": ach / peaks["tflops_sustained"],
+                          "frac_of_burst": ach / peaks["tflops_burst"], "frac_of_nominal_2250": ach / 2250.0,
+                          "work_per_step": amount})
+            else:
+                ach = amount / (per_step_ms * 1e-3) / 1e9
+                e.update({"bound": "hbm", "achieved": ach, "unit": "GB/s", "frac": ach / peaks["hbm_gbs"], "work_per_step": amount})
+        return e
+
+    launch_types, kernels = {}, {}
+    for name, rec in prof["kernels"].items():
+        fam = name.split("[")[0]
+        if "[" not in name:
+            kernels[fam] = entry(rec["ms"], rec["launches"], *family_work(fam, shapes, plan))
+            continue
+        sub = shapes_of_launch_type(name, shapes)
+        share = 1.0
+        if fam in GEMM_X:           # plain and fused X updates of one bucket share its X updates, by launch count
+            twins = [n for n in prof["kernels"] if n.split("[")[0] in GEMM_X and "[" in n and launch_type_key(n) == launch_type_key(name)]
+            share = rec["launches"] / sum(prof["kernels"][n]["launches"] for n in twins)
+        launch_types[name] = entry(rec["ms"], rec["launches"], *family_work(fam, sub, plan, share))
+        m_pad, n_pad, tall = launch_type_key(name)
+        chunks = [b["count"] for b in plan["buckets"] if (b["m"], b["n"]) == (m_pad, n_pad) and (b.get("kind") == "tall") == tall]
+        launch_types[name]["matrices_per_launch"] = statistics.mean(chunks) if chunks else len(sub)
+    agg = {}
+    for name, e in launch_types.items():            # GEMM families: sum over buckets
+        a = agg.setdefault(name.split("[")[0], {"ms": 0.0, "launches": 0.0, "work": 0.0})
+        a["ms"] += e["ms_per_step"]
+        a["launches"] += e["launches_per_step"]
+        a["work"] += e.get("work_per_step", 0.0)
+    for fam, a in agg.items():
+        ach = a["work"] / (a["ms"] * 1e-3) / 1e12 if a["ms"] > 0 else 0.0
+        kernels[fam] = {"launches_per_step": a["launches"], "ms_per_step": a["ms"], "share": a["ms"] / ms, "bound": "tensor",
+                        "achieved": ach, "unit": "TFLOP/s", "frac": ach / peaks["tflops_sustained"]}
+    dom = max(launch_types, key=lambda k: launch_types[k]["ms_per_step"], default=None)
+    return kernels, launch_types, dom
 
 
 # ------------------------------------------------------------------------------------------------ clocks
@@ -166,7 +250,7 @@ def oracle_sample(config: int, max_seconds: float = 30.0):
     oracle.ns(torch.zeros(8, 8).double().numpy())          # build + load outside the timed region
     done, flops, secs = [], 0.0, 0.0
     for s in distinct:
-        est = dense_flops([s]) / 7e10                       # ~70 GFLOP/s plain loops on 16 cores: skip what cannot fit the budget
+        est = dense_flops([s]) / 4.5e10                     # ~45 GFLOP/s plain loops on 16 cores: skip what cannot fit the budget
         if done and secs + est > max_seconds:
             break
         i = shapes.index(s)
@@ -201,7 +285,8 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * dense_flops(shapes) / (value * 1e12), "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": WORKLOADS[args.config], "note": "ms_per_step extrapolated from the sample by FLOPs"},
+        "config": {"workload": WORKLOADS[args.config], "ns_steps": NS_STEPS, "coeffs": [3.4445, -4.7750, 2.0315], "lr": LR,
+                   "mu": MU, "wd": WD, "note": "ms_per_step extrapolated from the sample by FLOPs"},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
                          "seconds_per_sample": statistics.mean(secs)},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -260,11 +345,9 @@ def run_ours(args):
     peaks = load_peaks()
     dm.set_option("mode", "tc")
     dm.set_option("steps", NS_STEPS)
-    dm.set_option("profile", 1)
-    if args.variants:
-        dm.set_option("variants", args.variants)
-    dm.set_option("overlap", args.overlap)
-    t_setup = time.perf_counter()
+    dm.set_option("profile", 0)
+    dm.set_option("keep_ns_output", 0)
+    dm.set_option("fuse_epilogue", args.fuse)
     if cfg == 1:
         _, W = synth.ns_inputs("cuda")
         G = M = None
@@ -278,9 +361,11 @@ def run_ours(args):
         else:
             dm.muon_step(W, G, M, LR, MU, WD)
 
+    torch.cuda.synchronize()
+    t_plan = time.perf_counter()
     step()                                    # first call: plan + workspace + autotune (reported, not timed)
     torch.cuda.synchronize()
-    plan_s = time.perf_counter() - t_setup
+    plan_s = time.perf_counter() - t_plan
     for _ in range(max(0, args.warmup - 1)):
         step()
     barrier()
@@ -297,47 +382,28 @@ def run_ours(args):
     torch.cuda.nvtx.range_pop()
     barrier()
     ms = max_over_ranks(e0.elapsed_time(e1)) / args.steps
-    prof = dm.profile_read()
+    gpu_launches = dm.profile_read()["launches"]
     clocks = sampler.stop() if rank == 0 else {}
 
     plan_desc = dm.describe_plan(shapes, NS_STEPS)
     dflops, xflops = dense_flops(shapes), executed_flops(shapes, plan_desc)
     value = whole_job_value(world, dflops, ms)
 
-    # per-kernel rooflines from the library's own CUDA events (recorded on the launching stream, in the timed region).
-    # The library names GEMM launches family[m x n] per shape bucket; `kernels` aggregates per family, `launch_types`
-    # keeps the buckets apart, and `roofline` is the launch type that takes the most time.
-    work = kernel_work(shapes, plan_desc)
-
-    def entry(ms_tot, launches, kind, amount):
-        per_step_ms = ms_tot / args.steps
-        e = {"launches_per_step": launches / args.steps, "ms_per_step": per_step_ms, "share": per_step_ms / ms}
-        if kind and per_step_ms > 0:
-            if kind == "flop":
-                ach = amount / (per_step_ms * 1e-3) / 1e12
-                e.update({"bound": "tensor", "achieved": ach, "unit": "TFLOP/s", "frac": ach / peaks["tflops_sustained"],
-                          "frac_of_burst": ach / peaks["tflops_burst"], "frac_of_nominal_2250": ach / 2250.0})
-            else:
-                ach = amount / (per_step_ms * 1e-3) / 1e9
-                e.update({"bound": "hbm", "achieved": ach, "unit": "GB/s", "frac": ach / peaks["hbm_gbs"]})
-        return e
-
-    fam = {}
-    for name, rec in prof["kernels"].items():
-        f = fam.setdefault(name.split("[")[0], {"ms": 0.0, "launches": 0})
-        f["ms"] += rec["ms"]
-        f["launches"] += rec["launches"]
-    kernels = {f: entry(v["ms"], v["launches"], *work.get(f, (None, 0))) for f, v in fam.items()}
-    launch_types = {}
-    for name, rec in prof["kernels"].items():
-        if "[" not in name:
-            continue
-        f, dims = name[:-1].split("[")
-        bm, bn = (int(v) for v in dims.split("x"))
-        sub = [sh for sh in shapes if (pad128(min(sh)), pad128(max(sh))) == (bm, bn)]
-        launch_types[name] = entry(rec["ms"], rec["launches"], *kernel_work(sub, plan_desc)[f])
-        launch_types[name]["matrices_per_launch"] = len(sub)
-    dom = max(launch_types, key=lambda k: launch_types[k]["ms_per_step"], default=None)
+    # ---- second pass of the same K steps with the library's events around every launch: per-kernel rooflines.  The
+    #      library names GEMM launches family[rows x cols] per shape bucket; `kernels` aggregates per family,
+    #      `launch_types` keeps the buckets apart, and `roofline` is the launch type that takes the most time.
+    dm.set_option("profile", 1)
+    step()
+    dm.profile_reset()
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms_prof = e0.elapsed_time(e1) / args.steps
+    prof = dm.profile_read()
+    dm.set_option("profile", 0)
+    kernels, launch_types, dom = profile_breakdown(prof, args.steps, ms_prof, shapes, plan_desc, peaks)
     traffic = None
     tpath = os.path.join(ROOT, "profiles", "roofline_traffic.csv")
     if dom and os.path.exists(tpath):
@@ -351,21 +417,23 @@ def run_ours(args):
         roofline = {"kernel": dom, "bound": "tensor", "achieved": k["achieved"], "peak": peaks["tflops_sustained"],
                     "unit": "TFLOP/s", "frac": k["frac"], "traffic": traffic,
                     "launches_per_step": k["launches_per_step"], "matrices_per_launch": k["matrices_per_launch"],
-                    "peak_kind": f"{peaks['source']} bf16 cuBLAS, sustained (kernel timed inside a long step); "
-                                 f"burst {peaks['tflops_burst']}, nominal 2250",
+                    "peak_kind": f"{peaks['source']} bf16 cuBLAS 8192^3, sustained (kernel timed inside a long step); "
+                                 f"burst {peaks['tflops_burst']}, nominal 2250; cuBLAS fp16 on THIS kernel's shape and "
+                                 f"operand bits: profiles/r2_energy_per_flop.md",
                     "flops_counted": "algorithmic FLOPs per launch: 2 m^2 n per matrix for an X update (dense, no "
                                      "symmetry); (T+1)/(2T) of 2 m^2 n or 2 m^3 per matrix for the symmetric products "
                                      "(upper-triangular 128-blocks; the mirror is not arithmetic)",
-                    "traffic_unit": "bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum, ncu --set full; "
-                                    "profiles/roofline_traffic.csv)"}
+                    "traffic_unit": "bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum of one launch of this "
+                                    "type in the full-size step; profiles/roofline_traffic.md)"}
 
-    # ---- the HBM-bound kernels timed without the GEMM phase around them (steps = 0: momentum, norms, normalise,
-    #      apply run back to back at the clocks a memory-bound phase gets); the in-step figures above inherit the
-    #      ~1 GHz SM clock of the power-capped GEMM phase
+    # ---- the HBM-bound kernels timed without the GEMM phase around them (steps = 0: momentum, norms, normalise, apply
+    #      run back to back at the clocks a memory-bound phase gets); the in-step figures above inherit the ~1 GHz SM
+    #      clock of the power-capped GEMM phase.  (With steps > 0 the apply pass does not exist: it is the last X
+    #      update's epilogue.)
     hbm_alone = None
     if cfg != 1:
         dm.set_option("steps", 0)
-        dm.set_option("overlap", 0)           # one stream: the passes are timed one after the other
+        dm.set_option("profile", 1)
         for _ in range(2):
             step()
         torch.cuda.synchronize()
@@ -376,11 +444,11 @@ def run_ours(args):
         torch.cuda.synchronize()
         pa = dm.profile_read()["kernels"]
         dm.set_option("steps", NS_STEPS)
-        dm.set_option("overlap", args.overlap)
+        dm.set_option("profile", 0)
         hbm_alone = {}
-        for name in ("momentum_nesterov_sumsq", "normalize_orient_cast", "apply_update"):
+        for name in ("momentum_nesterov_sumsq", "normalize_cast", "apply_update"):
             if name in pa and pa[name]["ms"] > 0:
-                gbs = work[name][1] / (pa[name]["ms"] / n_alone * 1e-3) / 1e9
+                gbs = family_work(name, shapes, plan_desc)[1] / (pa[name]["ms"] / n_alone * 1e-3) / 1e9
                 hbm_alone[name] = {"ms": pa[name]["ms"] / n_alone, "achieved": gbs, "unit": "GB/s", "peak": peaks["hbm_gbs"],
                                    "frac": gbs / peaks["hbm_gbs"]}
 
@@ -426,22 +494,29 @@ def run_ours(args):
         cpu_baseline = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc, "seconds": secs}
 
     if rank == 0:
+        xt = xflops / (ms * 1e-3) / 1e12
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f16",
             "data": "synthetic",
             "config": {"workload": WORKLOADS[cfg] + (f" -- REDUCED to the first {args.layers} layers (profiling run, not a bench value)" if indices is not None else ""), "ns_steps": NS_STEPS, "coeffs": [3.4445, -4.7750, 2.0315], "lr": LR,
-                       "mu": MU, "wd": WD, "schedule": plan_desc["buckets"],
-                       "overlap": bool(args.overlap), "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "mu": MU, "wd": WD, "schedule": plan_desc["buckets"], "workspace_bytes": plan_desc.get("workspace_bytes"),
+                       "fused_epilogue": bool(args.fuse), "parallelism": "replicas only" if world > 1 else "single GPU",
                        "l2": "inputs (W, G, M + workspace, tens of GB) exceed the 126 MB L2; no flush needed",
                        "arithmetic": "bf16 in/out, fp16 operands on tcgen05 with fp32 TMEM accumulation, fp32 elementwise"},
-            "muon_step_ms": ms, "ns_tflops_dense_equiv": value / world, "ns_tflops_executed": xflops / (ms * 1e-3) / 1e12,
-            "pct_of_bf16_peak": {"dense_equiv_of_measured_sustained": 100 * value / world / peaks["tflops_sustained"],
-                                 "dense_equiv_of_measured_burst": 100 * value / world / peaks["tflops_burst"],
-                                 "dense_equiv_of_nominal_2250": 100 * value / world / 2250.0,
-                                 "executed_of_measured_sustained": 100 * xflops / (ms * 1e-3) / 1e12 / peaks["tflops_sustained"]},
-            "roofline": roofline, "kernels": kernels, "launch_types": launch_types, "hbm_kernels_alone": hbm_alone, "cpu_baseline": cpu_baseline, "e2e": e2e,
-            "gpu_launches": prof["launches"], "clocks": clocks, "plan_autotune_seconds": plan_s,
+            "muon_step_ms": ms, "ns_tflops_dense_equiv": value / world, "ns_tflops_executed": xt,
+            "pct_of_bf16_peak": {"executed_of_measured_sustained": 100 * xt / peaks["tflops_sustained"],
+                                 "executed_of_measured_burst": 100 * xt / peaks["tflops_burst"],
+                                 "executed_of_nominal_2250": 100 * xt / 2250.0},
+            "algorithmic_speed_vs_dense_at_peak": {
+                "note": "dense-equivalent TFLOP/s (the metric's count) over a peak: NOT a hardware utilisation -- symmetry and "
+                        "Gram blocks execute fewer FLOPs than the dense count",
+                "vs_measured_sustained": value / world / peaks["tflops_sustained"],
+                "vs_nominal_2250": value / world / 2250.0},
+            "roofline": roofline, "kernels": kernels, "launch_types": launch_types, "profiled_pass_ms_per_step": ms_prof,
+            "hbm_kernels_alone": hbm_alone, "cpu_baseline": cpu_baseline, "e2e": e2e,
+            "gpu_launches": gpu_launches, "clocks": clocks, "plan_autotune_seconds": plan_s,
+            "tune_seconds": plan_desc.get("tune_seconds"),
             "paper_context": "DMuon reports 6.85x-163x optimizer-step and 1.48x-3.01x end-to-end speedups on 8-256 A800 "
                              "(PAPER.md:5, :274) and ~2x on one GPU (:329): other hardware, context only",
         }
@@ -452,21 +527,33 @@ def run_ours(args):
 
 def run_sweep(args):
     """BASELINE.json configs[4]: the NS kernel alone (dmuon_ns_batched, 5 steps) over a shape sweep, one JSON line per
-    shape with dense-equivalent and executed TFLOP/s.  Not the bench line: a per-shape table for profiles/."""
+    shape with dense-equivalent and executed TFLOP/s and the roofline fraction of the executed rate.  Batches are the
+    config's own (squares: 2^32 / n^2 matrices, i.e. 8 GiB of bf16 per shape); the library runs a bucket that needs
+    more than its workspace cap ("chunk_mb", 12 GiB) as chunks of fewer matrices.  The MoE expert set is ONE call of
+    128 matrices.  Not the bench line: a per-shape table for profiles/."""
     import paper_2606_27153_b200 as dm
     from paper_2606_27153_b200 import synth
     if not torch.cuda.is_available():
         raise SystemExit("bench.py --sweep needs a B200")
     torch.cuda.set_device(0)
+    peaks = load_peaks()
     dm.set_option("mode", "tc")
-    cap = 16384                      # bounds plan-building time (TMA descriptors per matrix); said in the output
-    for (r, c), batch in synth.sweep_shapes():
-        b = min(batch, cap)
-        g = torch.Generator(device="cuda")
-        g.manual_seed(5000 + r + c)
-        big = torch.randn((b, r, c), generator=g, device="cuda", dtype=torch.float32).to(torch.bfloat16)
-        Xs = [big[i] for i in range(b)]
-        shapes = [(r, c)] * b
+    dm.set_option("keep_ns_output", 0)
+    points = [([s], b) for s, b in synth.sweep_shapes() if s not in ((2048, 1408), (1408, 2048))]
+    points.append(([(2048, 1408), (1408, 2048)], 64))          # the MoE expert batch: 64 + 64 in one call
+    for shape_list, batch in points:
+        shapes, Xs, keep = [], [], []
+        for r, c in shape_list:
+            g = torch.Generator(device="cuda")
+            g.manual_seed(5000 + r + c)
+            big = torch.empty((batch, r, c), device="cuda", dtype=torch.bfloat16)
+            per = max(1, (1 << 28) // (r * c))                  # fill 256 Mi elements at a time (fp32 staging)
+            for b0 in range(0, batch, per):
+                nb = min(per, batch - b0)
+                big[b0:b0 + nb] = torch.randn((nb, r, c), generator=g, device="cuda", dtype=torch.float32).to(torch.bfloat16)
+            keep.append(big)
+            Xs += [big[i] for i in range(batch)]
+            shapes += [(r, c)] * batch
         t0 = time.perf_counter()
         dm.ns_batched(Xs, steps=NS_STEPS)      # plan + autotune
         torch.cuda.synchronize()
@@ -483,12 +570,13 @@ def run_sweep(args):
         e1.record()
         torch.cuda.synchronize()
         ms = e0.elapsed_time(e1) / reps
-        print(json.dumps({"sweep": True, "shape": [r, c], "batch": b, "batch_in_config": batch, "ms": ms,
-                          "tflops_dense_equiv": dense_flops(shapes) / ms / 1e9,
-                          "tflops_executed": executed_flops(shapes, plan) / ms / 1e9,
-                          "blocks": plan["buckets"][0]["blocks"], "variants": plan["buckets"][0]["variants"],
-                          "plan_seconds": plan_s, "includes": "norm + normalise + 5 NS steps + bf16 store"}), flush=True)
-        del Xs, big
+        xt = executed_flops(shapes, plan) / ms / 1e9
+        print(json.dumps({"sweep": True, "shapes": [list(s) for s in shape_list], "batch_per_shape": batch, "matrices": len(Xs), "ms": ms,
+                          "tflops_dense_equiv": dense_flops(shapes) / ms / 1e9, "tflops_executed": xt,
+                          "roofline_frac_executed_of_sustained": xt / peaks["tflops_sustained"],
+                          "buckets": plan["buckets"], "workspace_bytes": plan["workspace_bytes"],
+                          "plan_seconds": plan_s, "includes": "norm + normalise + 5 NS steps (bf16 store in the last epilogue)"}), flush=True)
+        del Xs, keep, big
         dm.shutdown()
         torch.cuda.empty_cache()
     # PAPER.md:188 (Fig. 7): per-matrix NS time against the number of same-shape matrices advanced together
@@ -518,51 +606,6 @@ def run_sweep(args):
             torch.cuda.empty_cache()
 
 
-def run_power_probe(args):
-    """Sustained throughput of the grouped X-update and SYRK kernels (dmuon_ns_gemm, CTA-pair tiling, 8 matrices of
-    4096 x 14336) against operand bit patterns: random fp16, low mantissa bits cleared, constant, zeros.  Shows how
-    much of the 1 kW cap is operand toggling.  One JSON line per (pattern, kernel)."""
-    import paper_2606_27153_b200 as dm
-    from paper_2606_27153_b200.binding import OP_BX, OP_SYRK
-    torch.cuda.set_device(0)
-    m, n, cnt = 4096, 14336, 8
-
-    def clear_low(x, bits):
-        return (x.view(torch.int16) & ~((1 << bits) - 1)).view(torch.float16)
-
-    for kind in ("random", "low3_cleared", "low6_cleared", "constant", "zeros", "random"):
-        g = torch.Generator(device="cuda")
-        g.manual_seed(1)
-        B = [(torch.randn((m, m), generator=g, device="cuda") * 0.02).half() for _ in range(cnt)]
-        X = [(torch.randn((m, n), generator=g, device="cuda") * 1e-2).half() for _ in range(cnt)]
-        if kind == "zeros":
-            B, X = [torch.zeros_like(t) for t in B], [torch.zeros_like(t) for t in X]
-        elif kind == "constant":
-            B, X = [torch.full_like(t, 0.01) for t in B], [torch.full_like(t, 0.01) for t in X]
-        elif kind.startswith("low"):
-            k = int(kind[3])
-            B, X = [clear_low(t, k) for t in B], [clear_low(t, k) for t in X]
-        C = [torch.empty((m, n), device="cuda", dtype=torch.float16) for _ in range(cnt)]
-        A = [torch.empty((m, m), device="cuda", dtype=torch.float16) for _ in range(cnt)]
-        for op, name, reps in ((OP_BX, "ns_bx_update_pair", 80), (OP_SYRK, "ns_syrk_xxt_pair", 150)):
-            call = (lambda: dm.ns_gemm(OP_BX, B, X, C, 1.0, 3.4445, variant=5)) if op == OP_BX else \
-                   (lambda: dm.ns_gemm(OP_SYRK, X, None, A, 1.0, 0.0, variant=4))
-            for _ in range(3):
-                call()
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            torch.cuda.synchronize()
-            e0.record()
-            for _ in range(reps):
-                call()
-            e1.record()
-            torch.cuda.synchronize()
-            ms = e0.elapsed_time(e1) / reps
-            flops = cnt * 2 * m * m * n * (1.0 if op == OP_BX else 136 * 4 / 1024)   # SYRK: 136 of 256 pair units
-            print(json.dumps({"probe": "power", "operands": kind, "kernel": name, "ms": ms, "seconds_timed": ms * reps / 1e3,
-                              "tflops_executed": flops / ms / 1e9}), flush=True)
-        del B, X, C, A
-
-
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -572,17 +615,13 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--layers", type=int, default=0, help="profiling aid: only the first L layers of the set (0 = all)")
     ap.add_argument("--sample-seconds", type=float, default=0.0, help="--impl reference: CPU seconds per step (0 = auto)")
-    ap.add_argument("--overlap", type=int, default=0, choices=[0, 1], help="library option 'overlap' (side-stream schedule)")
-    ap.add_argument("--variants", default="", help="tuning aid: force tile configurations 'syrk,sq,bx' (-1 = tuned)")
+    ap.add_argument("--fuse", type=int, default=1, choices=[0, 1], help="library option 'fuse_epilogue' (0: separate apply pass)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--power-probe", action="store_true", help="kernel throughput vs operand bit patterns (power cap)")
     ap.add_argument("--sweep", action="store_true", help="configs[4]: NS-only shape sweep, one JSON line per shape")
     args = ap.parse_args()
     if args.sweep:
         run_sweep(args)
-    elif args.power_probe:
-        run_power_probe(args)
     elif args.impl == "reference":
         run_reference(args)
     else:

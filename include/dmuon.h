@@ -2,13 +2,14 @@
  * dmuon.h -- C ABI of libdmuon: the single-GPU Muon optimizer step of DMuon (arxiv/paper_2606_27153)
  * for NVIDIA B200 (sm_100a).
  *
- * The path (Eq. 1; Eq. 2; Gram form PAPER.md:170; Algorithm 1 l.12-15, PAPER.md:232-238;
- * conventions the paper does not print are the readings N1..N15 of DESIGN.md):
+ * The path (Eq. 1; Eq. 2; Gram form PAPER.md:170; Algorithm 1 l.12-16, PAPER.md:232-239;
+ * conventions the paper does not print are the readings N1..N17 of DESIGN.md):
  *
  *     M' = mu M + G ;  U = bf16( G + mu M' )                         Nesterov momentum + the bf16 cast
- *     X0 = U / (||U||_F + 1e-7)        (transposed first when rows > cols)
+ *     X0 = U / (||U||_F + 1e-7)        (the Gram matrix is taken on the smaller side)
  *     k times:  A = X X^T ;  B = b A + c A A ;  X <- a X + B X       Newton-Schulz quintic, Gram form
  *     W' = W - lr ( sqrt(max(1, rows/cols)) X_k + wd W )             Eq. 1 with shape scale + decoupled decay
+ *                                                                    (applied in the last X update's epilogue)
  *
  * Every step runs in hand-written CUDA kernels (tcgen05/TMEM/TMA grouped GEMMs, vectorised elementwise
  * kernels).  There is no CPU fallback: on a machine without an sm_100 device every compute entry point
@@ -27,6 +28,9 @@
  *   - errors: return value 0 = DMUON_OK, negative = error; dmuon_last_error() gives a message for the calling
  *     thread's last failure.  Nothing throws or aborts across this boundary.  Non-finite inputs propagate.
  *   - count == 0 is a valid no-op.  Not thread-safe: serialise calls from several host threads.
+ *   - devices: every call works on the CURRENT CUDA device (cudaSetDevice before the call); plans, workspaces and
+ *     kernel attributes are kept per device.  Calls that share a device share that device's workspace: issue them
+ *     on one stream, or order the streams yourself.
  */
 #ifndef DMUON_H_
 #define DMUON_H_
@@ -74,8 +78,8 @@ DMUON_API int dmuon_ns_batched_sched(void* const* ptrs, const int32_t* shapes, i
  *   grads    HOST array[count] of DEVICE pointers to G (bf16), read only.
  *   momenta  HOST array[count] of DEVICE pointers to M (bf16), updated in place to mu M + G.
  *   lr, mu, wd  learning rate, momentum, decoupled weight decay.
- * Uses the NS step count and coefficients set through dmuon_set_option ("steps", "coeffs"; defaults 5 and the
- * standard quintic).
+ * Uses the NS step count and coefficients set through dmuon_set_option ("steps", "coeffs" or "coeffs_sched";
+ * defaults 5 and the standard quintic).
  */
 DMUON_API int dmuon_muon_step(void* const* params, const void* const* grads, void* const* momenta,
                               const int32_t* shapes, int32_t count, float lr, float mu, float wd,
@@ -95,9 +99,10 @@ DMUON_API int dmuon_muon_step_master(void* const* params, void* const* masters, 
 /*
  * The same step for tensors that live in HOST memory (pinned memory gives asynchronous copies): copies W, G, M of
  * every matrix to device staging buffers owned by the library, runs dmuon_muon_step there, and copies W and M
- * back.  The matrix list is processed in up to 8 groups of whole repetitions of its shape pattern (layers), so that
- * the host->device copies of one group, the step of the previous one and the device->host copies of the one before
- * overlap (two library-owned copy streams, both PCIe directions busy).  All work is ordered after what `stream`
+ * back.  The matrix list is processed in up to 32 groups of whole repetitions of its shape pattern (layers) through
+ * a ring of four staging slots (four groups resident, not the whole set; option "host_pipeline"), so that the
+ * host->device copies of one group, the step of the previous one and the device->host copies of the one before
+ * overlap (two library-owned copy streams, both PCIe directions busy).  On an error return nothing is left in flight.  All work is ordered after what `stream`
  * held at the call and `stream` waits for all of it: the caller synchronises `stream` before reading the results.
  * Host buffers should be pinned (pageable memory makes the copies synchronous).
  */
@@ -105,10 +110,53 @@ DMUON_API int dmuon_muon_step_host(void* const* params_host, const void* const* 
                                    void* const* momenta_host, const int32_t* shapes, int32_t count, float lr,
                                    float mu, float wd, dmuon_stream_t stream);
 
+/*
+ * Non-matrix parameters (embeddings, norms, biases; Alg. 1 l.16 "non-matrix params: AdamW"): one
+ * decoupled-weight-decay AdamW step (the paper's citation [16]; the convention of torch.optim.AdamW) over `count`
+ * tensors in ONE launch:
+ *     m <- beta1 m + (1 - beta1) g ;  v <- beta2 v + (1 - beta2) g^2
+ *     p <- p (1 - lr wd) - lr / (1 - beta1^step) * m / ( sqrt(v) / sqrt(1 - beta2^step) + eps )
+ *   params      HOST array[count] of DEVICE pointers, bf16, updated in place (fp32 arithmetic, one RNE rounding)
+ *   grads       HOST array[count] of DEVICE pointers, bf16, read only
+ *   exp_avg, exp_avg_sq   HOST arrays[count] of DEVICE pointers, fp32, updated in place
+ *   numel       HOST array[count], elements per tensor (> 0); all pointers 16-byte aligned
+ *   step        1-based step count (bias correction)
+ */
+DMUON_API int dmuon_adamw_step(void* const* params, const void* const* grads, void* const* exp_avg,
+                               void* const* exp_avg_sq, const int64_t* numel, int32_t count, float lr, float beta1,
+                               float beta2, float eps, float wd, int32_t step, dmuon_stream_t stream);
+
+/*
+ * c_{s,b} of PAPER.md:194: the measured time (ms) of the owner-local Muon update of ONE batch of `batch` matrices of
+ * shape rows x cols "including the complete execution path selected by the runtime" (bucketing, tuned tile
+ * configurations, block schedule, fused epilogue), averaged over `reps` steps after two warm-up steps.  Runs on
+ * library-owned scratch tensors; synchronises the device.
+ */
+DMUON_API int dmuon_measure_cost(int32_t rows, int32_t cols, int32_t batch, int32_t reps, float* ms_out,
+                                 dmuon_stream_t stream);
+
+/*
+ * Owner assignment from a measured cost model (Eq. 5).  HOST ONLY, no device needed.
+ *     minimise  max_r sum_{s,b} c[s,b] x[s,b,r]    subject to   sum_{r,b} b x[s,b,r] = n_s  for every shape s
+ *   counts       [num_shapes] n_s, matrices of shape s
+ *   num_batches  [num_shapes] |B_s|, candidate batch sizes of shape s (must contain 1 when n_s > 0)
+ *   batch_sizes, costs   concatenated over shapes: b and c[s,b] (e.g. from dmuon_measure_cost)
+ *   mode         0 greedy (longest processing time first, over several batch-size caps); 1 exact (branch and bound);
+ *                -1 exact when (sum_s |B_s|) * num_ranks <= threshold (S_thr of PAPER.md:206), greedy otherwise
+ *   x_out        [(sum_s |B_s|) * num_ranks] batches of configuration k = (s, b) given to rank r at x_out[k * R + r]
+ *   makespan_out the largest per-rank cost of the returned assignment
+ * Returns 1 when the result is a proven optimum, 0 for a greedy result, negative on error (an exact search that
+ * exceeds its node budget falls back to greedy and returns 0).
+ */
+DMUON_API int dmuon_assign_owners(const int32_t* counts, const int32_t* num_batches, const int32_t* batch_sizes,
+                                  const double* costs, int32_t num_shapes, int32_t num_ranks, int32_t mode,
+                                  int32_t threshold, int32_t* x_out, double* makespan_out);
+
 /* Plan + allocate + autotune for a shape set ahead of time (what the first dmuon_muon_step would do). */
 DMUON_API int dmuon_warmup(const int32_t* shapes, int32_t count, dmuon_stream_t stream);
 
-/* Bytes of device workspace a step over this shape set needs (0 on bad arguments). */
+/* Bytes of device workspace a step over this shape set needs with the current options (0 on bad arguments): the
+ * largest bucket's buffers, since buckets run one after another in one region ("chunk_mb" bounds a bucket). */
 DMUON_API size_t dmuon_workspace_bytes(const int32_t* shapes, int32_t count);
 
 /* Hand the library a caller-owned DEVICE workspace (256-byte aligned) to use instead of its own allocation;
@@ -119,6 +167,9 @@ DMUON_API int dmuon_set_workspace(void* dev_ptr, size_t bytes);
  * Options (string key/value).  Keys:
  *   "steps"       NS steps of dmuon_muon_step (default "5")
  *   "coeffs"      "a,b,c" used by dmuon_muon_step (default "3.4445,-4.7750,2.0315")
+ *   "coeffs_sched" "a0,b0,c0;a1,b1,c1;..." one triple per NS step for the Muon-step entry points (per-step sets such
+ *                 as Polar Express; the values are the caller's); must hold exactly "steps" triples when
+ *                 a step runs; "" = off (default)
  *   "mode"        "tc"  = fp16 operands on tcgen05 tensor cores, fp32 accumulation in TMEM (default; PAPER.md:262 runs NS in fp16);
  *                 "fp32_check" = fp32 operands, plain SIMT kernels: the <= 1e-4 check mode, small shapes only
  *   "schedule"    "auto" = on wide buckets (n >= 1.5 m, m >= 256) run the k steps as Gram blocks: G = X X^T once per block,
@@ -127,9 +178,16 @@ DMUON_API int dmuon_set_workspace(void* dev_ptr, size_t bytes);
  *                 reformulation of Eq. 2: same result up to rounding (default).
  *                 "x" = the plain iteration X <- (a I + B) X at every step, on every bucket
  *   "autotune"    "1"/"0": pick each bucket's tile configuration by on-device measurement (default "1")
- *   "overlap"     "1"/"0": dmuon_muon_step on several shape buckets runs the HBM-bound passes (momentum, norm, normalise,
- *                 apply) of one bucket on a library-owned side stream under the GEMMs of another; results are
- *                 identical either way.  Measured gain on configs[3]: <= 1 % (the step is power-bound) (default "0")
+ *   "fuse_epilogue" "1"/"0": for matrices whose rows and cols are multiples of 128, apply W' = W - lr (scale O + wd W)
+ *                 (or write the bf16 NS output) in the epilogue of the last X update instead of a separate pass
+ *                 (default "1").  Results agree to the rounding of the unfused path's fp16 O
+ *   "keep_ns_output" "1"/"0": keep every matrix's unrounded NS result readable after the call (dmuon_read_ns_output):
+ *                 fused epilogues also store it and buckets get disjoint workspace regions (default "0")
+ *   "chunk_mb"    workspace a bucket may use, MiB (default "12288"): a bucket whose matrices need more runs as
+ *                 chunks of fewer matrices, one after the other, through the same region
+ *   "host_pipeline" "groups,slots" of dmuon_muon_step_host (default "32,4")
+ *   "tune_ms"     autotune: milliseconds each candidate runs back to back (default "40": long enough for the
+ *                 board's power cap to act, as it does in the step)
  *   "variants"    "s,q,b": force the tile configuration (see dmuon_ns_gemm) of the SYRK, m x m and X-update products of
  *                 plans built from now on; -1 = measured / cached choice (default "-1,-1,-1")
  *   "cache_path"  file for the persistent tuning cache ("" disables; default $DMUON_CACHE or ~/.cache/dmuon/tune.txt)
@@ -140,8 +198,10 @@ DMUON_API int dmuon_set_option(const char* key, const char* value);
 
 /*
  * Describe how a shape set is executed: writes a JSON object
- *   {"buckets": [{"m": m_pad, "n": n_pad, "count": matrices, "blocks": [3, 2], "variants": [syrk, sq, bx]}, ...]}
- * for `steps` NS steps with the current options and default coefficients into buf (NUL terminated, truncated to
+ *   {"buckets": [{"m": m_pad, "n": n_pad, "kind": "wide" | "tall" | "generic", "count": matrices, "blocks": [3, 2],
+ *                 "variants": [gram, sq, xupdate], "fused": bool, "xscale": c, "gscale": g}, ...],   (execution order;
+ *    "workspace_bytes": B, "tune_seconds": t, "tune_cache_entries": n}                     chunks of a shape repeat)
+ * for `steps` NS steps with the current options into buf (NUL terminated, truncated to
  * len); builds the plan if needed (like dmuon_warmup).  Returns the bytes needed (excluding the NUL) or a negative error.
  */
 DMUON_API int dmuon_describe_plan(const int32_t* shapes, int32_t count, int32_t steps, char* buf, size_t len,
@@ -174,12 +234,13 @@ DMUON_API int dmuon_profile_reset(void);
  *   op 0 (SYRK, step a3):  C[m x m] = alpha * X X^T                X = in0[i] is m x k;  in1 ignored
  *   op 1 (SQ,   step a4):  C[m x m] = alpha * A A + beta * A       A = in0[i] is m x m, symmetric;  in1 ignored
  *   op 2 (BX,   step a5):  C[m x n] = alpha * B X + beta * X       B = in0[i] is m x m;  X = in1[i] is m x n
- * For op 0 `n` is k (the contraction length); for op 1 it is ignored.  Symmetric ops compute upper-triangular
+ *   op 4 (SYRK_T):         C[m x m] = alpha * Y^T Y                Y = in0[i] is n x m (a tall matrix as stored)
+ *   op 5 (XB):             C[n x m] = alpha * Y B + beta * Y       B = in0[i] is m x m SYMMETRIC;  Y = in1[i] is n x m
+ * For ops 0 and 4 `n` is the contraction length; for op 1 it is ignored.  Symmetric ops compute upper-triangular
  * tiles only and mirror them.  in0/in1/out are HOST arrays[count] of DEVICE pointers; out must not alias an input.
  * variant: -1 = the default tile configuration, >= 0 selects configuration `variant`: 0..3 = one CTA per unit,
  * UMMA 128 x 256 (0, 2) or 128 x 128 (1, 3), column-panel-major (0, 1) or row-major (2, 3) unit order; 4, 5 = CTA
- * pair (cta_group::2), UMMA 256 x 256, panel-major / row-major; 6 = CTA quad (cluster of two pairs whose units share
- * an operand panel, fetched once and multicast by TMA).  The symmetric ops accept 0, 1, 4, 6 only.
+ * pair (cta_group::2), UMMA 256 x 256, panel-major / row-major.  The symmetric ops accept 0, 1, 4 only.
  */
 DMUON_API int dmuon_ns_gemm(int32_t op, const void* const* in0, const void* const* in1, void* const* out,
                             int32_t m, int32_t n, int32_t count, float alpha, float beta, int32_t variant,
@@ -204,6 +265,8 @@ DMUON_API int dmuon_ns_gemm_variants(int32_t op);
  * Test hook: copies the Newton-Schulz result O = NS_k(X0) of matrix `index` of the MOST RECENT dmuon_muon_step /
  * dmuon_ns_batched call out of the library's workspace, before any rounding to bf16, as fp32 into out_dev
  * (DEVICE, rows*cols floats, the matrix's stored orientation).  Valid until the next call that uses the workspace.
+ * Needs option keep_ns_output=1 set BEFORE that call unless the call had a single bucket and no fused epilogue
+ * (otherwise buckets reuse one workspace region and the fused epilogue never stores O): DMUON_ERR_INVALID_ARG.
  */
 DMUON_API int dmuon_read_ns_output(int32_t index, float* out_dev, dmuon_stream_t stream);
 

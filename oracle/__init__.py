@@ -54,6 +54,9 @@ def _load():
         lib.oracle_muon_step.argtypes = [dp, dp, dp, ctypes.c_int, ctypes.c_int, ctypes.c_double,
                                          ctypes.c_double, ctypes.c_double, ctypes.c_int, dp, ctypes.c_int,
                                          ctypes.c_double, ctypes.c_int, ctypes.c_int, dp, dp, dp, dp]
+        lib.oracle_adamw_step.restype = ctypes.c_int
+        lib.oracle_adamw_step.argtypes = [dp, dp, dp, dp, ctypes.c_longlong, ctypes.c_double, ctypes.c_double,
+                                          ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_int, dp, dp, dp]
         _lib = lib
     return _lib
 
@@ -117,3 +120,19 @@ def muon_step(W, G, M, lr: float, mu: float, wd: float, steps: int = 5, coeffs=D
     if rc != 0:
         raise RuntimeError("oracle_muon_step failed")
     return {"M_new": Mo, "U": U, "O": O, "W_new": Wo}
+
+
+def adamw_step(p, g, m, v, lr: float, beta1: float, beta2: float, eps: float, wd: float, step: int):
+    """One decoupled-AdamW step (reading N17 of DESIGN.md) in float64.  Returns (p_new, m_new, v_new),
+    unrounded; the caller rounds p_new with round_bf16 to get the stored parameter."""
+    arrs = [np.ascontiguousarray(a, dtype=np.float64).reshape(-1) for a in (p, g, m, v)]
+    n = arrs[0].size
+    if any(a.size != n for a in arrs):
+        raise ValueError("p, g, m, v must have one size")
+    po, mo, vo = (np.empty(n) for _ in range(3))
+    rc = _load().oracle_adamw_step(_ptr(arrs[0]), _ptr(arrs[1]), _ptr(arrs[2]), _ptr(arrs[3]), n, float(lr), float(beta1),
+                                   float(beta2), float(eps), float(wd), int(step), _ptr(po), _ptr(mo), _ptr(vo))
+    if rc != 0:
+        raise RuntimeError("oracle_adamw_step failed")
+    shape = np.shape(p)
+    return po.reshape(shape), mo.reshape(shape), vo.reshape(shape)

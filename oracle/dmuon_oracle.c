@@ -28,6 +28,15 @@
  * exact polar factor; transpose equivariance; a hand-worked 2x3 Muon step.
  * Parity unpinned: the conventions N3 (momentum form), N4 (update scale), N5 (weight-decay form)
  * have no statement in the paper to pin them against; they are readings, listed in DESIGN.md.
+ *
+ *   AdamW for the non-matrix parameters (Alg. 1 l.16 "non-matrix params: sharded AdamW
+ *   through the host stack"; decoupled weight decay is the paper's citation [16]).  The
+ *   paper prints no formula; reading N17 takes the host stack's (PyTorch's) convention:
+ *       m_t = beta1 m + (1 - beta1) g ;  v_t = beta2 v + (1 - beta2) g^2
+ *       mhat = m_t / (1 - beta1^t) ;  vhat = v_t / (1 - beta2^t)
+ *       p_t = p - lr ( mhat / (sqrt(vhat) + eps) + wd p )
+ *   Pins: torch.optim.AdamW in float64 on the CPU over several steps (a library routine, not this
+ *   file); the closed form of step 1 (mhat = g, vhat = g^2).
  */
 #include <math.h>
 #include <stdlib.h>
@@ -203,4 +212,24 @@ ORACLE_API int oracle_muon_step(const double* W, const double* G, const double* 
   }
   free(Mn); free(U);
   return rc;
+}
+
+/* One decoupled-AdamW step over n elements (reading N17), all fp64.  step counts from 1.
+ * Outputs (each n doubles): p_out (unrounded), m_out, v_out. */
+ORACLE_API int oracle_adamw_step(const double* p, const double* g, const double* m, const double* v, long long n,
+                                 double lr, double beta1, double beta2, double eps, double wd, int step,
+                                 double* p_out, double* m_out, double* v_out) {
+  if (!p || !g || !m || !v || !p_out || !m_out || !v_out || n < 0 || step < 1) return -1;
+  const double bc1 = 1.0 - pow(beta1, (double)step);   /* bias corrections */
+  const double bc2 = 1.0 - pow(beta2, (double)step);
+  for (long long i = 0; i < n; ++i) {
+    const double mt = beta1 * m[i] + (1.0 - beta1) * g[i];
+    const double vt = beta2 * v[i] + (1.0 - beta2) * g[i] * g[i];
+    const double mhat = mt / bc1;
+    const double vhat = vt / bc2;
+    p_out[i] = p[i] - lr * (mhat / (sqrt(vhat) + eps) + wd * p[i]);
+    m_out[i] = mt;
+    v_out[i] = vt;
+  }
+  return 0;
 }

@@ -10,7 +10,7 @@ from typing import Iterable, List, Optional, Sequence
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libdmuon.so")
+LIB_PATH = os.environ.get("DMUON_LIB") or os.path.join(_HERE, "libdmuon.so")      # DMUON_LIB: another build of the same library (A/B measurements)
 
 OK = 0
 ERR_INVALID_ARG = -1
@@ -19,13 +19,14 @@ ERR_OOM = -3
 ERR_CUDA = -4
 ERR_INTERNAL = -5
 
-OP_SYRK, OP_SQ, OP_BX = 0, 1, 2
+OP_SYRK, OP_SQ, OP_BX, OP_SYRK_T, OP_XB = 0, 1, 2, 4, 5
 
 #: every symbol include/dmuon.h declares
 SYMBOLS = ("dmuon_ns_batched", "dmuon_ns_batched_sched", "dmuon_muon_step", "dmuon_muon_step_host", "dmuon_warmup",
            "dmuon_workspace_bytes", "dmuon_set_workspace", "dmuon_set_option", "dmuon_last_error",
            "dmuon_profile_read", "dmuon_profile_reset", "dmuon_ns_gemm", "dmuon_ns_gemm_variants", "dmuon_read_ns_output", "dmuon_shutdown",
-           "dmuon_version", "dmuon_describe_plan", "dmuon_ns_sym_mm", "dmuon_block_schedule", "dmuon_muon_step_master")
+           "dmuon_version", "dmuon_describe_plan", "dmuon_ns_sym_mm", "dmuon_block_schedule", "dmuon_muon_step_master",
+           "dmuon_adamw_step", "dmuon_measure_cost", "dmuon_assign_owners")
 
 
 class DmuonError(RuntimeError):
@@ -67,6 +68,11 @@ def lib() -> ctypes.CDLL:
         L.dmuon_block_schedule.argtypes = [i32, i32, i32, pf, i32, pi, i32]
         L.dmuon_describe_plan.argtypes = [pi, i32, i32, ctypes.c_char_p, ctypes.c_size_t, vp]
         L.dmuon_read_ns_output.argtypes = [i32, vp, vp]
+        pl = ctypes.POINTER(ctypes.c_int64)
+        pd = ctypes.POINTER(ctypes.c_double)
+        L.dmuon_adamw_step.argtypes = [pp, pp, pp, pp, pl, i32, f32, f32, f32, f32, f32, i32, vp]
+        L.dmuon_measure_cost.argtypes = [i32, i32, i32, i32, pf, vp]
+        L.dmuon_assign_owners.argtypes = [pi, pi, pi, pd, i32, i32, i32, i32, pi, pd]
         L.dmuon_shutdown.restype = None
         L.dmuon_version.restype = ctypes.c_char_p
         for name in SYMBOLS:
@@ -214,8 +220,13 @@ def ns_gemm(op: int, in0: Sequence[torch.Tensor], in1: Optional[Sequence[torch.T
         for t in ts:
             if t.dtype != torch.float16 or not t.is_contiguous() or t.device.type != "cuda" or t.dim() != 2:
                 raise ValueError("ns_gemm takes contiguous 2-D float16 cuda tensors")
-    m = in0[0].shape[0]
-    n = in0[0].shape[1] if op == OP_SYRK else (out[0].shape[1] if op == OP_BX else m)
+    if op == OP_SYRK_T:                      # in0 = Y [n x m]
+        m, n = in0[0].shape[1], in0[0].shape[0]
+    elif op == OP_XB:                        # in0 = B [m x m], in1 = Y [n x m]
+        m, n = in0[0].shape[0], out[0].shape[0]
+    else:
+        m = in0[0].shape[0]
+        n = in0[0].shape[1] if op == OP_SYRK else (out[0].shape[1] if op == OP_BX else m)
     _check(lib().dmuon_ns_gemm(op, _ptr_array(in0), _ptr_array(in1) if in1 else None, _ptr_array(out), m, n, len(in0),
                                float(alpha), float(beta), int(variant), _stream(stream)))
 
@@ -262,6 +273,62 @@ def read_ns_output(index: int, shape: Sequence[int], stream=None) -> torch.Tenso
     out = torch.empty(tuple(shape), dtype=torch.float32, device="cuda")
     _check(lib().dmuon_read_ns_output(int(index), ctypes.c_void_p(out.data_ptr()), _stream(stream)))
     return out
+
+
+def adamw_step(params: Sequence[torch.Tensor], grads: Sequence[torch.Tensor], exp_avg: Sequence[torch.Tensor],
+               exp_avg_sq: Sequence[torch.Tensor], lr: float, beta1: float, beta2: float, eps: float, wd: float, step: int,
+               stream=None) -> None:
+    """dmuon_adamw_step: decoupled AdamW over non-matrix parameters (bf16 p, g; fp32 moments), any shapes."""
+    n = len(params)
+    if not (len(grads) == len(exp_avg) == len(exp_avg_sq) == n):
+        raise ValueError("params, grads, exp_avg, exp_avg_sq must have one length")
+    for i in range(n):
+        p, g, m, v = params[i], grads[i], exp_avg[i], exp_avg_sq[i]
+        if p.dtype != torch.bfloat16 or g.dtype != torch.bfloat16 or m.dtype != torch.float32 or v.dtype != torch.float32:
+            raise ValueError(f"tensor {i}: params/grads must be bfloat16, moments float32")
+        if not (p.is_contiguous() and g.is_contiguous() and m.is_contiguous() and v.is_contiguous()):
+            raise ValueError(f"tensor {i}: tensors must be contiguous")
+        if not (p.numel() == g.numel() == m.numel() == v.numel()) or any(t.device.type != "cuda" for t in (p, g, m, v)):
+            raise ValueError(f"tensor {i}: sizes differ or not on cuda")
+    numel = (ctypes.c_int64 * n)(*[p.numel() for p in params])
+    _check(lib().dmuon_adamw_step(_ptr_array(params), _ptr_array(grads), _ptr_array(exp_avg), _ptr_array(exp_avg_sq),
+                                  numel, n, float(lr), float(beta1), float(beta2), float(eps), float(wd), int(step),
+                                  _stream(stream)))
+
+
+def measure_cost(shape: Sequence[int], batch: int, reps: int = 3, stream=None) -> float:
+    """dmuon_measure_cost: c_{s,b} (ms) of one batch of `batch` matrices of `shape` through the whole Muon step."""
+    out = ctypes.c_float(0.0)
+    _check(lib().dmuon_measure_cost(int(shape[0]), int(shape[1]), int(batch), int(reps), ctypes.byref(out), _stream(stream)))
+    return float(out.value)
+
+
+def assign_owners(counts: Sequence[int], batch_sizes: Sequence[Sequence[int]], costs: Sequence[Sequence[float]],
+                  num_ranks: int, mode: int = -1, threshold: int = 64):
+    """dmuon_assign_owners (host only).  batch_sizes[s], costs[s]: candidate batch sizes of shape s and their measured
+    costs.  Returns (x, makespan, exact) with x[s][j][r] = batches of batch_sizes[s][j] given to rank r."""
+    S = len(counts)
+    nb = [len(b) for b in batch_sizes]
+    flat_b = [int(v) for b in batch_sizes for v in b]
+    flat_c = [float(v) for c in costs for v in c]
+    if len(flat_b) != len(flat_c):
+        raise ValueError("batch_sizes and costs must have one shape")
+    K = len(flat_b)
+    x = (ctypes.c_int32 * max(1, K * num_ranks))()
+    ms = ctypes.c_double(0.0)
+    rc = lib().dmuon_assign_owners((ctypes.c_int32 * max(1, S))(*[int(c) for c in counts]), (ctypes.c_int32 * max(1, S))(*nb),
+                                   (ctypes.c_int32 * max(1, K))(*flat_b), (ctypes.c_double * max(1, K))(*flat_c), S,
+                                   int(num_ranks), int(mode), int(threshold), x, ctypes.byref(ms))
+    if rc < 0:
+        _check(rc)
+    out, k = [], 0
+    for s in range(S):
+        rows = []
+        for _ in range(nb[s]):
+            rows.append([int(x[k * num_ranks + r]) for r in range(num_ranks)])
+            k += 1
+        out.append(rows)
+    return out, float(ms.value), bool(rc == 1)
 
 
 def ns_gemm_variants(op: int) -> int:

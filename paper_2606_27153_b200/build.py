@@ -4,6 +4,7 @@
 """
 from __future__ import annotations
 
+import hashlib
 import os
 import subprocess
 import sys
@@ -13,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libdmuon.so")
-SOURCES = ["api.cu", "planner.cu", "elementwise.cu", "gemm_sm100.cu", "gemm_check.cu"]
+SOURCES = ["api.cu", "planner.cu", "assign.cu", "elementwise.cu", "gemm_sm100.cu", "gemm_check.cu"]
 HEADERS = ["common.h", "planner.h", "umma.cuh", os.path.join("..", "..", "include", "dmuon.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC,-fvisibility=hidden", "-diag-suppress", "177"]
@@ -33,16 +34,28 @@ def _stale(target: str, deps) -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build_library(force: bool = False, verbose: bool = False) -> str:
+def build_id() -> str:
+    """Hash of every source and header of the library: the key under which tuned tile configurations are cached, so
+    that a new build never trusts an older build's timings (PAPER.md:184 persistent kernel cache)."""
+    h = hashlib.sha1()
+    for name in sorted(SOURCES) + sorted(HEADERS):
+        with open(os.path.normpath(os.path.join(CSRC, name)), "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()[:12]
+
+
+def build_library(force: bool = False, verbose: bool = False, extra_flags=()) -> str:
     os.makedirs(OBJ, exist_ok=True)
     headers = [os.path.normpath(os.path.join(CSRC, h)) for h in HEADERS]
     nvcc = _nvcc()
     jobs = []
+    bid = build_id()
     for src in SOURCES:
         s = os.path.join(CSRC, src)
         o = os.path.join(OBJ, src.replace(".cu", ".o"))
         if force or _stale(o, [s] + headers):
-            jobs.append([nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", s, "-o", o])
+            defs = [f'-DDMUON_BUILD_ID="{bid}"'] if src == "planner.cu" else []
+            jobs.append([nvcc] + NVCC_FLAGS + list(extra_flags) + defs + (["-Xptxas", "-v"] if verbose else []) + ["-c", s, "-o", o])
 
     def run(cmd):
         r = subprocess.run(cmd, capture_output=True, text=True)

@@ -25,6 +25,8 @@ void set_error(const char* fmt, ...);
     }                                                                                            \
   } while (0)
 
+constexpr int kMaxDevices = 16;   // per-device state tables (kernel attributes, workspaces)
+
 // ---------------------------------------------------------------- GEMM family (gemm_sm100.cu)
 // Tile geometry: output tiles are built from 128 x 128 blocks.  A work unit of the single-CTA tiling is one block row
 // of 1 or 2 blocks (UMMA 128 x 128 or 128 x 256); a work unit of the CTA-pair tiling is 2 x 2 blocks (UMMA 256 x 256
@@ -32,44 +34,63 @@ void set_error(const char* fmt, ...);
 constexpr int kBlk = 128;     // block edge (UMMA_M)
 constexpr int kBlkK = 64;     // K elements per stage = one 128-byte swizzle row of fp16
 
-// OP_SYRK  C = alpha A B^T                      (symmetric result: upper blocks computed, mirrored)
-// OP_SQ    C = alpha A B^T + beta D             (symmetric result)
-// OP_BX    C = alpha A B   + beta D             (B operand MN-major; general result)
-// OP_SQ2   C = alpha A B^T + beta D + beta2 D2  (symmetric result; the product of the P_i of a Gram block)
-enum GemmOp : int { OP_SYRK = 0, OP_SQ = 1, OP_BX = 2, OP_SQ2 = 3 };
-constexpr int kNumOps = 4;
+// Products of the Gram-form NS step.  "wide" matrices (rows <= cols) are held as X [m x n]; "tall"
+// aligned matrices (rows > cols) are held AS STORED, Y = X^T [n x m], and use the two *_T / XB products, so that no
+// transposed copy of a tall matrix is ever made (PAPER.md:174 only asks that the Gram matrix be the small one).
+//   OP_SYRK    C = alpha A A^T                      A = X  [m x n] K-major                      (symmetric result)
+//   OP_SQ      C = alpha A B^T + beta D             A, B [m x m] K-major, symmetric result
+//   OP_BX      C = alpha A B   + beta D             A = R [m x m] K-major, B = D = X [m x n] MN-major; general result
+//   OP_SQ2     C = alpha A B^T + beta D + beta2 D2  symmetric result (running product of the P_i of a Gram block)
+//   OP_SYRK_T  C = alpha Y^T Y                      Y [n x m]: both operands MN-major             (symmetric result)
+//   OP_XB      C = alpha A B^T + beta D             A = D = Y [n x m] K-major, B = R [m x m] (R = R^T); general result
+enum GemmOp : int { OP_SYRK = 0, OP_SQ = 1, OP_BX = 2, OP_SQ2 = 3, OP_SYRK_T = 4, OP_XB = 5 };
+constexpr int kNumOps = 6;
+
+// What the epilogue does with x = alpha acc + beta D (+ beta2 D2), all in fp32 on the accumulator:
+//   EPI_F16           C = fp16(x)
+//   EPI_BF16          out = bf16(x / c)                               the last X update of dmuon_ns_batched
+//   EPI_APPLY         W' = bf16(W - (lr scale x / c + lr wd W))       the last X update of dmuon_muon_step: step a6
+//   EPI_APPLY_MASTER  W32' = W32 - (...), W' = bf16(W32')             (Eq. 1) fused into its epilogue
+// For the last three, C may also be written (fp16(x), the unrounded NS result kept for dmuon_read_ns_output).
+enum Epilogue : int { EPI_F16 = 0, EPI_BF16 = 1, EPI_APPLY = 2, EPI_APPLY_MASTER = 3 };
+constexpr int kNumEpi = 4;
 
 // One problem of a grouped launch.  Lives in device memory; the tensor maps are read by the TMA unit.
 struct alignas(128) GemmProblem {
-  CUtensorMap tmA;      // operand A: [rows, K] K-major, box {64, 128}
-  CUtensorMap tmB;      // operand B: K-major box {64, 128} (SYRK, SQ) or MN-major box {64 (n), 64 (k)} (BX)
-  const __half* D;      // addend matrix (SQ: A, BX: X), same leading dimension as C; null for SYRK
-  __half* C;            // output
+  CUtensorMap tmA;      // operand A: K-major box {64 (k), 128 (rows)}; MN-major (SYRK_T) box {64 (m), 64 (k)}
+  CUtensorMap tmB;      // operand B: K-major box {64, 128}; MN-major (BX, SYRK_T) box {64 (n), 64 (k)}
+  const __half* D;      // addend matrix (SQ: A, BX / XB: X), same leading dimension as C; null for SYRK
+  __half* C;            // output (fused epilogues write it only when the launch says store_c)
   const __half* D2;     // second addend (SQ2 only)
   int32_t ldc;          // leading dimension of C, D and D2, in elements
-  int32_t pad_[25];
+  int32_t rec;          // index of the matrix's MatRec (fused epilogues read W / W32 / scale there)
+  int32_t pad_[24];
 };
 static_assert(sizeof(GemmProblem) == 384, "GemmProblem layout");
 
 // One work unit of a problem.  Single-CTA tiling: block row, first block column, number of blocks (1 or 2), in
-// 128-blocks.  CTA-pair tiling: m_blk, n_blk index 256 x 256 units (width unused).  CTA-quad tiling: two 256 x 256
-// units, (m_blk, n_blk) for pair 0 and (width, flags) for pair 1, sharing a block row or a block column (both equal:
-// pair 1 shadows pair 0 and stores nothing -- the odd unit left over).
+// 128-blocks.  CTA-pair tiling: m_blk, n_blk index 256 x 256 units (width unused).
 struct TileUnit {
   int16_t m_blk, n_blk, width, flags;
 };
 
+struct MatRec;
+
 struct GemmLaunch {
   GemmOp op;
+  Epilogue epi = EPI_F16;
   const GemmProblem* problems;  // device
   const TileUnit* units;        // device, units_per_problem entries
+  const MatRec* recs = nullptr; // device (fused epilogues)
   int units_per_problem;
   int num_problems;
   int k_blocks;                 // K / 64
-  int m_blocks, n_blocks;       // extent of the output in 128-blocks
+  int m_blocks, n_blocks;       // extent of the output in 128-blocks (rows, columns)
   bool pair;                    // CTA-pair (cta_group::2) tiling
-  bool quad = false;            // CTA quad: two pairs sharing one operand panel by TMA multicast (units hold both)
   float alpha, beta, beta2;
+  float lr = 0.f, lrwd = 0.f;   // EPI_APPLY*: learning rate and lr * wd
+  bool store_c = true;          // fused epilogues: also store fp16(x) to C
+  int rec_base = 0;             // MatRec of problem p = recs[rec_base + problems[p].rec]
   int grid;                     // CTAs (<= #SM)
 };
 int launch_ns_gemm(const GemmLaunch& L, cudaStream_t stream);
@@ -80,19 +101,22 @@ int launch_check_gemm(GemmOp op, const float* in0, const float* in1, float* out,
                       float beta, cudaStream_t stream);
 
 // ---------------------------------------------------------------- elementwise family (elementwise.cu)
-// Per-matrix record used by every elementwise kernel (device array).
+// Per-matrix record used by every elementwise kernel and by the fused GEMM epilogues (device array).
 struct MatRec {
   void* W;              // bf16 parameter (muon) / in-out matrix (ns)
   const void* G;        // bf16 gradient (muon)
   void* M;              // bf16 momentum (muon)
   float* W32;           // fp32 master copy of W (dmuon_muon_step_master) or null
   void* U;              // bf16 staging of U, rows*cols, stored orientation (muon); unused (ns)
-  void* X0;             // internal buffer receiving the normalised, oriented, padded X0 (fp16 or fp32)
-  const void* O;        // internal buffer holding NS_k(X0), oriented + padded
+  void* X0;             // internal buffer receiving the normalised, scaled, padded X0 (fp16 or fp32)
+  const void* O;        // internal buffer holding NS_k(X0) (scaled by xscale)
   int32_t rows, cols;   // stored shape
-  int32_t m_pad, n_pad; // oriented, padded shape of the internal buffers (leading dimension n_pad)
-  int32_t transposed;   // rows > cols
-  float scale;          // sqrt(max(1, rows/cols))
+  int32_t m_pad, n_pad; // shape of the internal buffers: [m_pad x n_pad], leading dimension n_pad.  Generic matrices:
+                        // oriented (m <= n) and padded to 128; aligned matrices: the stored shape itself
+  int32_t transposed;   // internal buffer = transpose of the stored matrix (generic tall matrices only)
+  float scale;          // sqrt(max(1, rows/cols))                       (reading N4)
+  float xscale;         // power of two c: the internal buffers hold c X  (fp16 range)
+  float inv_xscale;     // 1 / c (exact)
   int64_t flat_chunk0;  // first chunk id of this matrix in the flat (momentum / sumsq) chunking
   int64_t tile0;        // first tile id of this matrix in the stored-orientation 64 x 64 tiling
   int64_t ptile0;       // first tile id in the padded, oriented 64 x 64 tiling
@@ -101,32 +125,45 @@ struct MatRec {
 constexpr int kFlatChunk = 8192;   // elements per flat chunk (one CTA pass)
 constexpr int kTile = 64;          // edge of the 2-D elementwise tiles
 
+// Work lists of one elementwise launch: the matrices of ONE bucket (the other matrices of the plan have no work items).
 struct ElemTables {
-  const MatRec* recs;          // device [count]
+  const MatRec* recs;          // device [count] (all matrices of the plan)
   const int64_t* flat_prefix;  // device [count + 1] chunk prefix
-  const int64_t* tile_prefix;  // device [count + 1] stored-orientation tile prefix
-  const int64_t* ptile_prefix; // device [count + 1] padded oriented tile prefix
-  // Fast paths of the normalise / apply passes (fp16 workspace only).  A matrix is on exactly one path; the other
-  // paths' prefix arrays give it zero work items.
-  const int64_t* fa_prefix;    // path A: not transposed, rows and cols multiples of 128 (workspace layout == stored
-                               //         layout): flat 8192-element chunks
-  const int64_t* fb_prefix;    // path B: transposed, rows and cols multiples of 128: 64 x 64 tiles, 16-bit transpose
+  const int64_t* tile_prefix;  // device [count + 1] stored-orientation tile prefix   (generic matrices)
+  const int64_t* ptile_prefix; // device [count + 1] padded oriented tile prefix      (generic matrices)
+  const int64_t* fa_prefix;    // device [count + 1] flat chunk prefix (aligned matrices: internal layout == stored layout)
   int count;
-  int64_t flat_chunks, tiles, ptiles, fa_chunks, fb_tiles;
+  int64_t flat_chunks, tiles, ptiles, fa_chunks;
   float* partials;             // device [flat_chunks] per-chunk sum of squares
-  float* inv_norm;             // device [count] 1 / (||U||_F + eps)
+  float* inv_norm;             // device [count] xscale / (||U||_F + eps)
 };
 
 int launch_fill_scratch(void* ptr, size_t bytes, cudaStream_t s);            // autotune operands
-int launch_momentum(const ElemTables& T, float mu, cudaStream_t s);          // a1 + a2 partials
+int launch_momentum(const ElemTables& T, float mu, bool exact, cudaStream_t s);   // a1 + a2 partials (exact: fp64 decisions)
 int launch_sumsq(const ElemTables& T, cudaStream_t s);                       // a2 alone (ns_batched)
 int launch_finalize_norms(const ElemTables& T, float eps, cudaStream_t s);
 int launch_normalize(const ElemTables& T, bool from_user, bool fp32_internal, cudaStream_t s);
-int launch_apply(const ElemTables& T, float lr, float wd, bool fp32_internal, bool master, cudaStream_t s);   // a6
-int launch_store_ns(const ElemTables& T, bool fp32_internal, cudaStream_t s);                    // ns_batched output
+int launch_apply(const ElemTables& T, float lr, float wd, bool fp32_internal, bool master, cudaStream_t s);   // a6 (not fused)
+int launch_store_ns(const ElemTables& T, bool fp32_internal, cudaStream_t s);                    // ns_batched output (not fused)
+
+// Non-matrix parameters (Alg. 1 l.16): decoupled AdamW, one flat launch over all tensors.
+struct AdamRec {
+  void* p;              // bf16 parameter, updated in place
+  const void* g;        // bf16 gradient
+  float* m;             // fp32 first moment
+  float* v;             // fp32 second moment
+  int64_t numel;
+};
+struct AdamScalars {
+  float lr, beta1, beta2, eps, wd;
+  float inv_bc1;        // 1 / (1 - beta1^t)
+  float inv_sqrt_bc2;   // 1 / sqrt(1 - beta2^t)
+};
+int launch_adamw(const AdamRec* d_recs, const int64_t* d_prefix, int count, int64_t total_chunks, const AdamScalars& sc,
+                 cudaStream_t s);
 
 int launch_export(const void* O, float* out, int rows, int cols, int n_pad, bool transposed, bool fp32_internal,
-                  cudaStream_t s);                                                               // test hook
+                  float inv_xscale, cudaStream_t s);                                             // test hook
 
 // ---------------------------------------------------------------- profiling (api.cu)
 void prof_begin(const char* name, cudaStream_t s);

@@ -7,8 +7,13 @@
 //                     128-multiples the GEMM tiles want, cast to the internal dtype (fp16, or fp32 in check mode)
 //   apply_kernel      W' = W - lr (scale O + wd W)  (a6; Eq. 1)  /  out = bf16(O) for dmuon_ns_batched
 //
+//   adamw_kernel      decoupled AdamW for the non-matrix parameters (Alg. 1 l.16)
+//
 // All global accesses are 128-bit and coalesced on the fast path (cols % 8 == 0); other shapes take a scalar path.
-// Work is cut into fixed-size chunks/tiles over ALL matrices of the call, so one launch covers the whole set.
+// Work is cut into fixed-size chunks/tiles over all matrices of a bucket, so one launch covers the whole bucket.
+// Aligned matrices (rows and cols multiples of 128) keep the stored layout in the workspace -- tall ones included,
+// the GEMM family has products for both orientations -- so their passes are flat streams; for them a6 and the NS
+// output are fused into the last X-update epilogue (gemm_sm100.cu) and the kernels here run only when steps = 0.
 #include "common.h"
 
 namespace dmuon {
@@ -67,8 +72,19 @@ __device__ __forceinline__ float block_sum(float v, float* red) {
 }
 
 // ---------------------------------------------------------------------------------------------- a1 + a2
+// double -> bf16 with ONE rounding (RNE): round to odd at binary32 (truncate, set the last bit when inexact; binary32
+// carries 16 more bits than bf16, so no tie of the second rounding can be created or lost), then RNE to bf16.
+__device__ __forceinline__ uint32_t double_to_bf16_bits(double x) {
+  float f = __double2float_rz(x);
+  if (static_cast<double>(f) != x) f = __uint_as_float(__float_as_uint(f) | 1u);
+  return float_to_bf16_bits(f);
+}
+
 // kMomentum: read G, M; write M' (in place) and U; accumulate |bf16(U)|^2.   !kMomentum: accumulate |X|^2 of rec.W.
-template <bool kMomentum>
+// kExact (check mode): M' and U are formed in binary64 and rounded once, i.e. the two quantisation decisions are taken
+// exactly as the fp64 oracle takes them; the fast path forms them in binary32 (one fused rounding each), which lands
+// on the neighbouring bf16 value for the ~1.5 % of elements whose exact value sits within 2^-24 of a bf16 tie.
+template <bool kMomentum, bool kExact>
 __global__ void __launch_bounds__(kThreads) flat_kernel(const MatRec* __restrict__ recs,
                                                         const int64_t* __restrict__ prefix, int count,
                                                         int64_t total_chunks, float mu, float* __restrict__ partials) {
@@ -108,10 +124,20 @@ __global__ void __launch_bounds__(kThreads) flat_kernel(const MatRec* __restrict
           for (int e = 0; e < 4; ++e) {
             const float2 gf = bf16x2_to_float2(gw[e]);
             const float2 mf = bf16x2_to_float2(mw[e]);
-            const float2 mn = __ffma2_rn(mu2, mf, gf);            // M' = mu M + G
-            const float2 uf = __ffma2_rn(mu2, mn, gf);            // U  = G + mu M'   (from the unrounded M')
-            mo[e] = float2_to_bf16x2(mn);
-            uo[e] = float2_to_bf16x2(uf);
+            if (kExact) {
+              const double mud = static_cast<double>(mu);
+              const double mnx = mud * static_cast<double>(mf.x) + static_cast<double>(gf.x);     // M' = mu M + G
+              const double mny = mud * static_cast<double>(mf.y) + static_cast<double>(gf.y);
+              const double ux = static_cast<double>(gf.x) + mud * mnx;                            // U = G + mu M'
+              const double uy = static_cast<double>(gf.y) + mud * mny;
+              mo[e] = double_to_bf16_bits(mnx) | (double_to_bf16_bits(mny) << 16);
+              uo[e] = double_to_bf16_bits(ux) | (double_to_bf16_bits(uy) << 16);
+            } else {
+              const float2 mn = __ffma2_rn(mu2, mf, gf);            // M' = mu M + G
+              const float2 uf = __ffma2_rn(mu2, mn, gf);            // U  = G + mu M'   (from the unrounded M')
+              mo[e] = float2_to_bf16x2(mn);
+              uo[e] = float2_to_bf16x2(uf);
+            }
             const float2 ur = bf16x2_to_float2(uo[e]);            // the rounded U is what the norm is taken of
             acc2 = __ffma2_rn(ur, ur, acc2);
           }
@@ -120,9 +146,18 @@ __global__ void __launch_bounds__(kThreads) flat_kernel(const MatRec* __restrict
         } else {
           for (int64_t j = i; j < end; ++j) {       // ragged tail of the matrix
             const float g = bf16_bits_to_float(G[j]), m = bf16_bits_to_float(M[j]);
-            const float mn = fmaf(mu, m, g);
-            const uint32_t ub = float_to_bf16_bits(fmaf(mu, mn, g));
-            M[j] = static_cast<uint16_t>(float_to_bf16_bits(mn));
+            uint32_t ub, mb;
+            if (kExact) {
+              const double mud = static_cast<double>(mu);
+              const double mn = mud * static_cast<double>(m) + static_cast<double>(g);
+              mb = double_to_bf16_bits(mn);
+              ub = double_to_bf16_bits(static_cast<double>(g) + mud * mn);
+            } else {
+              const float mn = fmaf(mu, m, g);
+              mb = float_to_bf16_bits(mn);
+              ub = float_to_bf16_bits(fmaf(mu, mn, g));
+            }
+            M[j] = static_cast<uint16_t>(mb);
             U[j] = static_cast<uint16_t>(ub);
             const float uf = bf16_bits_to_float(ub);
             acc = fmaf(uf, uf, acc);
@@ -161,7 +196,8 @@ __global__ void __launch_bounds__(kThreads) flat_kernel(const MatRec* __restrict
 }
 
 // One block per matrix: fixed-order sum of that matrix's chunk partials, in double.
-__global__ void __launch_bounds__(kThreads) finalize_norms_kernel(const int64_t* __restrict__ prefix,
+__global__ void __launch_bounds__(kThreads) finalize_norms_kernel(const MatRec* __restrict__ recs,
+                                                                  const int64_t* __restrict__ prefix,
                                                                   const float* __restrict__ partials, float eps,
                                                                   float* __restrict__ inv_norm) {
   __shared__ double red[kThreads];
@@ -176,7 +212,9 @@ __global__ void __launch_bounds__(kThreads) finalize_norms_kernel(const int64_t*
     if (threadIdx.x < s) red[threadIdx.x] += red[threadIdx.x + s];
     __syncthreads();
   }
-  if (threadIdx.x == 0) inv_norm[mat] = static_cast<float>(1.0 / (sqrt(red[0]) + static_cast<double>(eps)));
+  // the internal buffers hold c X0 with c = rec.xscale, a power of two (exact; keeps fp16 away from its subnormals)
+  if (threadIdx.x == 0)
+    inv_norm[mat] = static_cast<float>(static_cast<double>(recs[mat].xscale) / (sqrt(red[0]) + static_cast<double>(eps)));
 }
 
 // ---------------------------------------------------------------------------------------------- 2-D tile helpers
@@ -304,7 +342,7 @@ __global__ void __launch_bounds__(kThreads) apply_kernel(const MatRec* __restric
     const T* __restrict__ O = static_cast<const T*>(rec.O);
     uint16_t* __restrict__ W = static_cast<uint16_t*>(rec.W);
     const bool vec_ok = (rec.cols & 7) == 0;
-    const float s_o = lr * rec.scale;
+    const float s_o = kApply ? lr * rec.scale * rec.inv_xscale : rec.inv_xscale;    // the buffer holds c O
     if (rec.transposed) {
       // O(R, C) = Obuf[C][R]: stage Obuf rows [tC*64, +64), cols [tR*64, +64)  (always inside the padded buffer)
       __syncthreads();
@@ -346,12 +384,12 @@ __global__ void __launch_bounds__(kThreads) apply_kernel(const MatRec* __restric
           for (int e = 0; e < 8; ++e) w[e] = w[e] - fmaf(s_o, o[e], lr * wd * w[e]);
         } else {
 #pragma unroll
-          for (int e = 0; e < 8; ++e) w[e] = o[e];
+          for (int e = 0; e < 8; ++e) w[e] = o[e] * s_o;
         }
         *reinterpret_cast<uint4*>(wp) = pack8_bf16(w);
       } else {
         for (int e = 0; e < 8 && C + e < rec.cols; ++e) {
-          float w = o[e];
+          float w = o[e] * s_o;
           if (kApply) {
             const float w0 = bf16_bits_to_float(wp[e]);
             w = w0 - fmaf(s_o, o[e], lr * wd * w0);
@@ -364,8 +402,8 @@ __global__ void __launch_bounds__(kThreads) apply_kernel(const MatRec* __restric
 }
 
 // ---------------------------------------------------------------------------------------------- fast paths
-// Path A (matrix not transposed, rows and cols multiples of 128, fp16 workspace): the workspace buffer has the stored
-// layout, so normalise and apply are flat streaming passes: 4 x 16-byte loads per thread in flight, two elements per
+// Aligned matrices (rows and cols multiples of 128, fp16 workspace): the workspace buffer has the stored layout, so
+// normalise and (for steps = 0) apply are flat streaming passes: 4 x 16-byte loads per thread in flight, two elements per
 // arithmetic instruction (f32x2), one 16-byte store per 8 elements.
 __device__ __forceinline__ uint32_t float2_to_half2_bits(float2 f) {
   const __half2 h = __float22half2_rn(f);
@@ -440,7 +478,7 @@ __global__ void __launch_bounds__(kThreads) apply_flat_kernel(const MatRec* __re
     const int64_t start = (chunk - __ldg(prefix + mat)) * kFlatChunk;
     const uint16_t* __restrict__ O = static_cast<const uint16_t*>(rec.O) + start;
     uint16_t* __restrict__ W = static_cast<uint16_t*>(rec.W) + start;
-    const float so = lr * rec.scale, lrwd = lr * wd;
+    const float so = kApply ? lr * rec.scale * rec.inv_xscale : rec.inv_xscale, lrwd = lr * wd;   // the buffer holds c O
     const float2 so2 = make_float2(so, so), lrwd2 = make_float2(lrwd, lrwd);
     uint4 o4[kIter], w4[kIter];
     if (kMaster) {
@@ -467,119 +505,65 @@ __global__ void __launch_bounds__(kThreads) apply_flat_kernel(const MatRec* __re
       uint32_t r[4];
 #pragma unroll
       for (int e = 0; e < 4; ++e)
-        r[e] = kApply ? apply_word(ww[e], ow[e], so2, lrwd2) : float2_to_bf16x2(half2_bits_to_float2(ow[e]));
+        r[e] = kApply ? apply_word(ww[e], ow[e], so2, lrwd2) : float2_to_bf16x2(__fmul2_rn(half2_bits_to_float2(ow[e]), so2));
       *reinterpret_cast<uint4*>(W + (it * kThreads + threadIdx.x) * 8) = make_uint4(r[0], r[1], r[2], r[3]);
     }
   }
 }
 
-// Path B (matrix transposed, rows and cols multiples of 128, fp16 workspace): 64 x 64 tiles transposed as raw 16-bit
-// elements.  Thread (a, b) = (tid / 8, tid % 8) loads the source rows 2a, 2a+1, columns 8b .. 8b+7 (two 16-byte
-// loads), pairs the two rows column by column with PRMT into 32-bit words (src[2a][c], src[2a+1][c]) and stores word
-// a of transposed row c; then thread (c', k') reads 16 bytes = transposed row c', elements 8k' .. 8k'+7.  The 16-byte
-// chunks of a transposed row (128 B) are XOR-swizzled with (c & 7) ^ (c >> 3) so that both the word stores and the
-// 16-byte loads are free of bank conflicts.
-__device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {
-  uint32_t r;
-  asm("prmt.b32 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(sel));
-  return r;
-}
-__device__ __forceinline__ void transpose_tile16(const uint16_t* __restrict__ src, int64_t ld, uint32_t* tile,
-                                                 uint4 (&out)[2]) {
-  const int a = threadIdx.x >> 3, b = threadIdx.x & 7;
-  const uint4 r0 = __ldcs(reinterpret_cast<const uint4*>(src + static_cast<int64_t>(2 * a) * ld + 8 * b));
-  const uint4 r1 = __ldcs(reinterpret_cast<const uint4*>(src + static_cast<int64_t>(2 * a + 1) * ld + 8 * b));
-  const uint32_t w0[4] = {r0.x, r0.y, r0.z, r0.w}, w1[4] = {r1.x, r1.y, r1.z, r1.w};
-  __syncthreads();                                   // the previous tile has been read out
-#pragma unroll
-  for (int w = 0; w < 4; ++w) {
-#pragma unroll
-    for (int odd = 0; odd < 2; ++odd) {
-      const int c = 8 * b + 2 * w + odd;             // transposed row = source column
-      const int chunk = (a >> 2) ^ (c & 7) ^ (c >> 3);
-      tile[c * 32 + chunk * 4 + (a & 3)] = prmt(w0[w], w1[w], odd ? 0x7632u : 0x5410u);
-    }
-  }
-  __syncthreads();
-#pragma unroll
-  for (int h = 0; h < 2; ++h) {
-    const int c = a + 32 * h, k = b;
-    const int chunk = k ^ (c & 7) ^ ((c >> 3) & 7);
-    out[h] = *reinterpret_cast<const uint4*>(tile + c * 32 + chunk * 4);
-  }
+// ---------------------------------------------------------------------------------------------- AdamW
+// Non-matrix parameters (embeddings, norms, biases; PAPER.md:239 / Alg. 1 l.16 "non-matrix params: AdamW"): decoupled
+// weight decay (the paper's citation [16]), bias-corrected moments, fp32 moments and arithmetic, bf16
+// parameter rounded once (reading N17 of DESIGN.md).  One flat launch over all tensors: 24 B/element
+// (read p, g, m, v; write p, m, v).
+__device__ __forceinline__ float adamw_one(float p, float g, float& m, float& v, const AdamScalars& sc) {
+  m = fmaf(sc.beta1, m, (1.f - sc.beta1) * g);
+  v = fmaf(sc.beta2, v, (1.f - sc.beta2) * g * g);
+  const float denom = fmaf(sqrtf(v), sc.inv_sqrt_bc2, sc.eps);
+  const float decayed = p * (1.f - sc.lr * sc.wd);
+  return decayed - (sc.lr * sc.inv_bc1) * (m / denom);
 }
 
-template <bool kFromUser>
-__global__ void __launch_bounds__(kThreads) normalize_tr_kernel(const MatRec* __restrict__ recs,
-                                                                const int64_t* __restrict__ prefix, int count,
-                                                                int64_t total_tiles, const float* __restrict__ inv_norm) {
-  __shared__ __align__(16) uint32_t tile[kTile * 32];
-  for (int64_t t = blockIdx.x; t < total_tiles; t += gridDim.x) {
-    const int mat = find_matrix(prefix, count, t);
-    const MatRec& rec = recs[mat];
-    const int64_t local = t - __ldg(prefix + mat);
-    const int tiles_c = rec.cols / kTile;
-    const int tR = static_cast<int>(local / tiles_c), tC = static_cast<int>(local % tiles_c);
-    const uint16_t* __restrict__ src = static_cast<const uint16_t*>(kFromUser ? rec.W : rec.U);
-    uint16_t* __restrict__ dst = static_cast<uint16_t*>(rec.X0);
-    const float inv = __ldg(inv_norm + mat);
-    const float2 inv2 = make_float2(inv, inv);
-    uint4 v[2];
-    transpose_tile16(src + static_cast<int64_t>(tR) * kTile * rec.cols + tC * kTile, rec.cols, tile, v);
+__global__ void __launch_bounds__(kThreads) adamw_kernel(const AdamRec* __restrict__ recs,
+                                                         const int64_t* __restrict__ prefix, int count,
+                                                         int64_t total_chunks, const AdamScalars sc) {
+  constexpr int kIter = kFlatChunk / (kThreads * 8);
+  for (int64_t chunk = blockIdx.x; chunk < total_chunks; chunk += gridDim.x) {
+    const int t = find_matrix(prefix, count, chunk);
+    const AdamRec rec = recs[t];
+    const int64_t start = (chunk - __ldg(prefix + t)) * kFlatChunk;
+    const int64_t end = min(start + static_cast<int64_t>(kFlatChunk), rec.numel);
+    uint16_t* __restrict__ P = static_cast<uint16_t*>(rec.p);
+    const uint16_t* __restrict__ G = static_cast<const uint16_t*>(rec.g);
+    float* __restrict__ M = rec.m;
+    float* __restrict__ V = rec.v;
 #pragma unroll
-    for (int h = 0; h < 2; ++h) {
-      const uint32_t w[4] = {v[h].x, v[h].y, v[h].z, v[h].w};
-      uint32_t o[4];
+    for (int it = 0; it < kIter; ++it) {
+      const int64_t i = start + (static_cast<int64_t>(it) * kThreads + threadIdx.x) * 8;
+      if (i + 8 <= end) {
+        float p[8], g[8];
+        unpack8(__ldcs(reinterpret_cast<const uint4*>(P + i)), p);
+        unpack8(__ldcs(reinterpret_cast<const uint4*>(G + i)), g);
+        const float4 m0 = __ldcs(reinterpret_cast<const float4*>(M + i)), m1 = __ldcs(reinterpret_cast<const float4*>(M + i) + 1);
+        const float4 v0 = __ldcs(reinterpret_cast<const float4*>(V + i)), v1 = __ldcs(reinterpret_cast<const float4*>(V + i) + 1);
+        float m[8] = {m0.x, m0.y, m0.z, m0.w, m1.x, m1.y, m1.z, m1.w};
+        float v[8] = {v0.x, v0.y, v0.z, v0.w, v1.x, v1.y, v1.z, v1.w};
 #pragma unroll
-      for (int e = 0; e < 4; ++e) o[e] = float2_to_half2_bits(__fmul2_rn(bf16x2_to_float2(w[e]), inv2));
-      // X0[i][j] = src[j][i]: oriented row = stored column, leading dimension n_pad (= rows)
-      const int64_t i = tC * kTile + (threadIdx.x >> 3) + 32 * h, j = tR * kTile + (threadIdx.x & 7) * 8;
-      *reinterpret_cast<uint4*>(dst + i * rec.n_pad + j) = make_uint4(o[0], o[1], o[2], o[3]);
-    }
-  }
-}
-
-template <bool kApply, bool kMaster>
-__global__ void __launch_bounds__(kThreads) apply_tr_kernel(const MatRec* __restrict__ recs,
-                                                            const int64_t* __restrict__ prefix, int count,
-                                                            int64_t total_tiles, float lr, float wd) {
-  __shared__ __align__(16) uint32_t tile[kTile * 32];
-  for (int64_t t = blockIdx.x; t < total_tiles; t += gridDim.x) {
-    const int mat = find_matrix(prefix, count, t);
-    const MatRec& rec = recs[mat];
-    const int64_t local = t - __ldg(prefix + mat);
-    const int tiles_c = rec.cols / kTile;
-    const int tR = static_cast<int>(local / tiles_c), tC = static_cast<int>(local % tiles_c);
-    const uint16_t* __restrict__ O = static_cast<const uint16_t*>(rec.O);
-    uint16_t* __restrict__ W = static_cast<uint16_t*>(rec.W);
-    const float so = lr * rec.scale, lrwd = lr * wd;
-    const float2 so2 = make_float2(so, so), lrwd2 = make_float2(lrwd, lrwd);
-    // O(R, C) = Obuf[C][R]: the source tile is Obuf rows tC*64.., columns tR*64.. (leading dimension n_pad = rows)
-    uint4 w4[2];
-    constexpr bool master = kMaster;
-    if (kApply && !master) {
-#pragma unroll
-      for (int h = 0; h < 2; ++h) {
-        const int64_t R = tR * kTile + (threadIdx.x >> 3) + 32 * h, C = tC * kTile + (threadIdx.x & 7) * 8;
-        w4[h] = __ldcs(reinterpret_cast<const uint4*>(W + R * rec.cols + C));
+        for (int e = 0; e < 8; ++e) p[e] = adamw_one(p[e], g[e], m[e], v[e], sc);
+        *reinterpret_cast<uint4*>(P + i) = pack8_bf16(p);
+        reinterpret_cast<float4*>(M + i)[0] = make_float4(m[0], m[1], m[2], m[3]);
+        reinterpret_cast<float4*>(M + i)[1] = make_float4(m[4], m[5], m[6], m[7]);
+        reinterpret_cast<float4*>(V + i)[0] = make_float4(v[0], v[1], v[2], v[3]);
+        reinterpret_cast<float4*>(V + i)[1] = make_float4(v[4], v[5], v[6], v[7]);
+      } else {
+        for (int64_t j = i; j < end; ++j) {        // ragged tail of the tensor
+          float m = M[j], v = V[j];
+          const float pn = adamw_one(bf16_bits_to_float(P[j]), bf16_bits_to_float(G[j]), m, v, sc);
+          P[j] = static_cast<uint16_t>(float_to_bf16_bits(pn));
+          M[j] = m;
+          V[j] = v;
+        }
       }
-    }
-    uint4 v[2];
-    transpose_tile16(O + static_cast<int64_t>(tC) * kTile * rec.n_pad + tR * kTile, rec.n_pad, tile, v);
-#pragma unroll
-    for (int h = 0; h < 2; ++h) {
-      const int64_t R = tR * kTile + (threadIdx.x >> 3) + 32 * h, C = tC * kTile + (threadIdx.x & 7) * 8;
-      if (master) {
-        *reinterpret_cast<uint4*>(W + R * rec.cols + C) = apply8_master(rec.W32 + R * rec.cols + C, v[h], so2, lrwd2);
-        continue;
-      }
-      const uint32_t ow[4] = {v[h].x, v[h].y, v[h].z, v[h].w};
-      const uint32_t ww[4] = {w4[h].x, w4[h].y, w4[h].z, w4[h].w};
-      uint32_t r[4];
-#pragma unroll
-      for (int e = 0; e < 4; ++e)
-        r[e] = kApply ? apply_word(ww[e], ow[e], so2, lrwd2) : float2_to_bf16x2(half2_bits_to_float2(ow[e]));
-      *reinterpret_cast<uint4*>(W + R * rec.cols + C) = make_uint4(r[0], r[1], r[2], r[3]);
     }
   }
 }
@@ -601,13 +585,13 @@ __global__ void fill_scratch_kernel(uint32_t* __restrict__ p, size_t words) {
 // Test hook: copy one matrix's NS result out of the internal (oriented, padded) buffer as fp32, stored orientation.
 template <typename T>
 __global__ void export_kernel(const T* __restrict__ O, float* __restrict__ out, int rows, int cols, int n_pad,
-                              int transposed) {
+                              int transposed, float inv_xscale) {
   const int64_t total = static_cast<int64_t>(rows) * cols;
   for (int64_t i = blockIdx.x * static_cast<int64_t>(blockDim.x) + threadIdx.x; i < total;
        i += static_cast<int64_t>(gridDim.x) * blockDim.x) {
     const int r = static_cast<int>(i / cols), c = static_cast<int>(i % cols);
     const int64_t src = transposed ? static_cast<int64_t>(c) * n_pad + r : static_cast<int64_t>(r) * n_pad + c;
-    out[i] = static_cast<float>(O[src]);
+    out[i] = static_cast<float>(O[src]) * inv_xscale;
   }
 }
 
@@ -630,20 +614,21 @@ int launch_fill_scratch(void* ptr, size_t bytes, cudaStream_t s) {
 }
 
 int launch_export(const void* O, float* out, int rows, int cols, int n_pad, bool transposed, bool fp32_internal,
-                  cudaStream_t s) {
+                  float inv_xscale, cudaStream_t s) {
   const int64_t total = static_cast<int64_t>(rows) * cols;
   const int grid = grid_for((total + 255) / 256, 16);
-  if (fp32_internal) export_kernel<float><<<grid, 256, 0, s>>>(static_cast<const float*>(O), out, rows, cols, n_pad, transposed);
-  else export_kernel<__half><<<grid, 256, 0, s>>>(static_cast<const __half*>(O), out, rows, cols, n_pad, transposed);
+  if (fp32_internal) export_kernel<float><<<grid, 256, 0, s>>>(static_cast<const float*>(O), out, rows, cols, n_pad, transposed, inv_xscale);
+  else export_kernel<__half><<<grid, 256, 0, s>>>(static_cast<const __half*>(O), out, rows, cols, n_pad, transposed, inv_xscale);
   DMUON_CUDA_CHECK(cudaGetLastError());
   return DMUON_OK;
 }
 
-int launch_momentum(const ElemTables& T, float mu, cudaStream_t s) {
+int launch_momentum(const ElemTables& T, float mu, bool exact, cudaStream_t s) {
   if (T.flat_chunks == 0) return DMUON_OK;
   ProfScope ps("momentum_nesterov_sumsq", s);
-  flat_kernel<true><<<grid_for(T.flat_chunks, 8), kThreads, 0, s>>>(T.recs, T.flat_prefix, T.count, T.flat_chunks, mu,
-                                                                    T.partials);
+  if (exact) flat_kernel<true, true><<<grid_for(T.flat_chunks, 8), kThreads, 0, s>>>(T.recs, T.flat_prefix, T.count, T.flat_chunks, mu, T.partials);
+  else flat_kernel<true, false><<<grid_for(T.flat_chunks, 8), kThreads, 0, s>>>(T.recs, T.flat_prefix, T.count, T.flat_chunks, mu,
+                                                                          T.partials);
   DMUON_CUDA_CHECK(cudaGetLastError());
   return DMUON_OK;
 }
@@ -651,8 +636,8 @@ int launch_momentum(const ElemTables& T, float mu, cudaStream_t s) {
 int launch_sumsq(const ElemTables& T, cudaStream_t s) {
   if (T.flat_chunks == 0) return DMUON_OK;
   ProfScope ps("sumsq", s);
-  flat_kernel<false><<<grid_for(T.flat_chunks, 8), kThreads, 0, s>>>(T.recs, T.flat_prefix, T.count, T.flat_chunks, 0.f,
-                                                                     T.partials);
+  flat_kernel<false, false><<<grid_for(T.flat_chunks, 8), kThreads, 0, s>>>(T.recs, T.flat_prefix, T.count, T.flat_chunks, 0.f,
+                                                                            T.partials);
   DMUON_CUDA_CHECK(cudaGetLastError());
   return DMUON_OK;
 }
@@ -660,28 +645,22 @@ int launch_sumsq(const ElemTables& T, cudaStream_t s) {
 int launch_finalize_norms(const ElemTables& T, float eps, cudaStream_t s) {
   if (T.count == 0) return DMUON_OK;
   ProfScope ps("finalize_norms", s);
-  finalize_norms_kernel<<<T.count, kThreads, 0, s>>>(T.flat_prefix, T.partials, eps, T.inv_norm);
+  finalize_norms_kernel<<<T.count, kThreads, 0, s>>>(T.recs, T.flat_prefix, T.partials, eps, T.inv_norm);
   DMUON_CUDA_CHECK(cudaGetLastError());
   return DMUON_OK;
 }
 
 int launch_normalize(const ElemTables& T, bool from_user, bool fp32_internal, cudaStream_t s) {
-  if (T.ptiles + T.fa_chunks + T.fb_tiles == 0) return DMUON_OK;
+  if (T.ptiles + T.fa_chunks == 0) return DMUON_OK;
   if (T.fa_chunks > 0) {
-    ProfScope ps("normalize_orient_cast", s);
+    ProfScope ps("normalize_cast", s);
     const int g = grid_for(T.fa_chunks, 8);
     if (from_user) normalize_flat_kernel<true><<<g, kThreads, 0, s>>>(T.recs, T.fa_prefix, T.count, T.fa_chunks, T.inv_norm);
     else normalize_flat_kernel<false><<<g, kThreads, 0, s>>>(T.recs, T.fa_prefix, T.count, T.fa_chunks, T.inv_norm);
   }
-  if (T.fb_tiles > 0) {
-    ProfScope ps("normalize_orient_cast", s);
-    const int g = grid_for(T.fb_tiles, 8);
-    if (from_user) normalize_tr_kernel<true><<<g, kThreads, 0, s>>>(T.recs, T.fb_prefix, T.count, T.fb_tiles, T.inv_norm);
-    else normalize_tr_kernel<false><<<g, kThreads, 0, s>>>(T.recs, T.fb_prefix, T.count, T.fb_tiles, T.inv_norm);
-  }
   DMUON_CUDA_CHECK(cudaGetLastError());
   if (T.ptiles == 0) return DMUON_OK;
-  ProfScope ps("normalize_orient_cast", s);
+  ProfScope ps("normalize_cast", s);
   const int grid = grid_for(T.ptiles, 16);
 #define DMUON_NORM(TT, FU) \
   normalize_kernel<TT, FU><<<grid, kThreads, 0, s>>>(T.recs, T.ptile_prefix, T.count, T.ptiles, T.inv_norm)
@@ -693,16 +672,11 @@ int launch_normalize(const ElemTables& T, bool from_user, bool fp32_internal, cu
 }
 
 int launch_apply(const ElemTables& T, float lr, float wd, bool fp32_internal, bool master, cudaStream_t s) {
-  if (T.tiles + T.fa_chunks + T.fb_tiles == 0) return DMUON_OK;
+  if (T.tiles + T.fa_chunks == 0) return DMUON_OK;
   if (T.fa_chunks > 0) {
     ProfScope ps("apply_update", s);
     if (master) apply_flat_kernel<true, true><<<grid_for(T.fa_chunks, 8), kThreads, 0, s>>>(T.recs, T.fa_prefix, T.count, T.fa_chunks, lr, wd);
     else apply_flat_kernel<true, false><<<grid_for(T.fa_chunks, 8), kThreads, 0, s>>>(T.recs, T.fa_prefix, T.count, T.fa_chunks, lr, wd);
-  }
-  if (T.fb_tiles > 0) {
-    ProfScope ps("apply_update", s);
-    if (master) apply_tr_kernel<true, true><<<grid_for(T.fb_tiles, 8), kThreads, 0, s>>>(T.recs, T.fb_prefix, T.count, T.fb_tiles, lr, wd);
-    else apply_tr_kernel<true, false><<<grid_for(T.fb_tiles, 8), kThreads, 0, s>>>(T.recs, T.fb_prefix, T.count, T.fb_tiles, lr, wd);
   }
   DMUON_CUDA_CHECK(cudaGetLastError());
   if (T.tiles == 0) return DMUON_OK;
@@ -715,14 +689,10 @@ int launch_apply(const ElemTables& T, float lr, float wd, bool fp32_internal, bo
 }
 
 int launch_store_ns(const ElemTables& T, bool fp32_internal, cudaStream_t s) {
-  if (T.tiles + T.fa_chunks + T.fb_tiles == 0) return DMUON_OK;
+  if (T.tiles + T.fa_chunks == 0) return DMUON_OK;
   if (T.fa_chunks > 0) {
     ProfScope ps("store_ns_output", s);
     apply_flat_kernel<false, false><<<grid_for(T.fa_chunks, 8), kThreads, 0, s>>>(T.recs, T.fa_prefix, T.count, T.fa_chunks, 0.f, 0.f);
-  }
-  if (T.fb_tiles > 0) {
-    ProfScope ps("store_ns_output", s);
-    apply_tr_kernel<false, false><<<grid_for(T.fb_tiles, 8), kThreads, 0, s>>>(T.recs, T.fb_prefix, T.count, T.fb_tiles, 0.f, 0.f);
   }
   DMUON_CUDA_CHECK(cudaGetLastError());
   if (T.tiles == 0) return DMUON_OK;
@@ -730,6 +700,15 @@ int launch_store_ns(const ElemTables& T, bool fp32_internal, cudaStream_t s) {
   const int grid = grid_for(T.tiles, 16);
   if (fp32_internal) apply_kernel<float, false><<<grid, kThreads, 0, s>>>(T.recs, T.tile_prefix, T.count, T.tiles, 0.f, 0.f);
   else               apply_kernel<__half, false><<<grid, kThreads, 0, s>>>(T.recs, T.tile_prefix, T.count, T.tiles, 0.f, 0.f);
+  DMUON_CUDA_CHECK(cudaGetLastError());
+  return DMUON_OK;
+}
+
+int launch_adamw(const AdamRec* d_recs, const int64_t* d_prefix, int count, int64_t total_chunks, const AdamScalars& sc,
+                 cudaStream_t s) {
+  if (total_chunks == 0) return DMUON_OK;
+  ProfScope ps("adamw_update", s);
+  adamw_kernel<<<grid_for(total_chunks, 8), kThreads, 0, s>>>(d_recs, d_prefix, count, total_chunks, sc);
   DMUON_CUDA_CHECK(cudaGetLastError());
   return DMUON_OK;
 }

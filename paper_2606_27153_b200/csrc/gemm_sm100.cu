@@ -1,13 +1,20 @@
-// Persistent grouped GEMM family for the Gram-form Newton-Schulz step on sm_100a (steps a3, a4, a5 of DESIGN.md):
+// Persistent grouped GEMM family for the Gram-form Newton-Schulz step on sm_100a (steps a3, a4, a5 of DESIGN.md, and
+// step a6 fused into the last a5 epilogue):
 //
-//   OP_SYRK  C = alpha * X X^T                (PAPER.md:170 G = X X^T; symmetric kernel of PAPER.md:182)
-//   OP_SQ    C = alpha * A A + beta * A       (the polynomial in the Gram matrix; A A = A A^T)
-//   OP_BX    C = alpha * B X + beta * X       (X_{i+1} = P X_i with the a X term in the epilogue)
-//   OP_SQ2   C = alpha * A B + beta * D + beta2 * D2   (symmetric, two addends: the running product of the
-//                                              P_i = a_i I + B_i of a Gram block, Eq. 4)
+//   OP_SYRK    C = alpha X X^T                  (PAPER.md:170 G = X X^T; symmetric kernel of PAPER.md:182)
+//   OP_SYRK_T  C = alpha Y^T Y                  (the same Gram matrix of a tall matrix held as stored, Y = X^T)
+//   OP_SQ      C = alpha A B^T + beta D         (the polynomial in the Gram matrix; A A = A A^T)
+//   OP_SQ2     C = alpha A B^T + beta D + beta2 D2   (symmetric, two addends: the running product of the
+//                                                P_i = a_i I + B_i of a Gram block, Eq. 4)
+//   OP_BX      C = alpha R X + beta X           (X_{i+1} = P X_i with the a X term in the epilogue)
+//   OP_XB      C = alpha Y R + beta Y           (the same update of a tall matrix held as stored)
 //
-// Two tilings of the same warp-specialised pipeline (warp 0 = TMA producer, warp 1 = tcgen05.mma issuer and TMEM
-// owner, warps 2..5 = epilogue: TMEM -> registers -> global):
+// Epilogues of the two X updates ("elementwise operations ... fused into the same epilogue"): fp16 store
+// of the new X; or, for the LAST update of a call, the Muon update itself W' = W - lr (scale O + wd W) (Eq. 1
+// PAPER.md:51) on bf16 weights or on fp32 master weights, or the bf16 NS output of dmuon_ns_batched.
+//
+// Two tilings of one warp-specialised pipeline (warp 0 = TMA producer, warp 1 = tcgen05.mma issuer and TMEM owner,
+// warps 2..5 = epilogue: TMEM -> registers -> global):
 //
 //   single CTA  (cta_group::1)  one CTA per SM computes a 128 x 128 or 128 x 256 unit; 4-stage ring of 48 KB.
 //   CTA pair    (cta_group::2)  a cluster of two CTAs (one TPC) computes a 256 x 256 unit with UMMA M = 256, N = 256:
@@ -37,6 +44,9 @@ constexpr int kNumThreads = 192;
 constexpr int kTmemCols = 512;
 constexpr int kAccCols = 256;                   // columns per accumulator stage
 constexpr int kMaxStages = 6;
+#ifndef DMUON_EPI_SLEEP_NS
+#define DMUON_EPI_SLEEP_NS 256                  // back-off of the epilogue warps' accumulator wait (0 = plain polling)
+#endif
 
 template <bool kPair> struct Tiling;
 template <> struct Tiling<false> {              // one CTA: A block + up to two B blocks per stage
@@ -57,39 +67,77 @@ struct SmemCtl {
   uint32_t pad;
 };
 static_assert(sizeof(SmemCtl) <= 256, "SmemCtl");
+constexpr int kEpiTileBytes = 32 * 64;         // 32 rows x 32 fp16: one warp's 32-column chunk, or its transpose
+constexpr int kEpiStageBytes = 4 * 2 * kEpiTileBytes;   // per epilogue warp: a direct and a mirrored tile
 template <bool kPair> constexpr int smem_bytes() {
-  return Tiling<kPair>::kStages * Tiling<kPair>::kStageBytes + 1024 /*alignment slack*/ + 256 /*SmemCtl*/;
+  return Tiling<kPair>::kStages * Tiling<kPair>::kStageBytes + 1024 /*alignment slack*/ + 256 /*SmemCtl*/ + kEpiStageBytes;
 }
 
+struct Scalars {
+  float alpha, beta, beta2;
+  float lr, lrwd;
+  int store_c;     // fused epilogues: also store fp16(x) to C
+  int rec_base;    // MatRec of problem p = recs[rec_base + probs[p].rec]
+};
+
+__host__ __device__ constexpr bool op_symmetric(int op) { return op == OP_SYRK || op == OP_SQ || op == OP_SQ2 || op == OP_SYRK_T; }
+__host__ __device__ constexpr bool op_a_mn(int op) { return op == OP_SYRK_T; }
+__host__ __device__ constexpr bool op_b_mn(int op) { return op == OP_BX || op == OP_SYRK_T; }
+__host__ __device__ constexpr bool op_has_addend(int op) { return op != OP_SYRK && op != OP_SYRK_T; }
+
 // ------------------------------------------------------------------------------------------------ epilogue
-// Addend words of one 32-column chunk of one row: 64 bytes of D (and of D2 for OP_SQ2).  Loaded one chunk ahead of the
-// arithmetic (two register sets, alternating) so that their L2 latency overlaps the TMEM load and the stores of the
-// previous chunk: with short contractions (K <= 1024) the epilogue, not the mainloop, sets the pace.
+// Addend words of one 32-column chunk of one row: 64 bytes of D (and of D2 for OP_SQ2, of the bf16 W for EPI_APPLY).
+// Loaded one chunk ahead of the arithmetic (two register sets, alternating) so that their L2 latency overlaps the
+// TMEM load and the stores of the previous chunk: with short contractions (K <= 1024) the epilogue, not the mainloop,
+// sets the pace.
 struct Addends {
   uint4 d[4];
   uint4 e[4];
 };
-template <int kOp>
-__device__ __forceinline__ void load_addends(Addends& a, const __half* __restrict__ D, const __half* __restrict__ D2,
-                                             int64_t ldc, int64_t grow, int64_t gcol) {
-  if (kOp == OP_SYRK) return;
-  const uint4* dp = reinterpret_cast<const uint4*>(D + grow * ldc + gcol);
+// Per-unit epilogue context (pointers of the unit's problem).
+struct EpiCtx {
+  __half* C;
+  const __half* D;
+  const __half* D2;
+  uint16_t* W;        // bf16 parameter / output (fused epilogues)
+  float* W32;         // fp32 master (EPI_APPLY_MASTER)
+  int64_t ldc;
+  float so;           // EPI_APPLY*: lr * scale / c ; EPI_BF16: 1 / c
+};
+
+template <int kOp, int kEpi>
+__device__ __forceinline__ void load_addends(Addends& a, const EpiCtx& x, int64_t grow, int64_t gcol) {
+  if (op_has_addend(kOp)) {
+    const uint4* dp = reinterpret_cast<const uint4*>(x.D + grow * x.ldc + gcol);
 #pragma unroll
-  for (int g = 0; g < 4; ++g) a.d[g] = __ldg(dp + g);
+    for (int g = 0; g < 4; ++g) a.d[g] = __ldg(dp + g);
+  }
   if (kOp == OP_SQ2) {
-    const uint4* ep = reinterpret_cast<const uint4*>(D2 + grow * ldc + gcol);
+    const uint4* ep = reinterpret_cast<const uint4*>(x.D2 + grow * x.ldc + gcol);
 #pragma unroll
     for (int g = 0; g < 4; ++g) a.e[g] = __ldg(ep + g);
   }
+  if (kEpi == EPI_APPLY) {
+    // W comes from DRAM.  Through L1 (ld.global.nc): a lane reads its row's 64 bytes as four 16-byte loads, the first
+    // brings the sectors in and the other three hit.  A streaming load (ld.global.cs, evict-first) sent all four to
+    // L2/DRAM and halved the throughput of the whole fused X update (profiles/r2_experiments.md).
+    const uint4* wp = reinterpret_cast<const uint4*>(x.W + grow * x.ldc + gcol);
+#pragma unroll
+    for (int g = 0; g < 4; ++g) a.e[g] = __ldg(wp + g);
+  }
+}
+
+__device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
+  const __nv_bfloat162 b = __floats2bfloat162_rn(lo, hi);
+  return *reinterpret_cast<const uint32_t*>(&b);
 }
 
 // One 32-column chunk of one accumulator row: v = 32 fp32 accumulators of row `grow`, columns [gcol, gcol + 32).
-template <int kOp>
-__device__ __forceinline__ void epilogue_chunk(const uint32_t (&v)[32], const Addends& a, __half* __restrict__ C,
-                                               int64_t ldc, int64_t grow, int64_t gcol, float alpha, float beta,
-                                               float beta2, bool mirror) {
-  uint32_t o[16];
-  if (kOp != OP_SYRK) {
+template <int kOp, int kEpi>
+__device__ __forceinline__ void epilogue_chunk(const uint32_t (&v)[32], const Addends& a, const EpiCtx& x,
+                                               int64_t grow, int64_t gcol, const Scalars& sc, bool mirror, uint32_t stage) {
+  float r[32];
+  if (op_has_addend(kOp)) {
 #pragma unroll
     for (int g = 0; g < 4; ++g) {
       const uint32_t dw[4] = {a.d[g].x, a.d[g].y, a.d[g].z, a.d[g].w};
@@ -97,46 +145,119 @@ __device__ __forceinline__ void epilogue_chunk(const uint32_t (&v)[32], const Ad
 #pragma unroll
       for (int e = 0; e < 4; ++e) {
         const float2 df = __half22float2(*reinterpret_cast<const __half2*>(&dw[e]));
-        float ax = beta * df.x, ay = beta * df.y;
+        float ax = sc.beta * df.x, ay = sc.beta * df.y;
         if (kOp == OP_SQ2) {
           const float2 ef = __half22float2(*reinterpret_cast<const __half2*>(&ew[e]));
-          ax = fmaf(beta2, ef.x, ax);
-          ay = fmaf(beta2, ef.y, ay);
+          ax = fmaf(sc.beta2, ef.x, ax);
+          ay = fmaf(sc.beta2, ef.y, ay);
         }
-        const float lo = fmaf(alpha, __uint_as_float(v[g * 8 + e * 2]), ax);
-        const float hi = fmaf(alpha, __uint_as_float(v[g * 8 + e * 2 + 1]), ay);
-        o[g * 4 + e] = pack_half2(lo, hi);
+        r[g * 8 + e * 2] = fmaf(sc.alpha, __uint_as_float(v[g * 8 + e * 2]), ax);
+        r[g * 8 + e * 2 + 1] = fmaf(sc.alpha, __uint_as_float(v[g * 8 + e * 2 + 1]), ay);
       }
     }
   } else {
 #pragma unroll
-    for (int e = 0; e < 16; ++e)
-      o[e] = pack_half2(alpha * __uint_as_float(v[2 * e]), alpha * __uint_as_float(v[2 * e + 1]));
+    for (int e = 0; e < 32; ++e) r[e] = sc.alpha * __uint_as_float(v[e]);
   }
-  uint4* cp = reinterpret_cast<uint4*>(C + grow * ldc + gcol);
+  if (kEpi == EPI_F16 || sc.store_c) {
+    // fp16 store of the chunk (32 rows x 32 columns per warp) and, for symmetric results, of its mirror image.  Both go
+    // through a warp-private shared-memory tile so that every global store instruction writes whole 64-byte row segments
+    // (8 rows x 64 B per instruction): one lane per row would write 32 half-sectors per instruction, and the mirror
+    // would take 32 two-byte stores per lane.  Tile: 32 rows x 64 B, 16-byte chunks XOR-swizzled by (row >> 1) & 3.
+    uint32_t o[16];
 #pragma unroll
-  for (int g = 0; g < 4; ++g) cp[g] = make_uint4(o[g * 4], o[g * 4 + 1], o[g * 4 + 2], o[g * 4 + 3]);
-  if (kOp != OP_BX && mirror) {
-    // mirrored store C[col][row]: for a fixed column the 32 lanes hold 32 consecutive rows -> 64-byte runs
-    __half* mp = C + gcol * ldc + grow;
+    for (int e = 0; e < 16; ++e) o[e] = pack_half2(r[2 * e], r[2 * e + 1]);
+    const int lane = threadIdx.x & 31;
+    const bool do_mirror = op_symmetric(kOp) && mirror;
+    __syncwarp();                                        // the previous chunk's tiles have been read out
 #pragma unroll
-    for (int e = 0; e < 16; ++e) {
-      const __half2 h = *reinterpret_cast<const __half2*>(&o[e]);
-      mp[static_cast<int64_t>(2 * e) * ldc] = __low2half(h);
-      mp[static_cast<int64_t>(2 * e + 1) * ldc] = __high2half(h);
+    for (int g = 0; g < 4; ++g)
+      st_shared_v4(stage + lane * 64 + ((g ^ ((lane >> 1) & 3)) << 4), o[g * 4], o[g * 4 + 1], o[g * 4 + 2], o[g * 4 + 3]);
+    if (do_mirror) {
+      // transposed tile: T[c][lane] = element (row lane, column c)
+      const uint32_t tbase = stage + kEpiTileBytes + ((lane & 7) << 1);
+#pragma unroll
+      for (int e = 0; e < 16; ++e) {
+        const int c0 = 2 * e, c1 = 2 * e + 1;
+        st_shared_u16(tbase + c0 * 64 + (((lane >> 3) ^ ((c0 >> 1) & 3)) << 4), o[e] & 0xFFFFu);
+        st_shared_u16(tbase + c1 * 64 + (((lane >> 3) ^ ((c1 >> 1) & 3)) << 4), o[e] >> 16);
+      }
     }
+    __syncwarp();
+    const int64_t wrow0 = grow - lane;                   // first row of this warp's 32 rows
+    const int ch = lane & 3;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const int rr = (lane >> 2) + 8 * i;
+      const uint4 v = ld_shared_v4(stage + rr * 64 + ((ch ^ ((rr >> 1) & 3)) << 4));
+      *reinterpret_cast<uint4*>(x.C + (wrow0 + rr) * x.ldc + gcol + ch * 8) = v;
+    }
+    if (do_mirror) {
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        const int cc = (lane >> 2) + 8 * i;              // a column of the chunk = a row of the mirrored block
+        const uint4 v = ld_shared_v4(stage + kEpiTileBytes + cc * 64 + ((ch ^ ((cc >> 1) & 3)) << 4));
+        *reinterpret_cast<uint4*>(x.C + (gcol + cc) * x.ldc + wrow0 + ch * 8) = v;
+      }
+    }
+  }
+  if (kEpi == EPI_BF16) {
+    // NS output of dmuon_ns_batched: out = bf16(x / c), c a power of two
+    uint32_t o[16];
+#pragma unroll
+    for (int e = 0; e < 16; ++e) o[e] = pack_bf16x2(r[2 * e] * x.so, r[2 * e + 1] * x.so);
+    uint4* wp = reinterpret_cast<uint4*>(x.W + grow * x.ldc + gcol);
+#pragma unroll
+    for (int g = 0; g < 4; ++g) wp[g] = make_uint4(o[g * 4], o[g * 4 + 1], o[g * 4 + 2], o[g * 4 + 3]);
+  } else if (kEpi == EPI_APPLY) {
+    // a6 (Eq. 1; readings N4, N5): W' = W - (lr scale O + lr wd W), one fp32 expression, one RNE rounding
+    uint32_t o[16];
+#pragma unroll
+    for (int g = 0; g < 4; ++g) {
+      const uint32_t ww[4] = {a.e[g].x, a.e[g].y, a.e[g].z, a.e[g].w};
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {
+        const float w0 = __uint_as_float(ww[e] << 16), w1 = __uint_as_float(ww[e] & 0xFFFF0000u);
+        const float t0 = fmaf(x.so, r[g * 8 + e * 2], sc.lrwd * w0);
+        const float t1 = fmaf(x.so, r[g * 8 + e * 2 + 1], sc.lrwd * w1);
+        o[g * 4 + e] = pack_bf16x2(w0 - t0, w1 - t1);
+      }
+    }
+    uint4* wp = reinterpret_cast<uint4*>(x.W + grow * x.ldc + gcol);
+#pragma unroll
+    for (int g = 0; g < 4; ++g) wp[g] = make_uint4(o[g * 4], o[g * 4 + 1], o[g * 4 + 2], o[g * 4 + 3]);
+  } else if (kEpi == EPI_APPLY_MASTER) {
+    // fp32 master weights: the update lands in the master, the bf16 parameter is its rounding
+    float4* mp = reinterpret_cast<float4*>(x.W32 + grow * x.ldc + gcol);
+    uint32_t o[16];
+#pragma unroll
+    for (int g = 0; g < 8; ++g) {
+      const float4 w = mp[g];
+      float4 n;
+      n.x = w.x - fmaf(x.so, r[g * 4], sc.lrwd * w.x);
+      n.y = w.y - fmaf(x.so, r[g * 4 + 1], sc.lrwd * w.y);
+      n.z = w.z - fmaf(x.so, r[g * 4 + 2], sc.lrwd * w.z);
+      n.w = w.w - fmaf(x.so, r[g * 4 + 3], sc.lrwd * w.w);
+      mp[g] = n;
+      o[g * 2] = pack_bf16x2(n.x, n.y);
+      o[g * 2 + 1] = pack_bf16x2(n.z, n.w);
+    }
+    uint4* wp = reinterpret_cast<uint4*>(x.W + grow * x.ldc + gcol);
+#pragma unroll
+    for (int g = 0; g < 4; ++g) wp[g] = make_uint4(o[g * 4], o[g * 4 + 1], o[g * 4 + 2], o[g * 4 + 3]);
   }
 }
 
 // ------------------------------------------------------------------------------------------------ the kernel body
 // mb, nb: extent of the output in 128-blocks (rows, columns); pair units may overhang it (TMA zero-fills the
 // operands there, the epilogue skips those blocks).
-template <int kOp, bool kPair>
+template <int kOp, bool kPair, int kEpi>
 __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ probs, const TileUnit* __restrict__ units,
-                                             int units_per_problem, int total_units, int k_blocks, int mb, int nb,
-                                             float alpha, float beta, float beta2) {
-  constexpr bool kSym = (kOp != OP_BX);
-  constexpr bool kBMn = (kOp == OP_BX);
+                                             const MatRec* __restrict__ recs, int units_per_problem, int total_units,
+                                             int k_blocks, int mb, int nb, const Scalars sc) {
+  constexpr bool kSym = op_symmetric(kOp);
+  constexpr bool kAMn = op_a_mn(kOp);
+  constexpr bool kBMn = op_b_mn(kOp);
   constexpr int kCG = kPair ? 2 : 1;
   constexpr int kStages = Tiling<kPair>::kStages;
   constexpr int kStageBytes = Tiling<kPair>::kStageBytes;
@@ -204,7 +325,12 @@ __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ pro
           if (!kPair) {
             const uint32_t fb = bar_full + 8 * stage;
             mbar_expect_tx(fb, kBlockBytes + w * kBlockBytes);
-            tma_load_2d(sA, tmA, kb * kBlkK, a_blk * kBlk, fb);
+            if (!kAMn) {
+              tma_load_2d(sA, tmA, kb * kBlkK, a_blk * kBlk, fb);
+            } else {
+              tma_load_2d(sA, tmA, a_blk * kBlk, kb * kBlkK, fb);                 // 64 (m) x 64 (k) boxes, 8 KB each
+              tma_load_2d(sA + kBlockBytes / 2, tmA, a_blk * kBlk + 64, kb * kBlkK, fb);
+            }
             if (!kBMn) {
               for (int q = 0; q < w; ++q) tma_load_2d(sB + q * kBlockBytes, tmB, kb * kBlkK, (b_blk + q) * kBlk, fb);
             } else {
@@ -215,7 +341,12 @@ __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ pro
             // both halves of the stage are accounted on the leader's barrier (its MMA thread waits there)
             if (rank == 0) mbar_expect_tx(bar_full + 8 * stage, 2 * kStageBytes);
             const uint32_t fb = mapa(bar_full + 8 * stage, 0);
-            tma_load_2d_pair(sA, tmA, kb * kBlkK, a_blk * kBlk, fb);
+            if (!kAMn) {
+              tma_load_2d_pair(sA, tmA, kb * kBlkK, a_blk * kBlk, fb);
+            } else {
+              tma_load_2d_pair(sA, tmA, a_blk * kBlk, kb * kBlkK, fb);
+              tma_load_2d_pair(sA + kBlockBytes / 2, tmA, a_blk * kBlk + 64, kb * kBlkK, fb);
+            }
             if (!kBMn) {
               tma_load_2d_pair(sB, tmB, kb * kBlkK, b_blk * kBlk, fb);
             } else {
@@ -237,7 +368,7 @@ __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ pro
       for (int u = worker; u < total_units; u += num_workers, ++it) {
         const int p = u / units_per_problem;
         const TileUnit tu = units[u - p * units_per_problem];
-        const uint32_t idesc = make_idesc(kPair ? 256 : 128, kPair ? 256 : tu.width * kBlk, kBMn);
+        const uint32_t idesc = make_idesc(kPair ? 256 : 128, kPair ? 256 : tu.width * kBlk, kAMn, kBMn);
         const int as = it & 1;
         const uint32_t aphase = (it >> 1) & 1;
         mbar_wait(bar_tempty + 8 * as, aphase ^ 1);    // epilogue has drained this accumulator
@@ -250,7 +381,7 @@ __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ pro
           const uint32_t sB = sA + kBlockBytes;
 #pragma unroll
           for (int k = 0; k < kBlkK / 16; ++k) {
-            const uint64_t ad = desc_kmajor(sA + k * 32);
+            const uint64_t ad = kAMn ? desc_mnmajor(sA + k * 2048) : desc_kmajor(sA + k * 32);
             const uint64_t bd = kBMn ? desc_mnmajor(sB + k * 2048) : desc_kmajor(sB + k * 32);
             mma_f16<kCG>(d_tmem, ad, bd, idesc, (kb | k) != 0);
           }
@@ -267,16 +398,27 @@ __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ pro
     // ================================================================== epilogue (4 warps, one TMEM lane quarter each)
     const int q = warp & 3;
     const int row = q * 32 + lane;
+    const uint32_t epi_stage = ctl_addr + 256 + q * (2 * kEpiTileBytes);      // this warp's two store tiles
     const uint32_t tempty_leader = kPair ? mapa(bar_tempty, 0) : bar_tempty;
     int it = 0;
     for (int u = worker; u < total_units; u += num_workers, ++it) {
       const int p = u / units_per_problem;
       const TileUnit tu = units[u - p * units_per_problem];
       const GemmProblem* pr = probs + p;
-      __half* __restrict__ C = pr->C;
-      const __half* __restrict__ D = pr->D;
-      const __half* __restrict__ D2 = pr->D2;
-      const int64_t ldc = pr->ldc;
+      EpiCtx x;
+      x.C = pr->C;
+      x.D = pr->D;
+      x.D2 = pr->D2;
+      x.ldc = pr->ldc;
+      x.W = nullptr;
+      x.W32 = nullptr;
+      x.so = 0.f;
+      if (kEpi != EPI_F16) {
+        const MatRec& rec = recs[sc.rec_base + pr->rec];
+        x.W = static_cast<uint16_t*>(rec.W);
+        x.W32 = rec.W32;
+        x.so = kEpi == EPI_BF16 ? rec.inv_xscale : sc.lr * rec.scale * rec.inv_xscale;
+      }
       const int as = it & 1;
       const uint32_t aphase = (it >> 1) & 1;
       const int bi = kPair ? 2 * tu.m_blk + static_cast<int>(rank) : tu.m_blk;      // row block of this CTA
@@ -292,21 +434,21 @@ __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ pro
         c_hi = (nb - bj0 < nbk ? nb - bj0 : nbk) * 4;
       }
       Addends a0 = {}, a1 = {};
-      if (c_lo < c_hi) load_addends<kOp>(a0, D, D2, ldc, grow, gcol0 + c_lo * 32);   // before the accumulator is ready
-      mbar_wait(bar_tfull + 8 * as, aphase);
+      if (c_lo < c_hi) load_addends<kOp, kEpi>(a0, x, grow, gcol0 + c_lo * 32);   // before the accumulator is ready
+      mbar_wait_warp(bar_tfull + 8 * as, aphase, DMUON_EPI_SLEEP_NS);
       tcgen05_fence_after();
       const uint32_t taddr = tmem_base + as * kAccCols + (static_cast<uint32_t>(q * 32) << 16);
       for (int c = c_lo; c < c_hi; c += 2) {
         uint32_t v[32];
-        if (c + 1 < c_hi) load_addends<kOp>(a1, D, D2, ldc, grow, gcol0 + (c + 1) * 32);
+        if (c + 1 < c_hi) load_addends<kOp, kEpi>(a1, x, grow, gcol0 + (c + 1) * 32);
         tmem_ld_32x32(taddr + c * 32, v);
         tmem_wait_ld();
-        epilogue_chunk<kOp>(v, a0, C, ldc, grow, gcol0 + c * 32, alpha, beta, beta2, bj0 + (c >> 2) != bi);
+        epilogue_chunk<kOp, kEpi>(v, a0, x, grow, gcol0 + c * 32, sc, bj0 + (c >> 2) != bi, epi_stage);
         if (c + 1 < c_hi) {
-          if (c + 2 < c_hi) load_addends<kOp>(a0, D, D2, ldc, grow, gcol0 + (c + 2) * 32);
+          if (c + 2 < c_hi) load_addends<kOp, kEpi>(a0, x, grow, gcol0 + (c + 2) * 32);
           tmem_ld_32x32(taddr + (c + 1) * 32, v);
           tmem_wait_ld();
-          epilogue_chunk<kOp>(v, a1, C, ldc, grow, gcol0 + (c + 1) * 32, alpha, beta, beta2, bj0 + ((c + 1) >> 2) != bi);
+          epilogue_chunk<kOp, kEpi>(v, a1, x, grow, gcol0 + (c + 1) * 32, sc, bj0 + ((c + 1) >> 2) != bi, epi_stage);
         }
       }
       // accumulator fully read by this warp: hand it back to the MMA thread
@@ -323,258 +465,71 @@ __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ pro
   if (warp == 1) tmem_dealloc<kCG>(tmem_base, kTmemCols);
 }
 
-// ------------------------------------------------------------------------------------------------ CTA quad
-// Cluster of four CTAs = two CTA pairs (ranks 0,1 and 2,3), each pair computing one 256 x 256 unit with
-// cta_group::2 MMAs as above; the two units of a quad share one operand panel (same block row: operand A shared;
-// same block column: operand B shared), and the shared tiles are fetched from L2 ONCE and multicast by TMA into both
-// pairs' shared memories.  The pair tiling reads 128 FLOP per L2->SMEM byte, which is what bounds it (0.87-0.89 of the
-// tensor peak at any clock, profiles/r1_step_l4_ncu_full.md); a quad reads 171 FLOP/byte.
-//
-// Protocol differences to the pair tiling: the bytes landing in a pair's two shared memories are all accounted on that
-// pair leader's "full" barrier, whoever sent them (cta_group::2 TMA: unicast loads name the leader's barrier, multicast
-// loads name it through the cleared pair bit); "empty" barriers count two arrivals, one tcgen05.commit from each pair
-// leader, multicast to all four CTAs, so the quad moves through the ring in lockstep (a multicast may overwrite the
-// other pair's slot only when that pair has consumed it too).
-constexpr int kQuadThreads = 192;
-
-struct QuadCtl {
-  uint64_t full[kMaxStages];
-  uint64_t empty[kMaxStages];
-  uint64_t tmem_full[2];
-  uint64_t tmem_empty[2];
-  uint32_t tmem_base;
-  uint32_t pad;
-};
-static_assert(sizeof(QuadCtl) <= 256, "QuadCtl");
-
-template <int kOp>
-__device__ __forceinline__ void ns_gemm_quad_body(const GemmProblem* __restrict__ probs,
-                                                  const TileUnit* __restrict__ units, int units_per_problem,
-                                                  int total_units, int k_blocks, int mb, int nb, float alpha, float beta,
-                                                  float beta2) {
-  constexpr bool kSym = (kOp != OP_BX);
-  constexpr bool kBMn = (kOp == OP_BX);
-  constexpr int kStages = Tiling<true>::kStages;
-  constexpr int kStageBytes = Tiling<true>::kStageBytes;
-
-  extern __shared__ uint8_t smem_raw[];
-  const uint32_t raw = smem_u32(smem_raw);
-  const uint32_t base = (raw + 1023u) & ~1023u;
-  QuadCtl* ctl = reinterpret_cast<QuadCtl*>(smem_raw + (base - raw) + kStages * kStageBytes);
-  const uint32_t ctl_addr = base + kStages * kStageBytes;
-  const uint32_t bar_full = ctl_addr + offsetof(QuadCtl, full);
-  const uint32_t bar_empty = ctl_addr + offsetof(QuadCtl, empty);
-  const uint32_t bar_tfull = ctl_addr + offsetof(QuadCtl, tmem_full);
-  const uint32_t bar_tempty = ctl_addr + offsetof(QuadCtl, tmem_empty);
-
-  const int warp = threadIdx.x >> 5;
-  const int lane = threadIdx.x & 31;
-  const uint32_t rank = cluster_ctarank();          // 0..3
-  const uint32_t pair = rank >> 1;                  // which unit of the quad
-  const uint32_t half = rank & 1;                   // 0 = leader of the pair
-  const uint32_t leader = rank & ~1u;
-  const uint16_t pair_mask = static_cast<uint16_t>(3u << leader);
-  const int worker = blockIdx.x >> 2;
-  const int num_workers = gridDim.x >> 2;
-
-  if (threadIdx.x == 0) {
-    for (int s = 0; s < kStages; ++s) {
-      mbar_init(bar_full + 8 * s, 1);
-      mbar_init(bar_empty + 8 * s, 2);              // one commit from each pair leader
-    }
-    for (int s = 0; s < 2; ++s) {
-      mbar_init(bar_tfull + 8 * s, 1);
-      mbar_init(bar_tempty + 8 * s, 8);             // epilogue warps of both CTAs of the pair
-    }
-    fence_barrier_init();
-  }
-  if (warp == 1) tmem_alloc<2>(ctl_addr + offsetof(QuadCtl, tmem_base), kTmemCols);
-  tcgen05_fence_before();
-  cluster_sync();
-  tcgen05_fence_after();
-  const uint32_t tmem_base = ctl->tmem_base;
-
-  // unit of this CTA's pair within quad unit `tu`: pair 0 -> (m_blk, n_blk), pair 1 -> (width, flags)
-#define DMUON_QUAD_UNIT(tu, mu, nu, share_a, share_b)                      \
-  const int mu = pair ? (tu).width : (tu).m_blk;                          \
-  const int nu = pair ? (tu).flags : (tu).n_blk;                          \
-  const bool share_a = (tu).m_blk == (tu).width;                          \
-  const bool share_b = (tu).n_blk == (tu).flags;
-
-  if (warp == 0) {
-    // ================================================================== TMA producer (all four CTAs)
-    if (lane == 0) {
-      int stage = 0;
-      uint32_t phase = 0;
-      const uint16_t mc_mask = static_cast<uint16_t>((1u << half) | (1u << (half + 2)));   // same half of both pairs
-      for (int u = worker; u < total_units; u += num_workers) {
-        const int p = u / units_per_problem;
-        const TileUnit tu = units[u - p * units_per_problem];
-        const GemmProblem* pr = probs + p;
-        const uint64_t tmA = reinterpret_cast<uint64_t>(&pr->tmA);
-        const uint64_t tmB = reinterpret_cast<uint64_t>(&pr->tmB);
-        const int un = u + num_workers;
-        if (un < total_units) {
-          const int pn = un / units_per_problem;
-          if (pn != p) {
-            tma_prefetch_desc(reinterpret_cast<uint64_t>(&probs[pn].tmA));
-            tma_prefetch_desc(reinterpret_cast<uint64_t>(&probs[pn].tmB));
-          }
-        }
-        DMUON_QUAD_UNIT(tu, mu, nu, share_a, share_b)
-        const int a_blk = 2 * mu + static_cast<int>(half);
-        const int b_blk = 2 * nu + static_cast<int>(half);
-        for (int kb = 0; kb < k_blocks; ++kb) {
-          mbar_wait(bar_empty + 8 * stage, phase ^ 1);
-          const uint32_t sA = base + stage * kStageBytes;
-          const uint32_t sB = sA + kBlockBytes;
-          if (half == 0) mbar_expect_tx(bar_full + 8 * stage, 2 * kStageBytes);   // both CTAs' halves of the stage
-          const uint32_t fb = mapa(bar_full + 8 * stage, leader);                  // unicast: the leader's barrier
-          const uint32_t fm = bar_full + 8 * stage;                                // multicast: each pair's leader
-          if (!share_a) tma_load_2d_pair(sA, tmA, kb * kBlkK, a_blk * kBlk, fb);
-          else if (pair == 0) tma_load_2d_pair_mcast(sA, tmA, kb * kBlkK, a_blk * kBlk, fm, mc_mask);
-          if (!kBMn) {
-            if (!share_b) tma_load_2d_pair(sB, tmB, kb * kBlkK, b_blk * kBlk, fb);
-            else if (pair == 0) tma_load_2d_pair_mcast(sB, tmB, kb * kBlkK, b_blk * kBlk, fm, mc_mask);
-          } else {
-            if (!share_b) {
-              tma_load_2d_pair(sB, tmB, b_blk * kBlk, kb * kBlkK, fb);
-              tma_load_2d_pair(sB + kBlockBytes / 2, tmB, b_blk * kBlk + 64, kb * kBlkK, fb);
-            } else if (pair == 0) {
-              tma_load_2d_pair_mcast(sB, tmB, b_blk * kBlk, kb * kBlkK, fm, mc_mask);
-              tma_load_2d_pair_mcast(sB + kBlockBytes / 2, tmB, b_blk * kBlk + 64, kb * kBlkK, fm, mc_mask);
-            }
-          }
-          if (++stage == kStages) { stage = 0; phase ^= 1; }
-        }
-      }
-    }
-    __syncwarp();
-  } else if (warp == 1) {
-    // ================================================================== MMA issuer (leader CTA of each pair)
-    if (lane == 0 && half == 0) {
-      int stage = 0;
-      uint32_t phase = 0;
-      int it = 0;
-      const uint32_t idesc = make_idesc(256, 256, kBMn);
-      for (int u = worker; u < total_units; u += num_workers, ++it) {
-        const int as = it & 1;
-        const uint32_t aphase = (it >> 1) & 1;
-        mbar_wait(bar_tempty + 8 * as, aphase ^ 1);
-        tcgen05_fence_after();
-        const uint32_t d_tmem = tmem_base + as * kAccCols;
-        for (int kb = 0; kb < k_blocks; ++kb) {
-          mbar_wait(bar_full + 8 * stage, phase);
-          tcgen05_fence_after();
-          const uint32_t sA = base + stage * kStageBytes;
-          const uint32_t sB = sA + kBlockBytes;
-#pragma unroll
-          for (int k = 0; k < kBlkK / 16; ++k) {
-            const uint64_t ad = desc_kmajor(sA + k * 32);
-            const uint64_t bd = kBMn ? desc_mnmajor(sB + k * 2048) : desc_kmajor(sB + k * 32);
-            mma_f16<2>(d_tmem, ad, bd, idesc, (kb | k) != 0);
-          }
-          mma_commit_pair(bar_empty + 8 * stage, 0xF);           // slot consumed by this pair: tell all four CTAs
-          if (++stage == kStages) { stage = 0; phase ^= 1; }
-        }
-        mma_commit_pair(bar_tfull + 8 * as, pair_mask);
-      }
-    }
-    __syncwarp();
-  } else {
-    // ================================================================== epilogue (warps 2..5)
-    const int q = warp & 3;
-    const int row = q * 32 + lane;
-    const uint32_t tempty_leader = mapa(bar_tempty, leader);
-    int it = 0;
-    for (int u = worker; u < total_units; u += num_workers, ++it) {
-      const int p = u / units_per_problem;
-      const TileUnit tu = units[u - p * units_per_problem];
-      const GemmProblem* pr = probs + p;
-      __half* __restrict__ C = pr->C;
-      const __half* __restrict__ D = pr->D;
-      const __half* __restrict__ D2 = pr->D2;
-      const int64_t ldc = pr->ldc;
-      const int as = it & 1;
-      const uint32_t aphase = (it >> 1) & 1;
-      DMUON_QUAD_UNIT(tu, mu, nu, share_a, share_b)
-      const bool duplicate = share_a && share_b && pair == 1;     // odd leftover: pair 1 shadows pair 0, stores nothing
-      const int bi = 2 * mu + static_cast<int>(half);
-      const int bj0 = 2 * nu;
-      const int64_t grow = static_cast<int64_t>(bi) * kBlk + row;
-      const int64_t gcol0 = static_cast<int64_t>(bj0) * kBlk;
-      int c_lo = 0, c_hi = 0;
-      if (bi < mb && !duplicate) {
-        c_lo = (kSym && bi > bj0) ? (bi - bj0) * 4 : 0;
-        c_hi = (nb - bj0 < 2 ? nb - bj0 : 2) * 4;
-      }
-      Addends a0 = {}, a1 = {};
-      if (c_lo < c_hi) load_addends<kOp>(a0, D, D2, ldc, grow, gcol0 + c_lo * 32);
-      mbar_wait(bar_tfull + 8 * as, aphase);
-      tcgen05_fence_after();
-      const uint32_t taddr = tmem_base + as * kAccCols + (static_cast<uint32_t>(q * 32) << 16);
-      for (int c = c_lo; c < c_hi; c += 2) {
-        uint32_t v[32];
-        if (c + 1 < c_hi) load_addends<kOp>(a1, D, D2, ldc, grow, gcol0 + (c + 1) * 32);
-        tmem_ld_32x32(taddr + c * 32, v);
-        tmem_wait_ld();
-        epilogue_chunk<kOp>(v, a0, C, ldc, grow, gcol0 + c * 32, alpha, beta, beta2, bj0 + (c >> 2) != bi);
-        if (c + 1 < c_hi) {
-          if (c + 2 < c_hi) load_addends<kOp>(a0, D, D2, ldc, grow, gcol0 + (c + 2) * 32);
-          tmem_ld_32x32(taddr + (c + 1) * 32, v);
-          tmem_wait_ld();
-          epilogue_chunk<kOp>(v, a1, C, ldc, grow, gcol0 + (c + 1) * 32, alpha, beta, beta2, bj0 + ((c + 1) >> 2) != bi);
-        }
-      }
-      tcgen05_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive_cluster(tempty_leader + 8 * as);
-    }
-  }
-#undef DMUON_QUAD_UNIT
-
-  tcgen05_fence_before();
-  cluster_sync();
-  if (warp == 1) tmem_dealloc<2>(tmem_base, kTmemCols);
-}
-
-// One named entry point per product and tiling, so profiles (ncu -k) and launch lists tell them apart.
-#define DMUON_GEMM_ENTRY(name, op, pair)                                                                        \
+// One named entry point per product, tiling and epilogue, so profiles (ncu -k) and launch lists tell them apart.
+#define DMUON_GEMM_ENTRY(name, op, pair, epi)                                                                   \
   __global__ void __launch_bounds__(kNumThreads, 1)                                                             \
-  name(const GemmProblem* __restrict__ probs, const TileUnit* __restrict__ units, int units_per_problem,       \
-       int total_units, int k_blocks, int mb, int nb, float alpha, float beta, float beta2) {                   \
-    ns_gemm_body<op, pair>(probs, units, units_per_problem, total_units, k_blocks, mb, nb, alpha, beta, beta2); \
+  name(const GemmProblem* __restrict__ probs, const TileUnit* __restrict__ units,                               \
+       const MatRec* __restrict__ recs, int units_per_problem, int total_units, int k_blocks, int mb, int nb,   \
+       const Scalars sc) {                                                                                      \
+    ns_gemm_body<op, pair, epi>(probs, units, recs, units_per_problem, total_units, k_blocks, mb, nb, sc);      \
   }
-DMUON_GEMM_ENTRY(ns_syrk_xxt_kernel, OP_SYRK, false)
-DMUON_GEMM_ENTRY(ns_sq_poly_kernel, OP_SQ, false)
-DMUON_GEMM_ENTRY(ns_bx_update_kernel, OP_BX, false)
-DMUON_GEMM_ENTRY(ns_syrk_xxt_pair_kernel, OP_SYRK, true)
-DMUON_GEMM_ENTRY(ns_sq_poly_pair_kernel, OP_SQ, true)
-DMUON_GEMM_ENTRY(ns_bx_update_pair_kernel, OP_BX, true)
-DMUON_GEMM_ENTRY(ns_gram_acc_kernel, OP_SQ2, false)
-DMUON_GEMM_ENTRY(ns_gram_acc_pair_kernel, OP_SQ2, true)
+DMUON_GEMM_ENTRY(ns_syrk_xxt_kernel, OP_SYRK, false, EPI_F16)
+DMUON_GEMM_ENTRY(ns_syrk_xxt_pair_kernel, OP_SYRK, true, EPI_F16)
+DMUON_GEMM_ENTRY(ns_syrk_xtx_kernel, OP_SYRK_T, false, EPI_F16)
+DMUON_GEMM_ENTRY(ns_syrk_xtx_pair_kernel, OP_SYRK_T, true, EPI_F16)
+DMUON_GEMM_ENTRY(ns_sq_poly_kernel, OP_SQ, false, EPI_F16)
+DMUON_GEMM_ENTRY(ns_sq_poly_pair_kernel, OP_SQ, true, EPI_F16)
+DMUON_GEMM_ENTRY(ns_gram_acc_kernel, OP_SQ2, false, EPI_F16)
+DMUON_GEMM_ENTRY(ns_gram_acc_pair_kernel, OP_SQ2, true, EPI_F16)
+DMUON_GEMM_ENTRY(ns_bx_update_kernel, OP_BX, false, EPI_F16)
+DMUON_GEMM_ENTRY(ns_bx_update_pair_kernel, OP_BX, true, EPI_F16)
+DMUON_GEMM_ENTRY(ns_bx_out_kernel, OP_BX, false, EPI_BF16)
+DMUON_GEMM_ENTRY(ns_bx_out_pair_kernel, OP_BX, true, EPI_BF16)
+DMUON_GEMM_ENTRY(ns_bx_apply_kernel, OP_BX, false, EPI_APPLY)
+DMUON_GEMM_ENTRY(ns_bx_apply_pair_kernel, OP_BX, true, EPI_APPLY)
+DMUON_GEMM_ENTRY(ns_bx_apply_master_kernel, OP_BX, false, EPI_APPLY_MASTER)
+DMUON_GEMM_ENTRY(ns_bx_apply_master_pair_kernel, OP_BX, true, EPI_APPLY_MASTER)
+DMUON_GEMM_ENTRY(ns_xb_update_kernel, OP_XB, false, EPI_F16)
+DMUON_GEMM_ENTRY(ns_xb_update_pair_kernel, OP_XB, true, EPI_F16)
+DMUON_GEMM_ENTRY(ns_xb_out_kernel, OP_XB, false, EPI_BF16)
+DMUON_GEMM_ENTRY(ns_xb_out_pair_kernel, OP_XB, true, EPI_BF16)
+DMUON_GEMM_ENTRY(ns_xb_apply_kernel, OP_XB, false, EPI_APPLY)
+DMUON_GEMM_ENTRY(ns_xb_apply_pair_kernel, OP_XB, true, EPI_APPLY)
+DMUON_GEMM_ENTRY(ns_xb_apply_master_kernel, OP_XB, false, EPI_APPLY_MASTER)
+DMUON_GEMM_ENTRY(ns_xb_apply_master_pair_kernel, OP_XB, true, EPI_APPLY_MASTER)
 #undef DMUON_GEMM_ENTRY
 
-#define DMUON_QUAD_ENTRY(name, op)                                                                              \
-  __global__ void __launch_bounds__(kQuadThreads, 1)                                                            \
-  name(const GemmProblem* __restrict__ probs, const TileUnit* __restrict__ units, int units_per_problem,       \
-       int total_units, int k_blocks, int mb, int nb, float alpha, float beta, float beta2) {                   \
-    ns_gemm_quad_body<op>(probs, units, units_per_problem, total_units, k_blocks, mb, nb, alpha, beta, beta2);  \
-  }
-DMUON_QUAD_ENTRY(ns_syrk_xxt_quad_kernel, OP_SYRK)
-DMUON_QUAD_ENTRY(ns_sq_poly_quad_kernel, OP_SQ)
-DMUON_QUAD_ENTRY(ns_bx_update_quad_kernel, OP_BX)
-DMUON_QUAD_ENTRY(ns_gram_acc_quad_kernel, OP_SQ2)
-#undef DMUON_QUAD_ENTRY
+typedef void (*GemmKernel)(const GemmProblem*, const TileUnit*, const MatRec*, int, int, int, int, int, const Scalars);
 
-typedef void (*GemmKernel)(const GemmProblem*, const TileUnit*, int, int, int, int, int, float, float, float);
+struct KernelEntry {
+  GemmKernel fn[2];                      // [single, pair]
+  bool configured[2][kMaxDevices];       // cudaFuncSetAttribute is per device
+};
+
+// [op][epilogue]; null = combination does not exist (fused epilogues belong to the two X updates)
+KernelEntry g_kernels[kNumOps][kNumEpi] = {
+    /* OP_SYRK   */ {{{ns_syrk_xxt_kernel, ns_syrk_xxt_pair_kernel}}, {}, {}, {}},
+    /* OP_SQ     */ {{{ns_sq_poly_kernel, ns_sq_poly_pair_kernel}}, {}, {}, {}},
+    /* OP_BX     */ {{{ns_bx_update_kernel, ns_bx_update_pair_kernel}}, {{ns_bx_out_kernel, ns_bx_out_pair_kernel}},
+                     {{ns_bx_apply_kernel, ns_bx_apply_pair_kernel}},
+                     {{ns_bx_apply_master_kernel, ns_bx_apply_master_pair_kernel}}},
+    /* OP_SQ2    */ {{{ns_gram_acc_kernel, ns_gram_acc_pair_kernel}}, {}, {}, {}},
+    /* OP_SYRK_T */ {{{ns_syrk_xtx_kernel, ns_syrk_xtx_pair_kernel}}, {}, {}, {}},
+    /* OP_XB     */ {{{ns_xb_update_kernel, ns_xb_update_pair_kernel}}, {{ns_xb_out_kernel, ns_xb_out_pair_kernel}},
+                     {{ns_xb_apply_kernel, ns_xb_apply_pair_kernel}},
+                     {{ns_xb_apply_master_kernel, ns_xb_apply_master_pair_kernel}}},
+};
 
 template <bool kPair>
-int launch_op(GemmKernel kern, bool* configured, const GemmLaunch& L, cudaStream_t stream) {
+int launch_op(KernelEntry& ke, const GemmLaunch& L, cudaStream_t stream) {
   constexpr int kSmem = smem_bytes<kPair>();
-  if (!*configured) {
+  GemmKernel kern = ke.fn[kPair ? 1 : 0];
+  int dev = 0;
+  DMUON_CUDA_CHECK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kMaxDevices) { set_error("launch_ns_gemm: device ordinal %d is not supported", dev); return DMUON_ERR_UNSUPPORTED_DEVICE; }
+  if (!ke.configured[kPair ? 1 : 0][dev]) {
     DMUON_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem));
-    *configured = true;
+    ke.configured[kPair ? 1 : 0][dev] = true;
   }
   const int total = L.units_per_problem * L.num_problems;
   if (total <= 0) return DMUON_OK;
@@ -592,43 +547,9 @@ int launch_op(GemmKernel kern, bool* configured, const GemmLaunch& L, cudaStream
   attr[0].val.clusterDim.z = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  DMUON_CUDA_CHECK(cudaLaunchKernelEx(&cfg, kern, L.problems, L.units, L.units_per_problem, total, L.k_blocks,
-                                      L.m_blocks, L.n_blocks, L.alpha, L.beta, L.beta2));
-  return DMUON_OK;
-}
-
-// Quad launch: clusters of 4; as many clusters as can be co-resident (GPC boundaries may leave a few SMs unused).
-int launch_quad(GemmKernel kern, int slot, const GemmLaunch& L, cudaStream_t stream) {
-  static bool configured[kNumOps] = {};
-  static int max_clusters[kNumOps] = {};
-  constexpr int kSmem = smem_bytes<true>();
-  const int total = L.units_per_problem * L.num_problems;
-  if (total <= 0) return DMUON_OK;
-  cudaLaunchConfig_t cfg = {};
-  cfg.blockDim = dim3(kQuadThreads);
-  cfg.dynamicSmemBytes = kSmem;
-  cfg.stream = stream;
-  cudaLaunchAttribute attr[1];
-  attr[0].id = cudaLaunchAttributeClusterDimension;
-  attr[0].val.clusterDim.x = 4;
-  attr[0].val.clusterDim.y = 1;
-  attr[0].val.clusterDim.z = 1;
-  cfg.attrs = attr;
-  cfg.numAttrs = 1;
-  if (!configured[slot]) {
-    DMUON_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem));
-    cfg.gridDim = dim3(4 * (L.grid / 4));
-    int n = 0;
-    DMUON_CUDA_CHECK(cudaOccupancyMaxActiveClusters(&n, kern, &cfg));
-    if (n < 1) { set_error("launch_quad: no cluster of 4 CTAs fits"); return DMUON_ERR_CUDA; }
-    max_clusters[slot] = n < L.grid / 4 ? n : L.grid / 4;
-    configured[slot] = true;
-    if (getenv("DMUON_LOG")) fprintf(stderr, "[dmuon] quad tiling op %d: %d co-resident clusters of 4 (occupancy query %d, %d SMs)\n", slot, max_clusters[slot], n, L.grid);
-  }
-  const int use = max_clusters[slot] < total ? max_clusters[slot] : total;
-  cfg.gridDim = dim3(4 * use);
-  DMUON_CUDA_CHECK(cudaLaunchKernelEx(&cfg, kern, L.problems, L.units, L.units_per_problem, total, L.k_blocks,
-                                      L.m_blocks, L.n_blocks, L.alpha, L.beta, L.beta2));
+  Scalars sc{L.alpha, L.beta, L.beta2, L.lr, L.lrwd, L.store_c ? 1 : 0, L.rec_base};
+  DMUON_CUDA_CHECK(cudaLaunchKernelEx(&cfg, kern, L.problems, L.units, L.recs, L.units_per_problem, total, L.k_blocks,
+                                      L.m_blocks, L.n_blocks, sc));
   return DMUON_OK;
 }
 
@@ -637,19 +558,18 @@ int launch_quad(GemmKernel kern, int slot, const GemmLaunch& L, cudaStream_t str
 int gemm_smem_bytes() { return smem_bytes<false>() > smem_bytes<true>() ? smem_bytes<false>() : smem_bytes<true>(); }
 
 int launch_ns_gemm(const GemmLaunch& L, cudaStream_t stream) {
-  static bool configured[2 * kNumOps] = {};
-  if (L.op < OP_SYRK || L.op >= kNumOps) {
-    set_error("launch_ns_gemm: bad op %d", static_cast<int>(L.op));
+  if (L.op < 0 || L.op >= kNumOps || L.epi < 0 || L.epi >= kNumEpi) {
+    set_error("launch_ns_gemm: bad op %d / epilogue %d", static_cast<int>(L.op), static_cast<int>(L.epi));
     return DMUON_ERR_INVALID_ARG;
   }
-  static const GemmKernel kSingle[kNumOps] = {ns_syrk_xxt_kernel, ns_sq_poly_kernel, ns_bx_update_kernel, ns_gram_acc_kernel};
-  static const GemmKernel kPairK[kNumOps] = {ns_syrk_xxt_pair_kernel, ns_sq_poly_pair_kernel, ns_bx_update_pair_kernel,
-                                             ns_gram_acc_pair_kernel};
-  static const GemmKernel kQuadK[kNumOps] = {ns_syrk_xxt_quad_kernel, ns_sq_poly_quad_kernel, ns_bx_update_quad_kernel,
-                                             ns_gram_acc_quad_kernel};
-  if (L.quad) return launch_quad(kQuadK[L.op], L.op, L, stream);
-  if (L.pair) return launch_op<true>(kPairK[L.op], &configured[kNumOps + L.op], L, stream);
-  return launch_op<false>(kSingle[L.op], &configured[L.op], L, stream);
+  KernelEntry& ke = g_kernels[L.op][L.epi];
+  if (!ke.fn[0]) {
+    set_error("launch_ns_gemm: op %d has no epilogue %d", static_cast<int>(L.op), static_cast<int>(L.epi));
+    return DMUON_ERR_INVALID_ARG;
+  }
+  if (L.epi != EPI_F16 && !L.recs) { set_error("launch_ns_gemm: fused epilogue without matrix records"); return DMUON_ERR_INVALID_ARG; }
+  if (L.pair) return launch_op<true>(ke, L, stream);
+  return launch_op<false>(ke, L, stream);
 }
 
 }  // namespace dmuon

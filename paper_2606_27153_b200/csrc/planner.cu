@@ -3,6 +3,7 @@
 #include "planner.h"
 
 #include <algorithm>
+#include <chrono>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -10,6 +11,10 @@
 #include <fstream>
 #include <sstream>
 #include <sys/stat.h>
+
+#ifndef DMUON_BUILD_ID
+#define DMUON_BUILD_ID "dev"      // build.py passes a hash of csrc/: a new build never trusts an old build's timings
+#endif
 
 namespace dmuon {
 
@@ -19,13 +24,24 @@ bool gram_eligible(int m_pad, int n_pad, bool fp32) { return !fp32 && m_pad >= 2
 
 namespace {
 
+constexpr size_t kMaxPlans = 8;              // least-recently-used plans beyond this are dropped
 std::vector<std::unique_ptr<Plan>> g_plans;
-std::map<std::string, int> g_tune_cache;     // "op m_pad n_pad count" -> variant
+uint64_t g_stamp = 0;
+std::map<std::string, int> g_tune_cache;     // "build op kind m n countbucket" -> variant
 bool g_tune_loaded = false;
 std::string g_tune_loaded_path;
 
+// One grow-only workspace per device, used by every plan of that device (calls are stream-ordered and buckets run one
+// after the other, so nothing needs two regions at a time).
+struct DeviceWs {
+  uint8_t* ptr = nullptr;
+  size_t bytes = 0;
+};
+DeviceWs g_ws[kMaxDevices];
+
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 inline int pad128(int v) { return (v + kBlk - 1) / kBlk * kBlk; }
+inline int ceil_log2(double v) { int e = 0; while (std::ldexp(1.0, e) < v) ++e; return e; }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -67,30 +83,95 @@ int upload(Plan& p, T** out, const std::vector<T>& host) {
   return DMUON_OK;
 }
 
-void describe(const int32_t* shapes, int count, std::vector<MatrixInfo>& mats, size_t es, size_t* ws_bytes) {
-  mats.resize(count);
-  size_t off = 0;
+// ---------------------------------------------------------------------------------------------- layout (host only)
+struct Layout {
+  std::vector<MatrixInfo> mats;
+  std::vector<ShapeTables> shapes;          // layout fields only
+  std::vector<std::vector<int>> members;    // matrices of each shape, caller order
+  std::vector<BucketPlan> buckets;          // execution order; mats / rec0 / shape / work filled
+  size_t ws_bytes = 0;
+};
+
+void describe(const int32_t* shapes, int count, bool fp32, bool keep_o, size_t chunk_bytes, Layout& L) {
+  const size_t es = fp32 ? 4 : 2;
+  L.mats.resize(count);
+  std::map<std::tuple<int, int, int>, int> shape_of;
   for (int i = 0; i < count; ++i) {
-    MatrixInfo& mi = mats[i];
+    MatrixInfo& mi = L.mats[i];
     mi.rows = shapes[2 * i];
     mi.cols = shapes[2 * i + 1];
-    mi.transposed = mi.rows > mi.cols;            // work in the smaller Gram dimension
-    mi.m = std::min(mi.rows, mi.cols);
+    mi.m = std::min(mi.rows, mi.cols);               // the Gram matrix is the small one
     mi.n = std::max(mi.rows, mi.cols);
     mi.m_pad = pad128(mi.m);
     mi.n_pad = pad128(mi.n);
-    mi.bucket = -1;
-    const size_t xb = align_up(static_cast<size_t>(mi.m_pad) * mi.n_pad * es, 1024);
-    const size_t ab = align_up(static_cast<size_t>(mi.m_pad) * mi.m_pad * es, 1024);
-    mi.gram = gram_eligible(mi.m_pad, mi.n_pad, es == 4);
-    mi.off_p = off; off += xb;
-    mi.off_q = off; off += xb;
-    for (int k = 0; k < 5; ++k) {
-      mi.off_sq[k] = off;
-      if (k < 2 || mi.gram) off += ab;
+    const bool aligned = !fp32 && mi.rows % kBlk == 0 && mi.cols % kBlk == 0;
+    mi.kind = !aligned ? K_GENERIC : (mi.rows <= mi.cols ? K_WIDE : K_TALL);
+    mi.transposed = mi.kind == K_GENERIC && mi.rows > mi.cols;
+    mi.buf_rows = mi.kind == K_GENERIC ? mi.m_pad : mi.rows;
+    mi.buf_cols = mi.kind == K_GENERIC ? mi.n_pad : mi.cols;
+    mi.gram = gram_eligible(mi.m_pad, mi.n_pad, fp32);
+    // fp16 range: entries of the normalised X0 are ~1 / sqrt(m n), those of G0 ~1 / m, both near or below fp16's
+    // smallest normal (6.1e-5) for the large shapes; ||X||_2 <= 1.21 and ||G||_2 <= 1.45 bound the other end
+    mi.xscale = fp32 ? 1.f : std::ldexp(1.f, std::min(10, std::max(0, ceil_log2(std::sqrt(double(mi.m_pad) * mi.n_pad)) - 4)));
+    mi.gscale = fp32 ? 1.f : std::ldexp(1.f, std::min(10, std::max(0, ceil_log2(mi.m_pad) - 2)));
+    auto key = std::make_tuple(mi.m_pad, mi.n_pad, mi.kind);
+    auto it = shape_of.find(key);
+    if (it == shape_of.end()) {
+      it = shape_of.emplace(key, static_cast<int>(L.shapes.size())).first;
+      ShapeTables st;
+      st.m_pad = mi.m_pad; st.n_pad = mi.n_pad; st.kind = mi.kind; st.gram = mi.gram;
+      st.buf_rows = mi.buf_rows; st.buf_cols = mi.buf_cols;
+      st.xscale = mi.xscale; st.gscale = mi.gscale;
+      const size_t xb = align_up(static_cast<size_t>(mi.buf_rows) * mi.buf_cols * es, 1024);
+      const size_t ab = align_up(static_cast<size_t>(mi.m_pad) * mi.m_pad * es, 1024);
+      const int nsq = mi.gram ? 5 : 2;
+      st.off_p = 0; st.off_q = xb;
+      for (int k = 0; k < 5; ++k) st.off_sq[k] = 2 * xb + std::min(k, nsq - 1) * ab;
+      st.mat_bytes = 2 * xb + nsq * ab;
+      L.shapes.push_back(st);
+      L.members.emplace_back();
+    }
+    L.members[it->second].push_back(i);
+  }
+  // chunks: a bucket uses at most chunk_bytes of workspace (keep_o: every matrix keeps its own slot)
+  size_t off = 0;
+  for (size_t s = 0; s < L.shapes.size(); ++s) {
+    ShapeTables& st = L.shapes[s];
+    const int n = static_cast<int>(L.members[s].size());
+    int slots = n;
+    if (!keep_o) {
+      const size_t fit = std::max<size_t>(1, chunk_bytes / st.mat_bytes);
+      const int chunks = static_cast<int>((n + fit - 1) / fit);
+      slots = (n + chunks - 1) / chunks;
+    }
+    st.slots = slots;
+    st.base = keep_o ? off : 0;
+    off += static_cast<size_t>(slots) * st.mat_bytes;
+    L.ws_bytes = keep_o ? off : std::max(L.ws_bytes, static_cast<size_t>(slots) * st.mat_bytes);
+    for (int b0 = 0; b0 < n; b0 += slots) {
+      BucketPlan bp;
+      bp.shape = static_cast<int>(s);
+      bp.mats.assign(L.members[s].begin() + b0, L.members[s].begin() + std::min(n, b0 + slots));
+      bp.work = static_cast<double>(bp.mats.size()) * st.m_pad * st.m_pad * (2.0 * st.n_pad + st.m_pad);
+      L.buckets.push_back(bp);
     }
   }
-  *ws_bytes = off;
+  // execution order: most NS work first (stable: chunks of one shape stay together and in caller order)
+  std::stable_sort(L.buckets.begin(), L.buckets.end(), [&](const BucketPlan& a, const BucketPlan& b) {
+    const double wa = a.work / a.mats.size(), wb = b.work / b.mats.size();      // per matrix: chunks of a shape tie
+    return wa > wb;
+  });
+  int rec = 0;
+  for (size_t b = 0; b < L.buckets.size(); ++b) {
+    BucketPlan& bp = L.buckets[b];
+    bp.rec0 = rec;
+    for (size_t k = 0; k < bp.mats.size(); ++k) {
+      MatrixInfo& mi = L.mats[bp.mats[k]];
+      mi.bucket = static_cast<int>(b);
+      mi.slot = static_cast<int>(k);
+      mi.rec = rec++;
+    }
+  }
 }
 
 std::string resolve_cache_path(const Options& opt) {
@@ -100,6 +181,7 @@ std::string resolve_cache_path(const Options& opt) {
   return "";
 }
 
+// File format: one line per entry, "v5 <build> <op> <kind> <m> <n> <countbucket> <variant>".
 void load_tune_cache(const std::string& path) {
   if (g_tune_loaded && g_tune_loaded_path == path) return;
   g_tune_cache.clear();
@@ -110,11 +192,11 @@ void load_tune_cache(const std::string& path) {
   std::string line;
   while (std::getline(in, line)) {
     std::istringstream ss(line);
-    std::string tag;
-    int op, m, n, cnt, variant;
-    if (ss >> tag >> op >> m >> n >> cnt >> variant && tag == "v4" && variant >= 0 && variant < kNumVariants) {
-      char key[96];
-      snprintf(key, sizeof key, "%d %d %d %d", op, m, n, cnt);
+    std::string tag, build;
+    int op, kind, m, n, cb, variant;
+    if (ss >> tag >> build >> op >> kind >> m >> n >> cb >> variant && tag == "v5" && variant >= 0 && variant < kNumVariants) {
+      char key[160];
+      snprintf(key, sizeof key, "%s %d %d %d %d %d", build.c_str(), op, kind, m, n, cb);
       g_tune_cache[key] = variant;
     }
   }
@@ -129,131 +211,202 @@ void save_tune_cache(const std::string& path) {
       if (i == dir.size() || dir[i] == '/') mkdir(dir.substr(0, i).c_str(), 0755);
   }
   std::ofstream out(path, std::ios::trunc);
-  for (auto& kv : g_tune_cache) out << "v4 " << kv.first << " " << kv.second << "\n";
+  for (auto& kv : g_tune_cache) out << "v5 " << kv.first << " " << kv.second << "\n";
 }
 
-inline int tiling_op(GemmOp op) { return op == OP_SQ2 ? OP_SQ : op; }   // SQ2 shares SQ's units and variant
+// tiling op (unit table / variant slot) of a product: 0 = the Gram product, 1 = the m x m products, 2 = the X update
+inline int tiling_op(GemmOp op) {
+  switch (op) {
+    case OP_SYRK: case OP_SYRK_T: return 0;
+    case OP_SQ: case OP_SQ2: return 1;
+    default: return 2;
+  }
+}
+inline GemmOp gram_op(int kind) { return kind == K_TALL ? OP_SYRK_T : OP_SYRK; }
+inline GemmOp xupd_op(int kind) { return kind == K_TALL ? OP_XB : OP_BX; }
+// extent of an op's output in 128-blocks for a bucket shape
+inline void out_blocks(const ShapeTables& st, GemmOp op, int* mb, int* nb) {
+  *mb = st.m_pad / kBlk;
+  *nb = st.m_pad / kBlk;
+  if (op == OP_BX) *nb = st.n_pad / kBlk;
+  if (op == OP_XB) *mb = st.n_pad / kBlk;
+}
 
-int bucket_launch(const Plan& plan, const BucketPlan& b, GemmOp op, const GemmProblem* probs, float alpha, float beta,
-                  float beta2, cudaStream_t stream, const TileUnit* units_override = nullptr, int upp_override = 0,
-                  int variant_override = -1) {
+int shape_launch(const Plan& plan, const ShapeTables& st, int count, int rec0, GemmOp op, const GemmProblem* probs,
+                 float alpha, float beta, float beta2, const FinalEpilogue& fin, cudaStream_t stream,
+                 const TileUnit* units_override = nullptr, int upp_override = 0, int variant_override = -1) {
   const int top = tiling_op(op);
-  const bool pair = variant_config(variant_override >= 0 ? variant_override : b.variant[top]).pair;
+  const TileConfig cfg = variant_config(variant_override >= 0 ? variant_override : st.variant[top]);
   GemmLaunch L;
   L.op = op;
+  L.epi = fin.epi;
   L.problems = probs;
-  L.units = units_override ? units_override : b.units[top];
-  L.units_per_problem = units_override ? upp_override : b.units_per_problem[top];
-  L.num_problems = static_cast<int>(b.mats.size());
-  L.k_blocks = (op == OP_SYRK ? b.n_pad : b.m_pad) / kBlkK;
-  L.m_blocks = b.m_pad / kBlk;
-  L.n_blocks = (op == OP_BX ? b.n_pad : b.m_pad) / kBlk;
-  L.pair = pair;
-  L.quad = variant_config(variant_override >= 0 ? variant_override : b.variant[top]).quad;
+  L.units = units_override ? units_override : st.units[top];
+  L.recs = plan.d_recs;
+  L.units_per_problem = units_override ? upp_override : st.units_per_problem[top];
+  L.num_problems = count;
+  L.k_blocks = (top == 0 ? st.n_pad : st.m_pad) / kBlkK;
+  out_blocks(st, op, &L.m_blocks, &L.n_blocks);
+  L.pair = cfg.pair;
   L.alpha = alpha;
   L.beta = beta;
   L.beta2 = beta2;
+  L.lr = fin.lr;
+  L.lrwd = fin.lrwd;
+  L.store_c = fin.store_c;
+  L.rec_base = rec0;
   L.grid = plan.sm_count;
   return launch_ns_gemm(L, stream);
 }
 
-// Time each variant of each op of a bucket on the plan's own (scratch) workspace and keep the fastest.
-int autotune_bucket(Plan& plan, BucketPlan& b, const Options& opt, cudaStream_t stream) {
+int count_bucket(int count) { return ceil_log2(std::max(1, count)); }
+
+// Time each variant of each tiling op of a bucket shape on the plan's own (scratch-filled) workspace and keep the
+// fastest.  Each candidate runs back to back for opt.tune_ms: a handful of isolated launches at boost clock flatter the
+// configurations that move more bytes per FLOP, the step itself runs at the power cap ("benchmarked on
+// the target hardware").
+int autotune_shape(Plan& plan, ShapeTables& st, const Options& opt, cudaStream_t stream, bool* scratch_ready) {
   const std::string path = resolve_cache_path(opt);
   load_tune_cache(path);
   bool dirty = false;
-  for (int op = 0; op < 3; ++op) {
-    char key[96];
-    snprintf(key, sizeof key, "%d %d %d %d", op, b.m_pad, b.n_pad, static_cast<int>(b.mats.size()));
+  const GemmOp ops[3] = {gram_op(st.kind), OP_SQ, xupd_op(st.kind)};
+  for (int t = 0; t < 3; ++t) {
+    const GemmOp op = ops[t];
+    char key[160];
+    snprintf(key, sizeof key, "%s %d %d %d %d %d", DMUON_BUILD_ID, static_cast<int>(op), st.kind, st.m_pad, st.n_pad,
+             count_bucket(st.slots));
     auto it = g_tune_cache.find(key);
-    int best = 0;
-    if (opt.force_variant[op] >= 0 && variant_valid(static_cast<GemmOp>(op), opt.force_variant[op])) {
-      best = opt.force_variant[op];
-    } else if (it != g_tune_cache.end()) {
+    int best = st.m_pad >= 2 * kBlk ? 4 : 0;         // untuned default: CTA pair unless the Gram matrix is one block
+    if (opt.force_variant[t] >= 0 && variant_valid(op, opt.force_variant[t])) {
+      best = opt.force_variant[t];
+    } else if (it != g_tune_cache.end() && variant_valid(op, it->second)) {
       best = it->second;
     } else if (opt.autotune) {
+      const auto wall0 = std::chrono::steady_clock::now();
+      if (!*scratch_ready) {
+        int rc = launch_fill_scratch(plan.ws, plan.ws_bytes, stream);
+        if (rc) return rc;
+        *scratch_ready = true;
+      }
       cudaEvent_t e0, e1;
       DMUON_CUDA_CHECK(cudaEventCreate(&e0));
       DMUON_CUDA_CHECK(cudaEventCreate(&e1));
-      // the CTA-pair tilings are the incumbents: another configuration has to beat them by 10 % in this short, isolated
-      // measurement to be taken.  Timer noise must not flip the choice between runs, and a few launches at boost clock
-      // flatter the single-CTA tilings: they move 1.5x the L2->SMEM bytes per FLOP, which costs them more once the
-      // board sits at its power cap (measured: 25.8 against 18.4 ms per step for B = bG + cGG on 64 x 4096^2).  Unit order of the X update: row-major while X stays in
-      // L2, column-panel-major beyond (row-major then streams the whole X once per block row: measured 16 GB instead
-      // of 2.7 GB of DRAM reads per 12 matrices of 4096 x 14336)
-      const bool x_in_l2 = static_cast<size_t>(b.m_pad) * b.n_pad * sizeof(__half) <= (48u << 20);
-      const int preferred = op == OP_BX ? (x_in_l2 ? 5 : 4) : 4;
-      float best_ms = 1e30f, preferred_ms = 1e30f;
-      for (int v = 0; v < kNumVariants; ++v) {
-        if (!variant_valid(static_cast<GemmOp>(op), v)) continue;
-        const TileConfig cfg = variant_config(v);
-        // The quad tiling measured slower than the pair tiling on every bucket tried (TMA multicast at cluster size 4
-        // saves no L2 traffic over concurrent unicast loads, and only 33 clusters of 4 are co-resident on 148 SMs): it
-        // stays available through option "variants" but is not a tuning candidate.
-        if (cfg.quad) continue;
-        std::vector<TileUnit> hu = make_units(static_cast<GemmOp>(op), b.m_pad / kBlk, b.n_pad / kBlk, cfg);
-        TileUnit* du = nullptr;
-        DMUON_CUDA_CHECK(cudaMalloc(&du, hu.size() * sizeof(TileUnit)));
-        DMUON_CUDA_CHECK(cudaMemcpy(du, hu.data(), hu.size() * sizeof(TileUnit), cudaMemcpyHostToDevice));
-        int rc = DMUON_OK;
-        float ms = 1e30f;
-        for (int rep = 0; rep < 4 && rc == DMUON_OK; ++rep) {   // rep 0 warms up
+      int mb, nb;
+      out_blocks(st, op, &mb, &nb);
+      int rc = DMUON_OK;
+      struct Cand { int v; TileUnit* du; int n; float ms; };
+      std::vector<Cand> cands;
+      for (int v = 0; v < kNumVariants && rc == DMUON_OK; ++v) {
+        if (!variant_valid(op, v)) continue;
+        std::vector<TileUnit> hu = make_units(op, mb, nb, variant_config(v));
+        Cand c{v, nullptr, static_cast<int>(hu.size()), 1e30f};
+        if (cudaMalloc(&c.du, hu.size() * sizeof(TileUnit)) != cudaSuccess ||
+            cudaMemcpy(c.du, hu.data(), hu.size() * sizeof(TileUnit), cudaMemcpyHostToDevice) != cudaSuccess) rc = DMUON_ERR_CUDA;
+        cands.push_back(c);
+      }
+      // back-to-back launches of one candidate for about `ms_target`; returns the mean launch time
+      auto run = [&](const Cand& c, float ms_target, float* mean) {
+        float one = 0.f;
+        for (int pass = 0; pass < 2 && rc == DMUON_OK; ++pass) {
+          const int reps = pass == 0 ? 1 : std::max(2, std::min(4000, static_cast<int>(ms_target / std::max(one, 1e-3f))));
           cudaEventRecord(e0, stream);
-          rc = bucket_launch(plan, b, static_cast<GemmOp>(op), b.tune_probs[op], 1.f, 0.f, 0.f, stream, du, static_cast<int>(hu.size()), v);
+          for (int r = 0; r < reps && rc == DMUON_OK; ++r)
+            rc = shape_launch(plan, st, st.slots, 0, op, st.tune_probs[t], 1.f, 0.f, 0.f, FinalEpilogue(), stream, c.du, c.n, c.v);
           cudaEventRecord(e1, stream);
           if (cudaEventSynchronize(e1) != cudaSuccess) rc = DMUON_ERR_CUDA;
-          float t = 0.f;
-          cudaEventElapsedTime(&t, e0, e1);
-          if (rep > 0) ms = std::min(ms, t);
+          float total = 0.f;
+          cudaEventElapsedTime(&total, e0, e1);
+          one = total / reps;
         }
-        cudaFree(du);
-        if (rc) { cudaEventDestroy(e0); cudaEventDestroy(e1); set_error("autotune launch failed"); return rc; }
-        if (ms < best_ms) { best_ms = ms; best = v; }
-        if (v == preferred) preferred_ms = ms;
+        *mean = one;
+      };
+      // 1. bring the board to the state the step runs in: a few candidates' worth of back-to-back launches of the default
+      //    configuration (a cold board at boost clock flatters whichever candidate runs first)
+      float burn = 0.f;
+      for (const Cand& c : cands)
+        if (c.v == best) run(c, 4.f * opt.tune_ms, &burn);
+      // 2. every candidate for tune_ms
+      for (Cand& c : cands) {
+        run(c, opt.tune_ms, &c.ms);
+        if (getenv("DMUON_LOG")) fprintf(stderr, "[dmuon] tune op %d kind %d %dx%d x%d variant %d: %.4f ms\n", static_cast<int>(op), st.kind, st.m_pad, st.n_pad, st.slots, c.v, c.ms);
       }
-      if (best != preferred && best_ms > 0.90f * preferred_ms) best = preferred;
+      // 3. the two fastest once more, alternating, and the decision on the sum of both rounds
+      std::sort(cands.begin(), cands.end(), [](const Cand& a, const Cand& b) { return a.ms < b.ms; });
+      if (cands.size() >= 2 && rc == DMUON_OK) {
+        float again[2] = {0.f, 0.f};
+        for (int round = 0; round < 2; ++round)
+          for (int k = 0; k < 2; ++k) {
+            float ms = 0.f;
+            run(cands[k], 0.5f * opt.tune_ms, &ms);
+            again[k] += 0.5f * ms;
+          }
+        cands[0].ms = 0.5f * (cands[0].ms + again[0]);
+        cands[1].ms = 0.5f * (cands[1].ms + again[1]);
+        if (getenv("DMUON_LOG")) fprintf(stderr, "[dmuon] tune op %d: finalists %d (%.4f ms) and %d (%.4f ms)\n", static_cast<int>(op), cands[0].v, cands[0].ms, cands[1].v, cands[1].ms);
+        // a tie within 1 % goes to the lower variant number, so that two runs agree
+        if (cands[1].ms < cands[0].ms * (cands[1].v < cands[0].v ? 1.01f : 0.99f)) std::swap(cands[0], cands[1]);
+      }
+      for (Cand& c : cands) cudaFree(c.du);
+      if (rc) { cudaEventDestroy(e0); cudaEventDestroy(e1); set_error("autotune launch failed"); return rc; }
+      if (!cands.empty()) best = cands[0].v;
       cudaEventDestroy(e0);
       cudaEventDestroy(e1);
       g_tune_cache[key] = best;
       dirty = true;
+      st.tuned_now = true;
+      plan.tune_seconds += std::chrono::duration<double>(std::chrono::steady_clock::now() - wall0).count();
     }
-    b.variant[op] = best;
+    st.variant[t] = best;
   }
   if (dirty) save_tune_cache(path);
   return DMUON_OK;
 }
 
+void drop_plans_of_device(int device, bool shared_ws_only) {
+  for (size_t i = 0; i < g_plans.size();) {
+    if (g_plans[i]->device == device && (!shared_ws_only || !g_plans[i]->ext_ws)) g_plans.erase(g_plans.begin() + i);
+    else ++i;
+  }
+}
+
 }  // namespace
 
+int tune_cache_entries() { return static_cast<int>(g_tune_cache.size()); }
+
+void forget_tune_cache() {       // the in-memory copy; the file stays
+  g_tune_cache.clear();
+  g_tune_loaded = false;
+  g_tune_loaded_path.clear();
+}
+
 int fill_problem(GemmProblem& g, GemmOp op, const void* a_mat, uint64_t a_rows, uint64_t a_cols, const void* b_mat,
-                 uint64_t b_rows, uint64_t b_cols, const void* d, void* c, int ldc, const void* d2) {
+                 uint64_t b_rows, uint64_t b_cols, const void* d, void* c, int ldc, const void* d2, int rec) {
   memset(&g, 0, sizeof g);
-  int rc = encode_tmap_2d(&g.tmA, a_mat, a_rows, a_cols, kBlkK, kBlk);
+  int rc;
+  if (op == OP_SYRK_T) rc = encode_tmap_2d(&g.tmA, a_mat, a_rows, a_cols, 64, kBlkK);   // MN-major: 64 (m) x 64 (k) boxes
+  else rc = encode_tmap_2d(&g.tmA, a_mat, a_rows, a_cols, kBlkK, kBlk);
   if (rc) return rc;
-  if (op == OP_BX) rc = encode_tmap_2d(&g.tmB, b_mat, b_rows, b_cols, 64, kBlkK);   // MN-major: 64 (n) x 64 (k) boxes
+  if (op == OP_BX || op == OP_SYRK_T) rc = encode_tmap_2d(&g.tmB, b_mat, b_rows, b_cols, 64, kBlkK);   // MN-major: 64 (n) x 64 (k) boxes
   else rc = encode_tmap_2d(&g.tmB, b_mat, b_rows, b_cols, kBlkK, kBlk);
   if (rc) return rc;
   g.D = static_cast<const __half*>(d);
   g.C = static_cast<__half*>(c);
   g.D2 = static_cast<const __half*>(d2);
   g.ldc = ldc;
+  g.rec = rec;
   return DMUON_OK;
 }
 
 Plan::~Plan() {
+  int cur = 0;
+  cudaGetDevice(&cur);
+  if (cur != device) cudaSetDevice(device);
   for (void* p : d_allocs) cudaFree(p);
-  for (cudaEvent_t e : ev) cudaEventDestroy(e);
-  if (side) cudaStreamDestroy(side);
+  if (cur != device) cudaSetDevice(cur);
 }
 
 TileConfig variant_config(int variant) {
   TileConfig c;
-  if (variant == 6) {
-    c.pair = true;
-    c.quad = true;
-    c.order = 1;
-    return c;
-  }
   if (variant >= 4) {
     c.pair = true;
     c.order = variant & 1;
@@ -266,35 +419,17 @@ TileConfig variant_config(int variant) {
 
 bool variant_valid(GemmOp op, int variant) {
   if (variant < 0 || variant >= kNumVariants) return false;
-  if (variant == 6) return true;
-  return op == OP_BX || variant_config(variant).order == 0;   // symmetric ops have one ordering
+  return op == OP_BX || op == OP_XB || variant_config(variant).order == 0;   // symmetric ops have one ordering
 }
 
 std::vector<TileUnit> make_units(GemmOp op, int mb, int nb, const TileConfig& cfg) {
   std::vector<TileUnit> u;
   auto push = [&](int i, int j, int w) { u.push_back(TileUnit{static_cast<int16_t>(i), static_cast<int16_t>(j), static_cast<int16_t>(w), 0}); };
-  if (cfg.quad) {
-    // two 256 x 256 units per entry, sharing a block row (pairs along a row) or a block column (leftovers of rows
-    // with an odd number of units, paired down the last column); a final odd unit is paired with itself
-    const int MB = (mb + 1) / 2, NB = (nb + 1) / 2;
-    auto quad = [&](int m0, int n0, int m1, int n1) {
-      u.push_back(TileUnit{static_cast<int16_t>(m0), static_cast<int16_t>(n0), static_cast<int16_t>(m1), static_cast<int16_t>(n1)});
-    };
-    const int ncols = op == OP_BX ? NB : MB;
-    std::vector<std::pair<int, int>> left;
-    for (int i = 0; i < MB; ++i) {
-      int j = op == OP_BX ? 0 : i;
-      for (; j + 1 < ncols; j += 2) quad(i, j, i, j + 1);
-      if (j < ncols) left.push_back({i, j});
-    }
-    for (size_t k = 0; k + 1 < left.size(); k += 2) quad(left[k].first, left[k].second, left[k + 1].first, left[k + 1].second);
-    if (left.size() % 2) quad(left.back().first, left.back().second, left.back().first, left.back().second);
-    return u;
-  }
+  const bool general = op == OP_BX || op == OP_XB;
   if (cfg.pair) {
     // 256 x 256 units; an odd block count leaves a half-empty last unit (operands zero-filled, stores skipped)
     const int MB = (mb + 1) / 2, NB = (nb + 1) / 2;
-    if (op == OP_BX) {
+    if (general) {
       if (cfg.order == 0) { for (int j = 0; j < NB; ++j) for (int i = 0; i < MB; ++i) push(i, j, 2); }
       else                { for (int i = 0; i < MB; ++i) for (int j = 0; j < NB; ++j) push(i, j, 2); }
     } else {
@@ -302,7 +437,7 @@ std::vector<TileUnit> make_units(GemmOp op, int mb, int nb, const TileConfig& cf
     }
     return u;
   }
-  if (op == OP_BX) {
+  if (general) {
     if (cfg.order == 0) {
       for (int j = 0; j < nb; j += cfg.width)
         for (int i = 0; i < mb; ++i) push(i, j, std::min(cfg.width, nb - j));
@@ -352,42 +487,78 @@ int check_device() {
     set_error("libdmuon needs an sm_100 (B200) device; found compute capability major %d", major);
     return DMUON_ERR_UNSUPPORTED_DEVICE;
   }
+  if (dev >= kMaxDevices) {
+    set_error("device ordinal %d is not supported (max %d)", dev, kMaxDevices - 1);
+    return DMUON_ERR_UNSUPPORTED_DEVICE;
+  }
   return DMUON_OK;
 }
 
-size_t plan_workspace_bytes(const int32_t* shapes, int count, bool fp32) {
-  std::vector<MatrixInfo> mats;
-  size_t bytes = 0;
-  describe(shapes, count, mats, fp32 ? 4 : 2, &bytes);
-  return bytes;
+size_t plan_workspace_bytes(const int32_t* shapes, int count, const Options& opt) {
+  Layout L;
+  describe(shapes, count, opt.fp32_check, opt.keep_o, opt.chunk_bytes, L);
+  return L.ws_bytes;
 }
 
 void drop_plans() { g_plans.clear(); }
 
+Plan* find_plan(uint64_t id) {
+  for (auto& up : g_plans)
+    if (up->id == id) return up.get();
+  return nullptr;
+}
+
+void release_workspaces() {
+  int cur = 0;
+  if (cudaGetDevice(&cur) != cudaSuccess) { cudaGetLastError(); return; }
+  for (int d = 0; d < kMaxDevices; ++d) {
+    if (!g_ws[d].ptr) continue;
+    cudaSetDevice(d);
+    cudaFree(g_ws[d].ptr);
+    g_ws[d] = DeviceWs();
+  }
+  cudaSetDevice(cur);
+  cudaGetLastError();
+}
+
 int get_plan(const int32_t* shapes, int count, const Options& opt, void* ext_ws, size_t ext_bytes, cudaStream_t stream,
              Plan** out) {
+  int rc = check_device();
+  if (rc) return rc;
+  int dev = 0;
+  cudaGetDevice(&dev);
   for (auto& up : g_plans) {
     Plan& p = *up;
-    if (p.fp32 == opt.fp32_check && p.shapes.size() == static_cast<size_t>(2 * count) &&
+    if (p.device == dev && p.fp32 == opt.fp32_check && p.keep_o == opt.keep_o && p.chunk_bytes == opt.chunk_bytes &&
+        p.ext_ws == ext_ws && p.shapes.size() == static_cast<size_t>(2 * count) &&
         (count == 0 || memcmp(p.shapes.data(), shapes, sizeof(int32_t) * 2 * count) == 0)) {
+      p.stamp = ++g_stamp;
       *out = &p;
       return DMUON_OK;
     }
   }
-  int rc = check_device();
-  if (rc) return rc;
 
   std::unique_ptr<Plan> up(new Plan);
   Plan& p = *up;
   p.shapes.assign(shapes, shapes + 2 * count);
   p.fp32 = opt.fp32_check;
-  const size_t es = p.fp32 ? 4 : 2;
-  describe(shapes, count, p.mats, es, &p.ws_bytes);
-  int dev = 0;
-  cudaGetDevice(&dev);
+  p.keep_o = opt.keep_o;
+  p.chunk_bytes = opt.chunk_bytes;
+  p.device = dev;
+  p.ext_ws = ext_ws;
+  p.stamp = ++g_stamp;
+  p.id = p.stamp;
+  {
+    Layout L;
+    describe(shapes, count, p.fp32, p.keep_o, p.chunk_bytes, L);
+    p.mats = std::move(L.mats);
+    p.shapes_tbl = std::move(L.shapes);
+    p.buckets = std::move(L.buckets);
+    p.ws_bytes = L.ws_bytes;
+  }
   cudaDeviceGetAttribute(&p.sm_count, cudaDevAttrMultiProcessorCount, dev);
 
-  // ---- workspace
+  // ---- workspace: the caller's, or the device's shared grow-only region
   if (ext_ws) {
     if (ext_bytes < p.ws_bytes) {
       set_error("caller workspace of %zu bytes is smaller than the %zu bytes this shape set needs", ext_bytes, p.ws_bytes);
@@ -395,141 +566,131 @@ int get_plan(const int32_t* shapes, int count, const Options& opt, void* ext_ws,
     }
     p.ws = static_cast<uint8_t*>(ext_ws);
   } else {
-    rc = dev_alloc(p, &p.ws, p.ws_bytes);
-    if (rc) return rc;
-    p.ws_owned = true;
-  }
-
-  // scratch contents for the autotuner (tensor-core mode) / zeros (check mode)
-  if (!p.fp32) { if ((rc = launch_fill_scratch(p.ws, p.ws_bytes, stream))) return rc; }
-  else DMUON_CUDA_CHECK(cudaMemsetAsync(p.ws, 0, p.ws_bytes, stream));
-
-  // ---- buckets by padded oriented shape
-  std::map<std::pair<int, int>, int> bucket_of;
-  for (int i = 0; i < count; ++i) {
-    MatrixInfo& mi = p.mats[i];
-    auto key = std::make_pair(mi.m_pad, mi.n_pad);
-    auto it = bucket_of.find(key);
-    if (it == bucket_of.end()) {
-      it = bucket_of.emplace(key, static_cast<int>(p.buckets.size())).first;
-      p.buckets.emplace_back();
-      p.buckets.back().m_pad = mi.m_pad;
-      p.buckets.back().n_pad = mi.n_pad;
+    DeviceWs& w = g_ws[dev];
+    if (w.bytes < p.ws_bytes) {
+      // growing moves the region: plans that point into the old one are dropped (their tuned choices stay cached)
+      DMUON_CUDA_CHECK(cudaDeviceSynchronize());
+      drop_plans_of_device(dev, true);
+      if (w.ptr) cudaFree(w.ptr);
+      w = DeviceWs();
+      void* ptr = nullptr;
+      cudaError_t e = cudaMalloc(&ptr, std::max<size_t>(p.ws_bytes, 1));
+      if (e != cudaSuccess) {
+        cudaGetLastError();
+        set_error("cudaMalloc of the %zu-byte workspace failed: %s", p.ws_bytes, cudaGetErrorString(e));
+        return DMUON_ERR_OOM;
+      }
+      w.ptr = static_cast<uint8_t*>(ptr);
+      w.bytes = p.ws_bytes;
     }
-    mi.bucket = it->second;
-    p.buckets[it->second].mats.push_back(i);
+    p.ws = w.ptr;
   }
+  // check mode: padding of the fp32 buffers must be zero (the tensor-core path's padding is written by the normalise kernel
+  // for generic matrices and does not exist for aligned ones)
+  DMUON_CUDA_CHECK(cudaMemsetAsync(p.ws, 0, p.ws_bytes, stream));
 
-  // ---- elementwise tables.  One set over all matrices (`tables`) and, when there are several buckets, one set per
-  //      bucket (`parts`, in execution order) in which the matrices of the other buckets have no work items: the step
-  //      runs the elementwise passes of one bucket on a side stream under the GEMMs of another (api.cu).
-  p.h_recs.resize(count);
+  // ---- elementwise records and per-bucket work lists
+  const size_t nrec = std::max(count, 1);
+  p.h_recs.resize(nrec);
+  memset(p.h_recs.data(), 0, nrec * sizeof(MatRec));
   for (int i = 0; i < count; ++i) {
     const MatrixInfo& mi = p.mats[i];
-    MatRec& r = p.h_recs[i];
-    memset(&r, 0, sizeof r);
-    r.U = p.ws + mi.off_p;
-    r.X0 = p.ws + mi.off_q;
+    const ShapeTables& st = p.shapes_tbl[p.buckets[mi.bucket].shape];
+    uint8_t* slot = p.ws + st.base + static_cast<size_t>(mi.slot) * st.mat_bytes;
+    MatRec& r = p.h_recs[mi.rec];
+    r.U = slot + st.off_p;
+    r.X0 = slot + st.off_q;
     r.O = nullptr;
     r.rows = mi.rows; r.cols = mi.cols;
-    r.m_pad = mi.m_pad; r.n_pad = mi.n_pad;
+    r.m_pad = mi.buf_rows; r.n_pad = mi.buf_cols;
     r.transposed = mi.transposed ? 1 : 0;
     r.scale = static_cast<float>(std::sqrt(std::max(1.0, static_cast<double>(mi.rows) / mi.cols)));   // reading N4
+    r.xscale = mi.xscale;
+    r.inv_xscale = 1.f / mi.xscale;
   }
-  if ((rc = dev_alloc(p, &p.d_recs, count))) return rc;
-  if ((rc = dev_alloc(p, &p.d_inv_norm, count))) return rc;
-  auto build_tables = [&](int only_bucket, ElemTables* out) -> int {
-    std::vector<int64_t> flat_prefix(count + 1, 0), tile_prefix(count + 1, 0), ptile_prefix(count + 1, 0);
-    std::vector<int64_t> fa_prefix(count + 1, 0), fb_prefix(count + 1, 0);
-    for (int i = 0; i < count; ++i) {
-      const MatrixInfo& mi = p.mats[i];
-      const bool member = only_bucket < 0 || mi.bucket == only_bucket;
+  if ((rc = dev_alloc(p, &p.d_recs, nrec))) return rc;
+  if ((rc = dev_alloc(p, &p.d_inv_norm, nrec))) return rc;
+  std::vector<int> mat_of_rec(count, -1);
+  for (int i = 0; i < count; ++i) mat_of_rec[p.mats[i].rec] = i;
+  for (BucketPlan& bp : p.buckets) {
+    // prefix arrays over ALL records: the records outside the bucket have no work items
+    std::vector<int64_t> flat_prefix(count + 1, 0), tile_prefix(count + 1, 0), ptile_prefix(count + 1, 0), fa_prefix(count + 1, 0);
+    for (int r = 0; r < count; ++r) {
+      const MatrixInfo& mi = p.mats[mat_of_rec[r]];
+      const bool member = r >= bp.rec0 && r < bp.rec0 + static_cast<int>(bp.mats.size());
       const int64_t elems = static_cast<int64_t>(mi.rows) * mi.cols;
-      // normalise / apply path of this matrix: A (flat), B (16-bit tile transpose) or the generic tiles
-      const bool aligned = !p.fp32 && mi.rows % kBlk == 0 && mi.cols % kBlk == 0;
-      const bool path_a = aligned && !mi.transposed, path_b = aligned && mi.transposed;
-      const bool generic = !path_a && !path_b;
-      flat_prefix[i + 1] = flat_prefix[i] + (member ? (elems + kFlatChunk - 1) / kFlatChunk : 0);
-      fa_prefix[i + 1] = fa_prefix[i] + (member && path_a ? elems / kFlatChunk : 0);
-      fb_prefix[i + 1] = fb_prefix[i] + (member && path_b ? static_cast<int64_t>(mi.rows / kTile) * (mi.cols / kTile) : 0);
-      tile_prefix[i + 1] = tile_prefix[i] + (member && generic ? static_cast<int64_t>((mi.rows + kTile - 1) / kTile) * ((mi.cols + kTile - 1) / kTile) : 0);
-      ptile_prefix[i + 1] = ptile_prefix[i] + (member && generic ? static_cast<int64_t>(mi.m_pad / kTile) * (mi.n_pad / kTile) : 0);
+      const bool aligned = mi.kind != K_GENERIC;
+      flat_prefix[r + 1] = flat_prefix[r] + (member ? (elems + kFlatChunk - 1) / kFlatChunk : 0);
+      fa_prefix[r + 1] = fa_prefix[r] + (member && aligned ? elems / kFlatChunk : 0);
+      tile_prefix[r + 1] = tile_prefix[r] + (member && !aligned ? static_cast<int64_t>((mi.rows + kTile - 1) / kTile) * ((mi.cols + kTile - 1) / kTile) : 0);
+      ptile_prefix[r + 1] = ptile_prefix[r] + (member && !aligned ? static_cast<int64_t>(mi.m_pad / kTile) * (mi.n_pad / kTile) : 0);
     }
-    int64_t *d_flat = nullptr, *d_tile = nullptr, *d_ptile = nullptr, *d_fa = nullptr, *d_fb = nullptr;
+    int64_t *d_flat = nullptr, *d_tile = nullptr, *d_ptile = nullptr, *d_fa = nullptr;
     float* d_partials = nullptr;
-    int r2;
-    if ((r2 = upload(p, &d_flat, flat_prefix))) return r2;
-    if ((r2 = upload(p, &d_tile, tile_prefix))) return r2;
-    if ((r2 = upload(p, &d_ptile, ptile_prefix))) return r2;
-    if ((r2 = upload(p, &d_fa, fa_prefix))) return r2;
-    if ((r2 = upload(p, &d_fb, fb_prefix))) return r2;
-    if ((r2 = dev_alloc(p, &d_partials, static_cast<size_t>(flat_prefix[count])))) return r2;
-    out->recs = p.d_recs;
-    out->flat_prefix = d_flat;
-    out->tile_prefix = d_tile;
-    out->ptile_prefix = d_ptile;
-    out->fa_prefix = d_fa;
-    out->fb_prefix = d_fb;
-    out->count = count;
-    out->flat_chunks = flat_prefix[count];
-    out->tiles = tile_prefix[count];
-    out->ptiles = ptile_prefix[count];
-    out->fa_chunks = fa_prefix[count];
-    out->fb_tiles = fb_prefix[count];
-    out->partials = d_partials;
-    out->inv_norm = p.d_inv_norm;
-    return DMUON_OK;
-  };
-  if ((rc = build_tables(-1, &p.tables))) return rc;
-  // execution order of the buckets: most NS work first, so that the largest elementwise passes that can be hidden
-  // (normalise of the later buckets, apply of the earlier ones) run under the longest GEMM phases
-  p.order.resize(p.buckets.size());
-  for (size_t b = 0; b < p.buckets.size(); ++b) p.order[b] = static_cast<int>(b);
-  auto cost = [&](int b) {
-    const BucketPlan& bp = p.buckets[b];
-    return static_cast<double>(bp.mats.size()) * bp.m_pad * bp.m_pad * (2.0 * bp.n_pad + bp.m_pad);
-  };
-  std::stable_sort(p.order.begin(), p.order.end(), [&](int a, int b) { return cost(a) > cost(b); });
-  if (!p.fp32 && p.buckets.size() > 1) {
-    p.parts.resize(p.buckets.size());
-    for (size_t k = 0; k < p.order.size(); ++k)
-      if ((rc = build_tables(p.order[k], &p.parts[k]))) return rc;
-    DMUON_CUDA_CHECK(cudaStreamCreateWithFlags(&p.side, cudaStreamNonBlocking));
-    p.ev.resize(2 * p.buckets.size() + 2);
-    for (cudaEvent_t& e : p.ev) DMUON_CUDA_CHECK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    if ((rc = upload(p, &d_flat, flat_prefix))) return rc;
+    if ((rc = upload(p, &d_tile, tile_prefix))) return rc;
+    if ((rc = upload(p, &d_ptile, ptile_prefix))) return rc;
+    if ((rc = upload(p, &d_fa, fa_prefix))) return rc;
+    if ((rc = dev_alloc(p, &d_partials, static_cast<size_t>(flat_prefix[count])))) return rc;
+    ElemTables& T = bp.tables;
+    T.recs = p.d_recs;
+    T.flat_prefix = d_flat;
+    T.tile_prefix = d_tile;
+    T.ptile_prefix = d_ptile;
+    T.fa_prefix = d_fa;
+    T.count = count;
+    T.flat_chunks = flat_prefix[count];
+    T.tiles = tile_prefix[count];
+    T.ptiles = ptile_prefix[count];
+    T.fa_chunks = fa_prefix[count];
+    T.partials = d_partials;
+    T.inv_norm = p.d_inv_norm;
   }
 
   // ---- grouped GEMM tables (tensor-core mode only): scratch problems for the autotuner, tile units per op.  The
   //      launch programs of the NS steps are built on first use (build_program), they depend on the step count.
   if (!p.fp32) {
-    for (BucketPlan& b : p.buckets) {
-      const size_t nprob = b.mats.size();
-      b.gram = p.mats[b.mats[0]].gram;
+    bool scratch_ready = false;
+    for (ShapeTables& st : p.shapes_tbl) {
+      const size_t nprob = st.slots;
       std::vector<GemmProblem> tp[3];
-      for (int op = 0; op < 3; ++op) tp[op].resize(nprob);
+      for (int t = 0; t < 3; ++t) tp[t].resize(nprob);
       for (size_t k = 0; k < nprob; ++k) {
-        const MatrixInfo& mi = p.mats[b.mats[k]];
-        void* XQ = p.ws + mi.off_q;
-        void* XP = p.ws + mi.off_p;
-        void* A = p.ws + mi.off_sq[0];
-        void* B = p.ws + mi.off_sq[1];
-        const uint64_t m = mi.m_pad, n = mi.n_pad;
-        if ((rc = fill_problem(tp[OP_SYRK][k], OP_SYRK, XQ, m, n, XQ, m, n, nullptr, A, mi.m_pad))) return rc;
-        if ((rc = fill_problem(tp[OP_SQ][k], OP_SQ, A, m, m, A, m, m, A, B, mi.m_pad))) return rc;
-        if ((rc = fill_problem(tp[OP_BX][k], OP_BX, B, m, m, XQ, m, n, XQ, XP, mi.n_pad))) return rc;
+        uint8_t* slot = p.ws + st.base + k * st.mat_bytes;
+        void* XQ = slot + st.off_q;
+        void* XP = slot + st.off_p;
+        void* A = slot + st.off_sq[0];
+        void* B = slot + st.off_sq[1];
+        const uint64_t m = st.m_pad, br = st.buf_rows, bc = st.buf_cols;
+        if ((rc = fill_problem(tp[0][k], gram_op(st.kind), XQ, br, bc, XQ, br, bc, nullptr, A, st.m_pad))) return rc;
+        if ((rc = fill_problem(tp[1][k], OP_SQ, A, m, m, A, m, m, A, B, st.m_pad))) return rc;
+        if (st.kind == K_TALL) rc = fill_problem(tp[2][k], OP_XB, XQ, br, bc, B, m, m, XQ, XP, st.buf_cols);
+        else rc = fill_problem(tp[2][k], OP_BX, B, m, m, XQ, br, bc, XQ, XP, st.buf_cols);
+        if (rc) return rc;
       }
-      for (int op = 0; op < 3; ++op)
-        if ((rc = upload(p, &b.tune_probs[op], tp[op]))) return rc;
-      // tile configuration: tuned (cache or measurement) or default variant 0
-      if ((rc = autotune_bucket(p, b, opt, stream))) return rc;
-      for (int op = 0; op < 3; ++op) {
-        std::vector<TileUnit> hu = make_units(static_cast<GemmOp>(op), b.m_pad / kBlk, b.n_pad / kBlk, variant_config(b.variant[op]));
-        b.units_per_problem[op] = static_cast<int>(hu.size());
-        if ((rc = upload(p, &b.units[op], hu))) return rc;
+      for (int t = 0; t < 3; ++t)
+        if ((rc = upload(p, &st.tune_probs[t], tp[t]))) return rc;
+      // tile configuration: tuned (cache or measurement) or the default
+      if ((rc = autotune_shape(p, st, opt, stream, &scratch_ready))) return rc;
+      const GemmOp ops[3] = {gram_op(st.kind), OP_SQ, xupd_op(st.kind)};
+      for (int t = 0; t < 3; ++t) {
+        int mb, nb;
+        out_blocks(st, ops[t], &mb, &nb);
+        std::vector<TileUnit> hu = make_units(ops[t], mb, nb, variant_config(st.variant[t]));
+        st.units_per_problem[t] = static_cast<int>(hu.size());
+        if ((rc = upload(p, &st.units[t], hu))) return rc;
       }
     }
+    if (scratch_ready) DMUON_CUDA_CHECK(cudaMemsetAsync(p.ws, 0, p.ws_bytes, stream));
   }
   DMUON_CUDA_CHECK(cudaDeviceSynchronize());
+  // least-recently-used plans make room
+  while (g_plans.size() >= kMaxPlans) {
+    size_t victim = 0;
+    for (size_t i = 1; i < g_plans.size(); ++i)
+      if (g_plans[i]->stamp < g_plans[victim]->stamp) victim = i;
+    g_plans.erase(g_plans.begin() + victim);
+  }
   g_plans.push_back(std::move(up));
   *out = g_plans.back().get();
   return DMUON_OK;
@@ -569,64 +730,73 @@ Partition choose_partition(int steps, const float* coeffs, bool per_step, bool g
   return part;
 }
 
-int result_parity(const Plan& plan, const BucketPlan& b, int steps, const float* coeffs, bool per_step, const Options& opt) {
+int result_parity(const Plan& plan, const ShapeTables& st, int steps, const float* coeffs, bool per_step, const Options& opt) {
   if (plan.fp32) return steps & 1;
-  return static_cast<int>(choose_partition(steps, coeffs, per_step, b.gram && opt.gram_blocks).size()) & 1;
+  return static_cast<int>(choose_partition(steps, coeffs, per_step, st.gram && opt.gram_blocks).size()) & 1;
+}
+
+bool bucket_fuses(const Plan& plan, const ShapeTables& st, int steps, const Options& opt) {
+  return !plan.fp32 && opt.fuse && st.kind != K_GENERIC && steps > 0;
 }
 
 namespace {
 
-// Build the launch list of one bucket for a partition of the steps into blocks.  m x m buffers: 0 = G, 1/2 = B and B'
-// (alternating), 3 = T, 4 = R.
-int build_program(Plan& p, BucketPlan& b, const Partition& part, NsProgram& prog) {
-  const size_t nprob = b.mats.size();
-  const int kb_n = b.n_pad / kBlkK, kb_m = b.m_pad / kBlkK, nb_m = b.m_pad / kBlk, nb_n = b.n_pad / kBlk;
+// Build the launch list of one bucket shape for a partition of the steps into blocks.  m x m buffers: 0 = G, 1/2 = B
+// and B' (alternating), 3 = T, 4 = R.
+int build_program(Plan& p, ShapeTables& st, const Partition& part, NsProgram& prog) {
+  const size_t nprob = st.slots;
   int rc;
+  const bool tall = st.kind == K_TALL;
+  // stored-shape tag of the profile names: tall buckets read "rows x cols" of the stored matrices
+  const std::string dims = "[" + std::to_string(tall ? st.n_pad : st.m_pad) + "x" + std::to_string(tall ? st.m_pad : st.n_pad) + "]";
   auto emit = [&](GemmOp op, CoefKind ck, int s0, int s1, const char* name, int a_buf, int b_buf, int d_buf, int d2_buf,
                   int c_buf, int xsrc) -> int {
     // buffer ids: 0..4 = m x m buffers; 10 / 11 = X in Q / P
     std::vector<GemmProblem> hp(nprob);
     for (size_t k = 0; k < nprob; ++k) {
-      const MatrixInfo& mi = p.mats[b.mats[k]];
+      uint8_t* slot = p.ws + st.base + k * st.mat_bytes;
       auto buf = [&](int id) -> void* {
         if (id < 0) return nullptr;
-        if (id >= 10) return p.ws + (id == 10 ? mi.off_q : mi.off_p);
-        return p.ws + mi.off_sq[id];
+        if (id >= 10) return slot + (id == 10 ? st.off_q : st.off_p);
+        return slot + st.off_sq[id];
       };
-      const uint64_t m = mi.m_pad, n = mi.n_pad;
-      if (op == OP_SYRK) rc = fill_problem(hp[k], op, buf(xsrc), m, n, buf(xsrc), m, n, nullptr, buf(c_buf), mi.m_pad);
-      else if (op == OP_BX) rc = fill_problem(hp[k], op, buf(a_buf), m, m, buf(xsrc), m, n, buf(xsrc), buf(c_buf), mi.n_pad);
-      else rc = fill_problem(hp[k], op, buf(a_buf), m, m, buf(b_buf), m, m, buf(d_buf), buf(c_buf), mi.m_pad, buf(d2_buf));
+      const uint64_t m = st.m_pad, br = st.buf_rows, bc = st.buf_cols;
+      const int rec = static_cast<int>(k);
+      if (op == OP_SYRK || op == OP_SYRK_T) rc = fill_problem(hp[k], op, buf(xsrc), br, bc, buf(xsrc), br, bc, nullptr, buf(c_buf), st.m_pad, nullptr, rec);
+      else if (op == OP_BX) rc = fill_problem(hp[k], op, buf(a_buf), m, m, buf(xsrc), br, bc, buf(xsrc), buf(c_buf), st.buf_cols, nullptr, rec);
+      else if (op == OP_XB) rc = fill_problem(hp[k], op, buf(xsrc), br, bc, buf(a_buf), m, m, buf(xsrc), buf(c_buf), st.buf_cols, nullptr, rec);
+      else rc = fill_problem(hp[k], op, buf(a_buf), m, m, buf(b_buf), m, m, buf(d_buf), buf(c_buf), st.m_pad, buf(d2_buf), rec);
       if (rc) return rc;
     }
     NsLaunch L;
     L.op = op; L.ck = ck; L.s0 = s0; L.s1 = s1;
-    L.name = std::string(name) + "[" + std::to_string(b.m_pad) + "x" + std::to_string(b.n_pad) + "]";
-    L.k_blocks = op == OP_SYRK ? kb_n : kb_m;
-    L.n_blocks = op == OP_BX ? nb_n : nb_m;
+    L.name = std::string(name) + dims;
     if ((rc = upload(p, &L.probs, hp))) return rc;
     prog.launches.push_back(L);
     return DMUON_OK;
   };
+  const GemmOp syrk = gram_op(st.kind), xupd = xupd_op(st.kind);
+  const char* syrk_name = tall ? "ns_syrk_xtx" : "ns_syrk_xxt";
+  const char* xupd_name = tall ? "ns_xb_update" : "ns_bx_update";
   int s = 0, par = 0;   // X0 is in Q (parity 0)
   for (int L : part) {
-    if (L > 1 && !b.gram) { set_error("internal: Gram block on a bucket without Gram buffers"); return DMUON_ERR_INVALID_ARG; }
+    if (L > 1 && !st.gram) { set_error("internal: Gram block on a bucket without Gram buffers"); return DMUON_ERR_INVALID_ARG; }
     if (L > 3) { set_error("internal: Gram block longer than 3"); return DMUON_ERR_INVALID_ARG; }
     const int xs = 10 + par, xd = 10 + (1 - par);
     int g = 0, bc = 1, bn = 2, t = 3, r = 1;     // R_0 = B_0 (alias)
-    if ((rc = emit(OP_SYRK, CK_ONE, s, s, "ns_syrk_xxt", -1, -1, -1, -1, g, xs))) return rc;            // G = X X^T
+    if ((rc = emit(syrk, CK_GRAM, s, s, syrk_name, -1, -1, -1, -1, g, xs))) return rc;                  // G = X X^T
     if ((rc = emit(OP_SQ, CK_POLY, s, s, "ns_sq_poly", g, g, g, -1, bc, -1))) return rc;                // B = b G + c G G
     for (int i = 1; i < L; ++i) {
-      const int st = s + i;
-      if ((rc = emit(OP_SQ, CK_A, st - 1, st - 1, "ns_gram_mm", bc, g, g, -1, t, -1))) return rc;       // T = a G + B G
-      if ((rc = emit(OP_SQ, CK_A, st - 1, st - 1, "ns_gram_mm", t, bc, t, -1, g, -1))) return rc;       // G' = a T + T B
-      if ((rc = emit(OP_SQ, CK_POLY, st, st, "ns_sq_poly", g, g, g, -1, bn, -1))) return rc;            // B' = b G' + c G' G'
+      const int stp = s + i;
+      if ((rc = emit(OP_SQ, CK_A, stp - 1, stp - 1, "ns_gram_mm", bc, g, g, -1, t, -1))) return rc;     // T = a G + B G
+      if ((rc = emit(OP_SQ, CK_A, stp - 1, stp - 1, "ns_gram_mm", t, bc, t, -1, g, -1))) return rc;     // G' = a T + T B
+      if ((rc = emit(OP_SQ, CK_POLY, stp, stp, "ns_sq_poly", g, g, g, -1, bn, -1))) return rc;          // B' = b G' + c G' G'
       const int rn = (i == 1) ? 4 : t;            // free buffer: R (i = 1), then T (not needed after G')
-      if ((rc = emit(OP_SQ2, CK_RACC, s, st, "ns_gram_mm", bn, r, bn, r, rn, -1))) return rc;            // R' = (prod a) B' + a R + B' R
+      if ((rc = emit(OP_SQ2, CK_RACC, s, stp, "ns_gram_mm", bn, r, bn, r, rn, -1))) return rc;           // R' = (prod a) B' + a R + B' R
       r = rn;
       const int tmp = bc; bc = bn; bn = tmp;
     }
-    if ((rc = emit(OP_BX, CK_APOW, s, s + L - 1, "ns_bx_update", r, -1, -1, -1, xd, xs))) return rc;     // X' = (prod a) X + R X
+    if ((rc = emit(xupd, CK_APOW, s, s + L - 1, xupd_name, r, -1, -1, -1, xd, xs))) return rc;           // X' = (prod a) X + R X
     s += L;
     par ^= 1;
     ++prog.x_updates;
@@ -634,13 +804,15 @@ int build_program(Plan& p, BucketPlan& b, const Partition& part, NsProgram& prog
   return DMUON_OK;
 }
 
-void launch_coefs(const NsLaunch& L, const float* coeffs, bool per_step, float* alpha, float* beta, float* beta2) {
+void launch_coefs(const NsLaunch& L, const ShapeTables& st, const float* coeffs, bool per_step, float* alpha,
+                  float* beta, float* beta2) {
   auto co = [&](int step, int which) { return coeffs[(per_step ? 3 * step : 0) + which]; };
   *alpha = 1.f; *beta = 0.f; *beta2 = 0.f;
   double prod = 1.0;
+  const double g = st.gscale, cx = st.xscale;
   switch (L.ck) {
-    case CK_ONE: break;
-    case CK_POLY: *alpha = co(L.s1, 2); *beta = co(L.s1, 1); break;
+    case CK_GRAM: *alpha = static_cast<float>(g / (cx * cx)); break;
+    case CK_POLY: *alpha = static_cast<float>(co(L.s1, 2) / (g * g)); *beta = static_cast<float>(co(L.s1, 1) / g); break;
     case CK_A: *beta = co(L.s1, 0); break;
     case CK_RACC:
       for (int j = L.s0; j < L.s1; ++j) prod *= co(j, 0);
@@ -656,50 +828,48 @@ void launch_coefs(const NsLaunch& L, const float* coeffs, bool per_step, float* 
 
 }  // namespace
 
-int run_ns_steps(Plan& plan, int steps, const float* coeffs, bool per_step, const Options& opt, cudaStream_t stream) {
-  for (int bi : plan.order) {
-    int rc = run_ns_bucket(plan, bi, steps, coeffs, per_step, opt, stream);
-    if (rc) return rc;
-  }
-  return DMUON_OK;
-}
-
 int run_ns_bucket(Plan& plan, int bucket, int steps, const float* coeffs, bool per_step, const Options& opt,
-                  cudaStream_t stream) {
-  {
-    BucketPlan& b = plan.buckets[bucket];
-    if (!plan.fp32) {
-      const Partition part = choose_partition(steps, coeffs, per_step, b.gram && opt.gram_blocks);
-      const std::string key = partition_key(part);
-      auto it = b.programs.find(key);
-      if (it == b.programs.end()) {
-        NsProgram prog;
-        int rc = build_program(plan, b, part, prog);
-        if (rc) return rc;
-        it = b.programs.emplace(key, std::move(prog)).first;
-      }
-      for (const NsLaunch& L : it->second.launches) {
-        float alpha, beta, beta2;
-        launch_coefs(L, coeffs, per_step, &alpha, &beta, &beta2);
-        ProfScope ps(L.name.c_str(), stream);
-        int rc = bucket_launch(plan, b, L.op, L.probs, alpha, beta, beta2, stream);
-        if (rc) return rc;
-      }
-    } else {
-      for (int s = 0; s < steps; ++s) {
-        const float* q = coeffs + (per_step ? 3 * s : 0);
-        const float a = q[0], bb = q[1], c = q[2];
-        const int parity = s & 1;                 // step 0 reads Q (parity 0) and writes P
-        for (int idx : b.mats) {
-          const MatrixInfo& mi = plan.mats[idx];
-          float* X[2] = {reinterpret_cast<float*>(plan.ws + mi.off_q), reinterpret_cast<float*>(plan.ws + mi.off_p)};
-          float* A = reinterpret_cast<float*>(plan.ws + mi.off_sq[0]);
-          float* B = reinterpret_cast<float*>(plan.ws + mi.off_sq[1]);
-          int rc;
-          if ((rc = launch_check_gemm(OP_SYRK, X[parity], nullptr, A, mi.m_pad, mi.n_pad, 1.f, 0.f, stream))) return rc;
-          if ((rc = launch_check_gemm(OP_SQ, A, nullptr, B, mi.m_pad, mi.m_pad, c, bb, stream))) return rc;
-          if ((rc = launch_check_gemm(OP_BX, B, X[parity], X[1 - parity], mi.m_pad, mi.n_pad, 1.f, a, stream))) return rc;
-        }
+                  const FinalEpilogue& fin, cudaStream_t stream) {
+  BucketPlan& bp = plan.buckets[bucket];
+  ShapeTables& st = plan.shapes_tbl[bp.shape];
+  const int count = static_cast<int>(bp.mats.size());
+  if (!plan.fp32) {
+    const Partition part = choose_partition(steps, coeffs, per_step, st.gram && opt.gram_blocks);
+    const std::string key = partition_key(part);
+    auto it = st.programs.find(key);
+    if (it == st.programs.end()) {
+      NsProgram prog;
+      int rc = build_program(plan, st, part, prog);
+      if (rc) return rc;
+      it = st.programs.emplace(key, std::move(prog)).first;
+    }
+    const bool fused = bucket_fuses(plan, st, steps, opt) && fin.epi != EPI_F16;
+    const size_t nl = it->second.launches.size();
+    for (size_t li = 0; li < nl; ++li) {
+      const NsLaunch& L = it->second.launches[li];
+      float alpha, beta, beta2;
+      launch_coefs(L, st, coeffs, per_step, &alpha, &beta, &beta2);
+      const bool last = fused && li + 1 == nl;
+      std::string name = L.name;
+      if (last) name.replace(name.find("_update"), 7, fin.epi == EPI_BF16 ? "_out" : "_apply");
+      ProfScope ps(name.c_str(), stream);
+      int rc = shape_launch(plan, st, count, bp.rec0, L.op, L.probs, alpha, beta, beta2, last ? fin : FinalEpilogue(), stream);
+      if (rc) return rc;
+    }
+  } else {
+    for (int s = 0; s < steps; ++s) {
+      const float* q = coeffs + (per_step ? 3 * s : 0);
+      const float a = q[0], bb = q[1], c = q[2];
+      const int parity = s & 1;                 // step 0 reads Q (parity 0) and writes P
+      for (int k = 0; k < count; ++k) {
+        uint8_t* slot = plan.ws + st.base + static_cast<size_t>(k) * st.mat_bytes;
+        float* X[2] = {reinterpret_cast<float*>(slot + st.off_q), reinterpret_cast<float*>(slot + st.off_p)};
+        float* A = reinterpret_cast<float*>(slot + st.off_sq[0]);
+        float* B = reinterpret_cast<float*>(slot + st.off_sq[1]);
+        int rc;
+        if ((rc = launch_check_gemm(OP_SYRK, X[parity], nullptr, A, st.m_pad, st.n_pad, 1.f, 0.f, stream))) return rc;
+        if ((rc = launch_check_gemm(OP_SQ, A, nullptr, B, st.m_pad, st.m_pad, c, bb, stream))) return rc;
+        if ((rc = launch_check_gemm(OP_BX, B, X[parity], X[1 - parity], st.m_pad, st.n_pad, 1.f, a, stream))) return rc;
       }
     }
   }

@@ -1,7 +1,8 @@
 // Host-side planner of libdmuon: groups the heterogeneous matrices of a call into shape buckets (PAPER.md:180,
-// "grouped by shape and advanced ... together"), lays out the workspace, builds the TMA descriptors and grouped
-// launch tables once, and picks each bucket's tile configuration by on-device measurement with a persistent
-// cache keyed by problem shape and op (Fig. 6).
+// "grouped by shape and advanced ... together"), lays out ONE workspace region that the buckets use one after the
+// other, builds the TMA descriptors and grouped launch tables once per bucket shape, and picks each bucket shape's
+// tile configuration by on-device measurement with a persistent cache keyed by problem shape and op (PAPER.md:184,
+// Fig. 6).
 #pragma once
 
 #include <map>
@@ -14,39 +15,56 @@ namespace dmuon {
 struct Options {
   int steps = 5;
   float coeffs[3] = {3.4445f, -4.7750f, 2.0315f};
+  std::vector<float> sched;     // option "coeffs_sched": one (a, b, c) per step for the Muon-step entry points
+                                // (per-step sets such as Polar Express); empty = `coeffs` at every step
   bool fp32_check = false;
   bool autotune = true;
   bool profile = false;
   std::string cache_path;       // resolved lazily
   bool cache_path_set = false;
   float eps = 1e-7f;
-  int force_variant[3] = {-1, -1, -1};   // per tiling op (SYRK, SQ, BX): -1 = tuned, else this tile configuration
-  bool overlap = false;         // run the elementwise passes of one bucket under the GEMMs of another (side stream);
-                                // measured <= 1 % on config 4 (the step is power-bound: hiding a pass saves no energy)
+  int force_variant[3] = {-1, -1, -1};   // per tiling op (SYRK, SQ, X update): -1 = tuned, else this tile configuration
   bool gram_blocks = true;      // schedule "auto": Gram blocks (Eq. 4) on wide buckets; false = plain X iteration
+  bool fuse = true;             // a6 / the bf16 NS output fused into the last X-update epilogue (aligned buckets)
+  bool keep_o = false;          // keep every matrix's unrounded NS result readable after the call
+                                // (dmuon_read_ns_output): fused epilogues also store it, buckets do not share memory
+  size_t chunk_bytes = 12ull << 30;   // workspace a bucket may use; larger buckets run as chunks of fewer matrices
+  int host_groups = 32;         // dmuon_muon_step_host: at most this many groups of whole shape periods (layers) ...
+  int host_slots = 4;           // ... moving through this many device staging slots (measured: profiles/r2_experiments.md)
+  float tune_ms = 40.f;         // autotune: back-to-back time per candidate (long enough for the power cap to act)
+};
+
+// How a matrix is held in the workspace.
+enum MatKind : int {
+  K_WIDE = 0,      // rows <= cols, both multiples of 128: X [rows x cols] as stored; products SYRK, BX
+  K_TALL = 1,      // rows >  cols, both multiples of 128: Y = X^T [rows x cols] AS STORED; products SYRK_T, XB
+  K_GENERIC = 2    // any other shape (and every matrix in fp32 check mode): oriented (m <= n, transposed on the way in
+                   // and out by the elementwise kernels when rows > cols) and zero-padded to multiples of 128
 };
 
 struct MatrixInfo {
   int rows, cols;        // stored
   int m, n;              // oriented (m <= n)
   int m_pad, n_pad;      // padded to multiples of 128
-  bool transposed;
-  int bucket;
-  size_t off_p, off_q;   // byte offsets into the workspace: the two m_pad x n_pad X buffers
-  size_t off_sq[5];      // m_pad x m_pad buffers: G, B, and (Gram-block buckets only) B', T, R
+  int kind;              // MatKind
+  int buf_rows, buf_cols;// shape of the two X buffers: stored shape (aligned kinds) or m_pad x n_pad (generic)
+  bool transposed;       // generic and rows > cols
+  int bucket;            // index into Plan::buckets
+  int slot;              // position inside its bucket
+  int rec;               // index of its MatRec (records are ordered bucket by bucket)
   bool gram;             // bucket eligible for Gram blocks (wide enough that they save work)
+  float xscale, gscale;  // powers of two: the workspace holds xscale * X and gscale * G (fp16 range)
 };
 
 // Tile configuration of one op of one bucket ("variant" of dmuon_ns_gemm).
 struct TileConfig {
   bool pair = false;     // CTA-pair tiling: 256 x 256 units on two SMs (cta_group::2)
-  bool quad = false;     // CTA-quad tiling: two pair units per cluster of 4, shared operand panel multicast by TMA
   int width = 2;         // single-CTA tiling, blocks per work unit: 2 -> UMMA N = 256, 1 -> N = 128
-  int order = 0;         // 0: panel-major (all block rows of one column panel first), 1: row-major
+  int order = 0;         // 0: column-panel-major (all block rows of one column panel first), 1: row-major
 };
 // Variants 0..3: single CTA, (width, order) = (2,0), (1,0), (2,1), (1,1); 4, 5: CTA pair, order 0, 1.
-// 6: CTA quad.  The symmetric ops have one ordering: their variants are 0, 1 (single CTA), 4 (pair) and 6 (quad).
-constexpr int kNumVariants = 7;
+// The symmetric ops have one ordering: their variants are 0, 1 (single CTA) and 4 (pair).
+constexpr int kNumVariants = 6;
 bool variant_valid(GemmOp op, int variant);
 TileConfig variant_config(int variant);
 
@@ -59,20 +77,20 @@ typedef std::vector<int> Partition;
 Partition choose_partition(int steps, const float* coeffs, bool per_step, bool gram);
 bool gram_eligible(int m_pad, int n_pad, bool fp32);
 
-// How a launch's (alpha, beta, beta2) follow from the per-step coefficients (a_i, b_i, c_i).
+// How a launch's (alpha, beta, beta2) follow from the per-step coefficients (a_i, b_i, c_i) and the bucket's scales
+// (the workspace holds cx X and g G, powers of two).
 enum CoefKind : int {
-  CK_ONE = 0,    // alpha = 1                                            SYRK: G = X X^T
-  CK_POLY,       // alpha = c_s1, beta = b_s1                            B = b G + c G G
-  CK_A,          // alpha = 1, beta = a_s1                               T = a G + B G ; G' = a T + T B
+  CK_GRAM = 0,   // alpha = g / cx^2                                     SYRK: g G = (g / cx^2) (cx X)(cx X)^T
+  CK_POLY,       // alpha = c_s1 / g^2, beta = b_s1 / g                  B = b G + c G G  from g G
+  CK_A,          // alpha = 1, beta = a_s1                               T = a G + B G ; G' = a T + T B  (linear in g G)
   CK_RACC,       // alpha = 1, beta = prod a_[s0, s1), beta2 = a_s1      R' = (prod a) B' + a R + B' R
-  CK_APOW        // alpha = 1, beta = prod a_[s0, s1]                    X' = (prod a) X + R X
+  CK_APOW        // alpha = 1, beta = prod a_[s0, s1]                    X' = (prod a) X + R X           (linear in cx X)
 };
 struct NsLaunch {
   GemmOp op;
   CoefKind ck;
   int s0, s1;                  // step indices the coefficients come from
-  GemmProblem* probs;          // device, one per matrix of the bucket
-  int k_blocks, n_blocks;
+  GemmProblem* probs;          // device, one per matrix slot of the bucket shape
   std::string name;            // profiling name: family[m_pad x n_pad]
 };
 struct NsProgram {
@@ -80,61 +98,102 @@ struct NsProgram {
   int x_updates = 0;           // how many times X switched buffers (result parity)
 };
 
-struct BucketPlan {
-  int m_pad = 0, n_pad = 0;
+// Everything the buckets of one (m_pad, n_pad, kind) share: buckets that are chunks of one shape use the same
+// workspace slots, so the same problem tables, tile units and tuned variants serve all of them.
+struct ShapeTables {
+  int m_pad = 0, n_pad = 0, kind = K_WIDE;
   bool gram = false;
-  std::vector<int> mats;               // matrix indices
+  int slots = 0;                       // matrices per chunk (problems per table)
+  int buf_rows = 0, buf_cols = 0;
+  size_t mat_bytes = 0;                // workspace bytes per matrix slot
+  size_t off_p = 0, off_q = 0;         // offsets of the two X buffers inside a slot
+  size_t off_sq[5] = {0, 0, 0, 0, 0};  // m_pad x m_pad buffers: G, B, and (Gram-block buckets only) B', T, R
+  size_t base = 0;                     // offset of slot 0 in the workspace
+  float xscale = 1.f, gscale = 1.f;
   std::map<std::string, NsProgram> programs;   // by partition signature, e.g. "32"
-  TileUnit* units[3] = {nullptr, nullptr, nullptr};   // per tiling op (SYRK, SQ / SQ2, BX)
+  TileUnit* units[3] = {nullptr, nullptr, nullptr};   // per tiling op (SYRK*, SQ / SQ2, X update)
   int units_per_problem[3] = {0, 0, 0};
   int variant[3] = {0, 0, 0};
-  // scratch problem tables for the autotuner
-  GemmProblem* tune_probs[3] = {nullptr, nullptr, nullptr};
+  GemmProblem* tune_probs[3] = {nullptr, nullptr, nullptr};   // scratch problem tables for the autotuner
+  bool tuned_now = false;              // at least one op was timed (not cached) when this plan was built
+};
+
+struct BucketPlan {
+  int shape = 0;                       // index into Plan::shapes_tbl
+  std::vector<int> mats;               // matrix indices (caller order); slot k holds mats[k]
+  int rec0 = 0;                        // first MatRec of the bucket
+  ElemTables tables{};                 // work lists of the bucket's elementwise launches
+  double work = 0;
 };
 
 struct Plan {
   std::vector<int32_t> shapes;         // key
   bool fp32 = false;
+  bool keep_o = false;
+  size_t chunk_bytes = 0;
+  int device = 0;
+  void* ext_ws = nullptr;
+  uint64_t stamp = 0;                  // last use (LRU eviction)
+  uint64_t id = 0;                     // unique; find_plan(id) tells whether the plan still exists
+  bool o_valid = false;                // the last call left every matrix's NS result readable in the workspace
   std::vector<MatrixInfo> mats;
-  std::vector<BucketPlan> buckets;
+  std::vector<ShapeTables> shapes_tbl;
+  std::vector<BucketPlan> buckets;     // in execution order
   size_t ws_bytes = 0;
-  uint8_t* ws = nullptr;               // device workspace (owned unless external)
-  bool ws_owned = false;
-  // elementwise tables
-  std::vector<MatRec> h_recs;          // host mirror (pointers patched per call)
+  uint8_t* ws = nullptr;               // device workspace (the device's shared region, or the caller's)
+  // elementwise records, ordered bucket by bucket
+  std::vector<MatRec> h_recs;          // host mirror (pointers patched per call, uploaded through a pinned snapshot)
   MatRec* d_recs = nullptr;
   float* d_inv_norm = nullptr;
-  ElemTables tables{};                 // all matrices
-  std::vector<int> order;              // execution order of the buckets (most NS work first)
-  std::vector<ElemTables> parts;       // per bucket, in execution order (empty: one bucket or check mode)
-  cudaStream_t side = nullptr;         // side stream for the elementwise passes hidden under GEMMs
-  std::vector<cudaEvent_t> ev;         // fork / join events of the overlapped step
-  std::string bound_key;               // schedule signature rec.O was last bound for
+  int bound_kind = -1;                 // what rec.O was last bound for
+  std::string bound_key;
   std::vector<void*> d_allocs;         // everything to cudaFree
   int sm_count = 148;
+  double tune_seconds = 0;             // time spent measuring tile configurations while building this plan
   ~Plan();
 };
 
-size_t plan_workspace_bytes(const int32_t* shapes, int count, bool fp32);
-// Builds (or fetches) the plan for a shape set.  ext_ws/ext_bytes: caller workspace or (nullptr, 0).
+size_t plan_workspace_bytes(const int32_t* shapes, int count, const Options& opt);
+// Builds (or fetches) the plan for a shape set on the current device.  ext_ws/ext_bytes: caller workspace or (nullptr, 0).
 int get_plan(const int32_t* shapes, int count, const Options& opt, void* ext_ws, size_t ext_bytes, cudaStream_t stream,
              Plan** out);
 void drop_plans();
+Plan* find_plan(uint64_t id);
+void release_workspaces();
+int tune_cache_entries();
+void forget_tune_cache();
 
-// Enqueue k NS steps over every bucket of the plan; X0 is in buffer Q.  result_parity(...) tells where a bucket's
-// result ends (0 = Q, 1 = P) for the same arguments.
-int run_ns_steps(Plan& plan, int steps, const float* coeffs, bool per_step, const Options& opt, cudaStream_t stream);
+// What the last X update of a bucket does besides (or instead of) storing the new X.
+struct FinalEpilogue {
+  Epilogue epi = EPI_F16;
+  float lr = 0.f, lrwd = 0.f;
+  bool store_c = true;
+};
+// Enqueue k NS steps of one bucket; X0 is in buffer Q.  result_parity(...) tells where the result ends (0 = Q, 1 = P).
 int run_ns_bucket(Plan& plan, int bucket, int steps, const float* coeffs, bool per_step, const Options& opt,
-                  cudaStream_t stream);
-int result_parity(const Plan& plan, const BucketPlan& b, int steps, const float* coeffs, bool per_step, const Options& opt);
+                  const FinalEpilogue& fin, cudaStream_t stream);
+int result_parity(const Plan& plan, const ShapeTables& st, int steps, const float* coeffs, bool per_step, const Options& opt);
+bool bucket_fuses(const Plan& plan, const ShapeTables& st, int steps, const Options& opt);
 std::string partition_key(const Partition& p);
 
 // Build tile units for an op.
 std::vector<TileUnit> make_units(GemmOp op, int m_blocks, int n_blocks, const TileConfig& cfg);
 int encode_tmap_2d(CUtensorMap* out, const void* base, uint64_t rows, uint64_t cols, uint32_t box_cols,
                    uint32_t box_rows);
+// A, B: operand matrices with their (rows, cols) as laid out in memory.
 int fill_problem(GemmProblem& g, GemmOp op, const void* a_mat, uint64_t a_rows, uint64_t a_cols, const void* b_mat,
-                 uint64_t b_rows, uint64_t b_cols, const void* d, void* c, int ldc, const void* d2 = nullptr);
+                 uint64_t b_rows, uint64_t b_cols, const void* d, void* c, int ldc, const void* d2 = nullptr, int rec = 0);
 int check_device();
+
+// ---------------------------------------------------------------- owner assignment (assign.cu)
+struct AssignInput {
+  int num_shapes, num_ranks;
+  const int32_t* counts;        // [num_shapes] n_s
+  const int32_t* num_batches;   // [num_shapes] |B_s|
+  const int32_t* batch_sizes;   // concatenated B_s
+  const double* costs;          // concatenated c_{s,b}
+};
+int assign_owners_greedy(const AssignInput& in, int32_t* x_out, double* makespan);
+int assign_owners_exact(const AssignInput& in, int32_t* x_out, double* makespan, long long node_limit);
 
 }  // namespace dmuon

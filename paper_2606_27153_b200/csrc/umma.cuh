@@ -27,21 +27,49 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
   asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
 }
-// Spin on the phase parity.  A protocol bug would otherwise hang the GPU, so a (very large) poll bound traps instead.
+__device__ __forceinline__ uint32_t mbar_try_wait(uint32_t bar, uint32_t parity) {
+  uint32_t done;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(done)
+      : "r"(bar), "r"(parity)
+      : "memory");
+  return done;
+}
+__device__ __forceinline__ uint64_t global_timer_ns() {
+  uint64_t t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
+}
+// Wait for the phase with the given parity.  mbarrier.try_wait suspends the thread for a hardware-chosen time slice
+// before it returns false, so the loop is not a hot spin.  A protocol bug would hang the GPU: after 20 s of WALL time
+// (not a poll count: a time-sliced or profiled GPU may need many polls) the kernel traps instead.
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-  uint32_t done = 0;
+  if (mbar_try_wait(bar, parity)) return;
+  const uint64_t t0 = global_timer_ns();
   uint32_t polls = 0;
-  while (true) {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-        "selp.u32 %0, 1, 0, p;\n\t}"
-        : "=r"(done)
-        : "r"(bar), "r"(parity)
-        : "memory");
-    if (done) break;
-    if (++polls > (1u << 28)) __trap();
+  while (!mbar_try_wait(bar, parity)) {
+    if ((++polls & 0xFFFu) == 0 && global_timer_ns() - t0 > 20000000000ull) __trap();
   }
+}
+// Whole-warp wait of the epilogue warps: lane 0 polls, sleeping between polls (the accumulator of a 256-wide unit
+// takes tens of microseconds); the other 31 lanes park at the warp barrier and then confirm the phase with one
+// try_wait each (it succeeds at once; it is what orders their later tcgen05.ld after the commit).
+__device__ __forceinline__ void mbar_wait_warp(uint32_t bar, uint32_t parity, uint32_t sleep_ns) {
+  if ((threadIdx.x & 31) == 0) {
+    if (!mbar_try_wait(bar, parity)) {
+      const uint64_t t0 = global_timer_ns();
+      uint32_t polls = 0;
+      while (!mbar_try_wait(bar, parity)) {
+        if (sleep_ns) __nanosleep(sleep_ns);
+        if ((++polls & 0xFFFu) == 0 && global_timer_ns() - t0 > 20000000000ull) __trap();
+      }
+    }
+  }
+  __syncwarp();
+  mbar_wait(bar, parity);
 }
 
 // ------------------------------------------------------------------------------------------------ cluster
@@ -74,27 +102,6 @@ __device__ __forceinline__ void tma_load_2d_pair(uint32_t smem_dst, uint64_t tma
   asm volatile(
       "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
       ::"r"(smem_dst), "l"(tmap), "r"(c0), "r"(c1), "r"(bar)
-      : "memory");
-}
-// Multicast form: the tile lands at the same CTA-relative offset in every CTA of `cta_mask` (cluster ranks), and each
-// destination CTA's mbarrier at the CTA-relative offset of `bar` receives the bytes that landed in that CTA.
-__device__ __forceinline__ void tma_load_2d_mcast(uint32_t smem_dst, uint64_t tmap, int c0, int c1, uint32_t bar,
-                                                  uint16_t cta_mask) {
-  asm volatile(
-      "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.multicast::cluster"
-      " [%0], [%1, {%2, %3}], [%4], %5;"
-      ::"r"(smem_dst), "l"(tmap), "r"(c0), "r"(c1), "r"(bar), "h"(cta_mask)
-      : "memory");
-}
-// CTA-pair multicast form: as above, but every destination CTA's bytes are signalled on the barrier of ITS pair's
-// leader (the even CTA): `bar` is this CTA's own barrier address with the pair bit (bit 24 of the cluster shared
-// window, the lowest bit of the CTA rank) cleared.
-__device__ __forceinline__ void tma_load_2d_pair_mcast(uint32_t smem_dst, uint64_t tmap, int c0, int c1, uint32_t bar,
-                                                       uint16_t cta_mask) {
-  asm volatile(
-      "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster"
-      " [%0], [%1, {%2, %3}], [%4], %5;"
-      ::"r"(smem_dst), "l"(tmap), "r"(c0), "r"(c1), "r"(bar & 0xFEFFFFFFu), "h"(cta_mask)
       : "memory");
 }
 __device__ __forceinline__ void tma_prefetch_desc(uint64_t tmap) {
@@ -178,17 +185,29 @@ __device__ __forceinline__ uint64_t desc_kmajor(uint32_t saddr) {
   const uint32_t lo = ((saddr >> 4) & 0x3FFFu) | (1u << 16);            // LBO unused for swizzled K-major (set to 1)
   return (static_cast<uint64_t>(kDescHi) << 32) | lo;
 }
-// MN-major operand (B of X' = aX + BX): 64 K rows x 128 B per 64-wide N chunk; next N chunk LBO = 8192 B further,
-// next group of 8 K rows SBO = 1024 B further.
+// MN-major operand (X in X' = aX + BX; both operands of G = Y^T Y): 64 K rows x 128 B per 64-wide M/N chunk; next
+// M/N chunk LBO = 8192 B further, next group of 8 K rows SBO = 1024 B further.
 __device__ __forceinline__ uint64_t desc_mnmajor(uint32_t saddr) {
   const uint32_t lo = ((saddr >> 4) & 0x3FFFu) | ((8192u >> 4) << 16);
   return (static_cast<uint64_t>(kDescHi) << 32) | lo;
 }
 // Instruction descriptor for kind::f16: D = fp32 (bits [4,6) = 1), A/B format fp16 (0) in [7,10)/[10,13),
-// B major-ness in bit 16 (1 = MN-major), N >> 3 in [17,23), M >> 4 in [24,29).
-__device__ __forceinline__ uint32_t make_idesc(int m, int n, bool b_mn_major) {
-  return (1u << 4) | (static_cast<uint32_t>(b_mn_major) << 16) | (static_cast<uint32_t>(n >> 3) << 17) |
-         (static_cast<uint32_t>(m >> 4) << 24);
+// A / B major-ness in bits 15 / 16 (1 = MN-major), N >> 3 in [17,23), M >> 4 in [24,29).
+__device__ __forceinline__ uint32_t make_idesc(int m, int n, bool a_mn_major, bool b_mn_major) {
+  return (1u << 4) | (static_cast<uint32_t>(a_mn_major) << 15) | (static_cast<uint32_t>(b_mn_major) << 16) |
+         (static_cast<uint32_t>(n >> 3) << 17) | (static_cast<uint32_t>(m >> 4) << 24);
+}
+
+__device__ __forceinline__ void st_shared_v4(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+  asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
+__device__ __forceinline__ void st_shared_u16(uint32_t addr, uint32_t v) {
+  asm volatile("st.shared.u16 [%0], %1;" ::"r"(addr), "h"(static_cast<uint16_t>(v)) : "memory");
+}
+__device__ __forceinline__ uint4 ld_shared_v4(uint32_t addr) {
+  uint4 v;
+  asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr) : "memory");
+  return v;
 }
 
 __device__ __forceinline__ uint32_t pack_half2(float lo, float hi) {

@@ -108,3 +108,37 @@ def ns_inputs(device="cpu"):
     """configs[0]: the tiny NS batch, 8 x (128 x 512)."""
     shapes = config_shapes(1)
     return shapes, [iid_scaled(s, seed_for(1, i), device) for i, s in enumerate(shapes)]
+
+
+# ---------------------------------------------------------------- hostile spectra (Gram-block error study, DESIGN.md section 6)
+def with_spectrum(shape: Shape, sigmas: torch.Tensor, seed: int, device="cpu") -> torch.Tensor:
+    """A matrix with prescribed singular values: Q1 diag(sigmas) Q2^T with Haar-like orthonormal factors (QR of
+    Gaussians), rounded to bf16.  len(sigmas) = min(shape)."""
+    r, c = shape
+    m = min(r, c)
+    g = _gen(seed, device)
+    q1, _ = torch.linalg.qr(torch.randn((r, m), generator=g, device=device, dtype=torch.float64))
+    q2, _ = torch.linalg.qr(torch.randn((c, m), generator=g, device=device, dtype=torch.float64))
+    return ((q1 * sigmas.to(device=device, dtype=torch.float64)) @ q2.t()).to(torch.float32).to(torch.bfloat16)
+
+
+def hostile_inputs(shape: Shape, seed: int, device="cpu"):
+    """(name, matrix) pairs that stress 16-bit Newton-Schulz and the Gram-space recurrence in particular: spectra with a
+    huge dynamic range, clusters at both ends, low rank plus rounding noise, extreme overall scales."""
+    r, c = shape
+    m = min(r, c)
+    out = []
+    gen = _gen(seed, device)
+    z = torch.randn((r, c), generator=gen, device=device, dtype=torch.float32)
+    p = torch.randn((r, LOW_RANK), generator=gen, device=device, dtype=torch.float32)
+    q = torch.randn((c, LOW_RANK), generator=gen, device=device, dtype=torch.float32)
+    out.append(("rank8_energy_1000x", (SIGMA_G * z + SIGMA_G * math.sqrt(1000.0 / LOW_RANK) * (p @ q.t())).to(torch.bfloat16)))
+    out.append(("geometric_decay_1_to_1e-6", with_spectrum(shape, torch.logspace(0, -6, m, dtype=torch.float64), seed + 1, device)))
+    half = torch.cat([torch.ones(m // 2, dtype=torch.float64), torch.full((m - m // 2,), 1e-4, dtype=torch.float64)])
+    out.append(("half_converged_half_tiny", with_spectrum(shape, half, seed + 2, device)))
+    out.append(("exact_rank8_plus_bf16_noise", (p @ q.t()).to(torch.bfloat16)))
+    out.append(("iid_scale_1e-3", (z * 1e-3).to(torch.bfloat16)))
+    out.append(("iid_scale_1e1", (z * 1e1).to(torch.bfloat16)))
+    two = torch.cat([torch.full((m // 16,), 1.0, dtype=torch.float64), torch.full((m - m // 16,), 0.02, dtype=torch.float64)])
+    out.append(("spikes_over_flat_bulk", with_spectrum(shape, two, seed + 3, device)))
+    return out

@@ -25,20 +25,52 @@ def test_dense_flops_match_survey_table():
 
 def test_executed_flops_follow_the_block_schedule():
     m, n = 4096, 14336
-    plain = {"buckets": [{"m": m, "n": n, "count": 1, "blocks": [1, 1, 1, 1, 1]}]}
-    blocks = {"buckets": [{"m": m, "n": n, "count": 1, "blocks": [3, 2]}]}
+    plain = {"buckets": [{"m": m, "n": n, "kind": "wide", "count": 1, "blocks": [1, 1, 1, 1, 1]},
+                         {"m": m, "n": n, "kind": "tall", "count": 1, "blocks": [1, 1, 1, 1, 1]}]}
+    blocks = {"buckets": [{"m": m, "n": n, "kind": "wide", "count": 1, "blocks": [3, 2]},
+                          {"m": m, "n": n, "kind": "tall", "count": 1, "blocks": [3, 2]}]}
     sym = 33 / 64                                    # T = 32 blocks: (T + 1) / (2 T)
     want_plain = 5 * (sym * (2 * m * m * n + 2 * m ** 3) + 2 * m * m * n)
     want_blocks = 2 * sym * 2 * m * m * n + 14 * sym * 2 * m ** 3 + 2 * 2 * m * m * n
     assert bench.executed_flops([(m, n)], plain) == pytest.approx(want_plain)
     assert bench.executed_flops([(n, m)], blocks) == pytest.approx(want_blocks)     # tall: same oriented shape
-    w = bench.kernel_work([(m, n)], blocks)
-    assert w["ns_bx_update"] == ("flop", 2 * 2 * m * m * n)
-    assert w["ns_gram_mm"][1] == pytest.approx(9 * sym * 2 * m ** 3)
-    assert w["ns_sq_poly"][1] == pytest.approx(5 * sym * 2 * m ** 3)
-    assert w["momentum_nesterov_sumsq"] == ("byte", 8 * m * n)
-    total = sum(v[1] for v in w.values() if v[0] == "flop")
-    assert total == pytest.approx(want_blocks)
+    assert bench.family_work("ns_bx_update", [(m, n)], blocks) == ("flop", 2 * 2 * m * m * n)
+    assert bench.family_work("ns_xb_apply", [(n, m)], blocks, 0.5) == ("flop", 2 * m * m * n)     # the fused one of two X updates
+    assert bench.family_work("ns_gram_mm", [(m, n)], blocks)[1] == pytest.approx(9 * sym * 2 * m ** 3)
+    assert bench.family_work("ns_sq_poly", [(n, m)], blocks)[1] == pytest.approx(5 * sym * 2 * m ** 3)
+    assert bench.family_work("momentum_nesterov_sumsq", [(m, n)], blocks) == ("byte", 8 * m * n)
+    assert bench.family_work("normalize_cast", [(m, n)], blocks) == ("byte", 4 * m * n)
+    fams = ("ns_syrk_xxt", "ns_sq_poly", "ns_gram_mm", "ns_bx_update")
+    assert sum(bench.family_work(f, [(m, n)], blocks)[1] for f in fams) == pytest.approx(want_blocks)
+
+
+def test_profile_breakdown_maps_launch_types_to_buckets():
+    """bench.profile_breakdown on a synthetic profile of config 4's buckets: tall buckets are named by the stored shape
+    (rows x cols), chunks of one bucket accumulate under one name, plain and fused X updates share the bucket's work."""
+    shapes = synth.config_shapes(4)
+    plan = {"buckets": [{"m": 4096, "n": 14336, "kind": "tall", "count": 32, "blocks": [3, 2]},
+                        {"m": 4096, "n": 14336, "kind": "tall", "count": 32, "blocks": [3, 2]},
+                        {"m": 4096, "n": 14336, "kind": "wide", "count": 32, "blocks": [3, 2]},
+                        {"m": 4096, "n": 4096, "kind": "wide", "count": 64, "blocks": [1] * 5},
+                        {"m": 1024, "n": 4096, "kind": "wide", "count": 64, "blocks": [3, 2]}]}
+    assert bench.bucket_key((14336, 4096)) == (4096, 14336, "tall") and bench.bucket_key((100, 260)) == (128, 384, "generic")
+    assert len(bench.shapes_of_launch_type("ns_xb_update[14336x4096]", shapes)) == 64
+    assert len(bench.shapes_of_launch_type("ns_bx_update[4096x14336]", shapes)) == 32
+    assert len(bench.shapes_of_launch_type("ns_sq_poly[4096x4096]", shapes)) == 64
+    prof = {"kernels": {"ns_xb_update[14336x4096]": {"launches": 2, "ms": 30.0}, "ns_xb_apply[14336x4096]": {"launches": 2, "ms": 31.0},
+                        "ns_bx_update[4096x4096]": {"launches": 4, "ms": 32.0}, "ns_bx_apply[4096x4096]": {"launches": 1, "ms": 8.5},
+                        "momentum_nesterov_sumsq": {"launches": 5, "ms": 10.0}}}
+    peaks = {"hbm_gbs": 6500.0, "tflops_burst": 1600.0, "tflops_sustained": 1400.0}
+    kernels, lt, dom = bench.profile_breakdown(prof, 1, 300.0, shapes, plan, peaks)
+    one = 64 * 2 * 4096 * 4096 * 14336                # one X update of the 64 tall matrices
+    assert lt["ns_xb_update[14336x4096]"]["work_per_step"] == pytest.approx(one)
+    assert lt["ns_xb_apply[14336x4096]"]["work_per_step"] == pytest.approx(one)
+    assert lt["ns_xb_update[14336x4096]"]["matrices_per_launch"] == 32
+    assert lt["ns_bx_update[4096x4096]"]["work_per_step"] == pytest.approx(4 * 64 * 2 * 4096 ** 3)
+    assert lt["ns_bx_apply[4096x4096]"]["achieved"] == pytest.approx(64 * 2 * 4096 ** 3 / 8.5e-3 / 1e12)
+    assert dom == "ns_bx_update[4096x4096]"
+    assert kernels["momentum_nesterov_sumsq"]["achieved"] == pytest.approx(8 * sum(r * c for r, c in shapes) / 10e-3 / 1e9)
+    assert kernels["ns_xb_update"]["ms_per_step"] == 30.0
 
 
 def _worker(rank, world, port, out):

@@ -301,3 +301,40 @@ def test_oracle_on_config1_matrix_against_svd():
     shapes, Xs = synth.ns_inputs("cpu")
     X = Xs[3].to(torch.float64).numpy()
     assert rel(oracle.ns(X), svd_closed_form(X, eps=1e-7)) < 1e-10
+
+
+# ---------------------------------------------------------------- AdamW (non-matrix parameters)
+
+def test_adamw_against_torch_optim_float64():
+    """oracle.adamw_step against torch.optim.AdamW (CPU, float64) over 6 steps with changing gradients: moments, bias
+    correction, eps placement and the decoupled decay (reading N17: the host stack's convention)."""
+    g = torch.Generator().manual_seed(11)
+    p0 = torch.randn(257, generator=g, dtype=torch.float64) * 0.3
+    lr, b1, b2, eps, wd = 3e-3, 0.9, 0.95, 1e-8, 0.1
+    pt = torch.nn.Parameter(p0.clone())
+    opt = torch.optim.AdamW([pt], lr=lr, betas=(b1, b2), eps=eps, weight_decay=wd)
+    p, m, v = p0.numpy().copy(), np.zeros(257), np.zeros(257)
+    for step in range(1, 7):
+        grad = torch.randn(257, generator=g, dtype=torch.float64) * (0.1 * step)
+        pt.grad = grad.clone()
+        opt.step()
+        p, m, v = oracle.adamw_step(p, grad.numpy(), m, v, lr, b1, b2, eps, wd, step)
+        st = opt.state[pt]
+        assert np.abs(p - pt.detach().numpy()).max() < 1e-14
+        assert np.abs(m - st["exp_avg"].numpy()).max() < 1e-15 and np.abs(v - st["exp_avg_sq"].numpy()).max() < 1e-15
+
+
+def test_adamw_first_step_closed_form():
+    """Step 1 from zero moments: mhat = g, vhat = g^2, so p1 = p0 (1 - lr wd) - lr g / (|g| + eps)."""
+    p0 = np.array([0.5, -0.25, 1.0, 0.0, 2.0])
+    g = np.array([0.1, -3.0, 1e-4, 7.0, 0.0])
+    lr, b1, b2, eps, wd = 1e-2, 0.9, 0.999, 1e-8, 0.05
+    p1, m1, v1 = oracle.adamw_step(p0, g, np.zeros(5), np.zeros(5), lr, b1, b2, eps, wd, 1)
+    want = p0 * (1 - lr * wd) - lr * g / (np.abs(g) + eps)
+    assert np.abs(p1 - want).max() < 1e-12       # sqrt(vhat) = |g| up to an ulp of the division by (1 - beta2)
+    assert np.allclose(m1, (1 - b1) * g, rtol=0, atol=1e-17) and np.allclose(v1, (1 - b2) * g * g, rtol=1e-15, atol=0)
+    # zero gradient: pure decay
+    assert p1[4] == 2.0 * (1 - lr * wd)
+    # wd = 0 and a huge eps: p moves by ~ -lr mhat / eps
+    p2, _, _ = oracle.adamw_step(p0, g, np.zeros(5), np.zeros(5), lr, b1, b2, 1e6, 0.0, 1)
+    assert np.abs((p2 - p0) + lr * g / (np.abs(g) + 1e6)).max() < 2.3e-16      # one ulp of the subtraction p2 - p0

@@ -1,0 +1,117 @@
+"""Performance guard + the energy-per-FLOP table of profiles/r2_energy_per_flop.md: the dominant kernel (the X update
+of the 4096 x 14336 bucket) against torch.matmul (cuBLAS) on the SAME shape and the SAME operand bits, each run back
+to back for >= 1.5 s with the SM clock and board power sampled.  torch.matmul is here as a yardstick only; it is never
+on the product path.  Run with -s to see the table:
+
+    python -m pytest tests/test_perf_gpu.py -m gpu -q -s
+"""
+import json
+import os
+import statistics
+import subprocess
+import tempfile
+import time
+
+import pytest
+import torch
+
+import paper_2606_27153_b200 as dm
+from paper_2606_27153_b200.binding import OP_BX, OP_SYRK, OP_SYRK_T, OP_XB
+
+pytestmark = [pytest.mark.gpu, pytest.mark.slow]
+SECS = float(os.environ.get("DMUON_PERF_SECS", "1.5"))
+
+
+class _Sampler:
+    def __init__(self):
+        self.f = tempfile.NamedTemporaryFile("w", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(torch.cuda.current_device()), "--query-gpu=clocks.sm,power.draw",
+                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        if not self.p:
+            return None, None
+        self.p.terminate()
+        self.p.wait()
+        rows = []
+        for line in open(self.f.name):
+            try:
+                a, b = line.split(",")
+                rows.append((float(a), float(b)))
+            except ValueError:
+                pass
+        os.unlink(self.f.name)
+        rows = rows[4:] or rows
+        if not rows:
+            return None, None
+        return statistics.median(r[0] for r in rows), statistics.mean(r[1] for r in rows)
+
+
+def _run(name, fn, flops):
+    for _ in range(3):
+        fn()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(); fn(); e1.record(); torch.cuda.synchronize()
+    reps = max(3, int(SECS * 1e3 / e0.elapsed_time(e1)))
+    s = _Sampler()
+    time.sleep(0.2)
+    e0.record()
+    for _ in range(reps):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    mhz, watts = s.stop()
+    ms = e0.elapsed_time(e1) / reps
+    tf = flops / ms / 1e9
+    row = {"case": name, "ms": round(ms, 4), "tflops": round(tf, 1), "sm_mhz": mhz, "watts": round(watts, 1) if watts else None,
+           "joule_per_tflop": round(watts / tf, 4) if watts else None,
+           "of_clock_peak": round(tf / (8192 * 148 * mhz * 1e-6), 3) if mhz else None}
+    print(json.dumps(row), flush=True)
+    time.sleep(0.5)
+    return row
+
+
+def test_x_update_energy_per_flop_vs_cublas_same_bits():
+    m, n, cnt = 4096, 14336, 8
+    g = torch.Generator(device="cuda").manual_seed(1)
+    sym = lambda t: (torch.triu(t) + torch.triu(t, 1).t()).contiguous()
+    B = [sym((torch.randn((m, m), generator=g, device="cuda") * 0.02).half()) for _ in range(cnt)]
+    X = [(torch.randn((m, n), generator=g, device="cuda") * 1e-2).half() for _ in range(cnt)]
+    C = [torch.empty((m, n), device="cuda", dtype=torch.float16) for _ in range(cnt)]
+    A = [torch.empty((m, m), device="cuda", dtype=torch.float16) for _ in range(cnt)]
+    fl = cnt * 2 * m * m * n
+    ours = _run("libdmuon ns_bx_update_pair (X' = aX + BX), fp16, column-panel-major", lambda: dm.ns_gemm(OP_BX, B, X, C, 1.0, 3.4445, variant=4), fl)
+
+    def mm16():
+        for b, x, c in zip(B, X, C):
+            torch.matmul(b, x, out=c)
+    cublas = _run("torch.matmul fp16, same B and X bits (no addend)", mm16, fl)
+    Bb, Xb = [b.bfloat16() for b in B], [x.bfloat16() for x in X]
+    Cb = [torch.empty((m, n), device="cuda", dtype=torch.bfloat16) for _ in range(cnt)]
+
+    def mmb():
+        for b, x, c in zip(Bb, Xb, Cb):
+            torch.matmul(b, x, out=c)
+    _run("torch.matmul bf16, B and X rounded to bf16", mmb, fl)
+    del Bb, Xb, Cb
+    _run("libdmuon ns_syrk_xxt_pair (G = X X^T, upper blocks), fp16", lambda: dm.ns_gemm(OP_SYRK, X, None, A, 1.0, 0.0, variant=4), fl * 136 * 4 / 1024)
+    # the tall orientation: the same matrices held as stored (Y = X^T)
+    Y = [x.t().contiguous() for x in X]
+    Cy = [torch.empty((n, m), device="cuda", dtype=torch.float16) for _ in range(cnt)]
+    del X, C
+    tall = _run("libdmuon ns_xb_update_pair (Y' = aY + YB), fp16, row-major", lambda: dm.ns_gemm(OP_XB, B, Y, Cy, 1.0, 3.4445, variant=5), fl)
+    _run("libdmuon ns_syrk_xtx_pair (G = Y^T Y, upper blocks), fp16", lambda: dm.ns_gemm(OP_SYRK_T, Y, None, A, 1.0, 0.0, variant=4), fl * 136 * 4 / 1024)
+    del Y, Cy, B, A
+    torch.cuda.empty_cache()
+    N = 8192
+    a = torch.randn((N, N), generator=g, device="cuda").bfloat16()
+    b = torch.randn((N, N), generator=g, device="cuda").bfloat16()
+    c = torch.empty((N, N), device="cuda", dtype=torch.bfloat16)
+    _run("torch.matmul bf16 8192^3 randn (the MEASURED_PEAKS.json recipe: the roofline denominator)", lambda: torch.matmul(a, b, out=c), 2 * N ** 3)
+    # the guard: on the same shape and bits the hand-written kernel is not slower than the library GEMM (it also adds a X)
+    assert ours["tflops"] >= 0.95 * cublas["tflops"], (ours, cublas)
+    assert tall["tflops"] >= 0.90 * cublas["tflops"], (tall, cublas)
