@@ -14,7 +14,7 @@
 // PAPER.md:51) on bf16 weights or on fp32 master weights, or the bf16 NS output of dmuon_ns_batched.
 //
 // Two tilings of one warp-specialised pipeline (warp 0 = TMA producer, warp 1 = tcgen05.mma issuer and TMEM owner,
-// warps 2..5 = epilogue: TMEM -> registers -> global):
+// warps 2..5 = epilogue: TMEM -> registers -> shared-memory tile -> global):
 //
 //   single CTA  (cta_group::1)  one CTA per SM computes a 128 x 128 or 128 x 256 unit; 4-stage ring of 48 KB.
 //   CTA pair    (cta_group::2)  a cluster of two CTAs (one TPC) computes a 256 x 256 unit with UMMA M = 256, N = 256:
@@ -40,7 +40,9 @@ namespace {
 using namespace umma;
 
 constexpr int kBlockBytes = kBlk * kBlkK * 2;   // 16 KB: 128 rows x 128 B of one operand block
-constexpr int kNumThreads = 192;
+constexpr int kEpiWarps = 4;                    // 4: one per TMEM lane quarter; 8: two per quarter taking alternate 32-column
+                                                // chunks (measured: no gain on short contractions, -2 % on config 4)
+constexpr int kNumThreads = 64 + 32 * kEpiWarps;
 constexpr int kTmemCols = 512;
 constexpr int kAccCols = 256;                   // columns per accumulator stage
 constexpr int kMaxStages = 6;
@@ -68,7 +70,7 @@ struct SmemCtl {
 };
 static_assert(sizeof(SmemCtl) <= 256, "SmemCtl");
 constexpr int kEpiTileBytes = 32 * 64;         // 32 rows x 32 fp16: one warp's 32-column chunk, or its transpose
-constexpr int kEpiStageBytes = 4 * 2 * kEpiTileBytes;   // per epilogue warp: a direct and a mirrored tile
+constexpr int kEpiStageBytes = kEpiWarps * 2 * kEpiTileBytes;   // per epilogue warp: a direct and a mirrored tile
 template <bool kPair> constexpr int smem_bytes() {
   return Tiling<kPair>::kStages * Tiling<kPair>::kStageBytes + 1024 /*alignment slack*/ + 256 /*SmemCtl*/ + kEpiStageBytes;
 }
@@ -163,7 +165,8 @@ __device__ __forceinline__ void epilogue_chunk(const uint32_t (&v)[32], const Ad
     // fp16 store of the chunk (32 rows x 32 columns per warp) and, for symmetric results, of its mirror image.  Both go
     // through a warp-private shared-memory tile so that every global store instruction writes whole 64-byte row segments
     // (8 rows x 64 B per instruction): one lane per row would write 32 half-sectors per instruction, and the mirror
-    // would take 32 two-byte stores per lane.  Tile: 32 rows x 64 B, 16-byte chunks XOR-swizzled by (row >> 1) & 3.
+    // would take 32 two-byte global stores per lane.  Tile: 32 rows x 64 B, 16-byte chunks XOR-swizzled by (row >> 1) & 3
+    // (conflict-free for the row-wise 16-byte stores, for ldmatrix / stmatrix and for the 8-rows-per-instruction reads).
     uint32_t o[16];
 #pragma unroll
     for (int e = 0; e < 16; ++e) o[e] = pack_half2(r[2 * e], r[2 * e + 1]);
@@ -174,13 +177,16 @@ __device__ __forceinline__ void epilogue_chunk(const uint32_t (&v)[32], const Ad
     for (int g = 0; g < 4; ++g)
       st_shared_v4(stage + lane * 64 + ((g ^ ((lane >> 1) & 3)) << 4), o[g * 4], o[g * 4 + 1], o[g * 4 + 2], o[g * 4 + 3]);
     if (do_mirror) {
-      // transposed tile: T[c][lane] = element (row lane, column c)
-      const uint32_t tbase = stage + kEpiTileBytes + ((lane & 7) << 1);
+      // transposed tile T[c][r] from the direct tile, 8 x 8 blocks at a time: ldmatrix.trans reads block (rb, cb) of the
+      // direct tile transposed into the fragment layout, stmatrix writes it as block (cb, rb) of T (4 + 4 instructions
+      // per chunk; element-wise it took 32 two-byte shared stores per lane)
+      __syncwarp();
 #pragma unroll
-      for (int e = 0; e < 16; ++e) {
-        const int c0 = 2 * e, c1 = 2 * e + 1;
-        st_shared_u16(tbase + c0 * 64 + (((lane >> 3) ^ ((c0 >> 1) & 3)) << 4), o[e] & 0xFFFFu);
-        st_shared_u16(tbase + c1 * 64 + (((lane >> 3) ^ ((c1 >> 1) & 3)) << 4), o[e] >> 16);
+      for (int cb = 0; cb < 4; ++cb) {
+        uint32_t f0, f1, f2, f3;
+        ldmatrix_x4_trans(stage + lane * 64 + ((cb ^ ((lane >> 1) & 3)) << 4), f0, f1, f2, f3);
+        const int trow = 8 * cb + (lane & 7);
+        stmatrix_x4(stage + kEpiTileBytes + trow * 64 + (((lane >> 3) ^ ((trow >> 1) & 3)) << 4), f0, f1, f2, f3);
       }
     }
     __syncwarp();
@@ -285,7 +291,7 @@ __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ pro
     }
     for (int s = 0; s < 2; ++s) {
       mbar_init(bar_tfull + 8 * s, 1);
-      mbar_init(bar_tempty + 8 * s, kPair ? 8 : 4);              // one arrival per epilogue warp (of both CTAs)
+      mbar_init(bar_tempty + 8 * s, kPair ? 2 * kEpiWarps : kEpiWarps);   // one arrival per epilogue warp (of both CTAs)
     }
     fence_barrier_init();
   }
@@ -395,10 +401,13 @@ __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ pro
     }
     __syncwarp();
   } else {
-    // ================================================================== epilogue (4 warps, one TMEM lane quarter each)
+    // ================================================================== epilogue (kEpiWarps warps: TMEM lane quarter warp % 4;
+    // with 8 warps the two of a quarter take alternate 32-column chunks)
     const int q = warp & 3;
+    const int half = (warp - 2) >> 2;
+    constexpr int kStep = kEpiWarps / 4;                                          // chunks between two of this warp's
     const int row = q * 32 + lane;
-    const uint32_t epi_stage = ctl_addr + 256 + q * (2 * kEpiTileBytes);      // this warp's two store tiles
+    const uint32_t epi_stage = ctl_addr + 256 + (warp - 2) * (2 * kEpiTileBytes);      // this warp's two store tiles
     const uint32_t tempty_leader = kPair ? mapa(bar_tempty, 0) : bar_tempty;
     int it = 0;
     for (int u = worker; u < total_units; u += num_workers, ++it) {
@@ -434,21 +443,23 @@ __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ pro
         c_hi = (nb - bj0 < nbk ? nb - bj0 : nbk) * 4;
       }
       Addends a0 = {}, a1 = {};
-      if (c_lo < c_hi) load_addends<kOp, kEpi>(a0, x, grow, gcol0 + c_lo * 32);   // before the accumulator is ready
+      const int c0 = c_lo + half;                                                   // this warp's chunks: c0, c0 + kStep, ...
+      if (c0 < c_hi) load_addends<kOp, kEpi>(a0, x, grow, gcol0 + c0 * 32);         // before the accumulator is ready
       mbar_wait_warp(bar_tfull + 8 * as, aphase, DMUON_EPI_SLEEP_NS);
       tcgen05_fence_after();
       const uint32_t taddr = tmem_base + as * kAccCols + (static_cast<uint32_t>(q * 32) << 16);
-      for (int c = c_lo; c < c_hi; c += 2) {
+      for (int c = c0; c < c_hi; c += 2 * kStep) {
         uint32_t v[32];
-        if (c + 1 < c_hi) load_addends<kOp, kEpi>(a1, x, grow, gcol0 + (c + 1) * 32);
+        const int cn = c + kStep;
+        if (cn < c_hi) load_addends<kOp, kEpi>(a1, x, grow, gcol0 + cn * 32);
         tmem_ld_32x32(taddr + c * 32, v);
         tmem_wait_ld();
         epilogue_chunk<kOp, kEpi>(v, a0, x, grow, gcol0 + c * 32, sc, bj0 + (c >> 2) != bi, epi_stage);
-        if (c + 1 < c_hi) {
-          if (c + 2 < c_hi) load_addends<kOp, kEpi>(a0, x, grow, gcol0 + (c + 2) * 32);
-          tmem_ld_32x32(taddr + (c + 1) * 32, v);
+        if (cn < c_hi) {
+          if (cn + kStep < c_hi) load_addends<kOp, kEpi>(a0, x, grow, gcol0 + (cn + kStep) * 32);
+          tmem_ld_32x32(taddr + cn * 32, v);
           tmem_wait_ld();
-          epilogue_chunk<kOp, kEpi>(v, a1, x, grow, gcol0 + (c + 1) * 32, sc, bj0 + ((c + 1) >> 2) != bi, epi_stage);
+          epilogue_chunk<kOp, kEpi>(v, a1, x, grow, gcol0 + cn * 32, sc, bj0 + (cn >> 2) != bi, epi_stage);
         }
       }
       // accumulator fully read by this warp: hand it back to the MMA thread

@@ -152,6 +152,25 @@ def test_xb(m, n, count, variant):
         assert _rel(c, ref) < 1e-3
 
 
+@pytest.mark.parametrize("variant", [0, 4])
+def test_sq_small_m_many_problems(variant):
+    """64 problems of m = 1024 (config 4's k/v bucket): short contractions, where the epilogue sets the pace.  Also the
+    target of the small-m ncu capture in profiles/."""
+    m, count = 1024, 64
+    A = []
+    for i in range(count):
+        x = _rand((m, 256), 200 + i, 256 ** -0.5)
+        a = (x.float() @ x.float().t()).to(torch.float16)
+        A.append(torch.triu(a) + torch.triu(a, 1).t())
+    C = [torch.empty((m, m), device="cuda", dtype=torch.float16) for _ in range(count)]
+    for _ in range(3):
+        dm.ns_gemm(OP_SQ, A, None, C, alpha=2.0315, beta=-4.775, variant=variant)
+    torch.cuda.synchronize()
+    for i in (0, 31, 63):
+        ref = 2.0315 * (A[i].float() @ A[i].float()) - 4.775 * A[i].float()
+        assert _rel(C[i], ref) < 1e-3 and torch.equal(C[i], C[i].t())
+
+
 def test_variant_table():
     assert dm.binding.ns_gemm_variants(OP_BX) == 6
     x = _rand((128, 128), 1, 1.0)
