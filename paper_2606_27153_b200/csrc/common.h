@@ -59,14 +59,16 @@ constexpr int kNumEpi = 4;
 struct alignas(128) GemmProblem {
   CUtensorMap tmA;      // operand A: K-major box {64 (k), 128 (rows)}; MN-major (SYRK_T) box {64 (m), 64 (k)}
   CUtensorMap tmB;      // operand B: K-major box {64, 128}; MN-major (BX, SYRK_T) box {64 (n), 64 (k)}
-  const __half* D;      // addend matrix (SQ: A, BX / XB: X), same leading dimension as C; null for SYRK
-  __half* C;            // output (fused epilogues write it only when the launch says store_c)
-  const __half* D2;     // second addend (SQ2 only)
-  int32_t ldc;          // leading dimension of C, D and D2, in elements
+  CUtensorMap tmC;      // output C (fused epilogues write it only when the launch says store_c): box {32 (cols), 32 (rows)},
+                        // 64-byte swizzle -- the epilogue warps' staging tiles; the mirrored tile of a symmetric result
+                        // goes out through the same map at the transposed coordinates
+  CUtensorMap tmD;      // addend D (SQ: A, BX / XB: X), same shape and boxes as C; unused for SYRK
+  CUtensorMap tmD2;     // second addend (SQ2 only)
+  int32_t ldc;          // leading dimension of C (and of W / W32 in the fused epilogues), in elements
   int32_t rec;          // index of the matrix's MatRec (fused epilogues read W / W32 / scale there)
-  int32_t pad_[24];
+  int32_t pad_[30];
 };
-static_assert(sizeof(GemmProblem) == 384, "GemmProblem layout");
+static_assert(sizeof(GemmProblem) == 768, "GemmProblem layout");
 
 // One work unit of a problem.  Single-CTA tiling: block row, first block column, number of blocks (1 or 2), in
 // 128-blocks.  CTA-pair tiling: m_blk, n_blk index 256 x 256 units (width unused).

@@ -40,8 +40,7 @@ namespace {
 using namespace umma;
 
 constexpr int kBlockBytes = kBlk * kBlkK * 2;   // 16 KB: 128 rows x 128 B of one operand block
-constexpr int kEpiWarps = 4;                    // 4: one per TMEM lane quarter; 8: two per quarter taking alternate 32-column
-                                                // chunks (measured: no gain on short contractions, -2 % on config 4)
+constexpr int kEpiWarps = 4;                    // one per TMEM lane quarter
 constexpr int kNumThreads = 64 + 32 * kEpiWarps;
 constexpr int kTmemCols = 512;
 constexpr int kAccCols = 256;                   // columns per accumulator stage
@@ -50,13 +49,22 @@ constexpr int kMaxStages = 6;
 #define DMUON_EPI_SLEEP_NS 256                  // back-off of the epilogue warps' accumulator wait (0 = plain polling)
 #endif
 
+// Epilogue staging, per epilogue warp: tiles of 32 rows x 32 fp16 (64-byte rows, 16-byte chunks XOR-swizzled by
+// (row >> 1) & 3 = CU_TENSOR_MAP_SWIZZLE_64B, conflict-free for row-wise 16-byte accesses and for ldmatrix / stmatrix).
+//   2 output tiles + 2 mirrored tiles (double-buffered: a tile is rewritten two chunks after its bulk store was issued)
+//   4 addend tiles: a ring the warp's elected lane fills by TMA three chunks ahead (two-addend products: two pairs)
+constexpr int kEpiTileBytes = 32 * 64;
+constexpr int kEpiAddTiles = 4;
+constexpr int kEpiWarpBytes = (4 + kEpiAddTiles) * kEpiTileBytes;     // 16 KB
+constexpr int kEpiBytes = kEpiWarps * kEpiWarpBytes;                  // 64 KB
+
 template <bool kPair> struct Tiling;
 template <> struct Tiling<false> {              // one CTA: A block + up to two B blocks per stage
-  static constexpr int kStages = 4;
+  static constexpr int kStages = 3;
   static constexpr int kStageBytes = 3 * kBlockBytes;
 };
 template <> struct Tiling<true> {               // CTA pair: this CTA's A block + its B block per stage
-  static constexpr int kStages = 6;
+  static constexpr int kStages = 5;
   static constexpr int kStageBytes = 2 * kBlockBytes;
 };
 
@@ -65,15 +73,16 @@ struct SmemCtl {
   uint64_t empty[kMaxStages];
   uint64_t tmem_full[2];
   uint64_t tmem_empty[2];
+  uint64_t addend[kEpiWarps][kEpiAddTiles];     // "addend tile(s) of ring slot s have landed", per epilogue warp
   uint32_t tmem_base;
   uint32_t pad;
 };
-static_assert(sizeof(SmemCtl) <= 256, "SmemCtl");
-constexpr int kEpiTileBytes = 32 * 64;         // 32 rows x 32 fp16: one warp's 32-column chunk, or its transpose
-constexpr int kEpiStageBytes = kEpiWarps * 2 * kEpiTileBytes;   // per epilogue warp: a direct and a mirrored tile
+constexpr int kCtlBytes = 512;
+static_assert(sizeof(SmemCtl) <= kCtlBytes, "SmemCtl");
 template <bool kPair> constexpr int smem_bytes() {
-  return Tiling<kPair>::kStages * Tiling<kPair>::kStageBytes + 1024 /*alignment slack*/ + 256 /*SmemCtl*/ + kEpiStageBytes;
+  return Tiling<kPair>::kStages * Tiling<kPair>::kStageBytes + kEpiBytes + kCtlBytes + 1024 /*alignment slack*/;
 }
+static_assert(smem_bytes<true>() <= 232448 && smem_bytes<false>() <= 232448, "shared memory budget");
 
 struct Scalars {
   float alpha, beta, beta2;
@@ -86,64 +95,90 @@ __host__ __device__ constexpr bool op_symmetric(int op) { return op == OP_SYRK |
 __host__ __device__ constexpr bool op_a_mn(int op) { return op == OP_SYRK_T; }
 __host__ __device__ constexpr bool op_b_mn(int op) { return op == OP_BX || op == OP_SYRK_T; }
 __host__ __device__ constexpr bool op_has_addend(int op) { return op != OP_SYRK && op != OP_SYRK_T; }
+__host__ __device__ constexpr int op_addends(int op) { return op == OP_SQ2 ? 2 : (op_has_addend(op) ? 1 : 0); }
+// addend ring: entries in flight per warp (each entry = the addend tile(s) of one 32-column chunk)
+__host__ __device__ constexpr int op_ring(int op) { return op == OP_SQ2 ? kEpiAddTiles / 2 : kEpiAddTiles; }
 
 // ------------------------------------------------------------------------------------------------ epilogue
-// Addend words of one 32-column chunk of one row: 64 bytes of D (and of D2 for OP_SQ2, of the bf16 W for EPI_APPLY).
-// Loaded one chunk ahead of the arithmetic (two register sets, alternating) so that their L2 latency overlaps the
-// TMEM load and the stores of the previous chunk: with short contractions (K <= 1024) the epilogue, not the mainloop,
-// sets the pace.
-struct Addends {
-  uint4 d[4];
-  uint4 e[4];
-};
+// All fp16 traffic of the epilogue moves by TMA: the addend tiles come in through a per-warp ring (issued three chunks
+// ahead, so their L2 latency is off the critical path), the result tile and, for symmetric results, its transpose go
+// out as bulk tensor stores from shared memory.  What is left for the LSU per chunk and warp is 4 swizzled 16-byte
+// shared stores, the 4 + 4 ldmatrix.trans / stmatrix of a mirrored tile and 4 shared loads per addend: with short
+// contractions (K <= 1024) the epilogue, not the mainloop, sets the pace, and the LSU (shared-memory crossbar and
+// global store path, one per SM) was what bounded it when the tiles went out as st.global (profiles/r2_experiments.md).
+// Only the bf16 weights of the fused update (and fp32 masters) still take the register path: ld.global.nc / st.global.
+
 // Per-unit epilogue context (pointers of the unit's problem).
 struct EpiCtx {
-  __half* C;
-  const __half* D;
-  const __half* D2;
+  uint64_t tmC, tmD, tmD2;   // tensor maps (generic addresses of the CUtensorMap objects in the problem table)
   uint16_t* W;        // bf16 parameter / output (fused epilogues)
   float* W32;         // fp32 master (EPI_APPLY_MASTER)
-  int64_t ldc;
+  int64_t ldw;        // leading dimension of W / W32 (= of C)
   float so;           // EPI_APPLY*: lr * scale / c ; EPI_BF16: 1 / c
 };
-
-template <int kOp, int kEpi>
-__device__ __forceinline__ void load_addends(Addends& a, const EpiCtx& x, int64_t grow, int64_t gcol) {
-  if (op_has_addend(kOp)) {
-    const uint4* dp = reinterpret_cast<const uint4*>(x.D + grow * x.ldc + gcol);
-#pragma unroll
-    for (int g = 0; g < 4; ++g) a.d[g] = __ldg(dp + g);
-  }
-  if (kOp == OP_SQ2) {
-    const uint4* ep = reinterpret_cast<const uint4*>(x.D2 + grow * x.ldc + gcol);
-#pragma unroll
-    for (int g = 0; g < 4; ++g) a.e[g] = __ldg(ep + g);
-  }
-  if (kEpi == EPI_APPLY) {
-    // W comes from DRAM.  Through L1 (ld.global.nc): a lane reads its row's 64 bytes as four 16-byte loads, the first
-    // brings the sectors in and the other three hit.  A streaming load (ld.global.cs, evict-first) sent all four to
-    // L2/DRAM and halved the throughput of the whole fused X update (profiles/r2_experiments.md).
-    const uint4* wp = reinterpret_cast<const uint4*>(x.W + grow * x.ldc + gcol);
-#pragma unroll
-    for (int g = 0; g < 4; ++g) a.e[g] = __ldg(wp + g);
-  }
-}
+// Per-warp staging state; counters run over the whole kernel.
+struct EpiPipe {
+  uint32_t obuf;      // 2 output tiles, then 2 mirrored tiles, then the addend ring
+  uint32_t abar;      // this warp's addend barriers
+  uint32_t issued;    // addend ring entries requested so far
+  uint32_t consumed;  // ... and read so far
+  uint32_t nout;      // chunks stored so far (output tile toggle)
+};
 
 __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
   const __nv_bfloat162 b = __floats2bfloat162_rn(lo, hi);
   return *reinterpret_cast<const uint32_t*>(&b);
 }
 
+// Lane 0: request the addend tile(s) of rows [wrow0, wrow0 + 32), columns [gcol, gcol + 32) into the next ring entry.
+template <int kOp>
+__device__ __forceinline__ void addend_issue(EpiPipe& ep, const EpiCtx& x, int gcol, int wrow0) {
+  constexpr int kRing = op_ring(kOp);
+  constexpr int kTiles = op_addends(kOp);
+  const uint32_t s = ep.issued % kRing;
+  const uint32_t bar = ep.abar + 8 * s;
+  const uint32_t dst = ep.obuf + 4 * kEpiTileBytes + s * kTiles * kEpiTileBytes;
+  mbar_expect_tx(bar, kTiles * kEpiTileBytes);
+  tma_load_2d(dst, x.tmD, gcol, wrow0, bar);
+  if (kOp == OP_SQ2) tma_load_2d(dst + kEpiTileBytes, x.tmD2, gcol, wrow0, bar);
+  ++ep.issued;
+}
+
+// W words of one 32-column chunk of one row (EPI_APPLY), loaded one chunk ahead.  Through L1 (ld.global.nc): a lane
+// reads its row's 64 bytes as four 16-byte loads, the first brings the sectors in and the other three hit; a streaming
+// load (ld.global.cs) sent all four to L2/DRAM and halved the throughput of the fused X update.
+struct WWords { uint4 w[4]; };
+template <int kEpi>
+__device__ __forceinline__ void load_w(WWords& a, const EpiCtx& x, int64_t grow, int64_t gcol) {
+  if (kEpi == EPI_APPLY) {
+    const uint4* wp = reinterpret_cast<const uint4*>(x.W + grow * x.ldw + gcol);
+#pragma unroll
+    for (int g = 0; g < 4; ++g) a.w[g] = __ldg(wp + g);
+  }
+}
+
 // One 32-column chunk of one accumulator row: v = 32 fp32 accumulators of row `grow`, columns [gcol, gcol + 32).
 template <int kOp, int kEpi>
-__device__ __forceinline__ void epilogue_chunk(const uint32_t (&v)[32], const Addends& a, const EpiCtx& x,
-                                               int64_t grow, int64_t gcol, const Scalars& sc, bool mirror, uint32_t stage) {
+__device__ __forceinline__ void epilogue_chunk(const uint32_t (&v)[32], const WWords& ww, const EpiCtx& x, EpiPipe& ep,
+                                               int64_t grow, int64_t gcol, const Scalars& sc, bool mirror) {
+  const int lane = threadIdx.x & 31;
+  const int sw = (lane >> 1) & 3;                        // swizzle term of this lane's row
   float r[32];
   if (op_has_addend(kOp)) {
+    constexpr int kRing = op_ring(kOp);
+    constexpr int kTiles = op_addends(kOp);
+    const uint32_t s = ep.consumed % kRing;
+    mbar_wait(ep.abar + 8 * s, (ep.consumed / kRing) & 1);
+    const uint32_t src = ep.obuf + 4 * kEpiTileBytes + s * kTiles * kEpiTileBytes + lane * 64;
 #pragma unroll
     for (int g = 0; g < 4; ++g) {
-      const uint32_t dw[4] = {a.d[g].x, a.d[g].y, a.d[g].z, a.d[g].w};
-      const uint32_t ew[4] = {a.e[g].x, a.e[g].y, a.e[g].z, a.e[g].w};
+      const uint4 d = ld_shared_v4(src + ((g ^ sw) << 4));
+      const uint32_t dw[4] = {d.x, d.y, d.z, d.w};
+      uint32_t ew[4] = {0u, 0u, 0u, 0u};
+      if (kOp == OP_SQ2) {
+        const uint4 e = ld_shared_v4(src + kEpiTileBytes + ((g ^ sw) << 4));
+        ew[0] = e.x; ew[1] = e.y; ew[2] = e.z; ew[3] = e.w;
+      }
 #pragma unroll
       for (int e = 0; e < 4; ++e) {
         const float2 df = __half22float2(*reinterpret_cast<const __half2*>(&dw[e]));
@@ -157,62 +192,54 @@ __device__ __forceinline__ void epilogue_chunk(const uint32_t (&v)[32], const Ad
         r[g * 8 + e * 2 + 1] = fmaf(sc.alpha, __uint_as_float(v[g * 8 + e * 2 + 1]), ay);
       }
     }
+    ++ep.consumed;
+    __syncwarp();                                        // every lane has read the ring slot before lane 0 refills it
   } else {
 #pragma unroll
     for (int e = 0; e < 32; ++e) r[e] = sc.alpha * __uint_as_float(v[e]);
   }
   if (kEpi == EPI_F16 || sc.store_c) {
-    // fp16 store of the chunk (32 rows x 32 columns per warp) and, for symmetric results, of its mirror image.  Both go
-    // through a warp-private shared-memory tile so that every global store instruction writes whole 64-byte row segments
-    // (8 rows x 64 B per instruction): one lane per row would write 32 half-sectors per instruction, and the mirror
-    // would take 32 two-byte global stores per lane.  Tile: 32 rows x 64 B, 16-byte chunks XOR-swizzled by (row >> 1) & 3
-    // (conflict-free for the row-wise 16-byte stores, for ldmatrix / stmatrix and for the 8-rows-per-instruction reads).
+    // fp16 store of the chunk (32 rows x 32 columns per warp) and, for symmetric results, of its mirror image: staged in
+    // this warp's shared-memory tiles, sent as bulk tensor stores by lane 0
     uint32_t o[16];
 #pragma unroll
     for (int e = 0; e < 16; ++e) o[e] = pack_half2(r[2 * e], r[2 * e + 1]);
-    const int lane = threadIdx.x & 31;
     const bool do_mirror = op_symmetric(kOp) && mirror;
-    __syncwarp();                                        // the previous chunk's tiles have been read out
+    const uint32_t ot = ep.obuf + (ep.nout & 1) * kEpiTileBytes;
+    const uint32_t mt = ot + 2 * kEpiTileBytes;
+    // the bulk stores issued from these two tiles two chunks ago have read them (one group per chunk)
+    if (lane == 0) bulk_wait_read<1>();
+    __syncwarp();
 #pragma unroll
-    for (int g = 0; g < 4; ++g)
-      st_shared_v4(stage + lane * 64 + ((g ^ ((lane >> 1) & 3)) << 4), o[g * 4], o[g * 4 + 1], o[g * 4 + 2], o[g * 4 + 3]);
+    for (int g = 0; g < 4; ++g) st_shared_v4(ot + lane * 64 + ((g ^ sw) << 4), o[g * 4], o[g * 4 + 1], o[g * 4 + 2], o[g * 4 + 3]);
     if (do_mirror) {
       // transposed tile T[c][r] from the direct tile, 8 x 8 blocks at a time: ldmatrix.trans reads block (rb, cb) of the
-      // direct tile transposed into the fragment layout, stmatrix writes it as block (cb, rb) of T (4 + 4 instructions
-      // per chunk; element-wise it took 32 two-byte shared stores per lane)
+      // direct tile transposed into the fragment layout, stmatrix writes it as block (cb, rb) of T
       __syncwarp();
 #pragma unroll
       for (int cb = 0; cb < 4; ++cb) {
         uint32_t f0, f1, f2, f3;
-        ldmatrix_x4_trans(stage + lane * 64 + ((cb ^ ((lane >> 1) & 3)) << 4), f0, f1, f2, f3);
+        ldmatrix_x4_trans(ot + lane * 64 + ((cb ^ sw) << 4), f0, f1, f2, f3);
         const int trow = 8 * cb + (lane & 7);
-        stmatrix_x4(stage + kEpiTileBytes + trow * 64 + (((lane >> 3) ^ ((trow >> 1) & 3)) << 4), f0, f1, f2, f3);
+        stmatrix_x4(mt + trow * 64 + (((lane >> 3) ^ ((trow >> 1) & 3)) << 4), f0, f1, f2, f3);
       }
     }
+    fence_proxy_async();                                 // generic-proxy writes -> visible to the bulk (async-proxy) store
     __syncwarp();
-    const int64_t wrow0 = grow - lane;                   // first row of this warp's 32 rows
-    const int ch = lane & 3;
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-      const int rr = (lane >> 2) + 8 * i;
-      const uint4 v = ld_shared_v4(stage + rr * 64 + ((ch ^ ((rr >> 1) & 3)) << 4));
-      *reinterpret_cast<uint4*>(x.C + (wrow0 + rr) * x.ldc + gcol + ch * 8) = v;
+    if (lane == 0) {
+      const int wrow0 = static_cast<int>(grow);          // lane 0 holds the warp's first row
+      tma_store_2d(x.tmC, ot, static_cast<int>(gcol), wrow0);
+      if (do_mirror) tma_store_2d(x.tmC, mt, wrow0, static_cast<int>(gcol));
+      bulk_commit();
     }
-    if (do_mirror) {
-#pragma unroll
-      for (int i = 0; i < 4; ++i) {
-        const int cc = (lane >> 2) + 8 * i;              // a column of the chunk = a row of the mirrored block
-        const uint4 v = ld_shared_v4(stage + kEpiTileBytes + cc * 64 + ((ch ^ ((cc >> 1) & 3)) << 4));
-        *reinterpret_cast<uint4*>(x.C + (gcol + cc) * x.ldc + wrow0 + ch * 8) = v;
-      }
-    }
+    ++ep.nout;
   }
   if (kEpi == EPI_BF16) {
     // NS output of dmuon_ns_batched: out = bf16(x / c), c a power of two
     uint32_t o[16];
 #pragma unroll
     for (int e = 0; e < 16; ++e) o[e] = pack_bf16x2(r[2 * e] * x.so, r[2 * e + 1] * x.so);
-    uint4* wp = reinterpret_cast<uint4*>(x.W + grow * x.ldc + gcol);
+    uint4* wp = reinterpret_cast<uint4*>(x.W + grow * x.ldw + gcol);
 #pragma unroll
     for (int g = 0; g < 4; ++g) wp[g] = make_uint4(o[g * 4], o[g * 4 + 1], o[g * 4 + 2], o[g * 4 + 3]);
   } else if (kEpi == EPI_APPLY) {
@@ -220,21 +247,21 @@ __device__ __forceinline__ void epilogue_chunk(const uint32_t (&v)[32], const Ad
     uint32_t o[16];
 #pragma unroll
     for (int g = 0; g < 4; ++g) {
-      const uint32_t ww[4] = {a.e[g].x, a.e[g].y, a.e[g].z, a.e[g].w};
+      const uint32_t wd[4] = {ww.w[g].x, ww.w[g].y, ww.w[g].z, ww.w[g].w};
 #pragma unroll
       for (int e = 0; e < 4; ++e) {
-        const float w0 = __uint_as_float(ww[e] << 16), w1 = __uint_as_float(ww[e] & 0xFFFF0000u);
+        const float w0 = __uint_as_float(wd[e] << 16), w1 = __uint_as_float(wd[e] & 0xFFFF0000u);
         const float t0 = fmaf(x.so, r[g * 8 + e * 2], sc.lrwd * w0);
         const float t1 = fmaf(x.so, r[g * 8 + e * 2 + 1], sc.lrwd * w1);
         o[g * 4 + e] = pack_bf16x2(w0 - t0, w1 - t1);
       }
     }
-    uint4* wp = reinterpret_cast<uint4*>(x.W + grow * x.ldc + gcol);
+    uint4* wp = reinterpret_cast<uint4*>(x.W + grow * x.ldw + gcol);
 #pragma unroll
     for (int g = 0; g < 4; ++g) wp[g] = make_uint4(o[g * 4], o[g * 4 + 1], o[g * 4 + 2], o[g * 4 + 3]);
   } else if (kEpi == EPI_APPLY_MASTER) {
     // fp32 master weights: the update lands in the master, the bf16 parameter is its rounding
-    float4* mp = reinterpret_cast<float4*>(x.W32 + grow * x.ldc + gcol);
+    float4* mp = reinterpret_cast<float4*>(x.W32 + grow * x.ldw + gcol);
     uint32_t o[16];
 #pragma unroll
     for (int g = 0; g < 8; ++g) {
@@ -248,7 +275,7 @@ __device__ __forceinline__ void epilogue_chunk(const uint32_t (&v)[32], const Ad
       o[g * 2] = pack_bf16x2(n.x, n.y);
       o[g * 2 + 1] = pack_bf16x2(n.z, n.w);
     }
-    uint4* wp = reinterpret_cast<uint4*>(x.W + grow * x.ldc + gcol);
+    uint4* wp = reinterpret_cast<uint4*>(x.W + grow * x.ldw + gcol);
 #pragma unroll
     for (int g = 0; g < 4; ++g) wp[g] = make_uint4(o[g * 4], o[g * 4 + 1], o[g * 4 + 2], o[g * 4 + 3]);
   }
@@ -271,8 +298,10 @@ __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ pro
   extern __shared__ uint8_t smem_raw[];
   const uint32_t raw = smem_u32(smem_raw);
   const uint32_t base = (raw + 1023u) & ~1023u;    // swizzle-128B atoms need 1024-byte alignment
-  SmemCtl* ctl = reinterpret_cast<SmemCtl*>(smem_raw + (base - raw) + kStages * kStageBytes);
-  const uint32_t ctl_addr = base + kStages * kStageBytes;
+  // [operand ring | epilogue tiles (2 KB each, 1024-byte aligned) | barriers]
+  const uint32_t epi_addr = base + kStages * kStageBytes;
+  const uint32_t ctl_addr = epi_addr + kEpiBytes;
+  SmemCtl* ctl = reinterpret_cast<SmemCtl*>(smem_raw + (ctl_addr - raw));
   const uint32_t bar_full = ctl_addr + offsetof(SmemCtl, full);
   const uint32_t bar_empty = ctl_addr + offsetof(SmemCtl, empty);
   const uint32_t bar_tfull = ctl_addr + offsetof(SmemCtl, tmem_full);
@@ -293,6 +322,7 @@ __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ pro
       mbar_init(bar_tfull + 8 * s, 1);
       mbar_init(bar_tempty + 8 * s, kPair ? 2 * kEpiWarps : kEpiWarps);   // one arrival per epilogue warp (of both CTAs)
     }
+    for (int s = 0; s < kEpiWarps * kEpiAddTiles; ++s) mbar_init(ctl_addr + offsetof(SmemCtl, addend) + 8 * s, 1);
     fence_barrier_init();
   }
   if (warp == 1) tmem_alloc<kCG>(ctl_addr + offsetof(SmemCtl, tmem_base), kTmemCols);
@@ -401,13 +431,14 @@ __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ pro
     }
     __syncwarp();
   } else {
-    // ================================================================== epilogue (kEpiWarps warps: TMEM lane quarter warp % 4;
-    // with 8 warps the two of a quarter take alternate 32-column chunks)
+    // ================================================================== epilogue (4 warps: TMEM lane quarter warp % 4)
     const int q = warp & 3;
-    const int half = (warp - 2) >> 2;
-    constexpr int kStep = kEpiWarps / 4;                                          // chunks between two of this warp's
     const int row = q * 32 + lane;
-    const uint32_t epi_stage = ctl_addr + 256 + (warp - 2) * (2 * kEpiTileBytes);      // this warp's two store tiles
+    constexpr int kRing = op_ring(kOp);
+    EpiPipe ep;
+    ep.obuf = epi_addr + (warp - 2) * kEpiWarpBytes;
+    ep.abar = ctl_addr + offsetof(SmemCtl, addend) + (warp - 2) * (8 * kEpiAddTiles);
+    ep.issued = ep.consumed = ep.nout = 0;
     const uint32_t tempty_leader = kPair ? mapa(bar_tempty, 0) : bar_tempty;
     int it = 0;
     for (int u = worker; u < total_units; u += num_workers, ++it) {
@@ -415,10 +446,10 @@ __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ pro
       const TileUnit tu = units[u - p * units_per_problem];
       const GemmProblem* pr = probs + p;
       EpiCtx x;
-      x.C = pr->C;
-      x.D = pr->D;
-      x.D2 = pr->D2;
-      x.ldc = pr->ldc;
+      x.tmC = reinterpret_cast<uint64_t>(&pr->tmC);
+      x.tmD = reinterpret_cast<uint64_t>(&pr->tmD);
+      x.tmD2 = reinterpret_cast<uint64_t>(&pr->tmD2);
+      x.ldw = pr->ldc;
       x.W = nullptr;
       x.W32 = nullptr;
       x.so = 0.f;
@@ -434,7 +465,8 @@ __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ pro
       const int bj0 = kPair ? 2 * tu.n_blk : tu.n_blk;                               // first column block
       const int nbk = kPair ? 2 : tu.width;
       const int64_t grow = static_cast<int64_t>(bi) * kBlk + row;
-      const int64_t gcol0 = static_cast<int64_t>(bj0) * kBlk;
+      const int wrow0 = bi * kBlk + q * 32;                                          // first row of this warp
+      const int gcol0 = bj0 * kBlk;
       // chunks (32 columns each) this warp stores: inside the matrix and, for symmetric results, not left of the
       // diagonal block (those blocks are written by the mirror of another unit)
       int c_lo = 0, c_hi = 0;
@@ -442,24 +474,29 @@ __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ pro
         c_lo = (kSym && bi > bj0) ? (bi - bj0) * 4 : 0;
         c_hi = (nb - bj0 < nbk ? nb - bj0 : nbk) * 4;
       }
-      Addends a0 = {}, a1 = {};
-      const int c0 = c_lo + half;                                                   // this warp's chunks: c0, c0 + kStep, ...
-      if (c0 < c_hi) load_addends<kOp, kEpi>(a0, x, grow, gcol0 + c0 * 32);         // before the accumulator is ready
+      // addend tiles of the first chunks and the first W words: requested before the accumulator is ready
+      if (op_has_addend(kOp) && lane == 0) {
+        for (int c = c_lo; c < c_hi && c < c_lo + kRing - 1; ++c) addend_issue<kOp>(ep, x, gcol0 + c * 32, wrow0);
+      }
+      WWords w0 = {}, w1 = {};
+      if (c_lo < c_hi) load_w<kEpi>(w0, x, grow, gcol0 + c_lo * 32);
       mbar_wait_warp(bar_tfull + 8 * as, aphase, DMUON_EPI_SLEEP_NS);
       tcgen05_fence_after();
       const uint32_t taddr = tmem_base + as * kAccCols + (static_cast<uint32_t>(q * 32) << 16);
-      for (int c = c0; c < c_hi; c += 2 * kStep) {
+      for (int c = c_lo; c < c_hi; c += 2) {
         uint32_t v[32];
-        const int cn = c + kStep;
-        if (cn < c_hi) load_addends<kOp, kEpi>(a1, x, grow, gcol0 + cn * 32);
+        const int cn = c + 1;
+        if (op_has_addend(kOp) && lane == 0 && c + kRing - 1 < c_hi) addend_issue<kOp>(ep, x, gcol0 + (c + kRing - 1) * 32, wrow0);
+        if (cn < c_hi) load_w<kEpi>(w1, x, grow, gcol0 + cn * 32);
         tmem_ld_32x32(taddr + c * 32, v);
         tmem_wait_ld();
-        epilogue_chunk<kOp, kEpi>(v, a0, x, grow, gcol0 + c * 32, sc, bj0 + (c >> 2) != bi, epi_stage);
+        epilogue_chunk<kOp, kEpi>(v, w0, x, ep, grow, gcol0 + c * 32, sc, bj0 + (c >> 2) != bi);
         if (cn < c_hi) {
-          if (cn + kStep < c_hi) load_addends<kOp, kEpi>(a0, x, grow, gcol0 + (cn + kStep) * 32);
+          if (op_has_addend(kOp) && lane == 0 && cn + kRing - 1 < c_hi) addend_issue<kOp>(ep, x, gcol0 + (cn + kRing - 1) * 32, wrow0);
+          if (cn + 1 < c_hi) load_w<kEpi>(w0, x, grow, gcol0 + (cn + 1) * 32);
           tmem_ld_32x32(taddr + cn * 32, v);
           tmem_wait_ld();
-          epilogue_chunk<kOp, kEpi>(v, a1, x, grow, gcol0 + cn * 32, sc, bj0 + (cn >> 2) != bi, epi_stage);
+          epilogue_chunk<kOp, kEpi>(v, w1, x, ep, grow, gcol0 + cn * 32, sc, bj0 + (cn >> 2) != bi);
         }
       }
       // accumulator fully read by this warp: hand it back to the MMA thread
@@ -469,6 +506,9 @@ __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ pro
         if (kPair) mbar_arrive_cluster(tempty_leader + 8 * as); else mbar_arrive(bar_tempty + 8 * as);
       }
     }
+    // the bulk stores of this warp must have completed (not only read their tiles) before the CTA exits
+    if (lane == 0) bulk_wait_all();
+    __syncwarp();
   }
 
   tcgen05_fence_before();

@@ -389,9 +389,11 @@ int fill_problem(GemmProblem& g, GemmOp op, const void* a_mat, uint64_t a_rows, 
   if (op == OP_BX || op == OP_SYRK_T) rc = encode_tmap_2d(&g.tmB, b_mat, b_rows, b_cols, 64, kBlkK);   // MN-major: 64 (n) x 64 (k) boxes
   else rc = encode_tmap_2d(&g.tmB, b_mat, b_rows, b_cols, kBlkK, kBlk);
   if (rc) return rc;
-  g.D = static_cast<const __half*>(d);
-  g.C = static_cast<__half*>(c);
-  g.D2 = static_cast<const __half*>(d2);
+  // epilogue tiles: C, D, D2 share one shape (rows x ldc); 32 x 32 boxes with the 64-byte swizzle
+  const uint64_t c_rows = (op == OP_BX || op == OP_XB) ? a_rows : static_cast<uint64_t>(ldc);
+  if (c && (rc = encode_tmap_2d(&g.tmC, c, c_rows, ldc, 32, 32, CU_TENSOR_MAP_SWIZZLE_64B))) return rc;
+  if (d && (rc = encode_tmap_2d(&g.tmD, d, c_rows, ldc, 32, 32, CU_TENSOR_MAP_SWIZZLE_64B))) return rc;
+  if (d2 && (rc = encode_tmap_2d(&g.tmD2, d2, c_rows, ldc, 32, 32, CU_TENSOR_MAP_SWIZZLE_64B))) return rc;
   g.ldc = ldc;
   g.rec = rec;
   return DMUON_OK;
@@ -454,7 +456,7 @@ std::vector<TileUnit> make_units(GemmOp op, int mb, int nb, const TileConfig& cf
 }
 
 int encode_tmap_2d(CUtensorMap* out, const void* base, uint64_t rows, uint64_t cols, uint32_t box_cols,
-                   uint32_t box_rows) {
+                   uint32_t box_rows, CUtensorMapSwizzle swizzle) {
   int rc = load_encode();
   if (rc) return rc;
   const cuuint64_t gdim[2] = {cols, rows};
@@ -462,7 +464,7 @@ int encode_tmap_2d(CUtensorMap* out, const void* base, uint64_t rows, uint64_t c
   const cuuint32_t box[2] = {box_cols, box_rows};
   const cuuint32_t estr[2] = {1, 1};
   CUresult r = g_encode(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, const_cast<void*>(base), gdim, gstride, box, estr,
-                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, swizzle, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) {
     set_error("cuTensorMapEncodeTiled failed (%d) for %llu x %llu, box %u x %u, base %p", static_cast<int>(r),

@@ -179,7 +179,7 @@ std::string partition_key(const Partition& p);
 // Build tile units for an op.
 std::vector<TileUnit> make_units(GemmOp op, int m_blocks, int n_blocks, const TileConfig& cfg);
 int encode_tmap_2d(CUtensorMap* out, const void* base, uint64_t rows, uint64_t cols, uint32_t box_cols,
-                   uint32_t box_rows);
+                   uint32_t box_rows, CUtensorMapSwizzle swizzle = CU_TENSOR_MAP_SWIZZLE_128B);
 // A, B: operand matrices with their (rows, cols) as laid out in memory.
 int fill_problem(GemmProblem& g, GemmOp op, const void* a_mat, uint64_t a_rows, uint64_t a_cols, const void* b_mat,
                  uint64_t b_rows, uint64_t b_cols, const void* d, void* c, int ldc, const void* d2 = nullptr, int rec = 0);

@@ -104,6 +104,17 @@ __device__ __forceinline__ void tma_load_2d_pair(uint32_t smem_dst, uint64_t tma
       ::"r"(smem_dst), "l"(tmap), "r"(c0), "r"(c1), "r"(bar)
       : "memory");
 }
+// Bulk tensor store shared -> global (the epilogue's output tiles), tracked by the issuing thread's bulk async-groups.
+__device__ __forceinline__ void tma_store_2d(uint64_t tmap, uint32_t smem_src, int c0, int c1) {
+  asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.tile.bulk_group [%0, {%2, %3}], [%1];"
+               ::"l"(tmap), "r"(smem_src), "r"(c0), "r"(c1) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+// At most kPending of this thread's bulk groups may still be READING their shared-memory source.
+template <int kPending>
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(kPending) : "memory"); }
+// All bulk groups of this thread complete (writes performed).
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void tma_prefetch_desc(uint64_t tmap) {
   asm volatile("prefetch.tensormap [%0];" ::"l"(tmap) : "memory");
 }
