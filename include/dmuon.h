@@ -181,6 +181,9 @@ DMUON_API int dmuon_set_workspace(void* dev_ptr, size_t bytes);
  *   "fuse_epilogue" "1"/"0": for matrices whose rows and cols are multiples of 128, apply W' = W - lr (scale O + wd W)
  *                 (or write the bf16 NS output) in the epilogue of the last X update instead of a separate pass
  *                 (default "1").  Results agree to the rounding of the unfused path's fp16 O
+ *   "small_fused" "1"/"0": matrices whose padded oriented shape is 256 x 256 run ALL their NS steps in one on-chip
+ *                 kernel (X, G, B resident in the shared memory of a CTA pair; nothing stored between products), up to
+ *                 16 steps (default "1"; "0" = the grouped per-product launches, as for every other shape)
  *   "keep_ns_output" "1"/"0": keep every matrix's unrounded NS result readable after the call (dmuon_read_ns_output):
  *                 fused epilogues also store it and buckets get disjoint workspace regions (default "0")
  *   "chunk_mb"    workspace a bucket may use, MiB (default "12288"): a bucket whose matrices need more runs as

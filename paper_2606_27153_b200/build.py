@@ -14,8 +14,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libdmuon.so")
-SOURCES = ["api.cu", "planner.cu", "assign.cu", "elementwise.cu", "gemm_sm100.cu", "gemm_check.cu"]
-HEADERS = ["common.h", "planner.h", "umma.cuh", os.path.join("..", "..", "include", "dmuon.h")]
+SOURCES = ["api.cu", "planner.cu", "assign.cu", "elementwise.cu", "gemm_sm100.cu", "ns_small_sm100.cu", "gemm_check.cu"]
+HEADERS = ["common.h", "planner.h", "umma.cuh", "epilogue.cuh", os.path.join("..", "..", "include", "dmuon.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC,-fvisibility=hidden", "-diag-suppress", "177"]
 

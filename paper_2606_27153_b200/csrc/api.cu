@@ -376,6 +376,7 @@ DMUON_API int dmuon_set_option(const char* key, const char* value) {
   if (k == "autotune") { if (as_bool(&g_opt.autotune)) return DMUON_OK; set_error("option autotune: bad value '%s'", value); return DMUON_ERR_INVALID_ARG; }
   if (k == "profile") { if (as_bool(&g_opt.profile)) return DMUON_OK; set_error("option profile: bad value '%s'", value); return DMUON_ERR_INVALID_ARG; }
   if (k == "fuse_epilogue") { if (as_bool(&g_opt.fuse)) return DMUON_OK; set_error("option fuse_epilogue: bad value '%s'", value); return DMUON_ERR_INVALID_ARG; }
+  if (k == "small_fused") { if (as_bool(&g_opt.small_fused)) return DMUON_OK; set_error("option small_fused: bad value '%s'", value); return DMUON_ERR_INVALID_ARG; }
   if (k == "keep_ns_output") { if (as_bool(&g_opt.keep_o)) return DMUON_OK; set_error("option keep_ns_output: bad value '%s'", value); return DMUON_ERR_INVALID_ARG; }
   if (k == "schedule") {
     if (v == "auto") g_opt.gram_blocks = true;
@@ -673,8 +674,9 @@ DMUON_API int dmuon_describe_plan(const int32_t* shapes, int32_t count, int32_t 
                st.m_pad, st.n_pad, kKind[st.kind], static_cast<int>(bp.mats.size()));
       s += item;
       for (size_t k = 0; k < part.size(); ++k) s += (k ? ", " : "") + std::to_string(part[k]);
-      snprintf(item, sizeof item, "], \"variants\": [%d, %d, %d], \"fused\": %s, \"xscale\": %g, \"gscale\": %g}", st.variant[0],
-               st.variant[1], st.variant[2], bucket_fuses(*plan, st, steps, g_opt) ? "true" : "false", st.xscale, st.gscale);
+      snprintf(item, sizeof item, "], \"variants\": [%d, %d, %d], \"fused\": %s, \"onchip\": %s, \"xscale\": %g, \"gscale\": %g}", st.variant[0],
+               st.variant[1], st.variant[2], bucket_fuses(*plan, st, steps, g_opt) ? "true" : "false",
+               bucket_onchip(*plan, st, steps, g_opt) ? "true" : "false", st.xscale, st.gscale);
       s += item;
       first = false;
     }

@@ -98,6 +98,28 @@ struct GemmLaunch {
 int launch_ns_gemm(const GemmLaunch& L, cudaStream_t stream);
 int gemm_smem_bytes();
 
+// On-chip NS of small matrices (ns_small_sm100.cu): all k steps of every 256 x 256 (padded) matrix of a bucket in ONE
+// launch, X / G / B resident in the shared memory of a CTA pair (PAPER.md:170 Gram form, :180 batching by shape).
+constexpr int kSmallEdge = 256;        // m_pad = n_pad = 256
+constexpr int kSmallMaxSteps = 16;
+struct SmallLaunch {
+  const CUtensorMap* tmX;      // host copy of the 3-D map {256 cols, 256 rows, slots} over the bucket's X0 buffers
+  void* out;                   // fp16 X_k of slot s at out + s * slot_bytes (row stride 256); written for EPI_F16 or store_c
+  size_t slot_bytes;
+  const MatRec* recs = nullptr;
+  int rec_base = 0;
+  int count = 0;               // matrices (slots 0 .. count - 1)
+  int steps = 0;
+  float gram_alpha = 1.f;      // G~ = gram_alpha X~ X~^T
+  float poly_alpha[kSmallMaxSteps], poly_beta[kSmallMaxSteps];   // B = poly_beta G~ + poly_alpha G~ G~
+  float x_beta[kSmallMaxSteps];                                   // X~' = x_beta X~ + B X~
+  Epilogue epi = EPI_F16;      // what the last X update does (see Epilogue)
+  float lr = 0.f, lrwd = 0.f;
+  bool store_c = true;
+  int grid = 148;
+};
+int launch_ns_small(const SmallLaunch& L, cudaStream_t stream);
+
 // fp32 SIMT check-mode GEMMs (gemm_check.cu): same three ops on fp32 matrices, one problem per launch.
 int launch_check_gemm(GemmOp op, const float* in0, const float* in1, float* out, int m, int n, float alpha,
                       float beta, cudaStream_t stream);

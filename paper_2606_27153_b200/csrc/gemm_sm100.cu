@@ -32,6 +32,7 @@
 #include <cstdlib>
 
 #include "common.h"
+#include "epilogue.cuh"
 #include "umma.cuh"
 
 namespace dmuon {
@@ -111,10 +112,7 @@ __host__ __device__ constexpr int op_ring(int op) { return op == OP_SQ2 ? kEpiAd
 // Per-unit epilogue context (pointers of the unit's problem).
 struct EpiCtx {
   uint64_t tmC, tmD, tmD2;   // tensor maps (generic addresses of the CUtensorMap objects in the problem table)
-  uint16_t* W;        // bf16 parameter / output (fused epilogues)
-  float* W32;         // fp32 master (EPI_APPLY_MASTER)
-  int64_t ldw;        // leading dimension of W / W32 (= of C)
-  float so;           // EPI_APPLY*: lr * scale / c ; EPI_BF16: 1 / c
+  FinalCtx fin;              // fused epilogues: the caller's tensors of this matrix (ldw = leading dimension of C)
 };
 // Per-warp staging state; counters run over the whole kernel.
 struct EpiPipe {
@@ -124,11 +122,6 @@ struct EpiPipe {
   uint32_t consumed;  // ... and read so far
   uint32_t nout;      // chunks stored so far (output tile toggle)
 };
-
-__device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
-  const __nv_bfloat162 b = __floats2bfloat162_rn(lo, hi);
-  return *reinterpret_cast<const uint32_t*>(&b);
-}
 
 // Lane 0: request the addend tile(s) of rows [wrow0, wrow0 + 32), columns [gcol, gcol + 32) into the next ring entry.
 template <int kOp>
@@ -142,19 +135,6 @@ __device__ __forceinline__ void addend_issue(EpiPipe& ep, const EpiCtx& x, int g
   tma_load_2d(dst, x.tmD, gcol, wrow0, bar);
   if (kOp == OP_SQ2) tma_load_2d(dst + kEpiTileBytes, x.tmD2, gcol, wrow0, bar);
   ++ep.issued;
-}
-
-// W words of one 32-column chunk of one row (EPI_APPLY), loaded one chunk ahead.  Through L1 (ld.global.nc): a lane
-// reads its row's 64 bytes as four 16-byte loads, the first brings the sectors in and the other three hit; a streaming
-// load (ld.global.cs) sent all four to L2/DRAM and halved the throughput of the fused X update.
-struct WWords { uint4 w[4]; };
-template <int kEpi>
-__device__ __forceinline__ void load_w(WWords& a, const EpiCtx& x, int64_t grow, int64_t gcol) {
-  if (kEpi == EPI_APPLY) {
-    const uint4* wp = reinterpret_cast<const uint4*>(x.W + grow * x.ldw + gcol);
-#pragma unroll
-    for (int g = 0; g < 4; ++g) a.w[g] = __ldg(wp + g);
-  }
 }
 
 // One 32-column chunk of one accumulator row: v = 32 fp32 accumulators of row `grow`, columns [gcol, gcol + 32).
@@ -234,51 +214,7 @@ __device__ __forceinline__ void epilogue_chunk(const uint32_t (&v)[32], const WW
     }
     ++ep.nout;
   }
-  if (kEpi == EPI_BF16) {
-    // NS output of dmuon_ns_batched: out = bf16(x / c), c a power of two
-    uint32_t o[16];
-#pragma unroll
-    for (int e = 0; e < 16; ++e) o[e] = pack_bf16x2(r[2 * e] * x.so, r[2 * e + 1] * x.so);
-    uint4* wp = reinterpret_cast<uint4*>(x.W + grow * x.ldw + gcol);
-#pragma unroll
-    for (int g = 0; g < 4; ++g) wp[g] = make_uint4(o[g * 4], o[g * 4 + 1], o[g * 4 + 2], o[g * 4 + 3]);
-  } else if (kEpi == EPI_APPLY) {
-    // a6 (Eq. 1; readings N4, N5): W' = W - (lr scale O + lr wd W), one fp32 expression, one RNE rounding
-    uint32_t o[16];
-#pragma unroll
-    for (int g = 0; g < 4; ++g) {
-      const uint32_t wd[4] = {ww.w[g].x, ww.w[g].y, ww.w[g].z, ww.w[g].w};
-#pragma unroll
-      for (int e = 0; e < 4; ++e) {
-        const float w0 = __uint_as_float(wd[e] << 16), w1 = __uint_as_float(wd[e] & 0xFFFF0000u);
-        const float t0 = fmaf(x.so, r[g * 8 + e * 2], sc.lrwd * w0);
-        const float t1 = fmaf(x.so, r[g * 8 + e * 2 + 1], sc.lrwd * w1);
-        o[g * 4 + e] = pack_bf16x2(w0 - t0, w1 - t1);
-      }
-    }
-    uint4* wp = reinterpret_cast<uint4*>(x.W + grow * x.ldw + gcol);
-#pragma unroll
-    for (int g = 0; g < 4; ++g) wp[g] = make_uint4(o[g * 4], o[g * 4 + 1], o[g * 4 + 2], o[g * 4 + 3]);
-  } else if (kEpi == EPI_APPLY_MASTER) {
-    // fp32 master weights: the update lands in the master, the bf16 parameter is its rounding
-    float4* mp = reinterpret_cast<float4*>(x.W32 + grow * x.ldw + gcol);
-    uint32_t o[16];
-#pragma unroll
-    for (int g = 0; g < 8; ++g) {
-      const float4 w = mp[g];
-      float4 n;
-      n.x = w.x - fmaf(x.so, r[g * 4], sc.lrwd * w.x);
-      n.y = w.y - fmaf(x.so, r[g * 4 + 1], sc.lrwd * w.y);
-      n.z = w.z - fmaf(x.so, r[g * 4 + 2], sc.lrwd * w.z);
-      n.w = w.w - fmaf(x.so, r[g * 4 + 3], sc.lrwd * w.w);
-      mp[g] = n;
-      o[g * 2] = pack_bf16x2(n.x, n.y);
-      o[g * 2 + 1] = pack_bf16x2(n.z, n.w);
-    }
-    uint4* wp = reinterpret_cast<uint4*>(x.W + grow * x.ldw + gcol);
-#pragma unroll
-    for (int g = 0; g < 4; ++g) wp[g] = make_uint4(o[g * 4], o[g * 4 + 1], o[g * 4 + 2], o[g * 4 + 3]);
-  }
+  if (kEpi != EPI_F16) final_store<kEpi>(r, ww, x.fin, grow, gcol, sc.lrwd);
 }
 
 // ------------------------------------------------------------------------------------------------ the kernel body
@@ -449,15 +385,15 @@ __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ pro
       x.tmC = reinterpret_cast<uint64_t>(&pr->tmC);
       x.tmD = reinterpret_cast<uint64_t>(&pr->tmD);
       x.tmD2 = reinterpret_cast<uint64_t>(&pr->tmD2);
-      x.ldw = pr->ldc;
-      x.W = nullptr;
-      x.W32 = nullptr;
-      x.so = 0.f;
+      x.fin.ldw = pr->ldc;
+      x.fin.W = nullptr;
+      x.fin.W32 = nullptr;
+      x.fin.so = 0.f;
       if (kEpi != EPI_F16) {
         const MatRec& rec = recs[sc.rec_base + pr->rec];
-        x.W = static_cast<uint16_t*>(rec.W);
-        x.W32 = rec.W32;
-        x.so = kEpi == EPI_BF16 ? rec.inv_xscale : sc.lr * rec.scale * rec.inv_xscale;
+        x.fin.W = static_cast<uint16_t*>(rec.W);
+        x.fin.W32 = rec.W32;
+        x.fin.so = kEpi == EPI_BF16 ? rec.inv_xscale : sc.lr * rec.scale * rec.inv_xscale;
       }
       const int as = it & 1;
       const uint32_t aphase = (it >> 1) & 1;
@@ -479,7 +415,7 @@ __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ pro
         for (int c = c_lo; c < c_hi && c < c_lo + kRing - 1; ++c) addend_issue<kOp>(ep, x, gcol0 + c * 32, wrow0);
       }
       WWords w0 = {}, w1 = {};
-      if (c_lo < c_hi) load_w<kEpi>(w0, x, grow, gcol0 + c_lo * 32);
+      if (c_lo < c_hi) load_w<kEpi>(w0, x.fin, grow, gcol0 + c_lo * 32);
       mbar_wait_warp(bar_tfull + 8 * as, aphase, DMUON_EPI_SLEEP_NS);
       tcgen05_fence_after();
       const uint32_t taddr = tmem_base + as * kAccCols + (static_cast<uint32_t>(q * 32) << 16);
@@ -487,13 +423,13 @@ __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ pro
         uint32_t v[32];
         const int cn = c + 1;
         if (op_has_addend(kOp) && lane == 0 && c + kRing - 1 < c_hi) addend_issue<kOp>(ep, x, gcol0 + (c + kRing - 1) * 32, wrow0);
-        if (cn < c_hi) load_w<kEpi>(w1, x, grow, gcol0 + cn * 32);
+        if (cn < c_hi) load_w<kEpi>(w1, x.fin, grow, gcol0 + cn * 32);
         tmem_ld_32x32(taddr + c * 32, v);
         tmem_wait_ld();
         epilogue_chunk<kOp, kEpi>(v, w0, x, ep, grow, gcol0 + c * 32, sc, bj0 + (c >> 2) != bi);
         if (cn < c_hi) {
           if (op_has_addend(kOp) && lane == 0 && cn + kRing - 1 < c_hi) addend_issue<kOp>(ep, x, gcol0 + (cn + kRing - 1) * 32, wrow0);
-          if (cn + 1 < c_hi) load_w<kEpi>(w0, x, grow, gcol0 + (cn + 1) * 32);
+          if (cn + 1 < c_hi) load_w<kEpi>(w0, x.fin, grow, gcol0 + (cn + 1) * 32);
           tmem_ld_32x32(taddr + cn * 32, v);
           tmem_wait_ld();
           epilogue_chunk<kOp, kEpi>(v, w1, x, ep, grow, gcol0 + cn * 32, sc, bj0 + (cn >> 2) != bi);

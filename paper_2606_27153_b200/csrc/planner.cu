@@ -122,6 +122,7 @@ void describe(const int32_t* shapes, int count, bool fp32, bool keep_o, size_t c
       st.m_pad = mi.m_pad; st.n_pad = mi.n_pad; st.kind = mi.kind; st.gram = mi.gram;
       st.buf_rows = mi.buf_rows; st.buf_cols = mi.buf_cols;
       st.xscale = mi.xscale; st.gscale = mi.gscale;
+      st.onchip = !fp32 && mi.m_pad == kSmallEdge && mi.n_pad == kSmallEdge && mi.buf_rows == kSmallEdge && mi.buf_cols == kSmallEdge;
       const size_t xb = align_up(static_cast<size_t>(mi.buf_rows) * mi.buf_cols * es, 1024);
       const size_t ab = align_up(static_cast<size_t>(mi.m_pad) * mi.m_pad * es, 1024);
       const int nsq = mi.gram ? 5 : 2;
@@ -474,6 +475,27 @@ int encode_tmap_2d(CUtensorMap* out, const void* base, uint64_t rows, uint64_t c
   return DMUON_OK;
 }
 
+// {cols, rows, slots} over `slots` row-major fp16 matrices `slot_bytes` apart; box {box_cols, box_rows, 1}.
+int encode_tmap_3d(CUtensorMap* out, const void* base, uint64_t rows, uint64_t cols, uint64_t slots, uint64_t slot_bytes,
+                   uint32_t box_cols, uint32_t box_rows) {
+  int rc = load_encode();
+  if (rc) return rc;
+  const cuuint64_t gdim[3] = {cols, rows, slots};
+  const cuuint64_t gstride[2] = {cols * sizeof(__half), slot_bytes};
+  const cuuint32_t box[3] = {box_cols, box_rows, 1};
+  const cuuint32_t estr[3] = {1, 1, 1};
+  CUresult r = g_encode(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 3, const_cast<void*>(base), gdim, gstride, box, estr,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    set_error("cuTensorMapEncodeTiled (3-D) failed (%d) for %llu x %llu x %llu, slot stride %llu", static_cast<int>(r),
+              static_cast<unsigned long long>(rows), static_cast<unsigned long long>(cols),
+              static_cast<unsigned long long>(slots), static_cast<unsigned long long>(slot_bytes));
+    return DMUON_ERR_CUDA;
+  }
+  return DMUON_OK;
+}
+
 int check_device() {
   int dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
@@ -654,7 +676,13 @@ int get_plan(const int32_t* shapes, int count, const Options& opt, void* ext_ws,
   if (!p.fp32) {
     bool scratch_ready = false;
     for (ShapeTables& st : p.shapes_tbl) {
-      const size_t nprob = st.slots;
+      if (st.onchip &&
+          (rc = encode_tmap_3d(&st.tm_x0, p.ws + st.base + st.off_q, kSmallEdge, kSmallEdge, st.slots, st.mat_bytes, kBlkK, kBlk)))
+        return rc;
+      // buckets that run in the on-chip kernel need no tile configuration: no scratch tables, nothing to time (if the
+      // option is switched off later, the same plan runs the grouped products with the default configuration)
+      const bool tune = !(st.onchip && opt.small_fused);
+      const size_t nprob = tune ? st.slots : 0;
       std::vector<GemmProblem> tp[3];
       for (int t = 0; t < 3; ++t) tp[t].resize(nprob);
       for (size_t k = 0; k < nprob; ++k) {
@@ -673,7 +701,8 @@ int get_plan(const int32_t* shapes, int count, const Options& opt, void* ext_ws,
       for (int t = 0; t < 3; ++t)
         if ((rc = upload(p, &st.tune_probs[t], tp[t]))) return rc;
       // tile configuration: tuned (cache or measurement) or the default
-      if ((rc = autotune_shape(p, st, opt, stream, &scratch_ready))) return rc;
+      if (tune) { if ((rc = autotune_shape(p, st, opt, stream, &scratch_ready))) return rc; }
+      else for (int t = 0; t < 3; ++t) st.variant[t] = 4;
       const GemmOp ops[3] = {gram_op(st.kind), OP_SQ, xupd_op(st.kind)};
       for (int t = 0; t < 3; ++t) {
         int mb, nb;
@@ -732,8 +761,13 @@ Partition choose_partition(int steps, const float* coeffs, bool per_step, bool g
   return part;
 }
 
+bool bucket_onchip(const Plan& plan, const ShapeTables& st, int steps, const Options& opt) {
+  return !plan.fp32 && st.onchip && opt.small_fused && steps >= 1 && steps <= kSmallMaxSteps;
+}
+
 int result_parity(const Plan& plan, const ShapeTables& st, int steps, const float* coeffs, bool per_step, const Options& opt) {
   if (plan.fp32) return steps & 1;
+  if (bucket_onchip(plan, st, steps, opt)) return 1;      // reads Q, leaves X_k in P
   return static_cast<int>(choose_partition(steps, coeffs, per_step, st.gram && opt.gram_blocks).size()) & 1;
 }
 
@@ -835,6 +869,36 @@ int run_ns_bucket(Plan& plan, int bucket, int steps, const float* coeffs, bool p
   BucketPlan& bp = plan.buckets[bucket];
   ShapeTables& st = plan.shapes_tbl[bp.shape];
   const int count = static_cast<int>(bp.mats.size());
+  if (bucket_onchip(plan, st, steps, opt)) {
+    // every step in one launch; the workspace holds c X and the kernel keeps g G on chip (same scales and the same
+    // epilogue constants as the grouped products: launch_coefs)
+    const bool fused = bucket_fuses(plan, st, steps, opt) && fin.epi != EPI_F16;
+    SmallLaunch L;
+    L.tmX = &st.tm_x0;
+    L.out = plan.ws + st.base + st.off_p;
+    L.slot_bytes = st.mat_bytes;
+    L.recs = plan.d_recs;
+    L.rec_base = bp.rec0;
+    L.count = count;
+    L.steps = steps;
+    const double g = st.gscale, cx = st.xscale;
+    L.gram_alpha = static_cast<float>(g / (cx * cx));
+    for (int s = 0; s < steps; ++s) {
+      const float* q = coeffs + (per_step ? 3 * s : 0);
+      L.poly_alpha[s] = static_cast<float>(q[2] / (g * g));
+      L.poly_beta[s] = static_cast<float>(q[1] / g);
+      L.x_beta[s] = q[0];
+    }
+    L.epi = fused ? fin.epi : EPI_F16;
+    L.lr = fin.lr;
+    L.lrwd = fin.lrwd;
+    L.store_c = fused ? fin.store_c : true;
+    L.grid = plan.sm_count;
+    const std::string name = std::string(!fused ? "ns_small_fused" : fin.epi == EPI_BF16 ? "ns_small_fused_out" : "ns_small_fused_apply") + "[" +
+                             std::to_string(st.m_pad) + "x" + std::to_string(st.n_pad) + "]";
+    ProfScope ps(name.c_str(), stream);
+    return launch_ns_small(L, stream);
+  }
   if (!plan.fp32) {
     const Partition part = choose_partition(steps, coeffs, per_step, st.gram && opt.gram_blocks);
     const std::string key = partition_key(part);

@@ -72,6 +72,30 @@ __device__ __forceinline__ void mbar_wait_warp(uint32_t bar, uint32_t parity, ui
   mbar_wait(bar, parity);
 }
 
+// Cluster-scope acquire: the waiting thread then sees (and may hand to the async proxy) what threads of the PEER CTA
+// wrote before their release.cluster arrive -- the on-chip small-matrix kernel's "operand tile ready" barriers.
+__device__ __forceinline__ uint32_t mbar_try_wait_cluster(uint32_t bar, uint32_t parity) {
+  uint32_t done;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(done)
+      : "r"(bar), "r"(parity)
+      : "memory");
+  return done;
+}
+__device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity) {
+  if (mbar_try_wait_cluster(bar, parity)) return;
+  const uint64_t t0 = global_timer_ns();
+  uint32_t polls = 0;
+  while (!mbar_try_wait_cluster(bar, parity)) {
+    if ((++polls & 0xFFFu) == 0 && global_timer_ns() - t0 > 20000000000ull) __trap();
+  }
+}
+// Generic-proxy writes to shared memory of ANY CTA of the cluster (own or peer) -> visible to the async proxy (UMMA, TMA).
+__device__ __forceinline__ void fence_proxy_async_all() { asm volatile("fence.proxy.async;" ::: "memory"); }
+
 // ------------------------------------------------------------------------------------------------ cluster
 __device__ __forceinline__ uint32_t cluster_ctarank() {
   uint32_t r;
@@ -102,6 +126,13 @@ __device__ __forceinline__ void tma_load_2d_pair(uint32_t smem_dst, uint64_t tma
   asm volatile(
       "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
       ::"r"(smem_dst), "l"(tmap), "r"(c0), "r"(c1), "r"(bar)
+      : "memory");
+}
+// The same for a 3-D tensor (one matrix of a bucket's slot array per coordinate c2).
+__device__ __forceinline__ void tma_load_3d_pair(uint32_t smem_dst, uint64_t tmap, int c0, int c1, int c2, uint32_t bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+      ::"r"(smem_dst), "l"(tmap), "r"(c0), "r"(c1), "r"(c2), "r"(bar)
       : "memory");
 }
 // Bulk tensor store shared -> global (the epilogue's output tiles), tracked by the issuing thread's bulk async-groups.
@@ -202,6 +233,11 @@ __device__ __forceinline__ uint64_t desc_mnmajor(uint32_t saddr) {
   const uint32_t lo = ((saddr >> 4) & 0x3FFFu) | ((8192u >> 4) << 16);
   return (static_cast<uint64_t>(kDescHi) << 32) | lo;
 }
+// The same with the 64-wide M/N chunks `lbo` bytes apart (panels taller than one pipeline stage).
+__device__ __forceinline__ uint64_t desc_mnmajor_lbo(uint32_t saddr, uint32_t lbo) {
+  const uint32_t lo = ((saddr >> 4) & 0x3FFFu) | ((lbo >> 4) << 16);
+  return (static_cast<uint64_t>(kDescHi) << 32) | lo;
+}
 // Instruction descriptor for kind::f16: D = fp32 (bits [4,6) = 1), A/B format fp16 (0) in [7,10)/[10,13),
 // A / B major-ness in bits 15 / 16 (1 = MN-major), N >> 3 in [17,23), M >> 4 in [24,29).
 __device__ __forceinline__ uint32_t make_idesc(int m, int n, bool a_mn_major, bool b_mn_major) {
@@ -211,6 +247,10 @@ __device__ __forceinline__ uint32_t make_idesc(int m, int n, bool a_mn_major, bo
 
 __device__ __forceinline__ void st_shared_v4(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
   asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
+// 16-byte store to an address of the cluster window (own CTA's or the peer's shared memory; see mapa).
+__device__ __forceinline__ void st_cluster_v4(uint32_t cluster_addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+  asm volatile("st.shared::cluster.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(cluster_addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
 }
 // Four 8 x 8 b16 matrices; lanes 8k .. 8k+7 give the row addresses of matrix k.  ldmatrix.trans leaves matrix k
 // TRANSPOSED in register k (fragment layout: lane t holds row t/4, columns 2 (t%4), 2 (t%4) + 1); stmatrix stores
