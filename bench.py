@@ -38,6 +38,7 @@ NS_STEPS = 5
 WORKLOADS = {1: "config1: tiny NS batch 8 x (128x512)", 2: "config2: GPT-2-small-shaped, 72 matrices",
              3: "config3: Qwen-0.5B-style, 168 matrices", 4: "config4: Llama-3-8B-shaped, 224 matrices, 6.98 G elements"}
 GEMM_X = ("ns_bx_update", "ns_bx_apply", "ns_bx_out", "ns_xb_update", "ns_xb_apply", "ns_xb_out")
+SMALL_FUSED = ("ns_small_fused", "ns_small_fused_out", "ns_small_fused_apply")     # the on-chip kernel: all steps, one launch
 
 
 # ------------------------------------------------------------------------------------------------ accounting
@@ -68,27 +69,29 @@ def launch_counts(shapes, plan):
     """Per matrix (m, n, products): how many launches of each product family the library's block schedule
     (dmuon_describe_plan) runs.  A block of length L: 1 Gram product (SYRK), L polynomial products, 3 (L - 1)
     Gram-space products (T = aG + BG, G' = aT + TB, R' = pB' + aR + B'R), 1 X update."""
-    blocks = {}
+    blocks, onchip = {}, {}
     for b in plan["buckets"]:
         blocks[(b["m"], b["n"], b.get("kind", "wide"))] = b["blocks"]
         blocks.setdefault((b["m"], b["n"]), b["blocks"])          # plans described without a kind
+        onchip[(b["m"], b["n"], b.get("kind", "wide"))] = onchip[(b["m"], b["n"])] = bool(b.get("onchip", False))
     out = []
     for s in shapes:
         m, n = oriented(s)
         key = bucket_key(s)
         part = blocks.get(key) or blocks[key[:2]]
         out.append((m, n, {"syrk": len(part), "ns_sq_poly": sum(part), "ns_gram_mm": sum(3 * (L - 1) for L in part),
-                           "xupd": len(part)}))
+                           "xupd": len(part), "onchip": onchip.get(key, onchip.get(key[:2], False))}))
     return out
 
 
 def executed_flops(shapes, plan):
     """FLOPs the kernels execute: every m x m result and X X^T is symmetric and only its upper-triangular 128-blocks
-    are computed, a share (T+1)/(2T) of the dense product; X updates are dense."""
+    are computed, a share (T+1)/(2T) of the dense product; X updates are dense.  The on-chip small-matrix kernel
+    computes its 256 x 256 products in full."""
     tot = 0.0
     for m, n, cnt in launch_counts(shapes, plan):
         t = -(-m // 128)
-        sym = (t + 1) / (2 * t)
+        sym = 1.0 if cnt["onchip"] else (t + 1) / (2 * t)
         tot += sym * (cnt["syrk"] * 2 * m * m * n + (cnt["ns_sq_poly"] + cnt["ns_gram_mm"]) * 2 * m ** 3)
         tot += cnt["xupd"] * 2 * m * m * n
     return tot
@@ -110,7 +113,9 @@ def family_work(family, shapes, plan, x_share=1.0):
         return "byte", 6 * el                      # read O, W; write W'             (a6, when not fused)
     if family == "store_ns_output":
         return "byte", 4 * el
-    lc = launch_counts(shapes, plan)
+    if family in SMALL_FUSED:                      # every product of every step, dense, on the padded 256 x 256 matrix
+        return "flop", sum((c["syrk"] + c["ns_sq_poly"] + c["xupd"]) * 2 * 256 ** 3 for m, n, c in launch_counts(shapes, plan) if c["onchip"])
+    lc = [x for x in launch_counts(shapes, plan) if not x[2]["onchip"]]
     sym = lambda m: (-(-m // 128) + 1) / (2 * -(-m // 128))
     if family in ("ns_syrk_xxt", "ns_syrk_xtx"):
         return "flop", sum(c["syrk"] * sym(m) * 2 * m * m * n for m, n, c in lc)
@@ -554,6 +559,7 @@ def run_sweep(args):
             keep.append(big)
             Xs += [big[i] for i in range(batch)]
             shapes += [(r, c)] * batch
+        Xs = dm.binding.marshal(Xs)            # pointer / shape arrays built once: for 65 536 matrices that is 60 ms of host time
         t0 = time.perf_counter()
         dm.ns_batched(Xs, steps=NS_STEPS)      # plan + autotune
         torch.cuda.synchronize()
@@ -571,7 +577,7 @@ def run_sweep(args):
         torch.cuda.synchronize()
         ms = e0.elapsed_time(e1) / reps
         xt = executed_flops(shapes, plan) / ms / 1e9
-        print(json.dumps({"sweep": True, "shapes": [list(s) for s in shape_list], "batch_per_shape": batch, "matrices": len(Xs), "ms": ms,
+        print(json.dumps({"sweep": True, "shapes": [list(s) for s in shape_list], "batch_per_shape": batch, "matrices": Xs.count, "ms": ms,
                           "tflops_dense_equiv": dense_flops(shapes) / ms / 1e9, "tflops_executed": xt,
                           "roofline_frac_executed_of_sustained": xt / peaks["tflops_sustained"],
                           "buckets": plan["buckets"], "workspace_bytes": plan["workspace_bytes"],

@@ -113,6 +113,22 @@ def _check_mats(tensors: Sequence[torch.Tensor], device_type: str, what: str) ->
             raise ValueError(f"{what}[{i}] must be a contiguous 2-D bfloat16 {device_type} tensor")
 
 
+class Marshalled:
+    """The C arguments of a tensor list (pointer array, shape array, count), built once by marshal() and reusable for any
+    number of calls: for tens of thousands of small matrices building them costs more host time than the GPU call
+    itself.  Holds the tensors, so the pointers stay valid as long as this object lives."""
+
+    def __init__(self, tensors: Sequence[torch.Tensor], device_type: str = "cuda", what: str = "tensors"):
+        self.tensors = list(tensors)
+        _check_mats(self.tensors, device_type, what)
+        self.ptrs = _ptr_array(self.tensors)
+        self.shapes, self.count = _shape_array([t.shape for t in self.tensors])
+
+
+def marshal(tensors: Sequence[torch.Tensor]) -> Marshalled:
+    return tensors if isinstance(tensors, Marshalled) else Marshalled(tensors)
+
+
 # ---------------------------------------------------------------- entry points (names follow include/dmuon.h)
 
 def version() -> str:
@@ -128,20 +144,19 @@ def set_option(key: str, value) -> None:
 
 
 def ns_batched(tensors: Sequence[torch.Tensor], steps: int = 5, coeffs: Optional[Sequence[float]] = None, stream=None) -> None:
-    """dmuon_ns_batched: each tensor is overwritten by NS_steps(X / (||X||_F + 1e-7))."""
-    _check_mats(tensors, "cuda", "tensors")
-    shp, n = _shape_array([t.shape for t in tensors])
+    """dmuon_ns_batched: each tensor is overwritten by NS_steps(X / (||X||_F + 1e-7)).  `tensors`: a list of tensors or
+    the Marshalled form of one (marshal())."""
+    a = marshal(tensors)
     co = (ctypes.c_float * 3)(*coeffs) if coeffs is not None else None
-    _check(lib().dmuon_ns_batched(_ptr_array(tensors), shp, n, int(steps), co, _stream(stream)))
+    _check(lib().dmuon_ns_batched(a.ptrs, a.shapes, a.count, int(steps), co, _stream(stream)))
 
 
 def ns_batched_sched(tensors: Sequence[torch.Tensor], coeffs: Sequence[Sequence[float]], stream=None) -> None:
     """dmuon_ns_batched_sched: one (a, b, c) per step."""
-    _check_mats(tensors, "cuda", "tensors")
-    shp, n = _shape_array([t.shape for t in tensors])
+    a = marshal(tensors)
     flat = [float(v) for row in coeffs for v in row]
     co = (ctypes.c_float * len(flat))(*flat)
-    _check(lib().dmuon_ns_batched_sched(_ptr_array(tensors), shp, n, len(coeffs), co, _stream(stream)))
+    _check(lib().dmuon_ns_batched_sched(a.ptrs, a.shapes, a.count, len(coeffs), co, _stream(stream)))
 
 
 def muon_step(params: Sequence[torch.Tensor], grads: Sequence[torch.Tensor], momenta: Sequence[torch.Tensor],

@@ -93,8 +93,33 @@ __device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity)
     if ((++polls & 0xFFFu) == 0 && global_timer_ns() - t0 > 20000000000ull) __trap();
   }
 }
-// Generic-proxy writes to shared memory of ANY CTA of the cluster (own or peer) -> visible to the async proxy (UMMA, TMA).
-__device__ __forceinline__ void fence_proxy_async_all() { asm volatile("fence.proxy.async;" ::: "memory"); }
+// Latency-critical waits (the on-chip small-matrix kernel's product chain): mbarrier.test_wait never suspends the
+// thread, so the waiter sees the phase flip one poll after it happens instead of after try_wait's time slice.
+template <bool kCluster>
+__device__ __forceinline__ void mbar_spin_wait(uint32_t bar, uint32_t parity) {
+  uint32_t done = 0;
+  uint32_t polls = 0;
+  uint64_t t0 = 0;
+  while (true) {
+    if (kCluster)
+      asm volatile("{\n\t.reg .pred p;\n\tmbarrier.test_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                   : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+    else
+      asm volatile("{\n\t.reg .pred p;\n\tmbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                   : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+    if (done) return;
+    if ((++polls & 0xFFFFu) == 0) {
+      const uint64_t t = global_timer_ns();
+      if (t0 == 0) t0 = t;
+      else if (t - t0 > 20000000000ull) __trap();
+    }
+  }
+}
+__device__ __forceinline__ uint32_t atom_add_acqrel_shared(uint32_t addr, uint32_t v) {
+  uint32_t old;
+  asm volatile("atom.acq_rel.cta.shared::cta.add.u32 %0, [%1], %2;" : "=r"(old) : "r"(addr), "r"(v) : "memory");
+  return old;
+}
 
 // ------------------------------------------------------------------------------------------------ cluster
 __device__ __forceinline__ uint32_t cluster_ctarank() {
@@ -134,6 +159,13 @@ __device__ __forceinline__ void tma_load_3d_pair(uint32_t smem_dst, uint64_t tma
       "cp.async.bulk.tensor.3d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
       ::"r"(smem_dst), "l"(tmap), "r"(c0), "r"(c1), "r"(c2), "r"(bar)
       : "memory");
+}
+// Bulk copy shared -> shared inside the cluster (own CTA or peer): `dst` and `bar` are cluster-window addresses of the
+// DESTINATION CTA (mapa); completion is signalled as transaction bytes on that CTA's barrier.  The copy engine moves
+// the bytes: no thread waits for the (slow) remote stores.
+__device__ __forceinline__ void bulk_copy_to_cluster(uint32_t dst_cluster, uint32_t src_cta, uint32_t bytes, uint32_t bar_cluster) {
+  asm volatile("cp.async.bulk.shared::cluster.shared::cta.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(dst_cluster), "r"(src_cta), "r"(bytes), "r"(bar_cluster) : "memory");
 }
 // Bulk tensor store shared -> global (the epilogue's output tiles), tracked by the issuing thread's bulk async-groups.
 __device__ __forceinline__ void tma_store_2d(uint64_t tmap, uint32_t smem_src, int c0, int c1) {
@@ -247,10 +279,6 @@ __device__ __forceinline__ uint32_t make_idesc(int m, int n, bool a_mn_major, bo
 
 __device__ __forceinline__ void st_shared_v4(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
   asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
-}
-// 16-byte store to an address of the cluster window (own CTA's or the peer's shared memory; see mapa).
-__device__ __forceinline__ void st_cluster_v4(uint32_t cluster_addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
-  asm volatile("st.shared::cluster.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(cluster_addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
 }
 // Four 8 x 8 b16 matrices; lanes 8k .. 8k+7 give the row addresses of matrix k.  ldmatrix.trans leaves matrix k
 // TRANSPOSED in register k (fragment layout: lane t holds row t/4, columns 2 (t%4), 2 (t%4) + 1); stmatrix stores
