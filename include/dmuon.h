@@ -243,7 +243,8 @@ DMUON_API int dmuon_profile_reset(void);
  * tiles only and mirror them.  in0/in1/out are HOST arrays[count] of DEVICE pointers; out must not alias an input.
  * variant: -1 = the default tile configuration, >= 0 selects configuration `variant`: 0..3 = one CTA per unit,
  * UMMA 128 x 256 (0, 2) or 128 x 128 (1, 3), column-panel-major (0, 1) or row-major (2, 3) unit order; 4, 5 = CTA
- * pair (cta_group::2), UMMA 256 x 256, panel-major / row-major.  The symmetric ops accept 0, 1, 4 only.
+ * pair (cta_group::2), UMMA 256 x 256, panel-major / row-major; 6, 7 = the CTA pair with 8 epilogue warps (two per
+ * TMEM lane quarter: for short contractions, where the epilogue sets the pace).  The symmetric ops accept 0, 1, 4, 6 only.
  */
 DMUON_API int dmuon_ns_gemm(int32_t op, const void* const* in0, const void* const* in1, void* const* out,
                             int32_t m, int32_t n, int32_t count, float alpha, float beta, int32_t variant,

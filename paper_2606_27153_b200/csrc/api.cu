@@ -829,6 +829,7 @@ DMUON_API int dmuon_ns_gemm(int32_t op, const void* const* in0, const void* cons
   L.m_blocks = mb;
   L.n_blocks = nb;
   L.pair = variant_config(variant < 0 ? 0 : variant).pair;
+  L.epi_warps = variant_config(variant < 0 ? 0 : variant).epi_warps;
   L.alpha = alpha;
   L.beta = beta;
   L.beta2 = 0.f;
@@ -873,6 +874,7 @@ DMUON_API int dmuon_ns_sym_mm(const void* const* a, const void* const* b, const 
   L.m_blocks = m / kBlk;
   L.n_blocks = m / kBlk;
   L.pair = cfg.pair;
+  L.epi_warps = cfg.epi_warps;
   L.alpha = alpha;
   L.beta = beta;
   L.beta2 = beta2;

@@ -89,6 +89,7 @@ struct GemmLaunch {
   int k_blocks;                 // K / 64
   int m_blocks, n_blocks;       // extent of the output in 128-blocks (rows, columns)
   bool pair;                    // CTA-pair (cta_group::2) tiling
+  int epi_warps = 4;            // epilogue warps per CTA: 4, or 8 (CTA-pair tiling only)
   float alpha, beta, beta2;
   float lr = 0.f, lrwd = 0.f;   // EPI_APPLY*: learning rate and lr * wd
   bool store_c = true;          // fused epilogues: also store fp16(x) to C

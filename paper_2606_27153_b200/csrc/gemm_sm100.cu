@@ -41,8 +41,7 @@ namespace {
 using namespace umma;
 
 constexpr int kBlockBytes = kBlk * kBlkK * 2;   // 16 KB: 128 rows x 128 B of one operand block
-constexpr int kEpiWarps = 4;                    // one per TMEM lane quarter
-constexpr int kNumThreads = 64 + 32 * kEpiWarps;
+constexpr int kMaxEpiWarps = 8;
 constexpr int kTmemCols = 512;
 constexpr int kAccCols = 256;                   // columns per accumulator stage
 constexpr int kMaxStages = 6;
@@ -52,20 +51,33 @@ constexpr int kMaxStages = 6;
 
 // Epilogue staging, per epilogue warp: tiles of 32 rows x 32 fp16 (64-byte rows, 16-byte chunks XOR-swizzled by
 // (row >> 1) & 3 = CU_TENSOR_MAP_SWIZZLE_64B, conflict-free for row-wise 16-byte accesses and for ldmatrix / stmatrix).
-//   2 output tiles + 2 mirrored tiles (double-buffered: a tile is rewritten two chunks after its bulk store was issued)
+//   kOutBufs output tiles + kOutBufs mirrored tiles (a tile is rewritten kOutBufs chunks after its bulk store was issued)
 //   4 addend tiles: a ring the warp's elected lane fills by TMA three chunks ahead (two-addend products: two pairs)
+// Epilogue warps, kEW: 4 = one per TMEM lane quarter; 8 = two per quarter taking alternate 32-column chunks.  With
+// short contractions the epilogue sets the pace and one warp per scheduler hides none of its own latencies (TMEM load,
+// addend wait, shared-memory round trips); the second warp does, at the price of single-buffered output tiles and one
+// operand stage less.
 constexpr int kEpiTileBytes = 32 * 64;
 constexpr int kEpiAddTiles = 4;
-constexpr int kEpiWarpBytes = (4 + kEpiAddTiles) * kEpiTileBytes;     // 16 KB
-constexpr int kEpiBytes = kEpiWarps * kEpiWarpBytes;                  // 64 KB
+template <int kEW> struct EpiCfg {
+  static constexpr int kSub = kEW / 4;                                          // warps per lane quarter
+  static constexpr int kOutBufs = kEW == 4 ? 2 : 1;
+  static constexpr int kWarpBytes = (2 * kOutBufs + kEpiAddTiles) * kEpiTileBytes;   // 16 KB / 12 KB
+  static constexpr int kBytes = kEW * kWarpBytes;                               // 64 KB / 96 KB
+  static constexpr int kThreads = 64 + 32 * kEW;
+};
 
-template <bool kPair> struct Tiling;
-template <> struct Tiling<false> {              // one CTA: A block + up to two B blocks per stage
+template <bool kPair, int kEW> struct Tiling;
+template <> struct Tiling<false, 4> {           // one CTA: A block + up to two B blocks per stage
   static constexpr int kStages = 3;
   static constexpr int kStageBytes = 3 * kBlockBytes;
 };
-template <> struct Tiling<true> {               // CTA pair: this CTA's A block + its B block per stage
+template <> struct Tiling<true, 4> {            // CTA pair: this CTA's A block + its B block per stage
   static constexpr int kStages = 5;
+  static constexpr int kStageBytes = 2 * kBlockBytes;
+};
+template <> struct Tiling<true, 8> {
+  static constexpr int kStages = 4;
   static constexpr int kStageBytes = 2 * kBlockBytes;
 };
 
@@ -74,16 +86,16 @@ struct SmemCtl {
   uint64_t empty[kMaxStages];
   uint64_t tmem_full[2];
   uint64_t tmem_empty[2];
-  uint64_t addend[kEpiWarps][kEpiAddTiles];     // "addend tile(s) of ring slot s have landed", per epilogue warp
+  uint64_t addend[kMaxEpiWarps][kEpiAddTiles];     // "addend tile(s) of ring slot s have landed", per epilogue warp
   uint32_t tmem_base;
   uint32_t pad;
 };
 constexpr int kCtlBytes = 512;
 static_assert(sizeof(SmemCtl) <= kCtlBytes, "SmemCtl");
-template <bool kPair> constexpr int smem_bytes() {
-  return Tiling<kPair>::kStages * Tiling<kPair>::kStageBytes + kEpiBytes + kCtlBytes + 1024 /*alignment slack*/;
+template <bool kPair, int kEW> constexpr int smem_bytes() {
+  return Tiling<kPair, kEW>::kStages * Tiling<kPair, kEW>::kStageBytes + EpiCfg<kEW>::kBytes + kCtlBytes + 1024 /*alignment slack*/;
 }
-static_assert(smem_bytes<true>() <= 232448 && smem_bytes<false>() <= 232448, "shared memory budget");
+static_assert(smem_bytes<true, 4>() <= 232448 && smem_bytes<false, 4>() <= 232448 && smem_bytes<true, 8>() <= 232448, "shared memory budget");
 
 struct Scalars {
   float alpha, beta, beta2;
@@ -116,7 +128,7 @@ struct EpiCtx {
 };
 // Per-warp staging state; counters run over the whole kernel.
 struct EpiPipe {
-  uint32_t obuf;      // 2 output tiles, then 2 mirrored tiles, then the addend ring
+  uint32_t obuf;      // kOutBufs output tiles, then kOutBufs mirrored tiles, then the addend ring
   uint32_t abar;      // this warp's addend barriers
   uint32_t issued;    // addend ring entries requested so far
   uint32_t consumed;  // ... and read so far
@@ -124,13 +136,13 @@ struct EpiPipe {
 };
 
 // Lane 0: request the addend tile(s) of rows [wrow0, wrow0 + 32), columns [gcol, gcol + 32) into the next ring entry.
-template <int kOp>
+template <int kOp, int kEW>
 __device__ __forceinline__ void addend_issue(EpiPipe& ep, const EpiCtx& x, int gcol, int wrow0) {
   constexpr int kRing = op_ring(kOp);
   constexpr int kTiles = op_addends(kOp);
   const uint32_t s = ep.issued % kRing;
   const uint32_t bar = ep.abar + 8 * s;
-  const uint32_t dst = ep.obuf + 4 * kEpiTileBytes + s * kTiles * kEpiTileBytes;
+  const uint32_t dst = ep.obuf + 2 * EpiCfg<kEW>::kOutBufs * kEpiTileBytes + s * kTiles * kEpiTileBytes;
   mbar_expect_tx(bar, kTiles * kEpiTileBytes);
   tma_load_2d(dst, x.tmD, gcol, wrow0, bar);
   if (kOp == OP_SQ2) tma_load_2d(dst + kEpiTileBytes, x.tmD2, gcol, wrow0, bar);
@@ -138,7 +150,7 @@ __device__ __forceinline__ void addend_issue(EpiPipe& ep, const EpiCtx& x, int g
 }
 
 // One 32-column chunk of one accumulator row: v = 32 fp32 accumulators of row `grow`, columns [gcol, gcol + 32).
-template <int kOp, int kEpi>
+template <int kOp, int kEpi, int kEW>
 __device__ __forceinline__ void epilogue_chunk(const uint32_t (&v)[32], const WWords& ww, const EpiCtx& x, EpiPipe& ep,
                                                int64_t grow, int64_t gcol, const Scalars& sc, bool mirror) {
   const int lane = threadIdx.x & 31;
@@ -149,7 +161,7 @@ __device__ __forceinline__ void epilogue_chunk(const uint32_t (&v)[32], const WW
     constexpr int kTiles = op_addends(kOp);
     const uint32_t s = ep.consumed % kRing;
     mbar_wait(ep.abar + 8 * s, (ep.consumed / kRing) & 1);
-    const uint32_t src = ep.obuf + 4 * kEpiTileBytes + s * kTiles * kEpiTileBytes + lane * 64;
+    const uint32_t src = ep.obuf + 2 * EpiCfg<kEW>::kOutBufs * kEpiTileBytes + s * kTiles * kEpiTileBytes + lane * 64;
 #pragma unroll
     for (int g = 0; g < 4; ++g) {
       const uint4 d = ld_shared_v4(src + ((g ^ sw) << 4));
@@ -185,10 +197,11 @@ __device__ __forceinline__ void epilogue_chunk(const uint32_t (&v)[32], const WW
 #pragma unroll
     for (int e = 0; e < 16; ++e) o[e] = pack_half2(r[2 * e], r[2 * e + 1]);
     const bool do_mirror = op_symmetric(kOp) && mirror;
-    const uint32_t ot = ep.obuf + (ep.nout & 1) * kEpiTileBytes;
-    const uint32_t mt = ot + 2 * kEpiTileBytes;
-    // the bulk stores issued from these two tiles two chunks ago have read them (one group per chunk)
-    if (lane == 0) bulk_wait_read<1>();
+    constexpr int kOutBufs = EpiCfg<kEW>::kOutBufs;
+    const uint32_t ot = ep.obuf + (ep.nout % kOutBufs) * kEpiTileBytes;
+    const uint32_t mt = ot + kOutBufs * kEpiTileBytes;
+    // the bulk stores issued from these two tiles kOutBufs chunks ago have read them (one group per chunk)
+    if (lane == 0) bulk_wait_read<kOutBufs - 1>();
     __syncwarp();
 #pragma unroll
     for (int g = 0; g < 4; ++g) st_shared_v4(ot + lane * 64 + ((g ^ sw) << 4), o[g * 4], o[g * 4 + 1], o[g * 4 + 2], o[g * 4 + 3]);
@@ -220,7 +233,7 @@ __device__ __forceinline__ void epilogue_chunk(const uint32_t (&v)[32], const WW
 // ------------------------------------------------------------------------------------------------ the kernel body
 // mb, nb: extent of the output in 128-blocks (rows, columns); pair units may overhang it (TMA zero-fills the
 // operands there, the epilogue skips those blocks).
-template <int kOp, bool kPair, int kEpi>
+template <int kOp, bool kPair, int kEpi, int kEW>
 __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ probs, const TileUnit* __restrict__ units,
                                              const MatRec* __restrict__ recs, int units_per_problem, int total_units,
                                              int k_blocks, int mb, int nb, const Scalars sc) {
@@ -228,8 +241,11 @@ __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ pro
   constexpr bool kAMn = op_a_mn(kOp);
   constexpr bool kBMn = op_b_mn(kOp);
   constexpr int kCG = kPair ? 2 : 1;
-  constexpr int kStages = Tiling<kPair>::kStages;
-  constexpr int kStageBytes = Tiling<kPair>::kStageBytes;
+  constexpr int kStages = Tiling<kPair, kEW>::kStages;
+  constexpr int kStageBytes = Tiling<kPair, kEW>::kStageBytes;
+  constexpr int kEpiBytes = EpiCfg<kEW>::kBytes;
+  constexpr int kEpiWarpBytes = EpiCfg<kEW>::kWarpBytes;
+  constexpr int kSub = EpiCfg<kEW>::kSub;
 
   extern __shared__ uint8_t smem_raw[];
   const uint32_t raw = smem_u32(smem_raw);
@@ -256,9 +272,9 @@ __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ pro
     }
     for (int s = 0; s < 2; ++s) {
       mbar_init(bar_tfull + 8 * s, 1);
-      mbar_init(bar_tempty + 8 * s, kPair ? 2 * kEpiWarps : kEpiWarps);   // one arrival per epilogue warp (of both CTAs)
+      mbar_init(bar_tempty + 8 * s, kPair ? 2 * kEW : kEW);   // one arrival per epilogue warp (of both CTAs)
     }
-    for (int s = 0; s < kEpiWarps * kEpiAddTiles; ++s) mbar_init(ctl_addr + offsetof(SmemCtl, addend) + 8 * s, 1);
+    for (int s = 0; s < kEW * kEpiAddTiles; ++s) mbar_init(ctl_addr + offsetof(SmemCtl, addend) + 8 * s, 1);
     fence_barrier_init();
   }
   if (warp == 1) tmem_alloc<kCG>(ctl_addr + offsetof(SmemCtl, tmem_base), kTmemCols);
@@ -367,8 +383,10 @@ __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ pro
     }
     __syncwarp();
   } else {
-    // ================================================================== epilogue (4 warps: TMEM lane quarter warp % 4)
+    // ================================================================== epilogue (kEW warps: TMEM lane quarter warp % 4;
+    //                                                                    with two warps per quarter, alternate chunks)
     const int q = warp & 3;
+    const int sub = (warp - 2) >> 2;
     const int row = q * 32 + lane;
     constexpr int kRing = op_ring(kOp);
     EpiPipe ep;
@@ -410,29 +428,31 @@ __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ pro
         c_lo = (kSym && bi > bj0) ? (bi - bj0) * 4 : 0;
         c_hi = (nb - bj0 < nbk ? nb - bj0 : nbk) * 4;
       }
-      // addend tiles of the first chunks and the first W words: requested before the accumulator is ready
+      // addend tiles of this warp's first chunks and its first W words: requested before the accumulator is ready
+      const int c0 = c_lo + sub;
       if (op_has_addend(kOp) && lane == 0) {
-        for (int c = c_lo; c < c_hi && c < c_lo + kRing - 1; ++c) addend_issue<kOp>(ep, x, gcol0 + c * 32, wrow0);
+        for (int j = 0; j < kRing - 1; ++j)
+          if (c0 + j * kSub < c_hi) addend_issue<kOp, kEW>(ep, x, gcol0 + (c0 + j * kSub) * 32, wrow0);
       }
       WWords w0 = {}, w1 = {};
-      if (c_lo < c_hi) load_w<kEpi>(w0, x.fin, grow, gcol0 + c_lo * 32);
+      if (c0 < c_hi) load_w<kEpi>(w0, x.fin, grow, gcol0 + c0 * 32);
       mbar_wait_warp(bar_tfull + 8 * as, aphase, DMUON_EPI_SLEEP_NS);
       tcgen05_fence_after();
       const uint32_t taddr = tmem_base + as * kAccCols + (static_cast<uint32_t>(q * 32) << 16);
-      for (int c = c_lo; c < c_hi; c += 2) {
+      for (int c = c0; c < c_hi; c += 2 * kSub) {
         uint32_t v[32];
-        const int cn = c + 1;
-        if (op_has_addend(kOp) && lane == 0 && c + kRing - 1 < c_hi) addend_issue<kOp>(ep, x, gcol0 + (c + kRing - 1) * 32, wrow0);
+        const int cn = c + kSub;
+        if (op_has_addend(kOp) && lane == 0 && c + (kRing - 1) * kSub < c_hi) addend_issue<kOp, kEW>(ep, x, gcol0 + (c + (kRing - 1) * kSub) * 32, wrow0);
         if (cn < c_hi) load_w<kEpi>(w1, x.fin, grow, gcol0 + cn * 32);
         tmem_ld_32x32(taddr + c * 32, v);
         tmem_wait_ld();
-        epilogue_chunk<kOp, kEpi>(v, w0, x, ep, grow, gcol0 + c * 32, sc, bj0 + (c >> 2) != bi);
+        epilogue_chunk<kOp, kEpi, kEW>(v, w0, x, ep, grow, gcol0 + c * 32, sc, bj0 + (c >> 2) != bi);
         if (cn < c_hi) {
-          if (op_has_addend(kOp) && lane == 0 && cn + kRing - 1 < c_hi) addend_issue<kOp>(ep, x, gcol0 + (cn + kRing - 1) * 32, wrow0);
-          if (cn + 1 < c_hi) load_w<kEpi>(w0, x.fin, grow, gcol0 + (cn + 1) * 32);
+          if (op_has_addend(kOp) && lane == 0 && cn + (kRing - 1) * kSub < c_hi) addend_issue<kOp, kEW>(ep, x, gcol0 + (cn + (kRing - 1) * kSub) * 32, wrow0);
+          if (cn + kSub < c_hi) load_w<kEpi>(w0, x.fin, grow, gcol0 + (cn + kSub) * 32);
           tmem_ld_32x32(taddr + cn * 32, v);
           tmem_wait_ld();
-          epilogue_chunk<kOp, kEpi>(v, w1, x, ep, grow, gcol0 + cn * 32, sc, bj0 + (cn >> 2) != bi);
+          epilogue_chunk<kOp, kEpi, kEW>(v, w1, x, ep, grow, gcol0 + cn * 32, sc, bj0 + (cn >> 2) != bi);
         }
       }
       // accumulator fully read by this warp: hand it back to the MMA thread
@@ -453,70 +473,64 @@ __device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ pro
 }
 
 // One named entry point per product, tiling and epilogue, so profiles (ncu -k) and launch lists tell them apart.
-#define DMUON_GEMM_ENTRY(name, op, pair, epi)                                                                   \
-  __global__ void __launch_bounds__(kNumThreads, 1)                                                             \
+#define DMUON_GEMM_ENTRY(name, op, pair, epi, ew)                                                               \
+  __global__ void __launch_bounds__(EpiCfg<ew>::kThreads, 1)                                                    \
   name(const GemmProblem* __restrict__ probs, const TileUnit* __restrict__ units,                               \
        const MatRec* __restrict__ recs, int units_per_problem, int total_units, int k_blocks, int mb, int nb,   \
        const Scalars sc) {                                                                                      \
-    ns_gemm_body<op, pair, epi>(probs, units, recs, units_per_problem, total_units, k_blocks, mb, nb, sc);      \
+    ns_gemm_body<op, pair, epi, ew>(probs, units, recs, units_per_problem, total_units, k_blocks, mb, nb, sc);  \
   }
-DMUON_GEMM_ENTRY(ns_syrk_xxt_kernel, OP_SYRK, false, EPI_F16)
-DMUON_GEMM_ENTRY(ns_syrk_xxt_pair_kernel, OP_SYRK, true, EPI_F16)
-DMUON_GEMM_ENTRY(ns_syrk_xtx_kernel, OP_SYRK_T, false, EPI_F16)
-DMUON_GEMM_ENTRY(ns_syrk_xtx_pair_kernel, OP_SYRK_T, true, EPI_F16)
-DMUON_GEMM_ENTRY(ns_sq_poly_kernel, OP_SQ, false, EPI_F16)
-DMUON_GEMM_ENTRY(ns_sq_poly_pair_kernel, OP_SQ, true, EPI_F16)
-DMUON_GEMM_ENTRY(ns_gram_acc_kernel, OP_SQ2, false, EPI_F16)
-DMUON_GEMM_ENTRY(ns_gram_acc_pair_kernel, OP_SQ2, true, EPI_F16)
-DMUON_GEMM_ENTRY(ns_bx_update_kernel, OP_BX, false, EPI_F16)
-DMUON_GEMM_ENTRY(ns_bx_update_pair_kernel, OP_BX, true, EPI_F16)
-DMUON_GEMM_ENTRY(ns_bx_out_kernel, OP_BX, false, EPI_BF16)
-DMUON_GEMM_ENTRY(ns_bx_out_pair_kernel, OP_BX, true, EPI_BF16)
-DMUON_GEMM_ENTRY(ns_bx_apply_kernel, OP_BX, false, EPI_APPLY)
-DMUON_GEMM_ENTRY(ns_bx_apply_pair_kernel, OP_BX, true, EPI_APPLY)
-DMUON_GEMM_ENTRY(ns_bx_apply_master_kernel, OP_BX, false, EPI_APPLY_MASTER)
-DMUON_GEMM_ENTRY(ns_bx_apply_master_pair_kernel, OP_BX, true, EPI_APPLY_MASTER)
-DMUON_GEMM_ENTRY(ns_xb_update_kernel, OP_XB, false, EPI_F16)
-DMUON_GEMM_ENTRY(ns_xb_update_pair_kernel, OP_XB, true, EPI_F16)
-DMUON_GEMM_ENTRY(ns_xb_out_kernel, OP_XB, false, EPI_BF16)
-DMUON_GEMM_ENTRY(ns_xb_out_pair_kernel, OP_XB, true, EPI_BF16)
-DMUON_GEMM_ENTRY(ns_xb_apply_kernel, OP_XB, false, EPI_APPLY)
-DMUON_GEMM_ENTRY(ns_xb_apply_pair_kernel, OP_XB, true, EPI_APPLY)
-DMUON_GEMM_ENTRY(ns_xb_apply_master_kernel, OP_XB, false, EPI_APPLY_MASTER)
-DMUON_GEMM_ENTRY(ns_xb_apply_master_pair_kernel, OP_XB, true, EPI_APPLY_MASTER)
+// single CTA, CTA pair, CTA pair with 8 epilogue warps
+#define DMUON_GEMM_ENTRIES(stem, op, epi)                           \
+  DMUON_GEMM_ENTRY(stem##_kernel, op, false, epi, 4)                \
+  DMUON_GEMM_ENTRY(stem##_pair_kernel, op, true, epi, 4)            \
+  DMUON_GEMM_ENTRY(stem##_pair_ew8_kernel, op, true, epi, 8)
+DMUON_GEMM_ENTRIES(ns_syrk_xxt, OP_SYRK, EPI_F16)
+DMUON_GEMM_ENTRIES(ns_syrk_xtx, OP_SYRK_T, EPI_F16)
+DMUON_GEMM_ENTRIES(ns_sq_poly, OP_SQ, EPI_F16)
+DMUON_GEMM_ENTRIES(ns_gram_acc, OP_SQ2, EPI_F16)
+DMUON_GEMM_ENTRIES(ns_bx_update, OP_BX, EPI_F16)
+DMUON_GEMM_ENTRIES(ns_bx_out, OP_BX, EPI_BF16)
+DMUON_GEMM_ENTRIES(ns_bx_apply, OP_BX, EPI_APPLY)
+DMUON_GEMM_ENTRIES(ns_bx_apply_master, OP_BX, EPI_APPLY_MASTER)
+DMUON_GEMM_ENTRIES(ns_xb_update, OP_XB, EPI_F16)
+DMUON_GEMM_ENTRIES(ns_xb_out, OP_XB, EPI_BF16)
+DMUON_GEMM_ENTRIES(ns_xb_apply, OP_XB, EPI_APPLY)
+DMUON_GEMM_ENTRIES(ns_xb_apply_master, OP_XB, EPI_APPLY_MASTER)
+#undef DMUON_GEMM_ENTRIES
 #undef DMUON_GEMM_ENTRY
 
 typedef void (*GemmKernel)(const GemmProblem*, const TileUnit*, const MatRec*, int, int, int, int, int, const Scalars);
 
+constexpr int kNumTilings = 3;           // single CTA, CTA pair, CTA pair with 8 epilogue warps
 struct KernelEntry {
-  GemmKernel fn[2];                      // [single, pair]
-  bool configured[2][kMaxDevices];       // cudaFuncSetAttribute is per device
+  GemmKernel fn[kNumTilings];
+  bool configured[kNumTilings][kMaxDevices];       // cudaFuncSetAttribute is per device
 };
+#define DMUON_K(stem) {{stem##_kernel, stem##_pair_kernel, stem##_pair_ew8_kernel}}
 
 // [op][epilogue]; null = combination does not exist (fused epilogues belong to the two X updates)
 KernelEntry g_kernels[kNumOps][kNumEpi] = {
-    /* OP_SYRK   */ {{{ns_syrk_xxt_kernel, ns_syrk_xxt_pair_kernel}}, {}, {}, {}},
-    /* OP_SQ     */ {{{ns_sq_poly_kernel, ns_sq_poly_pair_kernel}}, {}, {}, {}},
-    /* OP_BX     */ {{{ns_bx_update_kernel, ns_bx_update_pair_kernel}}, {{ns_bx_out_kernel, ns_bx_out_pair_kernel}},
-                     {{ns_bx_apply_kernel, ns_bx_apply_pair_kernel}},
-                     {{ns_bx_apply_master_kernel, ns_bx_apply_master_pair_kernel}}},
-    /* OP_SQ2    */ {{{ns_gram_acc_kernel, ns_gram_acc_pair_kernel}}, {}, {}, {}},
-    /* OP_SYRK_T */ {{{ns_syrk_xtx_kernel, ns_syrk_xtx_pair_kernel}}, {}, {}, {}},
-    /* OP_XB     */ {{{ns_xb_update_kernel, ns_xb_update_pair_kernel}}, {{ns_xb_out_kernel, ns_xb_out_pair_kernel}},
-                     {{ns_xb_apply_kernel, ns_xb_apply_pair_kernel}},
-                     {{ns_xb_apply_master_kernel, ns_xb_apply_master_pair_kernel}}},
+    /* OP_SYRK   */ {DMUON_K(ns_syrk_xxt), {}, {}, {}},
+    /* OP_SQ     */ {DMUON_K(ns_sq_poly), {}, {}, {}},
+    /* OP_BX     */ {DMUON_K(ns_bx_update), DMUON_K(ns_bx_out), DMUON_K(ns_bx_apply), DMUON_K(ns_bx_apply_master)},
+    /* OP_SQ2    */ {DMUON_K(ns_gram_acc), {}, {}, {}},
+    /* OP_SYRK_T */ {DMUON_K(ns_syrk_xtx), {}, {}, {}},
+    /* OP_XB     */ {DMUON_K(ns_xb_update), DMUON_K(ns_xb_out), DMUON_K(ns_xb_apply), DMUON_K(ns_xb_apply_master)},
 };
+#undef DMUON_K
 
-template <bool kPair>
+template <bool kPair, int kEW>
 int launch_op(KernelEntry& ke, const GemmLaunch& L, cudaStream_t stream) {
-  constexpr int kSmem = smem_bytes<kPair>();
-  GemmKernel kern = ke.fn[kPair ? 1 : 0];
+  constexpr int kSmem = smem_bytes<kPair, kEW>();
+  constexpr int kTiling = !kPair ? 0 : (kEW == 4 ? 1 : 2);
+  GemmKernel kern = ke.fn[kTiling];
   int dev = 0;
   DMUON_CUDA_CHECK(cudaGetDevice(&dev));
   if (dev < 0 || dev >= kMaxDevices) { set_error("launch_ns_gemm: device ordinal %d is not supported", dev); return DMUON_ERR_UNSUPPORTED_DEVICE; }
-  if (!ke.configured[kPair ? 1 : 0][dev]) {
+  if (!ke.configured[kTiling][dev]) {
     DMUON_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem));
-    ke.configured[kPair ? 1 : 0][dev] = true;
+    ke.configured[kTiling][dev] = true;
   }
   const int total = L.units_per_problem * L.num_problems;
   if (total <= 0) return DMUON_OK;
@@ -524,7 +538,7 @@ int launch_op(KernelEntry& ke, const GemmLaunch& L, cudaStream_t stream) {
   const int use = workers < total ? workers : total;
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3(kPair ? 2 * use : use);
-  cfg.blockDim = dim3(kNumThreads);
+  cfg.blockDim = dim3(EpiCfg<kEW>::kThreads);
   cfg.dynamicSmemBytes = kSmem;
   cfg.stream = stream;
   cudaLaunchAttribute attr[1];
@@ -542,7 +556,10 @@ int launch_op(KernelEntry& ke, const GemmLaunch& L, cudaStream_t stream) {
 
 }  // namespace
 
-int gemm_smem_bytes() { return smem_bytes<false>() > smem_bytes<true>() ? smem_bytes<false>() : smem_bytes<true>(); }
+int gemm_smem_bytes() {
+  const int a = smem_bytes<false, 4>(), b = smem_bytes<true, 4>(), c = smem_bytes<true, 8>();
+  return a > b ? (a > c ? a : c) : (b > c ? b : c);
+}
 
 int launch_ns_gemm(const GemmLaunch& L, cudaStream_t stream) {
   if (L.op < 0 || L.op >= kNumOps || L.epi < 0 || L.epi >= kNumEpi) {
@@ -555,8 +572,9 @@ int launch_ns_gemm(const GemmLaunch& L, cudaStream_t stream) {
     return DMUON_ERR_INVALID_ARG;
   }
   if (L.epi != EPI_F16 && !L.recs) { set_error("launch_ns_gemm: fused epilogue without matrix records"); return DMUON_ERR_INVALID_ARG; }
-  if (L.pair) return launch_op<true>(ke, L, stream);
-  return launch_op<false>(ke, L, stream);
+  if (L.pair && L.epi_warps == 8) return launch_op<true, 8>(ke, L, stream);
+  if (L.pair) return launch_op<true, 4>(ke, L, stream);
+  return launch_op<false, 4>(ke, L, stream);
 }
 
 }  // namespace dmuon

@@ -249,6 +249,7 @@ int shape_launch(const Plan& plan, const ShapeTables& st, int count, int rec0, G
   L.k_blocks = (top == 0 ? st.n_pad : st.m_pad) / kBlkK;
   out_blocks(st, op, &L.m_blocks, &L.n_blocks);
   L.pair = cfg.pair;
+  L.epi_warps = cfg.epi_warps;
   L.alpha = alpha;
   L.beta = beta;
   L.beta2 = beta2;
@@ -413,6 +414,7 @@ TileConfig variant_config(int variant) {
   if (variant >= 4) {
     c.pair = true;
     c.order = variant & 1;
+    c.epi_warps = variant >= 6 ? 8 : 4;
   } else {
     c.width = (variant & 1) ? 1 : 2;
     c.order = (variant >> 1) & 1;

@@ -62,10 +62,11 @@ struct TileConfig {
   bool pair = false;     // CTA-pair tiling: 256 x 256 units on two SMs (cta_group::2)
   int width = 2;         // single-CTA tiling, blocks per work unit: 2 -> UMMA N = 256, 1 -> N = 128
   int order = 0;         // 0: column-panel-major (all block rows of one column panel first), 1: row-major
+  int epi_warps = 4;     // epilogue warps per CTA; 8 (pair tiling only) = two per TMEM lane quarter, for short contractions
 };
-// Variants 0..3: single CTA, (width, order) = (2,0), (1,0), (2,1), (1,1); 4, 5: CTA pair, order 0, 1.
-// The symmetric ops have one ordering: their variants are 0, 1 (single CTA) and 4 (pair).
-constexpr int kNumVariants = 6;
+// Variants 0..3: single CTA, (width, order) = (2,0), (1,0), (2,1), (1,1); 4, 5: CTA pair, order 0, 1; 6, 7: CTA pair
+// with 8 epilogue warps, order 0, 1.  The symmetric ops have one ordering: their variants are 0, 1, 4 and 6.
+constexpr int kNumVariants = 8;
 bool variant_valid(GemmOp op, int variant);
 TileConfig variant_config(int variant);
 

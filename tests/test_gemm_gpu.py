@@ -25,7 +25,7 @@ SHAPES = [(128, 128, 1), (128, 512, 3), (256, 256, 2), (384, 640, 2), (768, 3072
 
 
 @pytest.mark.parametrize("m,k,count", SHAPES)
-@pytest.mark.parametrize("variant", [0, 1, 4])   # single CTA N=256 / N=128, CTA pair 256 x 256
+@pytest.mark.parametrize("variant", [0, 1, 4, 6])   # single CTA N=256 / N=128, CTA pair 256 x 256, pair with 8 epilogue warps
 def test_syrk(m, k, count, variant):
     X = [_rand((m, k), 10 + i, k ** -0.5) for i in range(count)]
     C = [torch.full((m, m), float("nan"), device="cuda", dtype=torch.float16) for _ in range(count)]
@@ -39,7 +39,7 @@ def test_syrk(m, k, count, variant):
 
 
 @pytest.mark.parametrize("m,count", [(128, 1), (256, 3), (384, 2), (896, 2), (1024, 2), (4096, 1)])
-@pytest.mark.parametrize("variant", [0, 1, 4])
+@pytest.mark.parametrize("variant", [0, 1, 4, 6])
 def test_sq(m, count, variant):
     A = []
     for i in range(count):
@@ -67,7 +67,7 @@ def _commuting_pair(m, seed):
 
 
 @pytest.mark.parametrize("m,count", [(128, 2), (256, 3), (384, 2), (896, 2), (1024, 1), (2048, 1)])
-@pytest.mark.parametrize("variant", [0, 1, 4])
+@pytest.mark.parametrize("variant", [0, 1, 4, 6])
 def test_sym_mm(m, count, variant):
     """dmuon_ns_sym_mm: the Gram-block products T = a G + B G (one addend) and R' = p B' + a R + B' R (two addends)."""
     pairs = [_commuting_pair(m, 50 + i) for i in range(count)]
@@ -94,7 +94,7 @@ def test_sym_mm(m, count, variant):
 
 
 @pytest.mark.parametrize("m,n,count", SHAPES)
-@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5, 6, 7])
 def test_bx(m, n, count, variant):
     B = [_rand((m, m), 30 + i, m ** -0.5) for i in range(count)]       # not symmetric on purpose: catches a transposed operand
     X = [_rand((m, n), 40 + i, 1.0) for i in range(count)]
@@ -107,7 +107,7 @@ def test_bx(m, n, count, variant):
         assert _rel(c, ref) < 1e-3
 
 
-@pytest.mark.parametrize("variant", [0, 4])
+@pytest.mark.parametrize("variant", [0, 4, 6])
 def test_many_problems_more_units_than_sms(variant):
     """Persistent loop + double-buffered TMEM across many work units per CTA (or CTA pair)."""
     m, k, count = 256, 384, 200
@@ -120,7 +120,7 @@ def test_many_problems_more_units_than_sms(variant):
 
 
 @pytest.mark.parametrize("m,k,count", SHAPES)
-@pytest.mark.parametrize("variant", [0, 1, 4])
+@pytest.mark.parametrize("variant", [0, 1, 4, 6])
 def test_syrk_t(m, k, count, variant):
     """G = Y^T Y for a tall matrix held as stored (Y is k x m): both operands MN-major."""
     Y = [_rand((k, m), 60 + i, k ** -0.5) for i in range(count)]
@@ -135,7 +135,7 @@ def test_syrk_t(m, k, count, variant):
 
 
 @pytest.mark.parametrize("m,n,count", SHAPES)
-@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5, 6, 7])
 def test_xb(m, n, count, variant):
     """Y' = Y B + beta Y for a tall matrix held as stored (Y is n x m, B symmetric m x m)."""
     B = []
@@ -152,7 +152,7 @@ def test_xb(m, n, count, variant):
         assert _rel(c, ref) < 1e-3
 
 
-@pytest.mark.parametrize("variant", [0, 4])
+@pytest.mark.parametrize("variant", [0, 4, 6])
 def test_sq_small_m_many_problems(variant):
     """64 problems of m = 1024 (config 4's k/v bucket): short contractions, where the epilogue sets the pace.  Also the
     target of the small-m ncu capture in profiles/."""
@@ -172,9 +172,9 @@ def test_sq_small_m_many_problems(variant):
 
 
 def test_variant_table():
-    assert dm.binding.ns_gemm_variants(OP_BX) == 6
+    assert dm.binding.ns_gemm_variants(OP_BX) == 8
     x = _rand((128, 128), 1, 1.0)
     c = torch.empty_like(x)
-    for bad in (2, 3, 5, 6):           # symmetric ops have one ordering; 6 is out of range
+    for bad in (2, 3, 5, 7, 8):        # symmetric ops have one ordering; 8 is out of range
         with pytest.raises(dm.DmuonError):
             dm.ns_gemm(OP_SYRK, [x], None, [c], alpha=1.0, beta=0.0, variant=bad)
