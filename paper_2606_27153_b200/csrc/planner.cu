@@ -278,7 +278,16 @@ int autotune_shape(Plan& plan, ShapeTables& st, const Options& opt, cudaStream_t
     snprintf(key, sizeof key, "%s %d %d %d %d %d", DMUON_BUILD_ID, static_cast<int>(op), st.kind, st.m_pad, st.n_pad,
              count_bucket(st.slots));
     auto it = g_tune_cache.find(key);
+    // Unit order of the X update when X does not fit the L2 (126 MB, two halves): the order in which consecutive units
+    // share the tile of the LARGE operand reads X once; the other one re-reads all of X for every block of the m x m
+    // factor (measured on the 14336 x 4096 bucket: 51.8 GB per launch against 8.6 GB algorithmic, profiles/
+    // r2_step_ncu.md).  Isolated timings cannot see that (the products are power-bound either way), so the wasteful
+    // order is not a candidate: X' = R X (wide) walks column panels of X, Y' = Y R (tall) walks row blocks of Y.
+    const bool general = op == OP_BX || op == OP_XB;
+    const bool x_exceeds_l2 = general && static_cast<size_t>(st.buf_rows) * st.buf_cols * 2 > (48u << 20);
+    const int good_order = op == OP_XB ? 1 : 0;
     int best = st.m_pad >= 2 * kBlk ? 4 : 0;         // untuned default: CTA pair unless the Gram matrix is one block
+    if (x_exceeds_l2) best = 4 + good_order;
     if (opt.force_variant[t] >= 0 && variant_valid(op, opt.force_variant[t])) {
       best = opt.force_variant[t];
     } else if (it != g_tune_cache.end() && variant_valid(op, it->second)) {
@@ -300,6 +309,7 @@ int autotune_shape(Plan& plan, ShapeTables& st, const Options& opt, cudaStream_t
       std::vector<Cand> cands;
       for (int v = 0; v < kNumVariants && rc == DMUON_OK; ++v) {
         if (!variant_valid(op, v)) continue;
+        if (x_exceeds_l2 && variant_config(v).order != good_order) continue;
         std::vector<TileUnit> hu = make_units(op, mb, nb, variant_config(v));
         Cand c{v, nullptr, static_cast<int>(hu.size()), 1e30f};
         if (cudaMalloc(&c.du, hu.size() * sizeof(TileUnit)) != cudaSuccess ||
