@@ -284,7 +284,9 @@ int autotune_shape(Plan& plan, ShapeTables& st, const Options& opt, cudaStream_t
     // r2_step_ncu.md).  Isolated timings cannot see that (the products are power-bound either way), so the wasteful
     // order is not a candidate: X' = R X (wide) walks column panels of X, Y' = Y R (tall) walks row blocks of Y.
     const bool general = op == OP_BX || op == OP_XB;
-    const bool x_exceeds_l2 = general && static_cast<size_t>(st.buf_rows) * st.buf_cols * 2 > (48u << 20);
+    // (only when the m x m factor itself can stay resident: for 8192 x 8192 both operands stream and timing decides)
+    const bool x_exceeds_l2 = general && static_cast<size_t>(st.buf_rows) * st.buf_cols * 2 > (48u << 20) &&
+                              static_cast<size_t>(st.m_pad) * st.m_pad * 2 <= (48u << 20);
     const int good_order = op == OP_XB ? 1 : 0;
     int best = st.m_pad >= 2 * kBlk ? 4 : 0;         // untuned default: CTA pair unless the Gram matrix is one block
     if (x_exceeds_l2) best = 4 + good_order;
