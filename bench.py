@@ -38,6 +38,7 @@ NS_STEPS = 5
 WORKLOADS = {1: "config1: tiny NS batch 8 x (128x512)", 2: "config2: GPT-2-small-shaped, 72 matrices",
              3: "config3: Qwen-0.5B-style, 168 matrices", 4: "config4: Llama-3-8B-shaped, 224 matrices, 6.98 G elements"}
 GEMM_X = ("ns_bx_update", "ns_bx_apply", "ns_bx_out", "ns_xb_update", "ns_xb_apply", "ns_xb_out")
+PROGRAM = ("ns_program", "ns_program_out", "ns_program_apply")     # option program=1: a bucket's whole NS program, one launch
 SMALL_FUSED = ("ns_small_fused", "ns_small_fused_out", "ns_small_fused_apply")     # the on-chip kernel: all steps, one launch
 
 
@@ -113,6 +114,8 @@ def family_work(family, shapes, plan, x_share=1.0):
         return "byte", 6 * el                      # read O, W; write W'             (a6, when not fused)
     if family == "store_ns_output":
         return "byte", 4 * el
+    if family in PROGRAM:                          # every product of the bucket's schedule (symmetry-aware, as executed)
+        return "flop", executed_flops(shapes, plan)
     if family in SMALL_FUSED:                      # every product of every step, dense, on the padded 256 x 256 matrix
         return "flop", sum((c["syrk"] + c["ns_sq_poly"] + c["xupd"]) * 2 * 256 ** 3 for m, n, c in launch_counts(shapes, plan) if c["onchip"])
     lc = [x for x in launch_counts(shapes, plan) if not x[2]["onchip"]]

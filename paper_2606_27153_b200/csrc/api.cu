@@ -399,6 +399,18 @@ DMUON_API int dmuon_set_option(const char* key, const char* value) {
     g_opt.chunk_bytes = static_cast<size_t>(mb) << 20;
     return DMUON_OK;
   }
+  if (k == "program") {
+    if (v == "0" || v == "1") { g_opt.program = v == "1"; return DMUON_OK; }
+    set_error("option program: expected '0' or '1', got '%s'", value);
+    return DMUON_ERR_INVALID_ARG;
+  }
+  if (k == "l2_group_mb") {
+    char* end = nullptr;
+    long long mb = strtoll(value, &end, 10);
+    if (end == value || *end || mb < 1 || mb > (1 << 20)) { set_error("option l2_group_mb: bad value '%s'", value); return DMUON_ERR_INVALID_ARG; }
+    g_opt.l2_group_bytes = static_cast<size_t>(mb) << 20;
+    return DMUON_OK;
+  }
   if (k == "tune_ms") {
     char* end = nullptr;
     float ms = strtof(value, &end);

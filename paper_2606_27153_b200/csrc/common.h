@@ -99,6 +99,34 @@ struct GemmLaunch {
 int launch_ns_gemm(const GemmLaunch& L, cudaStream_t stream);
 int gemm_smem_bytes();
 
+// The whole NS program of a bucket in ONE launch (gemm_sm100.cu, ns_program_kernel): products chained by per-matrix
+// completion counters, matrices taken in L2-sized groups.  CTA-pair tiling; aligned wide / tall and generic buckets with
+// m_pad >= 256.
+constexpr int kMaxProgPhases = 32;
+struct ProgPhaseHost {
+  GemmOp op;
+  const GemmProblem* probs;     // device: one problem per slot of the bucket shape
+  float alpha, beta, beta2;
+};
+struct ProgLaunch {
+  ProgPhaseHost ph[kMaxProgPhases];
+  int num_phases = 0;
+  bool tall = false;            // SYRK_T / XB (a tall matrix held as stored) instead of SYRK / BX
+  Epilogue final_epi = EPI_F16; // epilogue of the last phase (an X update)
+  const TileUnit* units[3];     // CTA-pair unit tables per tiling op (Gram product, m x m products, X update)
+  int upp[3];
+  const MatRec* recs = nullptr;
+  int rec_base = 0;
+  int count = 0;                // matrices (slots 0 .. count - 1)
+  int group = 1;                // matrices per L2-resident group
+  int m_blocks = 0, n_blocks = 0;   // oriented padded shape in 128-blocks
+  uint32_t* done = nullptr;     // device [count] completion counters (zeroed by the launcher)
+  float lr = 0.f, lrwd = 0.f;
+  bool store_c = true;
+  int grid = 148;
+};
+int launch_ns_program(const ProgLaunch& L, cudaStream_t stream);
+
 // On-chip NS of small matrices (ns_small_sm100.cu): all k steps of every 256 x 256 (padded) matrix of a bucket in ONE
 // launch, X / G / B resident in the shared memory of a CTA pair (PAPER.md:170 Gram form, :180 batching by shape).
 constexpr int kSmallEdge = 256;        // m_pad = n_pad = 256

@@ -30,6 +30,7 @@
 // output later steps need is kept.
 #include <cstdio>
 #include <cstdlib>
+#include <cstring>
 
 #include "common.h"
 #include "epilogue.cuh"
@@ -132,6 +133,8 @@ struct EpiPipe {
   uint32_t abar;      // this warp's addend barriers
   uint32_t issued;    // addend ring entries requested so far
   uint32_t consumed;  // ... and read so far
+  uint32_t par;       // bit s: parity of the next completion of addend barrier s (the ring depth differs between
+                      // products, so in the program kernel the phases of the barriers cannot be derived from `consumed`)
   uint32_t nout;      // chunks stored so far (output tile toggle)
 };
 
@@ -160,7 +163,8 @@ __device__ __forceinline__ void epilogue_chunk(const uint32_t (&v)[32], const WW
     constexpr int kRing = op_ring(kOp);
     constexpr int kTiles = op_addends(kOp);
     const uint32_t s = ep.consumed % kRing;
-    mbar_wait(ep.abar + 8 * s, (ep.consumed / kRing) & 1);
+    mbar_wait(ep.abar + 8 * s, (ep.par >> s) & 1u);
+    ep.par ^= 1u << s;
     const uint32_t src = ep.obuf + 2 * EpiCfg<kEW>::kOutBufs * kEpiTileBytes + s * kTiles * kEpiTileBytes + lane * 64;
 #pragma unroll
     for (int g = 0; g < 4; ++g) {
@@ -231,245 +235,343 @@ __device__ __forceinline__ void epilogue_chunk(const uint32_t (&v)[32], const WW
 }
 
 // ------------------------------------------------------------------------------------------------ the kernel body
-// mb, nb: extent of the output in 128-blocks (rows, columns); pair units may overhang it (TMA zero-fills the
-// operands there, the epilogue skips those blocks).
-template <int kOp, bool kPair, int kEpi, int kEW>
-__device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ probs, const TileUnit* __restrict__ units,
-                                             const MatRec* __restrict__ recs, int units_per_problem, int total_units,
-                                             int k_blocks, int mb, int nb, const Scalars sc) {
-  constexpr bool kSym = op_symmetric(kOp);
+// The pipeline is written as three role functions over one PHASE (= one product over a range of problems), with the
+// pipeline state (ring position, accumulator turn, epilogue staging counters) held by the caller, so that the same code
+// serves the one-product kernels (one phase per launch) and the program kernel (all products of a bucket in one
+// launch, phases chained by per-matrix completion counters instead of kernel boundaries).
+struct PhaseArgs {
+  const GemmProblem* probs;     // problems of this phase (device)
+  const TileUnit* units;
+  const MatRec* recs;
+  int units_per_problem, total_units, k_blocks, mb, nb;   // mb, nb: extent of the output in 128-blocks; pair units may
+                                                           // overhang it (operands zero-filled, stores skipped)
+  Scalars sc;
+  // program kernel only
+  int first;                    // running index of the phase's first unit: worker w takes the units u with (first + u) % W == w
+  uint32_t* done;               // per-problem count of finished (unit, epilogue warp) pairs, or null
+  uint32_t need;                // value a problem's counter must have reached before its units of this phase may start
+};
+
+struct Ctx {
+  uint32_t base, epi_addr, ctl_addr, bar_full, bar_empty, bar_tfull, bar_tempty, tmem_base;
+  int warp, lane, worker, num_workers;
+  uint32_t rank;
+};
+struct RingState { int stage; uint32_t phase; };
+
+__device__ __forceinline__ uint32_t ld_acquire_gpu(const uint32_t* p) {
+  uint32_t v;
+  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void red_release_gpu_add(uint32_t* p, uint32_t v) {
+  asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+// Program kernel: wait until every unit of the earlier products of this matrix has been stored (by any CTA).  The
+// stores were bulk tensor stores (async proxy) completed before the release; the loads that follow are bulk tensor
+// loads: a proxy fence on each side.
+__device__ __forceinline__ void wait_done(const uint32_t* ctr, uint32_t need) {
+  if (ld_acquire_gpu(ctr) < need) {
+    const uint64_t t0 = global_timer_ns();
+    uint32_t polls = 0;
+    while (ld_acquire_gpu(ctr) < need) {
+      __nanosleep(100);
+      if ((++polls & 0x3FFu) == 0 && global_timer_ns() - t0 > 20000000000ull) __trap();
+    }
+  }
+  asm volatile("fence.proxy.async;" ::: "memory");
+}
+__device__ __forceinline__ int first_unit(const Ctx& c, const PhaseArgs& a) {
+  const int r = a.first % c.num_workers;
+  return c.worker >= r ? c.worker - r : c.worker + c.num_workers - r;
+}
+
+// ================================================================== TMA producer (one lane; both CTAs of a pair)
+template <int kOp, bool kPair, int kEW>
+__device__ __forceinline__ void produce_phase(const Ctx& c, const PhaseArgs& a, RingState& rs) {
+  constexpr bool kAMn = op_a_mn(kOp);
+  constexpr bool kBMn = op_b_mn(kOp);
+  constexpr int kStages = Tiling<kPair, kEW>::kStages;
+  constexpr int kStageBytes = Tiling<kPair, kEW>::kStageBytes;
+  int waited = -1;
+  for (int u = first_unit(c, a); u < a.total_units; u += c.num_workers) {
+    const int p = u / a.units_per_problem;
+    const TileUnit tu = a.units[u - p * a.units_per_problem];
+    const GemmProblem* pr = a.probs + p;
+    const uint64_t tmA = reinterpret_cast<uint64_t>(&pr->tmA);
+    const uint64_t tmB = reinterpret_cast<uint64_t>(&pr->tmB);
+    // the next unit of this worker usually belongs to another matrix: fetch its descriptors ahead of use
+    const int un = u + c.num_workers;
+    if (un < a.total_units) {
+      const int pn = un / a.units_per_problem;
+      if (pn != p) {
+        tma_prefetch_desc(reinterpret_cast<uint64_t>(&a.probs[pn].tmA));
+        tma_prefetch_desc(reinterpret_cast<uint64_t>(&a.probs[pn].tmB));
+      }
+    }
+    if (a.done && a.need && waited != p) { wait_done(a.done + pr->rec, a.need); waited = p; }
+    const int a_blk = kPair ? 2 * tu.m_blk + static_cast<int>(c.rank) : tu.m_blk;      // this CTA's 128 rows of A
+    const int b_blk = kPair ? 2 * tu.n_blk + static_cast<int>(c.rank) : tu.n_blk;      // its first 128 columns of B
+    const int w = kPair ? 1 : tu.width;
+    for (int kb = 0; kb < a.k_blocks; ++kb) {
+      mbar_wait(c.bar_empty + 8 * rs.stage, rs.phase ^ 1);
+      const uint32_t sA = c.base + rs.stage * kStageBytes;
+      const uint32_t sB = sA + kBlockBytes;
+      if (!kPair) {
+        const uint32_t fb = c.bar_full + 8 * rs.stage;
+        mbar_expect_tx(fb, kBlockBytes + w * kBlockBytes);
+        if (!kAMn) {
+          tma_load_2d(sA, tmA, kb * kBlkK, a_blk * kBlk, fb);
+        } else {
+          tma_load_2d(sA, tmA, a_blk * kBlk, kb * kBlkK, fb);                 // 64 (m) x 64 (k) boxes, 8 KB each
+          tma_load_2d(sA + kBlockBytes / 2, tmA, a_blk * kBlk + 64, kb * kBlkK, fb);
+        }
+        if (!kBMn) {
+          for (int q = 0; q < w; ++q) tma_load_2d(sB + q * kBlockBytes, tmB, kb * kBlkK, (b_blk + q) * kBlk, fb);
+        } else {
+          for (int q = 0; q < 2 * w; ++q)   // 64 (n) x 64 (k) boxes, 8 KB each
+            tma_load_2d(sB + q * (kBlockBytes / 2), tmB, b_blk * kBlk + q * 64, kb * kBlkK, fb);
+        }
+      } else {
+        // both halves of the stage are accounted on the leader's barrier (its MMA thread waits there)
+        if (c.rank == 0) mbar_expect_tx(c.bar_full + 8 * rs.stage, 2 * kStageBytes);
+        const uint32_t fb = mapa(c.bar_full + 8 * rs.stage, 0);
+        if (!kAMn) {
+          tma_load_2d_pair(sA, tmA, kb * kBlkK, a_blk * kBlk, fb);
+        } else {
+          tma_load_2d_pair(sA, tmA, a_blk * kBlk, kb * kBlkK, fb);
+          tma_load_2d_pair(sA + kBlockBytes / 2, tmA, a_blk * kBlk + 64, kb * kBlkK, fb);
+        }
+        if (!kBMn) {
+          tma_load_2d_pair(sB, tmB, kb * kBlkK, b_blk * kBlk, fb);
+        } else {
+          tma_load_2d_pair(sB, tmB, b_blk * kBlk, kb * kBlkK, fb);
+          tma_load_2d_pair(sB + kBlockBytes / 2, tmB, b_blk * kBlk + 64, kb * kBlkK, fb);
+        }
+      }
+      if (++rs.stage == kStages) { rs.stage = 0; rs.phase ^= 1; }
+    }
+  }
+}
+
+// ================================================================== MMA issuer (one lane; leader CTA only in a pair)
+template <int kOp, bool kPair, int kEW>
+__device__ __forceinline__ void mma_phase(const Ctx& c, const PhaseArgs& a, RingState& rs, int& it) {
   constexpr bool kAMn = op_a_mn(kOp);
   constexpr bool kBMn = op_b_mn(kOp);
   constexpr int kCG = kPair ? 2 : 1;
   constexpr int kStages = Tiling<kPair, kEW>::kStages;
   constexpr int kStageBytes = Tiling<kPair, kEW>::kStageBytes;
-  constexpr int kEpiBytes = EpiCfg<kEW>::kBytes;
-  constexpr int kEpiWarpBytes = EpiCfg<kEW>::kWarpBytes;
-  constexpr int kSub = EpiCfg<kEW>::kSub;
+  for (int u = first_unit(c, a); u < a.total_units; u += c.num_workers, ++it) {
+    const int p = u / a.units_per_problem;
+    const TileUnit tu = a.units[u - p * a.units_per_problem];
+    const uint32_t idesc = make_idesc(kPair ? 256 : 128, kPair ? 256 : tu.width * kBlk, kAMn, kBMn);
+    const int as = it & 1;
+    const uint32_t aphase = (it >> 1) & 1;
+    mbar_wait(c.bar_tempty + 8 * as, aphase ^ 1);    // epilogue has drained this accumulator
+    tcgen05_fence_after();
+    const uint32_t d_tmem = c.tmem_base + as * kAccCols;
+    for (int kb = 0; kb < a.k_blocks; ++kb) {
+      mbar_wait(c.bar_full + 8 * rs.stage, rs.phase);       // TMA bytes have landed (in both CTAs of a pair)
+      tcgen05_fence_after();
+      const uint32_t sA = c.base + rs.stage * kStageBytes;
+      const uint32_t sB = sA + kBlockBytes;
+#pragma unroll
+      for (int k = 0; k < kBlkK / 16; ++k) {
+        const uint64_t ad = kAMn ? desc_mnmajor(sA + k * 2048) : desc_kmajor(sA + k * 32);
+        const uint64_t bd = kBMn ? desc_mnmajor(sB + k * 2048) : desc_kmajor(sB + k * 32);
+        mma_f16<kCG>(d_tmem, ad, bd, idesc, (kb | k) != 0);
+      }
+      // frees the smem slot (in both CTAs) when these MMAs finish
+      if (kPair) mma_commit_pair(c.bar_empty + 8 * rs.stage, 3); else mma_commit(c.bar_empty + 8 * rs.stage);
+      if (++rs.stage == kStages) { rs.stage = 0; rs.phase ^= 1; }
+    }
+    // accumulator complete -> epilogue (of both CTAs)
+    if (kPair) mma_commit_pair(c.bar_tfull + 8 * as, 3); else mma_commit(c.bar_tfull + 8 * as);
+  }
+}
 
+// ================================================================== epilogue (kEW warps: TMEM lane quarter warp % 4;
+//                                                                    with two warps per quarter, alternate chunks)
+template <int kOp, bool kPair, int kEpi, int kEW>
+__device__ __forceinline__ void epilogue_phase(const Ctx& c, const PhaseArgs& a, EpiPipe& ep, int& it) {
+  constexpr bool kSym = op_symmetric(kOp);
+  constexpr int kSub = EpiCfg<kEW>::kSub;
+  constexpr int kRing = op_ring(kOp);
+  const int lane = c.lane;
+  const int q = c.warp & 3;
+  const int sub = (c.warp - 2) >> 2;
+  const int row = q * 32 + lane;
+  const uint32_t tempty_leader = kPair ? mapa(c.bar_tempty, 0) : c.bar_tempty;
+  const Scalars& sc = a.sc;
+  ep.issued = ep.consumed = 0;      // every requested addend tile was read by the end of its unit: ring slots restart at 0
+  for (int u = first_unit(c, a); u < a.total_units; u += c.num_workers, ++it) {
+    const int p = u / a.units_per_problem;
+    const TileUnit tu = a.units[u - p * a.units_per_problem];
+    const GemmProblem* pr = a.probs + p;
+    EpiCtx x;
+    x.tmC = reinterpret_cast<uint64_t>(&pr->tmC);
+    x.tmD = reinterpret_cast<uint64_t>(&pr->tmD);
+    x.tmD2 = reinterpret_cast<uint64_t>(&pr->tmD2);
+    x.fin.ldw = pr->ldc;
+    x.fin.W = nullptr;
+    x.fin.W32 = nullptr;
+    x.fin.so = 0.f;
+    if (kEpi != EPI_F16) {
+      const MatRec& rec = a.recs[sc.rec_base + pr->rec];
+      x.fin.W = static_cast<uint16_t*>(rec.W);
+      x.fin.W32 = rec.W32;
+      x.fin.so = kEpi == EPI_BF16 ? rec.inv_xscale : sc.lr * rec.scale * rec.inv_xscale;
+    }
+    const int as = it & 1;
+    const uint32_t aphase = (it >> 1) & 1;
+    const int bi = kPair ? 2 * tu.m_blk + static_cast<int>(c.rank) : tu.m_blk;      // row block of this CTA
+    const int bj0 = kPair ? 2 * tu.n_blk : tu.n_blk;                               // first column block
+    const int nbk = kPair ? 2 : tu.width;
+    const int64_t grow = static_cast<int64_t>(bi) * kBlk + row;
+    const int wrow0 = bi * kBlk + q * 32;                                          // first row of this warp
+    const int gcol0 = bj0 * kBlk;
+    // chunks (32 columns each) this warp stores: inside the matrix and, for symmetric results, not left of the
+    // diagonal block (those blocks are written by the mirror of another unit)
+    int c_lo = 0, c_hi = 0;
+    if (bi < a.mb) {
+      c_lo = (kSym && bi > bj0) ? (bi - bj0) * 4 : 0;
+      c_hi = (a.nb - bj0 < nbk ? a.nb - bj0 : nbk) * 4;
+    }
+    // addend tiles of this warp's first chunks and its first W words: requested before the accumulator is ready
+    const int c0 = c_lo + sub;
+    if (op_has_addend(kOp) && lane == 0) {
+      if (a.done && a.need && c0 < c_hi) wait_done(a.done + pr->rec, a.need);      // the addend is an earlier product's result
+      for (int j = 0; j < kRing - 1; ++j)
+        if (c0 + j * kSub < c_hi) addend_issue<kOp, kEW>(ep, x, gcol0 + (c0 + j * kSub) * 32, wrow0);
+    }
+    WWords w0 = {}, w1 = {};
+    if (c0 < c_hi) load_w<kEpi>(w0, x.fin, grow, gcol0 + c0 * 32);
+    mbar_wait_warp(c.bar_tfull + 8 * as, aphase, DMUON_EPI_SLEEP_NS);
+    tcgen05_fence_after();
+    const uint32_t taddr = c.tmem_base + as * kAccCols + (static_cast<uint32_t>(q * 32) << 16);
+    for (int cc = c0; cc < c_hi; cc += 2 * kSub) {
+      uint32_t v[32];
+      const int cn = cc + kSub;
+      if (op_has_addend(kOp) && lane == 0 && cc + (kRing - 1) * kSub < c_hi) addend_issue<kOp, kEW>(ep, x, gcol0 + (cc + (kRing - 1) * kSub) * 32, wrow0);
+      if (cn < c_hi) load_w<kEpi>(w1, x.fin, grow, gcol0 + cn * 32);
+      tmem_ld_32x32(taddr + cc * 32, v);
+      tmem_wait_ld();
+      epilogue_chunk<kOp, kEpi, kEW>(v, w0, x, ep, grow, gcol0 + cc * 32, sc, bj0 + (cc >> 2) != bi);
+      if (cn < c_hi) {
+        if (op_has_addend(kOp) && lane == 0 && cn + (kRing - 1) * kSub < c_hi) addend_issue<kOp, kEW>(ep, x, gcol0 + (cn + (kRing - 1) * kSub) * 32, wrow0);
+        if (cn + kSub < c_hi) load_w<kEpi>(w0, x.fin, grow, gcol0 + (cn + kSub) * 32);
+        tmem_ld_32x32(taddr + cn * 32, v);
+        tmem_wait_ld();
+        epilogue_chunk<kOp, kEpi, kEW>(v, w1, x, ep, grow, gcol0 + cn * 32, sc, bj0 + (cn >> 2) != bi);
+      }
+    }
+    // accumulator fully read by this warp: hand it back to the MMA thread
+    tcgen05_fence_before();
+    __syncwarp();
+    if (lane == 0) {
+      if (kPair) mbar_arrive_cluster(tempty_leader + 8 * as); else mbar_arrive(c.bar_tempty + 8 * as);
+      if (a.done) {
+        // program kernel: this warp's part of the unit is in global memory -> the matrix's later products may read it
+        bulk_wait_all();
+        asm volatile("fence.proxy.async;" ::: "memory");
+        red_release_gpu_add(a.done + pr->rec, 1u);
+      }
+    }
+  }
+}
+
+template <bool kPair, int kEW>
+__device__ __forceinline__ Ctx pipeline_setup() {
+  constexpr int kCG = kPair ? 2 : 1;
+  constexpr int kStages = Tiling<kPair, kEW>::kStages;
+  constexpr int kStageBytes = Tiling<kPair, kEW>::kStageBytes;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t raw = smem_u32(smem_raw);
-  const uint32_t base = (raw + 1023u) & ~1023u;    // swizzle-128B atoms need 1024-byte alignment
+  Ctx c;
+  c.base = (raw + 1023u) & ~1023u;    // swizzle-128B atoms need 1024-byte alignment
   // [operand ring | epilogue tiles (2 KB each, 1024-byte aligned) | barriers]
-  const uint32_t epi_addr = base + kStages * kStageBytes;
-  const uint32_t ctl_addr = epi_addr + kEpiBytes;
-  SmemCtl* ctl = reinterpret_cast<SmemCtl*>(smem_raw + (ctl_addr - raw));
-  const uint32_t bar_full = ctl_addr + offsetof(SmemCtl, full);
-  const uint32_t bar_empty = ctl_addr + offsetof(SmemCtl, empty);
-  const uint32_t bar_tfull = ctl_addr + offsetof(SmemCtl, tmem_full);
-  const uint32_t bar_tempty = ctl_addr + offsetof(SmemCtl, tmem_empty);
-
-  const int warp = threadIdx.x >> 5;
-  const int lane = threadIdx.x & 31;
-  const uint32_t rank = kPair ? cluster_ctarank() : 0u;          // 0 = leader of the pair
-  const int worker = kPair ? (blockIdx.x >> 1) : blockIdx.x;
-  const int num_workers = kPair ? (gridDim.x >> 1) : gridDim.x;
-
+  c.epi_addr = c.base + kStages * kStageBytes;
+  c.ctl_addr = c.epi_addr + EpiCfg<kEW>::kBytes;
+  SmemCtl* ctl = reinterpret_cast<SmemCtl*>(smem_raw + (c.ctl_addr - raw));
+  c.bar_full = c.ctl_addr + offsetof(SmemCtl, full);
+  c.bar_empty = c.ctl_addr + offsetof(SmemCtl, empty);
+  c.bar_tfull = c.ctl_addr + offsetof(SmemCtl, tmem_full);
+  c.bar_tempty = c.ctl_addr + offsetof(SmemCtl, tmem_empty);
+  c.warp = threadIdx.x >> 5;
+  c.lane = threadIdx.x & 31;
+  c.rank = kPair ? cluster_ctarank() : 0u;          // 0 = leader of the pair
+  c.worker = kPair ? (blockIdx.x >> 1) : blockIdx.x;
+  c.num_workers = kPair ? (gridDim.x >> 1) : gridDim.x;
   if (threadIdx.x == 0) {
     for (int s = 0; s < kStages; ++s) {
-      mbar_init(bar_full + 8 * s, 1);
-      mbar_init(bar_empty + 8 * s, 1);
+      mbar_init(c.bar_full + 8 * s, 1);
+      mbar_init(c.bar_empty + 8 * s, 1);
     }
     for (int s = 0; s < 2; ++s) {
-      mbar_init(bar_tfull + 8 * s, 1);
-      mbar_init(bar_tempty + 8 * s, kPair ? 2 * kEW : kEW);   // one arrival per epilogue warp (of both CTAs)
+      mbar_init(c.bar_tfull + 8 * s, 1);
+      mbar_init(c.bar_tempty + 8 * s, kPair ? 2 * kEW : kEW);   // one arrival per epilogue warp (of both CTAs)
     }
-    for (int s = 0; s < kEW * kEpiAddTiles; ++s) mbar_init(ctl_addr + offsetof(SmemCtl, addend) + 8 * s, 1);
+    for (int s = 0; s < kEW * kEpiAddTiles; ++s) mbar_init(c.ctl_addr + offsetof(SmemCtl, addend) + 8 * s, 1);
     fence_barrier_init();
   }
-  if (warp == 1) tmem_alloc<kCG>(ctl_addr + offsetof(SmemCtl, tmem_base), kTmemCols);
+  if (c.warp == 1) tmem_alloc<kCG>(c.ctl_addr + offsetof(SmemCtl, tmem_base), kTmemCols);
   tcgen05_fence_before();
   if (kPair) cluster_sync(); else __syncthreads();
   tcgen05_fence_after();
-  const uint32_t tmem_base = ctl->tmem_base;
+  c.tmem_base = ctl->tmem_base;
+  return c;
+}
+template <bool kPair, int kEW>
+__device__ __forceinline__ EpiPipe epilogue_pipe(const Ctx& c) {
+  EpiPipe ep;
+  ep.obuf = c.epi_addr + (c.warp - 2) * EpiCfg<kEW>::kWarpBytes;
+  ep.abar = c.ctl_addr + offsetof(SmemCtl, addend) + (c.warp - 2) * (8 * kEpiAddTiles);
+  ep.issued = ep.consumed = ep.nout = 0;
+  ep.par = 0;
+  return ep;
+}
+template <bool kPair>
+__device__ __forceinline__ void pipeline_teardown(const Ctx& c) {
+  tcgen05_fence_before();
+  if (kPair) cluster_sync(); else __syncthreads();
+  if (c.warp == 1) tmem_dealloc<kPair ? 2 : 1>(c.tmem_base, kTmemCols);
+}
 
-  if (warp == 0) {
-    // ================================================================== TMA producer (both CTAs of a pair)
-    if (lane == 0) {
-      int stage = 0;
-      uint32_t phase = 0;
-      for (int u = worker; u < total_units; u += num_workers) {
-        const int p = u / units_per_problem;
-        const TileUnit tu = units[u - p * units_per_problem];
-        const GemmProblem* pr = probs + p;
-        const uint64_t tmA = reinterpret_cast<uint64_t>(&pr->tmA);
-        const uint64_t tmB = reinterpret_cast<uint64_t>(&pr->tmB);
-        // the next unit of this worker usually belongs to another matrix: fetch its descriptors ahead of use
-        const int un = u + num_workers;
-        if (un < total_units) {
-          const int pn = un / units_per_problem;
-          if (pn != p) {
-            tma_prefetch_desc(reinterpret_cast<uint64_t>(&probs[pn].tmA));
-            tma_prefetch_desc(reinterpret_cast<uint64_t>(&probs[pn].tmB));
-          }
-        }
-        const int a_blk = kPair ? 2 * tu.m_blk + static_cast<int>(rank) : tu.m_blk;      // this CTA's 128 rows of A
-        const int b_blk = kPair ? 2 * tu.n_blk + static_cast<int>(rank) : tu.n_blk;      // its first 128 columns of B
-        const int w = kPair ? 1 : tu.width;
-        for (int kb = 0; kb < k_blocks; ++kb) {
-          mbar_wait(bar_empty + 8 * stage, phase ^ 1);
-          const uint32_t sA = base + stage * kStageBytes;
-          const uint32_t sB = sA + kBlockBytes;
-          if (!kPair) {
-            const uint32_t fb = bar_full + 8 * stage;
-            mbar_expect_tx(fb, kBlockBytes + w * kBlockBytes);
-            if (!kAMn) {
-              tma_load_2d(sA, tmA, kb * kBlkK, a_blk * kBlk, fb);
-            } else {
-              tma_load_2d(sA, tmA, a_blk * kBlk, kb * kBlkK, fb);                 // 64 (m) x 64 (k) boxes, 8 KB each
-              tma_load_2d(sA + kBlockBytes / 2, tmA, a_blk * kBlk + 64, kb * kBlkK, fb);
-            }
-            if (!kBMn) {
-              for (int q = 0; q < w; ++q) tma_load_2d(sB + q * kBlockBytes, tmB, kb * kBlkK, (b_blk + q) * kBlk, fb);
-            } else {
-              for (int q = 0; q < 2 * w; ++q)   // 64 (n) x 64 (k) boxes, 8 KB each
-                tma_load_2d(sB + q * (kBlockBytes / 2), tmB, b_blk * kBlk + q * 64, kb * kBlkK, fb);
-            }
-          } else {
-            // both halves of the stage are accounted on the leader's barrier (its MMA thread waits there)
-            if (rank == 0) mbar_expect_tx(bar_full + 8 * stage, 2 * kStageBytes);
-            const uint32_t fb = mapa(bar_full + 8 * stage, 0);
-            if (!kAMn) {
-              tma_load_2d_pair(sA, tmA, kb * kBlkK, a_blk * kBlk, fb);
-            } else {
-              tma_load_2d_pair(sA, tmA, a_blk * kBlk, kb * kBlkK, fb);
-              tma_load_2d_pair(sA + kBlockBytes / 2, tmA, a_blk * kBlk + 64, kb * kBlkK, fb);
-            }
-            if (!kBMn) {
-              tma_load_2d_pair(sB, tmB, kb * kBlkK, b_blk * kBlk, fb);
-            } else {
-              tma_load_2d_pair(sB, tmB, b_blk * kBlk, kb * kBlkK, fb);
-              tma_load_2d_pair(sB + kBlockBytes / 2, tmB, b_blk * kBlk + 64, kb * kBlkK, fb);
-            }
-          }
-          if (++stage == kStages) { stage = 0; phase ^= 1; }
-        }
-      }
+// One product per launch.
+template <int kOp, bool kPair, int kEpi, int kEW>
+__device__ __forceinline__ void ns_gemm_body(const GemmProblem* __restrict__ probs, const TileUnit* __restrict__ units,
+                                             const MatRec* __restrict__ recs, int units_per_problem, int total_units,
+                                             int k_blocks, int mb, int nb, const Scalars sc) {
+  const Ctx c = pipeline_setup<kPair, kEW>();
+  PhaseArgs a;
+  a.probs = probs; a.units = units; a.recs = recs;
+  a.units_per_problem = units_per_problem; a.total_units = total_units;
+  a.k_blocks = k_blocks; a.mb = mb; a.nb = nb;
+  a.sc = sc;
+  a.first = 0; a.done = nullptr; a.need = 0;
+  if (c.warp == 0) {
+    if (c.lane == 0) {
+      RingState rs{0, 0};
+      produce_phase<kOp, kPair, kEW>(c, a, rs);
     }
     __syncwarp();
-  } else if (warp == 1) {
-    // ================================================================== MMA issuer (leader CTA only in a pair)
-    if (lane == 0 && rank == 0) {
-      int stage = 0;
-      uint32_t phase = 0;
+  } else if (c.warp == 1) {
+    if (c.lane == 0 && c.rank == 0) {
+      RingState rs{0, 0};
       int it = 0;
-      for (int u = worker; u < total_units; u += num_workers, ++it) {
-        const int p = u / units_per_problem;
-        const TileUnit tu = units[u - p * units_per_problem];
-        const uint32_t idesc = make_idesc(kPair ? 256 : 128, kPair ? 256 : tu.width * kBlk, kAMn, kBMn);
-        const int as = it & 1;
-        const uint32_t aphase = (it >> 1) & 1;
-        mbar_wait(bar_tempty + 8 * as, aphase ^ 1);    // epilogue has drained this accumulator
-        tcgen05_fence_after();
-        const uint32_t d_tmem = tmem_base + as * kAccCols;
-        for (int kb = 0; kb < k_blocks; ++kb) {
-          mbar_wait(bar_full + 8 * stage, phase);       // TMA bytes have landed (in both CTAs of a pair)
-          tcgen05_fence_after();
-          const uint32_t sA = base + stage * kStageBytes;
-          const uint32_t sB = sA + kBlockBytes;
-#pragma unroll
-          for (int k = 0; k < kBlkK / 16; ++k) {
-            const uint64_t ad = kAMn ? desc_mnmajor(sA + k * 2048) : desc_kmajor(sA + k * 32);
-            const uint64_t bd = kBMn ? desc_mnmajor(sB + k * 2048) : desc_kmajor(sB + k * 32);
-            mma_f16<kCG>(d_tmem, ad, bd, idesc, (kb | k) != 0);
-          }
-          // frees the smem slot (in both CTAs) when these MMAs finish
-          if (kPair) mma_commit_pair(bar_empty + 8 * stage, 3); else mma_commit(bar_empty + 8 * stage);
-          if (++stage == kStages) { stage = 0; phase ^= 1; }
-        }
-        // accumulator complete -> epilogue (of both CTAs)
-        if (kPair) mma_commit_pair(bar_tfull + 8 * as, 3); else mma_commit(bar_tfull + 8 * as);
-      }
+      mma_phase<kOp, kPair, kEW>(c, a, rs, it);
     }
     __syncwarp();
   } else {
-    // ================================================================== epilogue (kEW warps: TMEM lane quarter warp % 4;
-    //                                                                    with two warps per quarter, alternate chunks)
-    const int q = warp & 3;
-    const int sub = (warp - 2) >> 2;
-    const int row = q * 32 + lane;
-    constexpr int kRing = op_ring(kOp);
-    EpiPipe ep;
-    ep.obuf = epi_addr + (warp - 2) * kEpiWarpBytes;
-    ep.abar = ctl_addr + offsetof(SmemCtl, addend) + (warp - 2) * (8 * kEpiAddTiles);
-    ep.issued = ep.consumed = ep.nout = 0;
-    const uint32_t tempty_leader = kPair ? mapa(bar_tempty, 0) : bar_tempty;
+    EpiPipe ep = epilogue_pipe<kPair, kEW>(c);
     int it = 0;
-    for (int u = worker; u < total_units; u += num_workers, ++it) {
-      const int p = u / units_per_problem;
-      const TileUnit tu = units[u - p * units_per_problem];
-      const GemmProblem* pr = probs + p;
-      EpiCtx x;
-      x.tmC = reinterpret_cast<uint64_t>(&pr->tmC);
-      x.tmD = reinterpret_cast<uint64_t>(&pr->tmD);
-      x.tmD2 = reinterpret_cast<uint64_t>(&pr->tmD2);
-      x.fin.ldw = pr->ldc;
-      x.fin.W = nullptr;
-      x.fin.W32 = nullptr;
-      x.fin.so = 0.f;
-      if (kEpi != EPI_F16) {
-        const MatRec& rec = recs[sc.rec_base + pr->rec];
-        x.fin.W = static_cast<uint16_t*>(rec.W);
-        x.fin.W32 = rec.W32;
-        x.fin.so = kEpi == EPI_BF16 ? rec.inv_xscale : sc.lr * rec.scale * rec.inv_xscale;
-      }
-      const int as = it & 1;
-      const uint32_t aphase = (it >> 1) & 1;
-      const int bi = kPair ? 2 * tu.m_blk + static_cast<int>(rank) : tu.m_blk;      // row block of this CTA
-      const int bj0 = kPair ? 2 * tu.n_blk : tu.n_blk;                               // first column block
-      const int nbk = kPair ? 2 : tu.width;
-      const int64_t grow = static_cast<int64_t>(bi) * kBlk + row;
-      const int wrow0 = bi * kBlk + q * 32;                                          // first row of this warp
-      const int gcol0 = bj0 * kBlk;
-      // chunks (32 columns each) this warp stores: inside the matrix and, for symmetric results, not left of the
-      // diagonal block (those blocks are written by the mirror of another unit)
-      int c_lo = 0, c_hi = 0;
-      if (bi < mb) {
-        c_lo = (kSym && bi > bj0) ? (bi - bj0) * 4 : 0;
-        c_hi = (nb - bj0 < nbk ? nb - bj0 : nbk) * 4;
-      }
-      // addend tiles of this warp's first chunks and its first W words: requested before the accumulator is ready
-      const int c0 = c_lo + sub;
-      if (op_has_addend(kOp) && lane == 0) {
-        for (int j = 0; j < kRing - 1; ++j)
-          if (c0 + j * kSub < c_hi) addend_issue<kOp, kEW>(ep, x, gcol0 + (c0 + j * kSub) * 32, wrow0);
-      }
-      WWords w0 = {}, w1 = {};
-      if (c0 < c_hi) load_w<kEpi>(w0, x.fin, grow, gcol0 + c0 * 32);
-      mbar_wait_warp(bar_tfull + 8 * as, aphase, DMUON_EPI_SLEEP_NS);
-      tcgen05_fence_after();
-      const uint32_t taddr = tmem_base + as * kAccCols + (static_cast<uint32_t>(q * 32) << 16);
-      for (int c = c0; c < c_hi; c += 2 * kSub) {
-        uint32_t v[32];
-        const int cn = c + kSub;
-        if (op_has_addend(kOp) && lane == 0 && c + (kRing - 1) * kSub < c_hi) addend_issue<kOp, kEW>(ep, x, gcol0 + (c + (kRing - 1) * kSub) * 32, wrow0);
-        if (cn < c_hi) load_w<kEpi>(w1, x.fin, grow, gcol0 + cn * 32);
-        tmem_ld_32x32(taddr + c * 32, v);
-        tmem_wait_ld();
-        epilogue_chunk<kOp, kEpi, kEW>(v, w0, x, ep, grow, gcol0 + c * 32, sc, bj0 + (c >> 2) != bi);
-        if (cn < c_hi) {
-          if (op_has_addend(kOp) && lane == 0 && cn + (kRing - 1) * kSub < c_hi) addend_issue<kOp, kEW>(ep, x, gcol0 + (cn + (kRing - 1) * kSub) * 32, wrow0);
-          if (cn + kSub < c_hi) load_w<kEpi>(w0, x.fin, grow, gcol0 + (cn + kSub) * 32);
-          tmem_ld_32x32(taddr + cn * 32, v);
-          tmem_wait_ld();
-          epilogue_chunk<kOp, kEpi, kEW>(v, w1, x, ep, grow, gcol0 + cn * 32, sc, bj0 + (cn >> 2) != bi);
-        }
-      }
-      // accumulator fully read by this warp: hand it back to the MMA thread
-      tcgen05_fence_before();
-      __syncwarp();
-      if (lane == 0) {
-        if (kPair) mbar_arrive_cluster(tempty_leader + 8 * as); else mbar_arrive(bar_tempty + 8 * as);
-      }
-    }
+    epilogue_phase<kOp, kPair, kEpi, kEW>(c, a, ep, it);
     // the bulk stores of this warp must have completed (not only read their tiles) before the CTA exits
-    if (lane == 0) bulk_wait_all();
+    if (c.lane == 0) bulk_wait_all();
     __syncwarp();
   }
-
-  tcgen05_fence_before();
-  if (kPair) cluster_sync(); else __syncthreads();
-  if (warp == 1) tmem_dealloc<kCG>(tmem_base, kTmemCols);
+  pipeline_teardown<kPair>(c);
 }
 
 // One named entry point per product, tiling and epilogue, so profiles (ncu -k) and launch lists tell them apart.
@@ -499,6 +601,94 @@ DMUON_GEMM_ENTRIES(ns_xb_apply, OP_XB, EPI_APPLY)
 DMUON_GEMM_ENTRIES(ns_xb_apply_master, OP_XB, EPI_APPLY_MASTER)
 #undef DMUON_GEMM_ENTRIES
 #undef DMUON_GEMM_ENTRY
+
+// ------------------------------------------------------------------------------------------------ program kernel
+// ALL products of a bucket's NS program in ONE launch ("grouped by shape and advanced together"): every
+// CTA pair walks the same list -- for each group of matrices, for each product of the program, the units of that
+// product over the group -- and takes every W-th unit.  A unit of product l of a matrix starts when every unit of
+// product l - 1 of THAT matrix has been stored (per-matrix counters in global memory, bumped by the epilogue warps after
+// their bulk stores completed); nothing else orders the products, so the pipeline never drains between them, there is
+// no launch gap, and a group sized to the L2 keeps its G, B, T, R and X in cache from one product to the next.
+// CTA-pair tiling, 4 epilogue warps.  Deadlock-free because every CTA visits the list in order and a unit only waits
+// for units earlier in the list (all CTAs are resident: grid <= number of SMs, one CTA per SM).
+constexpr int kProgKindGram = 0, kProgKindSq = 1, kProgKindSq2 = 2, kProgKindX = 3, kProgKindXFinal = 4;
+struct ProgPhase {
+  const GemmProblem* probs;
+  float alpha, beta, beta2;
+  uint32_t need;            // completions (units x 8 epilogue warps) of a matrix before this product may read its inputs
+  int kind;
+  int pad;
+};
+struct alignas(16) ProgParams {
+  ProgPhase ph[kMaxProgPhases];
+  const TileUnit* units[3];
+  const MatRec* recs;
+  uint32_t* done;
+  int upp[3];
+  int num_phases, count, group, rec_base;
+  int m_blocks, n_blocks;   // oriented shape in 128-blocks (m <= n)
+  float lr, lrwd;
+  int store_c;
+};
+
+template <int kOp, int kEpi>
+__device__ __forceinline__ void run_phase(const Ctx& c, const PhaseArgs& a, RingState& rs, int& it, EpiPipe& ep) {
+  if (c.warp == 0) {
+    if (c.lane == 0) produce_phase<kOp, true, 4>(c, a, rs);
+  } else if (c.warp == 1) {
+    if (c.lane == 0 && c.rank == 0) mma_phase<kOp, true, 4>(c, a, rs, it);
+  } else {
+    epilogue_phase<kOp, true, kEpi, 4>(c, a, ep, it);
+  }
+}
+
+template <bool kTall, int kFinalEpi>
+__global__ void __launch_bounds__(EpiCfg<4>::kThreads, 1) ns_program_kernel(const __grid_constant__ ProgParams P) {
+  constexpr int kGram = kTall ? OP_SYRK_T : OP_SYRK;
+  constexpr int kX = kTall ? OP_XB : OP_BX;
+  const Ctx c = pipeline_setup<true, 4>();
+  RingState rs{0, 0};
+  int it = 0;
+  EpiPipe ep = epilogue_pipe<true, 4>(c);
+  int first = 0;
+  for (int g0 = 0; g0 < P.count; g0 += P.group) {
+    const int gn = P.count - g0 < P.group ? P.count - g0 : P.group;
+    for (int li = 0; li < P.num_phases; ++li) {
+      const ProgPhase& ph = P.ph[li];
+      const int t = ph.kind == kProgKindGram ? 0 : (ph.kind >= kProgKindX ? 2 : 1);
+      PhaseArgs a;
+      a.probs = ph.probs + g0;
+      a.units = P.units[t];
+      a.recs = P.recs;
+      a.units_per_problem = P.upp[t];
+      a.total_units = gn * P.upp[t];
+      a.k_blocks = (t == 0 ? P.n_blocks : P.m_blocks) * (kBlk / kBlkK);
+      a.mb = (t == 2 && kTall) ? P.n_blocks : P.m_blocks;
+      a.nb = (t == 2 && !kTall) ? P.n_blocks : P.m_blocks;
+      a.sc = Scalars{ph.alpha, ph.beta, ph.beta2, P.lr, P.lrwd, ph.kind == kProgKindXFinal ? P.store_c : 1, P.rec_base};
+      a.first = first;
+      a.done = P.done;
+      a.need = ph.need;
+      switch (ph.kind) {
+        case kProgKindGram: run_phase<kGram, EPI_F16>(c, a, rs, it, ep); break;
+        case kProgKindSq: run_phase<OP_SQ, EPI_F16>(c, a, rs, it, ep); break;
+        case kProgKindSq2: run_phase<OP_SQ2, EPI_F16>(c, a, rs, it, ep); break;
+        case kProgKindX: run_phase<kX, EPI_F16>(c, a, rs, it, ep); break;
+        default: run_phase<kX, kFinalEpi>(c, a, rs, it, ep); break;
+      }
+      first += a.total_units;
+    }
+  }
+  if (c.warp >= 2 && c.lane == 0) bulk_wait_all();
+  __syncwarp();
+  pipeline_teardown<true>(c);
+}
+
+typedef void (*ProgKernel)(const ProgParams);
+ProgKernel g_prog[2][kNumEpi] = {
+    {ns_program_kernel<false, EPI_F16>, ns_program_kernel<false, EPI_BF16>, ns_program_kernel<false, EPI_APPLY>, ns_program_kernel<false, EPI_APPLY_MASTER>},
+    {ns_program_kernel<true, EPI_F16>, ns_program_kernel<true, EPI_BF16>, ns_program_kernel<true, EPI_APPLY>, ns_program_kernel<true, EPI_APPLY_MASTER>}};
+bool g_prog_configured[2][kNumEpi][kMaxDevices];
 
 typedef void (*GemmKernel)(const GemmProblem*, const TileUnit*, const MatRec*, int, int, int, int, int, const Scalars);
 
@@ -575,6 +765,71 @@ int launch_ns_gemm(const GemmLaunch& L, cudaStream_t stream) {
   if (L.pair && L.epi_warps == 8) return launch_op<true, 8>(ke, L, stream);
   if (L.pair) return launch_op<true, 4>(ke, L, stream);
   return launch_op<false, 4>(ke, L, stream);
+}
+
+int launch_ns_program(const ProgLaunch& L, cudaStream_t stream) {
+  if (L.num_phases < 1 || L.num_phases > kMaxProgPhases || L.final_epi < 0 || L.final_epi >= kNumEpi || L.group < 1) {
+    set_error("launch_ns_program: bad phase count %d / epilogue %d / group %d", L.num_phases, static_cast<int>(L.final_epi), L.group);
+    return DMUON_ERR_INVALID_ARG;
+  }
+  if (L.count <= 0) return DMUON_OK;
+  int dev = 0;
+  DMUON_CUDA_CHECK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kMaxDevices) { set_error("launch_ns_program: device ordinal %d is not supported", dev); return DMUON_ERR_UNSUPPORTED_DEVICE; }
+  ProgKernel kern = g_prog[L.tall ? 1 : 0][L.final_epi];
+  constexpr int kSmem = smem_bytes<true, 4>();
+  if (!g_prog_configured[L.tall ? 1 : 0][L.final_epi][dev]) {
+    DMUON_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem));
+    g_prog_configured[L.tall ? 1 : 0][L.final_epi][dev] = true;
+  }
+  ProgParams P;
+  memset(&P, 0, sizeof P);
+  uint32_t units_before = 0;
+  for (int li = 0; li < L.num_phases; ++li) {
+    const ProgPhaseHost& h = L.ph[li];
+    ProgPhase& ph = P.ph[li];
+    ph.probs = h.probs;
+    ph.alpha = h.alpha; ph.beta = h.beta; ph.beta2 = h.beta2;
+    const bool last = li + 1 == L.num_phases;
+    int t;
+    switch (h.op) {
+      case OP_SYRK: case OP_SYRK_T: ph.kind = kProgKindGram; t = 0; break;
+      case OP_SQ: ph.kind = kProgKindSq; t = 1; break;
+      case OP_SQ2: ph.kind = kProgKindSq2; t = 1; break;
+      default: ph.kind = last ? kProgKindXFinal : kProgKindX; t = 2; break;
+    }
+    ph.need = units_before * 8u;       // 2 CTAs x 4 epilogue warps signal each unit
+    units_before += static_cast<uint32_t>(L.upp[t]);
+  }
+  for (int t = 0; t < 3; ++t) { P.units[t] = L.units[t]; P.upp[t] = L.upp[t]; }
+  P.recs = L.recs;
+  P.done = L.done;
+  P.num_phases = L.num_phases;
+  P.count = L.count;
+  P.group = L.group;
+  P.rec_base = L.rec_base;
+  P.m_blocks = L.m_blocks;
+  P.n_blocks = L.n_blocks;
+  P.lr = L.lr;
+  P.lrwd = L.lrwd;
+  P.store_c = L.store_c ? 1 : 0;
+  DMUON_CUDA_CHECK(cudaMemsetAsync(L.done, 0, sizeof(uint32_t) * L.count, stream));
+  const int max_units = L.group * (L.upp[0] > L.upp[2] ? L.upp[0] : L.upp[2]);
+  const int workers = L.grid / 2 < max_units ? L.grid / 2 : max_units;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(2 * workers);
+  cfg.blockDim = dim3(EpiCfg<4>::kThreads);
+  cfg.dynamicSmemBytes = kSmem;
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = 2;
+  attr[0].val.clusterDim.y = 1;
+  attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  DMUON_CUDA_CHECK(cudaLaunchKernelEx(&cfg, kern, P));
+  return DMUON_OK;
 }
 
 }  // namespace dmuon

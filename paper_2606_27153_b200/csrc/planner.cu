@@ -725,6 +725,20 @@ int get_plan(const int32_t* shapes, int count, const Options& opt, void* ext_ws,
         st.units_per_problem[t] = static_cast<int>(hu.size());
         if ((rc = upload(p, &st.units[t], hu))) return rc;
       }
+      if (st.m_pad >= 2 * kBlk) {
+        // program kernel: CTA-pair units for every product; the X update in the tuned order (or the one that reads X once)
+        for (int t = 0; t < 3; ++t) {
+          int mb, nb;
+          out_blocks(st, ops[t], &mb, &nb);
+          TileConfig cfg;
+          cfg.pair = true;
+          cfg.order = t == 2 ? variant_config(st.variant[2]).order : 0;
+          std::vector<TileUnit> hu = make_units(ops[t], mb, nb, cfg);
+          st.prog_upp[t] = static_cast<int>(hu.size());
+          if ((rc = upload(p, &st.prog_units[t], hu))) return rc;
+        }
+        if ((rc = dev_alloc(p, &st.d_done, static_cast<size_t>(st.slots)))) return rc;
+      }
     }
     if (scratch_ready) DMUON_CUDA_CHECK(cudaMemsetAsync(p.ws, 0, p.ws_bytes, stream));
   }
@@ -777,6 +791,10 @@ Partition choose_partition(int steps, const float* coeffs, bool per_step, bool g
 
 bool bucket_onchip(const Plan& plan, const ShapeTables& st, int steps, const Options& opt) {
   return !plan.fp32 && st.onchip && opt.small_fused && steps >= 1 && steps <= kSmallMaxSteps;
+}
+
+bool bucket_program(const Plan& plan, const ShapeTables& st, size_t num_launches, const Options& opt) {
+  return !plan.fp32 && opt.program == 1 && st.d_done && num_launches <= static_cast<size_t>(kMaxProgPhases);
 }
 
 int result_parity(const Plan& plan, const ShapeTables& st, int steps, const float* coeffs, bool per_step, const Options& opt) {
@@ -925,6 +943,40 @@ int run_ns_bucket(Plan& plan, int bucket, int steps, const float* coeffs, bool p
     }
     const bool fused = bucket_fuses(plan, st, steps, opt) && fin.epi != EPI_F16;
     const size_t nl = it->second.launches.size();
+    if (bucket_program(plan, st, nl, opt)) {
+      ProgLaunch P;
+      P.num_phases = static_cast<int>(nl);
+      for (size_t li = 0; li < nl; ++li) {
+        const NsLaunch& L = it->second.launches[li];
+        P.ph[li].op = L.op;
+        P.ph[li].probs = L.probs;
+        launch_coefs(L, st, coeffs, per_step, &P.ph[li].alpha, &P.ph[li].beta, &P.ph[li].beta2);
+      }
+      P.tall = st.kind == K_TALL;
+      P.final_epi = fused ? fin.epi : EPI_F16;
+      for (int t = 0; t < 3; ++t) { P.units[t] = st.prog_units[t]; P.upp[t] = st.prog_upp[t]; }
+      P.recs = plan.d_recs;
+      P.rec_base = bp.rec0;
+      P.count = count;
+      // matrices per group: the group's buffers within the L2 budget, but enough units per product to fill the grid
+      // three times (a product of a group that is one wave long stalls on its predecessor's tail)
+      const int workers = plan.sm_count / 2;
+      const int fit = static_cast<int>(std::max<size_t>(1, opt.l2_group_bytes / st.mat_bytes));
+      const int min_upp = std::max(1, std::min(st.prog_upp[1], st.prog_upp[2]));
+      P.group = std::min(count, std::max(fit, (3 * workers + min_upp - 1) / min_upp));
+      P.m_blocks = st.m_pad / kBlk;
+      P.n_blocks = st.n_pad / kBlk;
+      P.done = st.d_done;
+      P.lr = fin.lr;
+      P.lrwd = fin.lrwd;
+      P.store_c = fused ? fin.store_c : true;
+      P.grid = plan.sm_count;
+      const bool tall = st.kind == K_TALL;
+      const std::string name = std::string(!fused ? "ns_program" : fin.epi == EPI_BF16 ? "ns_program_out" : "ns_program_apply") + "[" +
+                               std::to_string(tall ? st.n_pad : st.m_pad) + "x" + std::to_string(tall ? st.m_pad : st.n_pad) + "]";
+      ProfScope ps(name.c_str(), stream);
+      return launch_ns_program(P, stream);
+    }
     for (size_t li = 0; li < nl; ++li) {
       const NsLaunch& L = it->second.launches[li];
       float alpha, beta, beta2;

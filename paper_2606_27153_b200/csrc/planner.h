@@ -31,6 +31,9 @@ struct Options {
   size_t chunk_bytes = 12ull << 30;   // workspace a bucket may use; larger buckets run as chunks of fewer matrices
   int host_groups = 32;         // dmuon_muon_step_host: at most this many groups of whole shape periods (layers) ...
   int host_slots = 4;           // ... moving through this many device staging slots (measured: profiles/r2_experiments.md)
+  int program = 0;              // option "program": 1 = run a bucket's whole NS program in ONE launch (ns_program_kernel:
+                                // products chained by per-matrix completion counters, matrices in L2-sized groups)
+  size_t l2_group_bytes = 64ull << 20;   // option "l2_group_mb": buffers of one group of matrices in the program kernel
   bool small_fused = true;      // buckets of 256 x 256 (padded) matrices: all NS steps in ONE on-chip launch (ns_small_sm100.cu)
   float tune_ms = 40.f;         // autotune: back-to-back time per candidate (long enough for the power cap to act)
 };
@@ -117,6 +120,9 @@ struct ShapeTables {
   int units_per_problem[3] = {0, 0, 0};
   int variant[3] = {0, 0, 0};
   GemmProblem* tune_probs[3] = {nullptr, nullptr, nullptr};   // scratch problem tables for the autotuner
+  TileUnit* prog_units[3] = {nullptr, nullptr, nullptr};   // CTA-pair unit tables of the program kernel
+  int prog_upp[3] = {0, 0, 0};
+  uint32_t* d_done = nullptr;          // [slots] completion counters of the program kernel
   bool onchip = false;                 // m_pad = n_pad = 256: eligible for the on-chip kernel (option small_fused)
   CUtensorMap tm_x0;                   // ... its 3-D map {cols, rows, slot} over the slots' X0 buffers (buffer Q)
   bool tuned_now = false;              // at least one op was timed (not cached) when this plan was built
@@ -180,6 +186,8 @@ int result_parity(const Plan& plan, const ShapeTables& st, int steps, const floa
 bool bucket_fuses(const Plan& plan, const ShapeTables& st, int steps, const Options& opt);
 // The bucket shape runs its NS steps in the on-chip small-matrix kernel (one launch, nothing stored between products).
 bool bucket_onchip(const Plan& plan, const ShapeTables& st, int steps, const Options& opt);
+// The bucket shape runs its NS program in the one-launch program kernel (option "program").
+bool bucket_program(const Plan& plan, const ShapeTables& st, size_t num_launches, const Options& opt);
 std::string partition_key(const Partition& p);
 
 // Build tile units for an op.

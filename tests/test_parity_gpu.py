@@ -305,6 +305,12 @@ def test_config4_full_size_sampled():
               f"(oracle {secs:.0f} s on {oracle.num_threads()} threads)")
         del orc, w0, g0, m0
     print("config4 plan:", plan["buckets"])
+    # X larger than the L2 (117 MB per matrix): the X update's unit order is the one that reads X once -- row blocks of Y
+    # for the tall buckets (odd tile variant), column panels of X for the wide one (even); measured 51.8 GB -> 9.8 GB of
+    # DRAM reads per launch of the tall update (profiles/r2_step_ncu.md)
+    for b in plan["buckets"]:
+        if b["n"] == 14336:
+            assert b["variants"][2] % 2 == (1 if b["kind"] == "tall" else 0), b
 
 
 # ------------------------------------------------------------------------------------------------ edge cases

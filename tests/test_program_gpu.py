@@ -1,0 +1,130 @@
+"""The one-launch program kernel (option program=1: every product of a bucket's NS program in ONE launch, products
+chained by per-matrix completion counters, matrices in L2-sized groups) against the PLAIN fp64 oracle, and against the
+per-product launches of the same library (program=0) on every matrix.
+
+Bars as in test_parity_gpu.py: O <= 1e-2 relative Frobenius error, M' <= 1 bf16 ulp, W' no worse than the output
+rounding plus 1 % of the update.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_2606_27153_b200 as dm
+from paper_2606_27153_b200 import synth
+from helpers import LR, LR_F, MU, MU_F, TOL_TC, WD, WD_F, bf16_ulp, rel_fro, to64
+
+pytestmark = pytest.mark.gpu
+
+SEED = 88000
+
+
+@pytest.fixture(autouse=True)
+def _reset_options():
+    def base():
+        dm.set_option("mode", "tc")
+        dm.set_option("steps", 5)
+        dm.set_option("coeffs", "3.4445,-4.7750,2.0315")
+        dm.set_option("coeffs_sched", "")
+        dm.set_option("schedule", "auto")
+        dm.set_option("fuse_epilogue", 1)
+        dm.set_option("l2_group_mb", 64)
+    base()
+    dm.set_option("program", 1)
+    dm.set_option("keep_ns_output", 1)
+    yield
+    base()
+    dm.set_option("program", 0)
+    dm.set_option("keep_ns_output", 0)
+
+
+def _check_step(i, shape, W0, G0, M0, Wg, Mg, Og):
+    orc = oracle.muon_step(W0, G0, M0, LR_F, MU_F, WD_F)
+    e = rel_fro(to64(Og), orc["O"])
+    assert e <= TOL_TC, f"matrix {i} {shape}: O rel err {e:.3e}"
+    m_orc = oracle.round_bf16(orc["M_new"])
+    assert (np.abs(to64(Mg) - m_orc) <= bf16_ulp(np.maximum(np.abs(to64(Mg)), np.abs(m_orc)))).all()
+    w_orc = orc["W_new"]
+    err = np.linalg.norm(to64(Wg) - w_orc)
+    bound = 1.02 * np.linalg.norm(oracle.round_bf16(w_orc) - w_orc) + TOL_TC * np.linalg.norm(w_orc - W0)
+    assert err <= bound, f"matrix {i}: W' err {err:.3e} > {bound:.3e}"
+    return e
+
+
+@pytest.mark.parametrize("config,sample", [(2, [0, 3, 4, 5, 35, 70, 71]), (3, [0, 1, 3, 4, 6, 83, 166, 167])])
+def test_muon_step_configs(config, sample):
+    """Square buckets (plain steps), wide and tall buckets (Gram blocks [3, 2]), the 128-row bucket of config 3 (stays on
+    the per-product launches: one block row): oracle on a sample, per-product launches on every matrix."""
+    shapes, W, G, M = synth.muon_inputs(config, "cuda", True)
+    pre = {i: (to64(W[i]), to64(G[i]), to64(M[i])) for i in sample}
+    W2, M2 = [w.clone() for w in W], [m.clone() for m in M]
+    dm.muon_step(W, G, M, LR, MU, WD)
+    torch.cuda.synchronize()
+    worst = 0.0
+    for i in sample:
+        worst = max(worst, _check_step(i, shapes[i], *pre[i], W[i], M[i], dm.binding.read_ns_output(i, shapes[i])))
+    O1 = [dm.binding.read_ns_output(i, s).clone() for i, s in enumerate(shapes)]
+    dm.set_option("program", 0)
+    dm.muon_step(W2, G, M2, LR, MU, WD)
+    torch.cuda.synchronize()
+    for i, s in enumerate(shapes):
+        assert torch.equal(M[i], M2[i])
+        e = rel_fro(to64(O1[i]), to64(dm.binding.read_ns_output(i, s)))
+        assert e <= 2e-3, f"matrix {i} {s}: program vs per-product launches {e:.3e}"
+    print(f"program kernel, config {config}: worst sampled O rel err vs oracle {worst:.2e}")
+
+
+def test_groups_of_many_matrices():
+    """300 matrices of 512 x 512 with a 16 MB group budget: several groups per launch, every CTA pair crosses product
+    and group boundaries many times."""
+    dm.set_option("l2_group_mb", 16)
+    shapes = [(512, 512)] * 300
+    Xs = [synth.iid_scaled(s, SEED + i, "cuda") for i, s in enumerate(shapes)]
+    X64 = {i: to64(Xs[i]) for i in (0, 1, 73, 74, 149, 150, 298, 299)}
+    dm.ns_batched(Xs, steps=5)
+    torch.cuda.synchronize()
+    for i, x in X64.items():
+        e = rel_fro(to64(dm.binding.read_ns_output(i, shapes[i])), oracle.ns(x))
+        assert e <= TOL_TC, f"matrix {i}: {e:.3e}"
+    O1 = [dm.binding.read_ns_output(i, s).clone() for i, s in enumerate(shapes)]
+    dm.set_option("program", 0)
+    Ys = [synth.iid_scaled(s, SEED + i, "cuda") for i, s in enumerate(shapes)]
+    dm.ns_batched(Ys, steps=5)
+    torch.cuda.synchronize()
+    for i, s in enumerate(shapes):
+        assert rel_fro(to64(O1[i]), to64(dm.binding.read_ns_output(i, s))) <= 2e-3
+        assert rel_fro(to64(Xs[i]), to64(Ys[i])) <= 2.0 ** -7
+
+
+@pytest.mark.parametrize("steps", [1, 2, 3, 4, 6, 7])
+def test_step_counts_and_ragged_shapes(steps):
+    """Every block partition [1] ... [3, 2, 2] on wide, tall, square and ragged (generic, padded) matrices."""
+    shapes = [(512, 1536), (1536, 512), (384, 384), (300, 700), (700, 300), (257, 513)]
+    Xs = [synth.iid_normal(s, SEED + 1000 + 10 * steps + i, "cuda") for i, s in enumerate(shapes)]
+    X64 = [to64(x) for x in Xs]
+    dm.ns_batched(Xs, steps=steps)
+    torch.cuda.synchronize()
+    for i, s in enumerate(shapes):
+        o = oracle.ns(X64[i], steps=steps)
+        e = rel_fro(to64(dm.binding.read_ns_output(i, s)), o)
+        assert e <= TOL_TC, f"steps {steps} matrix {i} {s}: {e:.3e}"
+        assert rel_fro(to64(Xs[i]), o) <= TOL_TC + 2.0 ** -8
+
+
+def test_deterministic_without_kept_output():
+    """The bench configuration (keep_ns_output = 0: buckets share one workspace region, fused update, nothing stored):
+    two runs agree bit for bit, and with the per-product launches to the update's rounding."""
+    dm.set_option("keep_ns_output", 0)
+    shapes, W, G, M = synth.muon_inputs(2, "cuda", True)
+    Wa, Ma = [w.clone() for w in W], [m.clone() for m in M]
+    Wb, Mb = [w.clone() for w in W], [m.clone() for m in M]
+    dm.muon_step(Wa, G, Ma, LR, MU, WD)
+    dm.muon_step(Wb, G, Mb, LR, MU, WD)
+    torch.cuda.synchronize()
+    assert all(torch.equal(a, b) for a, b in zip(Wa + Ma, Wb + Mb))
+    dm.set_option("program", 0)
+    dm.muon_step(W, G, M, LR, MU, WD)
+    torch.cuda.synchronize()
+    for a, b in zip(Wa, W):
+        d = (a.float() - b.float()).abs()
+        assert (d <= 2.0 ** -7 * b.float().abs() + 1e-9).all()
