@@ -189,6 +189,13 @@ DMUON_API int dmuon_set_workspace(void* dev_ptr, size_t bytes);
  *   "chunk_mb"    workspace a bucket may use, MiB (default "12288"): a bucket whose matrices need more runs as
  *                 chunks of fewer matrices, one after the other, through the same region
  *   "host_pipeline" "groups,slots" of dmuon_muon_step_host (default "32,4")
+ *   "program"     "auto" (default) / "1" / "0": run ALL products of a bucket's NS program in ONE launch, chained by
+ *                 per-matrix completion counters instead of kernel boundaries, the matrices taken in groups whose
+ *                 buffers fit the L2 ("l2_group_mb").  "auto" = buckets whose small side is >= 2048 (there it is 5-10 %
+ *                 faster: fewer DRAM bytes, more clock under the power cap); "1" = every bucket with a small side
+ *                 >= 256 and <= 32 products; "0" = one launch per product everywhere.  Same arithmetic either way
+ *   "l2_group_mb" budget for the buffers of one group of matrices in the program kernel, MiB (default "64"; a group is
+ *                 never smaller than three waves of work units)
  *   "tune_ms"     autotune: milliseconds each candidate runs back to back (default "40": long enough for the
  *                 board's power cap to act, as it does in the step)
  *   "variants"    "s,q,b": force the tile configuration (see dmuon_ns_gemm) of the SYRK, m x m and X-update products of
@@ -202,7 +209,7 @@ DMUON_API int dmuon_set_option(const char* key, const char* value);
 /*
  * Describe how a shape set is executed: writes a JSON object
  *   {"buckets": [{"m": m_pad, "n": n_pad, "kind": "wide" | "tall" | "generic", "count": matrices, "blocks": [3, 2],
- *                 "variants": [gram, sq, xupdate], "fused": bool, "xscale": c, "gscale": g}, ...],   (execution order;
+ *                 "variants": [gram, sq, xupdate], "fused": bool, "onchip": bool, "program": bool, "xscale": c, "gscale": g}, ...],   (execution order;
  *    "workspace_bytes": B, "tune_seconds": t, "tune_cache_entries": n}                     chunks of a shape repeat)
  * for `steps` NS steps with the current options into buf (NUL terminated, truncated to
  * len); builds the plan if needed (like dmuon_warmup).  Returns the bytes needed (excluding the NUL) or a negative error.

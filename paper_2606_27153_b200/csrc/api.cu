@@ -400,8 +400,8 @@ DMUON_API int dmuon_set_option(const char* key, const char* value) {
     return DMUON_OK;
   }
   if (k == "program") {
-    if (v == "0" || v == "1") { g_opt.program = v == "1"; return DMUON_OK; }
-    set_error("option program: expected '0' or '1', got '%s'", value);
+    if (v == "0" || v == "1" || v == "auto") { g_opt.program = v == "auto" ? 2 : (v == "1" ? 1 : 0); return DMUON_OK; }
+    set_error("option program: expected '0', '1' or 'auto', got '%s'", value);
     return DMUON_ERR_INVALID_ARG;
   }
   if (k == "l2_group_mb") {
@@ -686,9 +686,11 @@ DMUON_API int dmuon_describe_plan(const int32_t* shapes, int32_t count, int32_t 
                st.m_pad, st.n_pad, kKind[st.kind], static_cast<int>(bp.mats.size()));
       s += item;
       for (size_t k = 0; k < part.size(); ++k) s += (k ? ", " : "") + std::to_string(part[k]);
-      snprintf(item, sizeof item, "], \"variants\": [%d, %d, %d], \"fused\": %s, \"onchip\": %s, \"xscale\": %g, \"gscale\": %g}", st.variant[0],
+      snprintf(item, sizeof item, "], \"variants\": [%d, %d, %d], \"fused\": %s, \"onchip\": %s, \"program\": %s, \"xscale\": %g, \"gscale\": %g}", st.variant[0],
                st.variant[1], st.variant[2], bucket_fuses(*plan, st, steps, g_opt) ? "true" : "false",
-               bucket_onchip(*plan, st, steps, g_opt) ? "true" : "false", st.xscale, st.gscale);
+               bucket_onchip(*plan, st, steps, g_opt) ? "true" : "false",
+               !bucket_onchip(*plan, st, steps, g_opt) && bucket_program(*plan, st, program_launches(part), g_opt) ? "true" : "false",
+               st.xscale, st.gscale);
       s += item;
       first = false;
     }

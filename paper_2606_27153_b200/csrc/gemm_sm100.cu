@@ -133,6 +133,7 @@ struct EpiPipe {
   uint32_t abar;      // this warp's addend barriers
   uint32_t issued;    // addend ring entries requested so far
   uint32_t consumed;  // ... and read so far
+  int pend;           // program kernel: matrix whose previous unit this warp has stored but not yet announced, or -1
   uint32_t par;       // bit s: parity of the next completion of addend barrier s (the ring depth differs between
                       // products, so in the program kernel the phases of the barriers cannot be derived from `consumed`)
   uint32_t nout;      // chunks stored so far (output tile toggle)
@@ -280,6 +281,29 @@ __device__ __forceinline__ void wait_done(const uint32_t* ctr, uint32_t need) {
     }
   }
   asm volatile("fence.proxy.async;" ::: "memory");
+}
+// At most n of this thread's most recent bulk groups may still be in flight (n <= 8: chunks of one unit and warp).
+__device__ __forceinline__ void bulk_wait_pending(int n) {
+  switch (n) {
+    case 0: asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); break;
+    case 1: asm volatile("cp.async.bulk.wait_group 1;" ::: "memory"); break;
+    case 2: asm volatile("cp.async.bulk.wait_group 2;" ::: "memory"); break;
+    case 3: asm volatile("cp.async.bulk.wait_group 3;" ::: "memory"); break;
+    case 4: asm volatile("cp.async.bulk.wait_group 4;" ::: "memory"); break;
+    case 5: asm volatile("cp.async.bulk.wait_group 5;" ::: "memory"); break;
+    case 6: asm volatile("cp.async.bulk.wait_group 6;" ::: "memory"); break;
+    case 7: asm volatile("cp.async.bulk.wait_group 7;" ::: "memory"); break;
+    default: asm volatile("cp.async.bulk.wait_group 8;" ::: "memory"); break;
+  }
+}
+// Program kernel, lane 0 of an epilogue warp: announce the unit stored before the current one.  `newer` = bulk groups
+// committed since (those of the current unit, which may still be in flight).
+__device__ __forceinline__ void announce_pending(EpiPipe& ep, uint32_t* done, int newer) {
+  if (ep.pend < 0) return;
+  bulk_wait_pending(newer);
+  asm volatile("fence.proxy.async;" ::: "memory");
+  red_release_gpu_add(done + ep.pend, 1u);
+  ep.pend = -1;
 }
 __device__ __forceinline__ int first_unit(const Ctx& c, const PhaseArgs& a) {
   const int r = a.first % c.num_workers;
@@ -441,12 +465,18 @@ __device__ __forceinline__ void epilogue_phase(const Ctx& c, const PhaseArgs& a,
     // addend tiles of this warp's first chunks and its first W words: requested before the accumulator is ready
     const int c0 = c_lo + sub;
     if (op_has_addend(kOp) && lane == 0) {
-      if (a.done && a.need && c0 < c_hi) wait_done(a.done + pr->rec, a.need);      // the addend is an earlier product's result
+      if (a.done && a.need && c0 < c_hi) {     // the addend is an earlier product's result
+        // (never block with an unannounced unit: another CTA's wait may be for it)
+        if (ep.pend >= 0 && ld_acquire_gpu(a.done + pr->rec) < a.need) announce_pending(ep, a.done, 0);
+        wait_done(a.done + pr->rec, a.need);
+      }
       for (int j = 0; j < kRing - 1; ++j)
         if (c0 + j * kSub < c_hi) addend_issue<kOp, kEW>(ep, x, gcol0 + (c0 + j * kSub) * 32, wrow0);
     }
     WWords w0 = {}, w1 = {};
     if (c0 < c_hi) load_w<kEpi>(w0, x.fin, grow, gcol0 + c0 * 32);
+    if (a.done && lane == 0 && ep.pend >= 0 && !mbar_try_wait(c.bar_tfull + 8 * as, aphase)) announce_pending(ep, a.done, 0);
+    const uint32_t nout0 = ep.nout;
     mbar_wait_warp(c.bar_tfull + 8 * as, aphase, DMUON_EPI_SLEEP_NS);
     tcgen05_fence_after();
     const uint32_t taddr = c.tmem_base + as * kAccCols + (static_cast<uint32_t>(q * 32) << 16);
@@ -472,13 +502,15 @@ __device__ __forceinline__ void epilogue_phase(const Ctx& c, const PhaseArgs& a,
     if (lane == 0) {
       if (kPair) mbar_arrive_cluster(tempty_leader + 8 * as); else mbar_arrive(c.bar_tempty + 8 * as);
       if (a.done) {
-        // program kernel: this warp's part of the unit is in global memory -> the matrix's later products may read it
-        bulk_wait_all();
-        asm volatile("fence.proxy.async;" ::: "memory");
-        red_release_gpu_add(a.done + pr->rec, 1u);
+        // program kernel: once this warp's part of a unit is in global memory the matrix's later products may read it.
+        // Announced one unit late (its bulk stores have completed by then, nothing stalls), or earlier whenever this
+        // warp would otherwise block (above) and at the end of the phase.
+        announce_pending(ep, a.done, static_cast<int>(ep.nout - nout0));
+        ep.pend = pr->rec;
       }
     }
   }
+  if (a.done && lane == 0) announce_pending(ep, a.done, 0);
 }
 
 template <bool kPair, int kEW>
@@ -529,6 +561,7 @@ __device__ __forceinline__ EpiPipe epilogue_pipe(const Ctx& c) {
   ep.abar = c.ctl_addr + offsetof(SmemCtl, addend) + (c.warp - 2) * (8 * kEpiAddTiles);
   ep.issued = ep.consumed = ep.nout = 0;
   ep.par = 0;
+  ep.pend = -1;
   return ep;
 }
 template <bool kPair>

@@ -793,8 +793,17 @@ bool bucket_onchip(const Plan& plan, const ShapeTables& st, int steps, const Opt
   return !plan.fp32 && st.onchip && opt.small_fused && steps >= 1 && steps <= kSmallMaxSteps;
 }
 
+size_t program_launches(const Partition& part) {
+  size_t n = 0;
+  for (int L : part) n += 3 + 4 * static_cast<size_t>(L - 1);
+  return n;
+}
+
 bool bucket_program(const Plan& plan, const ShapeTables& st, size_t num_launches, const Options& opt) {
-  return !plan.fp32 && opt.program == 1 && st.d_done && num_launches <= static_cast<size_t>(kMaxProgPhases);
+  // "auto": where the m x m factors are L2-sized (m >= 2048) the program kernel wins 5-10 % (fewer DRAM bytes, hence
+  // more clock under the power cap); below that the per-product launches with their tuned tilings are as fast or faster
+  const bool wanted = opt.program == 1 || (opt.program == 2 && st.m_pad >= 2048);
+  return !plan.fp32 && wanted && st.d_done && num_launches >= 1 && num_launches <= static_cast<size_t>(kMaxProgPhases);
 }
 
 int result_parity(const Plan& plan, const ShapeTables& st, int steps, const float* coeffs, bool per_step, const Options& opt) {
@@ -959,7 +968,9 @@ int run_ns_bucket(Plan& plan, int bucket, int steps, const float* coeffs, bool p
       P.rec_base = bp.rec0;
       P.count = count;
       // matrices per group: the group's buffers within the L2 budget, but enough units per product to fill the grid
-      // three times (a product of a group that is one wave long stalls on its predecessor's tail)
+      // three times (a product of a group that is one wave long stalls on its predecessor's tail).  Measured on
+      // config 4 (profiles/r2_program.md): groups of 2 matrices for the 4096-row buckets; 1 stalls, 3 and more spill
+      // the L2 and cost clock under the power cap; the whole bucket as one group is 25 % slower than separate launches.
       const int workers = plan.sm_count / 2;
       const int fit = static_cast<int>(std::max<size_t>(1, opt.l2_group_bytes / st.mat_bytes));
       const int min_upp = std::max(1, std::min(st.prog_upp[1], st.prog_upp[2]));

@@ -31,8 +31,9 @@ struct Options {
   size_t chunk_bytes = 12ull << 30;   // workspace a bucket may use; larger buckets run as chunks of fewer matrices
   int host_groups = 32;         // dmuon_muon_step_host: at most this many groups of whole shape periods (layers) ...
   int host_slots = 4;           // ... moving through this many device staging slots (measured: profiles/r2_experiments.md)
-  int program = 0;              // option "program": 1 = run a bucket's whole NS program in ONE launch (ns_program_kernel:
-                                // products chained by per-matrix completion counters, matrices in L2-sized groups)
+  int program = 2;              // option "program": run a bucket's whole NS program in ONE launch (ns_program_kernel: products
+                                // chained by per-matrix completion counters, matrices in L2-sized groups): 0 = never,
+                                // 1 = every eligible bucket (m_pad >= 256, <= 32 products), 2 = "auto": m_pad >= 2048
   size_t l2_group_bytes = 64ull << 20;   // option "l2_group_mb": buffers of one group of matrices in the program kernel
   bool small_fused = true;      // buckets of 256 x 256 (padded) matrices: all NS steps in ONE on-chip launch (ns_small_sm100.cu)
   float tune_ms = 40.f;         // autotune: back-to-back time per candidate (long enough for the power cap to act)
@@ -188,6 +189,7 @@ bool bucket_fuses(const Plan& plan, const ShapeTables& st, int steps, const Opti
 bool bucket_onchip(const Plan& plan, const ShapeTables& st, int steps, const Options& opt);
 // The bucket shape runs its NS program in the one-launch program kernel (option "program").
 bool bucket_program(const Plan& plan, const ShapeTables& st, size_t num_launches, const Options& opt);
+size_t program_launches(const Partition& part);      // products of a block schedule: per block of L steps 3 + 4 (L - 1)
 std::string partition_key(const Partition& p);
 
 // Build tile units for an op.

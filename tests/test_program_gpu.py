@@ -34,7 +34,7 @@ def _reset_options():
     dm.set_option("keep_ns_output", 1)
     yield
     base()
-    dm.set_option("program", 0)
+    dm.set_option("program", "auto")
     dm.set_option("keep_ns_output", 0)
 
 
