@@ -356,6 +356,7 @@ def run_ours(args):
     dm.set_option("profile", 0)
     dm.set_option("keep_ns_output", 0)
     dm.set_option("fuse_epilogue", args.fuse)
+    dm.set_option("program", args.program)
     if cfg == 1:
         _, W = synth.ns_inputs("cuda")
         G = M = None
@@ -509,7 +510,7 @@ def run_ours(args):
             "data": "synthetic",
             "config": {"workload": WORKLOADS[cfg] + (f" -- REDUCED to the first {args.layers} layers (profiling run, not a bench value)" if indices is not None else ""), "ns_steps": NS_STEPS, "coeffs": [3.4445, -4.7750, 2.0315], "lr": LR,
                        "mu": MU, "wd": WD, "schedule": plan_desc["buckets"], "workspace_bytes": plan_desc.get("workspace_bytes"),
-                       "fused_epilogue": bool(args.fuse), "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "fused_epilogue": bool(args.fuse), "program_kernel": args.program, "parallelism": "replicas only" if world > 1 else "single GPU",
                        "l2": "inputs (W, G, M + workspace, tens of GB) exceed the 126 MB L2; no flush needed",
                        "arithmetic": "bf16 in/out, fp16 operands on tcgen05 with fp32 TMEM accumulation, fp32 elementwise"},
             "muon_step_ms": ms, "ns_tflops_dense_equiv": value / world, "ns_tflops_executed": xt,
@@ -625,6 +626,8 @@ def main():
     ap.add_argument("--layers", type=int, default=0, help="profiling aid: only the first L layers of the set (0 = all)")
     ap.add_argument("--sample-seconds", type=float, default=0.0, help="--impl reference: CPU seconds per step (0 = auto)")
     ap.add_argument("--fuse", type=int, default=1, choices=[0, 1], help="library option 'fuse_epilogue' (0: separate apply pass)")
+    ap.add_argument("--program", default="auto", choices=["auto", "0", "1"],
+                    help="library option 'program' (one launch per bucket's NS program: auto = small side >= 2048; 0: one launch per product)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="configs[4]: NS-only shape sweep, one JSON line per shape")
