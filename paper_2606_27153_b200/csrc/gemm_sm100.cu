@@ -854,27 +854,15 @@ int launch_ns_program(const ProgLaunch& L, cudaStream_t stream) {
   cfg.blockDim = dim3(EpiCfg<4>::kThreads);
   cfg.dynamicSmemBytes = kSmem;
   cfg.stream = stream;
-  cudaLaunchAttribute attr[2];
+  cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeClusterDimension;
   attr[0].val.clusterDim.x = 2;
   attr[0].val.clusterDim.y = 1;
   attr[0].val.clusterDim.z = 1;
-  // Units wait for units of other CTAs, so every CTA of the grid must be resident at once: a cooperative launch makes
-  // the driver guarantee that (grid <= one CTA per SM) even when other work shares the GPU.  Tried once per process;
-  // if this driver does not combine it with clusters the plain launch is used (correct whenever the step has the GPU
-  // to itself, which dmuon.h asks for).
-  static int coop = -1;            // -1 untried, 0 unsupported, 1 supported
-  attr[1].id = cudaLaunchAttributeCooperative;
-  attr[1].val.cooperative = 1;
+  // Units wait for units of other CTAs, so every CTA of the grid must be resident at once: grid <= one CTA per SM, and
+  // the step has the GPU to itself (dmuon.h).  (A cooperative launch would make the driver guarantee it, but Nsight
+  // Compute fails such a launch when it is combined with a cluster dimension: LaunchFailed under ncu, measured.)
   cfg.attrs = attr;
-  if (coop != 0) {
-    cfg.numAttrs = 2;
-    cudaError_t e = cudaLaunchKernelEx(&cfg, kern, P);
-    if (e == cudaSuccess) { coop = 1; return DMUON_OK; }
-    if (coop == 1) { set_error("cudaLaunchKernelEx(ns_program_kernel) failed: %s", cudaGetErrorString(e)); return DMUON_ERR_CUDA; }
-    cudaGetLastError();
-    coop = 0;
-  }
   cfg.numAttrs = 1;
   DMUON_CUDA_CHECK(cudaLaunchKernelEx(&cfg, kern, P));
   return DMUON_OK;

@@ -131,7 +131,7 @@ def test_deterministic_without_kept_output():
 
 
 def test_cuda_graph_replay():
-    """The program launch (a memset of the completion counters + one cooperative cluster launch) can be captured into a
+    """The program launch (a memset of the completion counters + one cluster launch) can be captured into a
     CUDA graph; the replay equals the eager step bit for bit."""
     dm.set_option("keep_ns_output", 0)
     shapes, W, G, M = synth.muon_inputs(2, "cuda", True, indices=list(range(12)))
