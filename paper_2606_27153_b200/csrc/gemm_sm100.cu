@@ -13,21 +13,28 @@
 // of the new X; or, for the LAST update of a call, the Muon update itself W' = W - lr (scale O + wd W) (Eq. 1
 // PAPER.md:51) on bf16 weights or on fp32 master weights, or the bf16 NS output of dmuon_ns_batched.
 //
-// Two tilings of one warp-specialised pipeline (warp 0 = TMA producer, warp 1 = tcgen05.mma issuer and TMEM owner,
-// warps 2..5 = epilogue: TMEM -> registers -> shared-memory tile -> global):
+// Three tilings of one warp-specialised pipeline (warp 0 = TMA producer, warp 1 = tcgen05.mma issuer and TMEM owner,
+// then the epilogue warps: TMEM -> registers -> shared-memory tile -> bulk tensor store):
 //
-//   single CTA  (cta_group::1)  one CTA per SM computes a 128 x 128 or 128 x 256 unit; 4-stage ring of 48 KB.
+//   single CTA  (cta_group::1)  one CTA per SM computes a 128 x 128 or 128 x 256 unit; 3-stage ring of 48 KB.
 //   CTA pair    (cta_group::2)  a cluster of two CTAs (one TPC) computes a 256 x 256 unit with UMMA M = 256, N = 256:
 //                               each CTA stages its 128 rows of operand A and its 128 columns of operand B (32 KB per
-//                               stage, 6 stages) and holds its 128 accumulator rows in its own TMEM, so a unit moves
+//                               stage, 5 stages) and holds its 128 accumulator rows in its own TMEM, so a unit moves
 //                               2/3 of the L2->SMEM bytes per FLOP of the single-CTA tiling.  The leader CTA issues the
 //                               MMAs; both producers signal the leader's "full" barrier; tcgen05.commit multicasts the
 //                               "slot free" and "accumulator ready" arrivals to both CTAs.
+//   CTA pair, 8 epilogue warps  two warps per TMEM lane quarter take alternate 32-column chunks (short contractions,
+//                               where the epilogue sets the pace); 4 stages.
 //
 // Operands are fp16, 128-byte-swizzled tiles moved by cp.async.bulk.tensor; accumulators are fp32 in TMEM, two
 // of them (2 x 256 columns) so the epilogue of one unit overlaps the mainloop of the next.  The symmetric ops visit
 // only upper-triangular blocks and store each off-diagonal 128 x 128 block twice (direct and mirrored), so the dense
 // output later steps need is kept.
+//
+// Two kinds of kernels are built from the same role functions (produce_phase / mma_phase / epilogue_phase): one
+// product per launch (ns_*_kernel, any tiling), and the PROGRAM kernel (ns_program_kernel, CTA pair): every product
+// of a bucket's NS program in one launch, chained by per-matrix completion counters, the matrices taken in groups
+// sized to the L2 (see "program kernel" below).
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
