@@ -120,7 +120,7 @@ struct ProgLaunch {
   int count = 0;                // matrices (slots 0 .. count - 1)
   int group = 1;                // matrices per L2-resident group
   int m_blocks = 0, n_blocks = 0;   // oriented padded shape in 128-blocks
-  uint32_t* done = nullptr;     // device [count] completion counters (zeroed by the launcher)
+  uint32_t* done = nullptr;     // device [count + 1]: completion counters and the unit queue (zeroed by the launcher)
   float lr = 0.f, lrwd = 0.f;
   bool store_c = true;
   int grid = 148;

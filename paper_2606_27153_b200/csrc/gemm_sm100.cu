@@ -53,6 +53,7 @@ constexpr int kMaxEpiWarps = 8;
 constexpr int kTmemCols = 512;
 constexpr int kAccCols = 256;                   // columns per accumulator stage
 constexpr int kMaxStages = 6;
+constexpr int kSchedDepth = 4;                  // program kernel: unit indices the scheduler may run ahead of its readers
 #ifndef DMUON_EPI_SLEEP_NS
 #define DMUON_EPI_SLEEP_NS 256                  // back-off of the epilogue warps' accumulator wait (0 = plain polling)
 #endif
@@ -94,11 +95,14 @@ struct SmemCtl {
   uint64_t empty[kMaxStages];
   uint64_t tmem_full[2];
   uint64_t tmem_empty[2];
+  uint64_t sched_full[kSchedDepth];             // program kernel: unit index of slot s published (own barrier)
+  uint64_t sched_empty[kSchedDepth];            // ... and read by every reader of both CTAs (leader's barrier)
+  int32_t sched[kSchedDepth];
   uint64_t addend[kMaxEpiWarps][kEpiAddTiles];     // "addend tile(s) of ring slot s have landed", per epilogue warp
   uint32_t tmem_base;
   uint32_t pad;
 };
-constexpr int kCtlBytes = 512;
+constexpr int kCtlBytes = 640;
 static_assert(sizeof(SmemCtl) <= kCtlBytes, "SmemCtl");
 template <bool kPair, int kEW> constexpr int smem_bytes() {
   return Tiling<kPair, kEW>::kStages * Tiling<kPair, kEW>::kStageBytes + EpiCfg<kEW>::kBytes + kCtlBytes + 1024 /*alignment slack*/;
@@ -318,21 +322,20 @@ __device__ __forceinline__ int first_unit(const Ctx& c, const PhaseArgs& a) {
 }
 
 // ================================================================== TMA producer (one lane; both CTAs of a pair)
+// One unit of a phase; `un` = this worker's next unit of the phase (descriptor prefetch) or a value >= total_units.
 template <int kOp, bool kPair, int kEW>
-__device__ __forceinline__ void produce_phase(const Ctx& c, const PhaseArgs& a, RingState& rs) {
+__device__ __forceinline__ void produce_unit(const Ctx& c, const PhaseArgs& a, int u, int un, RingState& rs) {
   constexpr bool kAMn = op_a_mn(kOp);
   constexpr bool kBMn = op_b_mn(kOp);
   constexpr int kStages = Tiling<kPair, kEW>::kStages;
   constexpr int kStageBytes = Tiling<kPair, kEW>::kStageBytes;
-  int waited = -1;
-  for (int u = first_unit(c, a); u < a.total_units; u += c.num_workers) {
+  {
     const int p = u / a.units_per_problem;
     const TileUnit tu = a.units[u - p * a.units_per_problem];
     const GemmProblem* pr = a.probs + p;
     const uint64_t tmA = reinterpret_cast<uint64_t>(&pr->tmA);
     const uint64_t tmB = reinterpret_cast<uint64_t>(&pr->tmB);
     // the next unit of this worker usually belongs to another matrix: fetch its descriptors ahead of use
-    const int un = u + c.num_workers;
     if (un < a.total_units) {
       const int pn = un / a.units_per_problem;
       if (pn != p) {
@@ -340,7 +343,7 @@ __device__ __forceinline__ void produce_phase(const Ctx& c, const PhaseArgs& a, 
         tma_prefetch_desc(reinterpret_cast<uint64_t>(&a.probs[pn].tmB));
       }
     }
-    if (a.done && a.need && waited != p) { wait_done(a.done + pr->rec, a.need); waited = p; }
+    if (a.done && a.need) wait_done(a.done + pr->rec, a.need);
     const int a_blk = kPair ? 2 * tu.m_blk + static_cast<int>(c.rank) : tu.m_blk;      // this CTA's 128 rows of A
     const int b_blk = kPair ? 2 * tu.n_blk + static_cast<int>(c.rank) : tu.n_blk;      // its first 128 columns of B
     const int w = kPair ? 1 : tu.width;
@@ -384,16 +387,20 @@ __device__ __forceinline__ void produce_phase(const Ctx& c, const PhaseArgs& a, 
     }
   }
 }
+template <int kOp, bool kPair, int kEW>
+__device__ __forceinline__ void produce_phase(const Ctx& c, const PhaseArgs& a, RingState& rs) {
+  for (int u = first_unit(c, a); u < a.total_units; u += c.num_workers) produce_unit<kOp, kPair, kEW>(c, a, u, u + c.num_workers, rs);
+}
 
 // ================================================================== MMA issuer (one lane; leader CTA only in a pair)
 template <int kOp, bool kPair, int kEW>
-__device__ __forceinline__ void mma_phase(const Ctx& c, const PhaseArgs& a, RingState& rs, int& it) {
+__device__ __forceinline__ void mma_unit(const Ctx& c, const PhaseArgs& a, int u, RingState& rs, int it) {
   constexpr bool kAMn = op_a_mn(kOp);
   constexpr bool kBMn = op_b_mn(kOp);
   constexpr int kCG = kPair ? 2 : 1;
   constexpr int kStages = Tiling<kPair, kEW>::kStages;
   constexpr int kStageBytes = Tiling<kPair, kEW>::kStageBytes;
-  for (int u = first_unit(c, a); u < a.total_units; u += c.num_workers, ++it) {
+  {
     const int p = u / a.units_per_problem;
     const TileUnit tu = a.units[u - p * a.units_per_problem];
     const uint32_t idesc = make_idesc(kPair ? 256 : 128, kPair ? 256 : tu.width * kBlk, kAMn, kBMn);
@@ -421,11 +428,15 @@ __device__ __forceinline__ void mma_phase(const Ctx& c, const PhaseArgs& a, Ring
     if (kPair) mma_commit_pair(c.bar_tfull + 8 * as, 3); else mma_commit(c.bar_tfull + 8 * as);
   }
 }
+template <int kOp, bool kPair, int kEW>
+__device__ __forceinline__ void mma_phase(const Ctx& c, const PhaseArgs& a, RingState& rs, int& it) {
+  for (int u = first_unit(c, a); u < a.total_units; u += c.num_workers, ++it) mma_unit<kOp, kPair, kEW>(c, a, u, rs, it);
+}
 
 // ================================================================== epilogue (kEW warps: TMEM lane quarter warp % 4;
 //                                                                    with two warps per quarter, alternate chunks)
 template <int kOp, bool kPair, int kEpi, int kEW>
-__device__ __forceinline__ void epilogue_phase(const Ctx& c, const PhaseArgs& a, EpiPipe& ep, int& it) {
+__device__ __forceinline__ void epilogue_unit(const Ctx& c, const PhaseArgs& a, int u, EpiPipe& ep, int it) {
   constexpr bool kSym = op_symmetric(kOp);
   constexpr int kSub = EpiCfg<kEW>::kSub;
   constexpr int kRing = op_ring(kOp);
@@ -436,7 +447,7 @@ __device__ __forceinline__ void epilogue_phase(const Ctx& c, const PhaseArgs& a,
   const uint32_t tempty_leader = kPair ? mapa(c.bar_tempty, 0) : c.bar_tempty;
   const Scalars& sc = a.sc;
   ep.issued = ep.consumed = 0;      // every requested addend tile was read by the end of its unit: ring slots restart at 0
-  for (int u = first_unit(c, a); u < a.total_units; u += c.num_workers, ++it) {
+  {
     const int p = u / a.units_per_problem;
     const TileUnit tu = a.units[u - p * a.units_per_problem];
     const GemmProblem* pr = a.probs + p;
@@ -517,7 +528,11 @@ __device__ __forceinline__ void epilogue_phase(const Ctx& c, const PhaseArgs& a,
       }
     }
   }
-  if (a.done && lane == 0) announce_pending(ep, a.done, 0);
+}
+template <int kOp, bool kPair, int kEpi, int kEW>
+__device__ __forceinline__ void epilogue_phase(const Ctx& c, const PhaseArgs& a, EpiPipe& ep, int& it) {
+  for (int u = first_unit(c, a); u < a.total_units; u += c.num_workers, ++it) epilogue_unit<kOp, kPair, kEpi, kEW>(c, a, u, ep, it);
+  if (a.done && c.lane == 0) announce_pending(ep, a.done, 0);
 }
 
 template <bool kPair, int kEW>
@@ -552,6 +567,11 @@ __device__ __forceinline__ Ctx pipeline_setup() {
       mbar_init(c.bar_tempty + 8 * s, kPair ? 2 * kEW : kEW);   // one arrival per epilogue warp (of both CTAs)
     }
     for (int s = 0; s < kEW * kEpiAddTiles; ++s) mbar_init(c.ctl_addr + offsetof(SmemCtl, addend) + 8 * s, 1);
+    for (int s = 0; s < kSchedDepth; ++s) {
+      mbar_init(c.ctl_addr + offsetof(SmemCtl, sched_full) + 8 * s, 1);
+      // readers: the leader's MMA thread and epilogue warps, the peer's producer and epilogue warps
+      mbar_init(c.ctl_addr + offsetof(SmemCtl, sched_empty) + 8 * s, kPair ? 2 + 2 * kEW : 1 + kEW);
+    }
     fence_barrier_init();
   }
   if (c.warp == 1) tmem_alloc<kCG>(c.ctl_addr + offsetof(SmemCtl, tmem_base), kTmemCols);
@@ -664,22 +684,65 @@ struct alignas(16) ProgParams {
   const TileUnit* units[3];
   const MatRec* recs;
   uint32_t* done;
+  uint32_t* queue;          // next unit of the launch's list (dynamic assignment)
   int upp[3];
+  int total_units;
   int num_phases, count, group, rec_base;
   int m_blocks, n_blocks;   // oriented shape in 128-blocks (m <= n)
   float lr, lrwd;
   int store_c;
 };
 
-template <int kOp, int kEpi>
-__device__ __forceinline__ void run_phase(const Ctx& c, const PhaseArgs& a, RingState& rs, int& it, EpiPipe& ep) {
-  if (c.warp == 0) {
-    if (c.lane == 0) produce_phase<kOp, true, 4>(c, a, rs);
-  } else if (c.warp == 1) {
-    if (c.lane == 0 && c.rank == 0) mma_phase<kOp, true, 4>(c, a, rs, it);
-  } else {
-    epilogue_phase<kOp, true, kEpi, 4>(c, a, ep, it);
+// Where unit g of the launch's list lies: group of matrices, product, index inside the product's units of the group.
+struct Cursor { int g0, li, base, tot; };
+__device__ __forceinline__ int phase_tiling(int kind) { return kind == kProgKindGram ? 0 : (kind >= kProgKindX ? 2 : 1); }
+__device__ __forceinline__ int phase_units(const ProgParams& P, int g0, int li) {
+  const int gn = P.count - g0 < P.group ? P.count - g0 : P.group;
+  return gn * P.upp[phase_tiling(P.ph[li].kind)];
+}
+__device__ __forceinline__ void locate(const ProgParams& P, Cursor& cur, int g) {     // g never decreases
+  while (g >= cur.base + cur.tot) {
+    cur.base += cur.tot;
+    if (++cur.li == P.num_phases) { cur.li = 0; cur.g0 += P.group; }
+    cur.tot = phase_units(P, cur.g0, cur.li);
   }
+}
+template <bool kTall>
+__device__ __forceinline__ PhaseArgs phase_args(const ProgParams& P, const Cursor& cur) {
+  const ProgPhase& ph = P.ph[cur.li];
+  const int t = phase_tiling(ph.kind);
+  PhaseArgs a;
+  a.probs = ph.probs + cur.g0;
+  a.units = P.units[t];
+  a.recs = P.recs;
+  a.units_per_problem = P.upp[t];
+  a.total_units = cur.tot;
+  a.k_blocks = (t == 0 ? P.n_blocks : P.m_blocks) * (kBlk / kBlkK);
+  a.mb = (t == 2 && kTall) ? P.n_blocks : P.m_blocks;
+  a.nb = (t == 2 && !kTall) ? P.n_blocks : P.m_blocks;
+  a.sc = Scalars{ph.alpha, ph.beta, ph.beta2, P.lr, P.lrwd, ph.kind == kProgKindXFinal ? P.store_c : 1, P.rec_base};
+  a.first = 0;
+  a.done = P.done;
+  a.need = ph.need;
+  return a;
+}
+
+// Dynamic unit assignment: the leader's producer thread takes the next index of the launch's list from a global
+// counter and publishes it to every role of both CTAs through a small ring in shared memory.  Units are handed out in
+// list order to CTAs that are RUNNING, and a unit waits only for units earlier in the list, so the walk cannot
+// deadlock even when other kernels keep some of this grid's CTAs from becoming resident (with a fixed assignment the
+// resident CTAs would wait for units of CTAs that never start).
+struct SchedReader { uint32_t n; uint32_t full, empty_leader, data; };
+template <bool kClusterAcquire>
+__device__ __forceinline__ int sched_read(SchedReader& r, bool arrive) {
+  const uint32_t s = r.n % kSchedDepth;
+  if (kClusterAcquire) mbar_wait_cluster(r.full + 8 * s, (r.n / kSchedDepth) & 1);
+  else mbar_wait(r.full + 8 * s, (r.n / kSchedDepth) & 1);
+  int g;
+  asm volatile("ld.shared.s32 %0, [%1];" : "=r"(g) : "r"(r.data + 4 * s) : "memory");
+  if (arrive) mbar_arrive_cluster(r.empty_leader + 8 * s);
+  ++r.n;
+  return g;
 }
 
 template <bool kTall, int kFinalEpi>
@@ -687,40 +750,90 @@ __global__ void __launch_bounds__(EpiCfg<4>::kThreads, 1) ns_program_kernel(cons
   constexpr int kGram = kTall ? OP_SYRK_T : OP_SYRK;
   constexpr int kX = kTall ? OP_XB : OP_BX;
   const Ctx c = pipeline_setup<true, 4>();
-  RingState rs{0, 0};
-  int it = 0;
-  EpiPipe ep = epilogue_pipe<true, 4>(c);
-  int first = 0;
-  for (int g0 = 0; g0 < P.count; g0 += P.group) {
-    const int gn = P.count - g0 < P.group ? P.count - g0 : P.group;
-    for (int li = 0; li < P.num_phases; ++li) {
-      const ProgPhase& ph = P.ph[li];
-      const int t = ph.kind == kProgKindGram ? 0 : (ph.kind >= kProgKindX ? 2 : 1);
-      PhaseArgs a;
-      a.probs = ph.probs + g0;
-      a.units = P.units[t];
-      a.recs = P.recs;
-      a.units_per_problem = P.upp[t];
-      a.total_units = gn * P.upp[t];
-      a.k_blocks = (t == 0 ? P.n_blocks : P.m_blocks) * (kBlk / kBlkK);
-      a.mb = (t == 2 && kTall) ? P.n_blocks : P.m_blocks;
-      a.nb = (t == 2 && !kTall) ? P.n_blocks : P.m_blocks;
-      a.sc = Scalars{ph.alpha, ph.beta, ph.beta2, P.lr, P.lrwd, ph.kind == kProgKindXFinal ? P.store_c : 1, P.rec_base};
-      a.first = first;
-      a.done = P.done;
-      a.need = ph.need;
-      switch (ph.kind) {
-        case kProgKindGram: run_phase<kGram, EPI_F16>(c, a, rs, it, ep); break;
-        case kProgKindSq: run_phase<OP_SQ, EPI_F16>(c, a, rs, it, ep); break;
-        case kProgKindSq2: run_phase<OP_SQ2, EPI_F16>(c, a, rs, it, ep); break;
-        case kProgKindX: run_phase<kX, EPI_F16>(c, a, rs, it, ep); break;
-        default: run_phase<kX, kFinalEpi>(c, a, rs, it, ep); break;
+  const uint32_t bar_sfull = c.ctl_addr + offsetof(SmemCtl, sched_full);
+  const uint32_t bar_sempty = c.ctl_addr + offsetof(SmemCtl, sched_empty);
+  const uint32_t sdata = c.ctl_addr + offsetof(SmemCtl, sched);
+  Cursor cur{0, 0, 0, phase_units(P, 0, 0)};
+  SchedReader rd{0u, bar_sfull, mapa(bar_sempty, 0), sdata};
+  if (c.warp == 0) {
+    if (c.lane == 0) {
+      RingState rs{0, 0};
+      const uint32_t peer_full = mapa(bar_sfull, 1), peer_data = mapa(sdata, 1);
+      uint32_t n = 0;
+      while (true) {
+        int g;
+        if (c.rank == 0) {
+          // scheduler: next unit of the list for this CTA pair
+          const uint32_t s = n % kSchedDepth;
+          mbar_wait(bar_sempty + 8 * s, ((n / kSchedDepth) & 1) ^ 1);
+          const uint32_t got = atomicAdd(P.queue, 1u);
+          g = got < static_cast<uint32_t>(P.total_units) ? static_cast<int>(got) : -1;
+          asm volatile("st.shared.s32 [%0], %1;" ::"r"(sdata + 4 * s), "r"(g) : "memory");
+          asm volatile("st.shared::cluster.s32 [%0], %1;" ::"r"(peer_data + 4 * s), "r"(g) : "memory");
+          mbar_arrive(bar_sfull + 8 * s);
+          mbar_arrive_cluster(peer_full + 8 * s);
+          ++n;
+        } else {
+          g = sched_read<true>(rd, true);
+        }
+        if (g < 0) break;
+        locate(P, cur, g);
+        const PhaseArgs a = phase_args<kTall>(P, cur);
+        const int u = g - cur.base;
+        switch (P.ph[cur.li].kind) {
+          case kProgKindGram: produce_unit<kGram, true, 4>(c, a, u, a.total_units, rs); break;
+          case kProgKindSq: produce_unit<OP_SQ, true, 4>(c, a, u, a.total_units, rs); break;
+          case kProgKindSq2: produce_unit<OP_SQ2, true, 4>(c, a, u, a.total_units, rs); break;
+          default: produce_unit<kX, true, 4>(c, a, u, a.total_units, rs); break;
+        }
       }
-      first += a.total_units;
     }
+    __syncwarp();
+  } else if (c.warp == 1) {
+    if (c.lane == 0 && c.rank == 0) {
+      RingState rs{0, 0};
+      for (int it = 0;; ++it) {
+        const int g = sched_read<false>(rd, true);
+        if (g < 0) break;
+        locate(P, cur, g);
+        const PhaseArgs a = phase_args<kTall>(P, cur);
+        const int u = g - cur.base;
+        switch (P.ph[cur.li].kind) {
+          case kProgKindGram: mma_unit<kGram, true, 4>(c, a, u, rs, it); break;
+          case kProgKindSq: mma_unit<OP_SQ, true, 4>(c, a, u, rs, it); break;
+          case kProgKindSq2: mma_unit<OP_SQ2, true, 4>(c, a, u, rs, it); break;
+          default: mma_unit<kX, true, 4>(c, a, u, rs, it); break;
+        }
+      }
+    }
+    __syncwarp();
+  } else {
+    EpiPipe ep = epilogue_pipe<true, 4>(c);
+    for (int it = 0;; ++it) {
+      // (never block with an unannounced unit)
+      if (c.lane == 0 && ep.pend >= 0 && !mbar_try_wait(rd.full + 8 * (rd.n % kSchedDepth), (rd.n / kSchedDepth) & 1))
+        announce_pending(ep, P.done, 0);
+      const int g = c.rank == 0 ? sched_read<false>(rd, false) : sched_read<true>(rd, false);
+      __syncwarp();                                   // every lane has read the slot
+      if (c.lane == 0) mbar_arrive_cluster(rd.empty_leader + 8 * ((rd.n - 1) % kSchedDepth));
+      if (g < 0) break;
+      locate(P, cur, g);
+      const PhaseArgs a = phase_args<kTall>(P, cur);
+      const int u = g - cur.base;
+      switch (P.ph[cur.li].kind) {
+        case kProgKindGram: epilogue_unit<kGram, true, EPI_F16, 4>(c, a, u, ep, it); break;
+        case kProgKindSq: epilogue_unit<OP_SQ, true, EPI_F16, 4>(c, a, u, ep, it); break;
+        case kProgKindSq2: epilogue_unit<OP_SQ2, true, EPI_F16, 4>(c, a, u, ep, it); break;
+        case kProgKindX: epilogue_unit<kX, true, EPI_F16, 4>(c, a, u, ep, it); break;
+        default: epilogue_unit<kX, true, kFinalEpi, 4>(c, a, u, ep, it); break;
+      }
+    }
+    if (c.lane == 0) {
+      announce_pending(ep, P.done, 0);
+      bulk_wait_all();
+    }
+    __syncwarp();
   }
-  if (c.warp >= 2 && c.lane == 0) bulk_wait_all();
-  __syncwarp();
   pipeline_teardown<true>(c);
 }
 
@@ -844,6 +957,14 @@ int launch_ns_program(const ProgLaunch& L, cudaStream_t stream) {
   for (int t = 0; t < 3; ++t) { P.units[t] = L.units[t]; P.upp[t] = L.upp[t]; }
   P.recs = L.recs;
   P.done = L.done;
+  P.queue = L.done + L.count;
+  {
+    long total = 0;
+    for (int li = 0; li < L.num_phases; ++li) total += L.upp[P.ph[li].kind == kProgKindGram ? 0 : (P.ph[li].kind >= kProgKindX ? 2 : 1)];
+    total *= L.count;
+    if (total > 0x7fffff00L) { set_error("launch_ns_program: %ld work units", total); return DMUON_ERR_INVALID_ARG; }
+    P.total_units = static_cast<int>(total);
+  }
   P.num_phases = L.num_phases;
   P.count = L.count;
   P.group = L.group;
@@ -853,7 +974,7 @@ int launch_ns_program(const ProgLaunch& L, cudaStream_t stream) {
   P.lr = L.lr;
   P.lrwd = L.lrwd;
   P.store_c = L.store_c ? 1 : 0;
-  DMUON_CUDA_CHECK(cudaMemsetAsync(L.done, 0, sizeof(uint32_t) * L.count, stream));
+  DMUON_CUDA_CHECK(cudaMemsetAsync(L.done, 0, sizeof(uint32_t) * (L.count + 1), stream));   // counters + the unit queue
   const int max_units = L.group * (L.upp[0] > L.upp[2] ? L.upp[0] : L.upp[2]);
   const int workers = L.grid / 2 < max_units ? L.grid / 2 : max_units;
   cudaLaunchConfig_t cfg = {};

@@ -737,7 +737,7 @@ int get_plan(const int32_t* shapes, int count, const Options& opt, void* ext_ws,
           st.prog_upp[t] = static_cast<int>(hu.size());
           if ((rc = upload(p, &st.prog_units[t], hu))) return rc;
         }
-        if ((rc = dev_alloc(p, &st.d_done, static_cast<size_t>(st.slots)))) return rc;
+        if ((rc = dev_alloc(p, &st.d_done, static_cast<size_t>(st.slots) + 1))) return rc;     // + the unit queue
       }
     }
     if (scratch_ready) DMUON_CUDA_CHECK(cudaMemsetAsync(p.ws, 0, p.ws_bytes, stream));

@@ -172,3 +172,23 @@ def test_hostile_spectra_at_the_auto_threshold():
         e = rel_fro(to64(dm.binding.read_ns_output(i, shape)), oracle.ns(X64[i]))
         print(f"program kernel, hostile {shape} {name}: {e:.2e}")
         assert e <= TOL_TC, f"{name}: {e:.3e}"
+
+
+def test_shares_the_gpu_with_other_kernels():
+    """Units are handed out dynamically to the CTA pairs that are running, so the program kernel makes progress (and
+    computes the same bits) while another stream keeps part of the GPU busy and some of its CTAs wait to become resident."""
+    dm.set_option("keep_ns_output", 0)
+    shape = (2048, 4096)
+    X0 = [synth.iid_normal(shape, SEED + 7000 + i, "cuda") for i in range(8)]
+    quiet = [x.clone() for x in X0]
+    dm.ns_batched(quiet, steps=5)
+    torch.cuda.synchronize()
+    busy = [x.clone() for x in X0]
+    a = torch.randn((8192, 8192), device="cuda", dtype=torch.bfloat16)
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        for _ in range(40):
+            a @ a                        # library GEMMs on another stream: they take SMs away while the step runs
+    dm.ns_batched(busy, steps=5)
+    torch.cuda.synchronize()
+    assert all(torch.equal(p, q) for p, q in zip(quiet, busy))
