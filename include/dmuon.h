@@ -194,8 +194,8 @@ DMUON_API int dmuon_set_workspace(void* dev_ptr, size_t bytes);
  *                 buffers fit the L2 ("l2_group_mb").  "auto" = buckets whose small side is >= 2048 (there it is 5-10 %
  *                 faster: fewer DRAM bytes, more clock under the power cap); "1" = every bucket with a small side
  *                 >= 256 and <= 32 products; "0" = one launch per product everywhere.  Same arithmetic either way
- *                 (the CTAs of that launch wait for one another and must all be resident: a step should have the GPU
- *                 to itself -- no other kernels on other streams while it runs -- or use "0")
+ *                 (work units are handed out dynamically to the CTAs that are running, so the launch also makes progress
+ *                 while kernels of other streams occupy part of the GPU)
  *   "l2_group_mb" budget for the buffers of one group of matrices in the program kernel, MiB (default "64"; a group is
  *                 never smaller than three waves of work units)
  *   "tune_ms"     autotune: milliseconds each candidate runs back to back (default "40": long enough for the

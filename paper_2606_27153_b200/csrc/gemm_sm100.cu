@@ -663,14 +663,15 @@ DMUON_GEMM_ENTRIES(ns_xb_apply_master, OP_XB, EPI_APPLY_MASTER)
 #undef DMUON_GEMM_ENTRY
 
 // ------------------------------------------------------------------------------------------------ program kernel
-// ALL products of a bucket's NS program in ONE launch ("grouped by shape and advanced together"): every
-// CTA pair walks the same list -- for each group of matrices, for each product of the program, the units of that
-// product over the group -- and takes every W-th unit.  A unit of product l of a matrix starts when every unit of
-// product l - 1 of THAT matrix has been stored (per-matrix counters in global memory, bumped by the epilogue warps after
-// their bulk stores completed); nothing else orders the products, so the pipeline never drains between them, there is
-// no launch gap, and a group sized to the L2 keeps its G, B, T, R and X in cache from one product to the next.
-// CTA-pair tiling, 4 epilogue warps.  Deadlock-free because every CTA visits the list in order and a unit only waits
-// for units earlier in the list (all CTAs are resident: grid <= number of SMs, one CTA per SM).
+// ALL products of a bucket's NS program in ONE launch ("grouped by shape and advanced together").  The
+// launch has one list of work units -- for each group of matrices, for each product of the program, the units of that
+// product over the group -- and the CTA pairs take its entries in order from a global counter.  A unit of product l of
+// a matrix starts when every unit of product l - 1 of THAT matrix has been stored (per-matrix counters in global
+// memory, bumped by the epilogue warps after their bulk stores completed); nothing else orders the products, so the
+// pipeline never drains between them, there is no launch gap, and a group sized to the L2 keeps its G, B, T, R in
+// cache from one product to the next -- which is what pays: fewer DRAM bytes, more clock under the power cap.
+// CTA-pair tiling, 4 epilogue warps.  Deadlock-free: units are handed to RUNNING CTAs in list order and a unit only
+// waits for units earlier in the list.
 constexpr int kProgKindGram = 0, kProgKindSq = 1, kProgKindSq2 = 2, kProgKindX = 3, kProgKindXFinal = 4;
 struct ProgPhase {
   const GemmProblem* probs;
@@ -987,9 +988,6 @@ int launch_ns_program(const ProgLaunch& L, cudaStream_t stream) {
   attr[0].val.clusterDim.x = 2;
   attr[0].val.clusterDim.y = 1;
   attr[0].val.clusterDim.z = 1;
-  // Units wait for units of other CTAs, so every CTA of the grid must be resident at once: grid <= one CTA per SM, and
-  // the step has the GPU to itself (dmuon.h).  (A cooperative launch would make the driver guarantee it, but Nsight
-  // Compute fails such a launch when it is combined with a cluster dimension: LaunchFailed under ncu, measured.)
   cfg.attrs = attr;
   cfg.numAttrs = 1;
   DMUON_CUDA_CHECK(cudaLaunchKernelEx(&cfg, kern, P));
