@@ -760,24 +760,7 @@ __global__ void __launch_bounds__(EpiCfg<4>::kThreads, 1) ns_program_kernel(cons
     if (c.lane == 0) {
       RingState rs{0, 0};
       const uint32_t peer_full = mapa(bar_sfull, 1), peer_data = mapa(sdata, 1);
-      uint32_t n = 0;
-      while (true) {
-        int g;
-        if (c.rank == 0) {
-          // scheduler: next unit of the list for this CTA pair
-          const uint32_t s = n % kSchedDepth;
-          mbar_wait(bar_sempty + 8 * s, ((n / kSchedDepth) & 1) ^ 1);
-          const uint32_t got = atomicAdd(P.queue, 1u);
-          g = got < static_cast<uint32_t>(P.total_units) ? static_cast<int>(got) : -1;
-          asm volatile("st.shared.s32 [%0], %1;" ::"r"(sdata + 4 * s), "r"(g) : "memory");
-          asm volatile("st.shared::cluster.s32 [%0], %1;" ::"r"(peer_data + 4 * s), "r"(g) : "memory");
-          mbar_arrive(bar_sfull + 8 * s);
-          mbar_arrive_cluster(peer_full + 8 * s);
-          ++n;
-        } else {
-          g = sched_read<true>(rd, true);
-        }
-        if (g < 0) break;
+      auto produce = [&](int g) {
         locate(P, cur, g);
         const PhaseArgs a = phase_args<kTall>(P, cur);
         const int u = g - cur.base;
@@ -786,6 +769,46 @@ __global__ void __launch_bounds__(EpiCfg<4>::kThreads, 1) ns_program_kernel(cons
           case kProgKindSq: produce_unit<OP_SQ, true, 4>(c, a, u, a.total_units, rs); break;
           case kProgKindSq2: produce_unit<OP_SQ2, true, 4>(c, a, u, a.total_units, rs); break;
           default: produce_unit<kX, true, 4>(c, a, u, a.total_units, rs); break;
+        }
+      };
+      if (c.rank == 0) {
+        // scheduler: takes the next unit of the list for this CTA pair and publishes it to every role of both CTAs
+        uint32_t n = 0;
+        auto publish = [&](int g) {
+          const uint32_t s = n % kSchedDepth;
+          mbar_wait(bar_sempty + 8 * s, ((n / kSchedDepth) & 1) ^ 1);
+          asm volatile("st.shared.s32 [%0], %1;" ::"r"(sdata + 4 * s), "r"(g) : "memory");
+          asm volatile("st.shared::cluster.s32 [%0], %1;" ::"r"(peer_data + 4 * s), "r"(g) : "memory");
+          mbar_arrive(bar_sfull + 8 * s);
+          mbar_arrive_cluster(peer_full + 8 * s);
+          ++n;
+        };
+        const uint32_t total = static_cast<uint32_t>(P.total_units);
+        uint32_t got = atomicAdd(P.queue, 1u);
+        int g = got < total ? static_cast<int>(got) : -1;
+        publish(g);
+        while (g >= 0) {
+          // the next index is requested before this unit's loads go out and used after them: the round trip of the
+          // atomic (~1 us) is off the producer's critical path
+          got = atomicAdd(P.queue, 1u);
+          produce(g);
+          g = got < total ? static_cast<int>(got) : -1;
+          publish(g);
+          if (g >= 0) {
+            // descriptors of the next unit's problem, ahead of its first load
+            Cursor nx = cur;
+            locate(P, nx, g);
+            const int t = phase_tiling(P.ph[nx.li].kind);
+            const GemmProblem* pr = P.ph[nx.li].probs + nx.g0 + (g - nx.base) / P.upp[t];
+            tma_prefetch_desc(reinterpret_cast<uint64_t>(&pr->tmA));
+            tma_prefetch_desc(reinterpret_cast<uint64_t>(&pr->tmB));
+          }
+        }
+      } else {
+        while (true) {
+          const int g = sched_read<true>(rd, true);
+          if (g < 0) break;
+          produce(g);
         }
       }
     }
