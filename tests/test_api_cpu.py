@@ -40,6 +40,14 @@ def test_options_validation():
     dm.set_option("keep_ns_output", "0")
     dm.set_option("chunk_mb", "12288")
     dm.set_option("tune_ms", "40")
+    for v in ("0", "1", "auto"):
+        dm.set_option("program", v)                 # one launch per bucket's NS program: never / always / from 2048 rows up
+    dm.set_option("l2_group_mb", "64")
+    dm.set_option("small_fused", "1")
+    for key, val in (("program", "2"), ("program", "yes"), ("l2_group_mb", "0"), ("l2_group_mb", "x"), ("small_fused", "2")):
+        with pytest.raises(dm.DmuonError) as ei:
+            dm.set_option(key, val)
+        assert ei.value.code == binding.ERR_INVALID_ARG
     for key, val in (("steps", "-1"), ("steps", "abc"), ("coeffs", "1,2"), ("mode", "bogus"), ("nope", "1"),
                      ("autotune", "maybe"), ("schedule", "gram"), ("coeffs_sched", "1,2;3"), ("coeffs_sched", "1,2,3/4,5,6"),
                      ("chunk_mb", "0"), ("tune_ms", "-1"), ("fuse_epilogue", "2"), ("overlap", "1")):
