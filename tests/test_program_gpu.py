@@ -192,3 +192,36 @@ def test_shares_the_gpu_with_other_kernels():
     dm.ns_batched(busy, steps=5)
     torch.cuda.synchronize()
     assert all(torch.equal(p, q) for p, q in zip(quiet, busy))
+
+
+def test_same_bits_as_separate_launches_at_full_size():
+    """The shapes of config 4 that `auto` sends through the program kernel (4096-row buckets: groups of 2 matrices, 18 or 15
+    products per launch): W' and M' are the SAME BITS as with one launch per product (same tiles, same arithmetic; only
+    the order in time differs), and five repetitions -- two of them next to another stream's GEMMs -- never differ."""
+    dm.set_option("keep_ns_output", 0)
+    dm.set_option("program", "auto")
+    shapes = [(4096, 14336)] * 3 + [(14336, 4096)] * 3 + [(4096, 4096)] * 4
+    G = [synth.gradient(s, SEED + 9000 + i, "cuda") for i, s in enumerate(shapes)]
+    W0 = [synth.weight(s, SEED + 9100 + i, "cuda") for i, s in enumerate(shapes)]
+    M0 = [synth.gradient(s, SEED + 9200 + i, "cuda") for i, s in enumerate(shapes)]
+    assert all(b["program"] for b in dm.describe_plan(shapes, 5)["buckets"])
+    a = torch.randn((4096, 4096), device="cuda", dtype=torch.bfloat16)
+    side = torch.cuda.Stream()
+    ref = None
+    for it in range(5):
+        W, M = [w.clone() for w in W0], [m.clone() for m in M0]
+        if it in (2, 4):
+            with torch.cuda.stream(side):
+                for _ in range(30):
+                    a @ a
+        dm.muon_step(W, G, M, LR, MU, WD)
+        torch.cuda.synchronize()
+        if ref is None:
+            ref = (W, M)
+        else:
+            assert all(torch.equal(x, y) for x, y in zip(ref[0] + ref[1], W + M)), f"repetition {it} differs"
+    dm.set_option("program", 0)
+    W, M = [w.clone() for w in W0], [m.clone() for m in M0]
+    dm.muon_step(W, G, M, LR, MU, WD)
+    torch.cuda.synchronize()
+    assert all(torch.equal(x, y) for x, y in zip(ref[0] + ref[1], W + M)), "program kernel and separate launches differ"
