@@ -225,3 +225,35 @@ def test_same_bits_as_separate_launches_at_full_size():
     dm.muon_step(W, G, M, LR, MU, WD)
     torch.cuda.synchronize()
     assert all(torch.equal(x, y) for x, y in zip(ref[0] + ref[1], W + M)), "program kernel and separate launches differ"
+
+
+def test_master_weights_and_per_step_schedule():
+    """The other final epilogues and coefficient paths of the program kernel: fp32 master weights (EPI_APPLY_MASTER) and a
+    per-step coefficient schedule (option coeffs_sched), against the oracle."""
+    sched = [(4.0848, -6.8946, 2.9270), (3.9505, -6.3029, 2.6377), (3.7418, -5.5913, 2.3037), (2.8769, -3.1427, 1.2046),
+             (2.8366, -3.0525, 1.2012)]
+    shapes = [(512, 1536), (1536, 512), (768, 768)]
+    W = [synth.weight(s, SEED + 9500 + i, "cuda") for i, s in enumerate(shapes)]
+    G = [synth.gradient(s, SEED + 9600 + i, "cuda") for i, s in enumerate(shapes)]
+    M = [synth.gradient(s, SEED + 9700 + i, "cuda") for i, s in enumerate(shapes)]
+    masters = [w.to(torch.float32) + 1e-4 * torch.randn_like(w, dtype=torch.float32) for w in W]
+    P0, G0, M0 = [to64(p) for p in masters], [to64(g) for g in G], [to64(m) for m in M]
+    assert all(b["program"] for b in dm.describe_plan(shapes, 5)["buckets"])
+    dm.muon_step_master(W, masters, G, M, LR, MU, WD)
+    torch.cuda.synchronize()
+    for i in range(len(shapes)):
+        orc = oracle.muon_step(P0[i], G0[i], M0[i], LR_F, MU_F, WD_F)
+        assert torch.equal(W[i], masters[i].to(torch.bfloat16)), "bf16 parameter = RNE of the new master"
+        upd, upd_orc = to64(masters[i]) - P0[i], orc["W_new"] - P0[i]
+        assert np.linalg.norm(upd - upd_orc) <= (TOL_TC + 1e-4) * np.linalg.norm(upd_orc)
+    # per-step schedule through the Muon-step entry point
+    dm.set_option("coeffs_sched", ";".join(",".join(str(v) for v in row) for row in sched))
+    W = [synth.weight(s, SEED + 9500 + i, "cuda") for i, s in enumerate(shapes)]
+    M = [synth.gradient(s, SEED + 9700 + i, "cuda") for i, s in enumerate(shapes)]
+    W0 = [to64(w) for w in W]
+    dm.muon_step(W, G, M, LR, MU, WD)
+    torch.cuda.synchronize()
+    for i, s in enumerate(shapes):
+        orc = oracle.muon_step(W0[i], G0[i], M0[i], LR_F, MU_F, WD_F, coeffs=sched)
+        e = rel_fro(to64(dm.binding.read_ns_output(i, s)), orc["O"])
+        assert e <= TOL_TC, f"per-step schedule, matrix {i} {s}: {e:.3e}"
