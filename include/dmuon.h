@@ -127,6 +127,38 @@ DMUON_API int dmuon_adamw_step(void* const* params, const void* const* grads, vo
                                float beta2, float eps, float wd, int32_t step, dmuon_stream_t stream);
 
 /*
+ * dmuon_adamw_step for callers that cannot allocate device memory.
+ *
+ * Who that is: an optimizer step that runs inside a training process whose framework allocator has already taken
+ * (nearly) all of the GPU's memory for its own pool, so a raw cudaMalloc from a library fails although the framework
+ * could still hand out tensors; a step issued while collectives of another stream are in flight, where cudaMalloc and
+ * cudaFree are unwelcome because they synchronise the whole device; and tight loops that cannot afford that
+ * synchronisation at all.  dmuon_adamw_step allocates its per-call work table (one record per tensor) with cudaMalloc
+ * whenever the tensor list changes.  This entry point never does: the table lives in a fixed array that is part of the
+ * library's device image, 192 KiB on every GPU that has loaded libdmuon, held until the process exits.
+ *
+ * Arguments, arithmetic and results are those of dmuon_adamw_step (same kernel; results are bitwise equal).  Differences:
+ *   - count must be <= DMUON_ADAMW_NOALLOC_MAX_TENSORS, else DMUON_ERR_INVALID_ARG and nothing is enqueued.  Longer
+ *     lists: several calls on one stream.
+ *   - no cudaMalloc, cudaFree, cudaMallocHost or other allocating routine is called, on any call.
+ *   - the FIRST call on each device looks up the array's address on that device (cudaGetSymbolAddress, with the
+ *     caller's current device) and remembers it.  Make that first call during start-up, on the device you will use and
+ *     before any stream capture begins.
+ *   - the table is uploaded from host memory at every call (two small asynchronous copies on `stream` ahead of the kernel), so the
+ *     call may wait for earlier work of `stream` to drain before it returns; everything it enqueues is ordered on `stream`.
+ *   - ALL calls on a device share the one array.  Each call rewrites every table entry its kernel reads, so nothing
+ *     from an earlier call is reused and nothing needs clearing; but two calls whose GPU work can overlap (different
+ *     streams without an event between them) race on the table and may update the wrong tensors.  Keep the calls of a
+ *     device on one stream, or order the streams yourself.
+ *   - launches are not recorded by the "profile" option.
+ */
+#define DMUON_ADAMW_NOALLOC_MAX_TENSORS 4096
+DMUON_API int dmuon_adamw_step_noalloc(void* const* params, const void* const* grads, void* const* exp_avg,
+                                       void* const* exp_avg_sq, const int64_t* numel, int32_t count, float lr,
+                                       float beta1, float beta2, float eps, float wd, int32_t step,
+                                       dmuon_stream_t stream);
+
+/*
  * c_{s,b} of PAPER.md:194: the measured time (ms) of the owner-local Muon update of ONE batch of `batch` matrices of
  * shape rows x cols "including the complete execution path selected by the runtime" (bucketing, tuned tile
  * configurations, block schedule, fused epilogue), averaged over `reps` steps after two warm-up steps.  Runs on

@@ -26,7 +26,7 @@ SYMBOLS = ("dmuon_ns_batched", "dmuon_ns_batched_sched", "dmuon_muon_step", "dmu
            "dmuon_workspace_bytes", "dmuon_set_workspace", "dmuon_set_option", "dmuon_last_error",
            "dmuon_profile_read", "dmuon_profile_reset", "dmuon_ns_gemm", "dmuon_ns_gemm_variants", "dmuon_read_ns_output", "dmuon_shutdown",
            "dmuon_version", "dmuon_describe_plan", "dmuon_ns_sym_mm", "dmuon_block_schedule", "dmuon_muon_step_master",
-           "dmuon_adamw_step", "dmuon_measure_cost", "dmuon_assign_owners")
+           "dmuon_adamw_step", "dmuon_adamw_step_noalloc", "dmuon_measure_cost", "dmuon_assign_owners")
 
 
 class DmuonError(RuntimeError):
@@ -71,6 +71,7 @@ def lib() -> ctypes.CDLL:
         pl = ctypes.POINTER(ctypes.c_int64)
         pd = ctypes.POINTER(ctypes.c_double)
         L.dmuon_adamw_step.argtypes = [pp, pp, pp, pp, pl, i32, f32, f32, f32, f32, f32, i32, vp]
+        L.dmuon_adamw_step_noalloc.argtypes = L.dmuon_adamw_step.argtypes
         L.dmuon_measure_cost.argtypes = [i32, i32, i32, i32, pf, vp]
         L.dmuon_assign_owners.argtypes = [pi, pi, pi, pd, i32, i32, i32, i32, pi, pd]
         L.dmuon_shutdown.restype = None
@@ -309,6 +310,34 @@ def adamw_step(params: Sequence[torch.Tensor], grads: Sequence[torch.Tensor], ex
     _check(lib().dmuon_adamw_step(_ptr_array(params), _ptr_array(grads), _ptr_array(exp_avg), _ptr_array(exp_avg_sq),
                                   numel, n, float(lr), float(beta1), float(beta2), float(eps), float(wd), int(step),
                                   _stream(stream)))
+
+
+ADAMW_NOALLOC_MAX_TENSORS = 4096      # DMUON_ADAMW_NOALLOC_MAX_TENSORS
+
+
+def adamw_step_noalloc(params: Sequence[torch.Tensor], grads: Sequence[torch.Tensor], exp_avg: Sequence[torch.Tensor],
+                       exp_avg_sq: Sequence[torch.Tensor], lr: float, beta1: float, beta2: float, eps: float, wd: float,
+                       step: int, stream=None) -> None:
+    """dmuon_adamw_step_noalloc: adamw_step for processes where the library must not call cudaMalloc (a framework pool
+    owns the GPU's memory, collectives are in flight, or the loop cannot take the device-wide synchronisation).  Same
+    results; at most ADAMW_NOALLOC_MAX_TENSORS tensors per call; the per-call table sits in a fixed 192 KiB array inside
+    the library that every call on the device shares, so keep these calls on one stream.  The first call on a device
+    does a one-time address lookup: make it at start-up."""
+    n = len(params)
+    if not (len(grads) == len(exp_avg) == len(exp_avg_sq) == n):
+        raise ValueError("params, grads, exp_avg, exp_avg_sq must have one length")
+    for i in range(n):
+        p, g, m, v = params[i], grads[i], exp_avg[i], exp_avg_sq[i]
+        if p.dtype != torch.bfloat16 or g.dtype != torch.bfloat16 or m.dtype != torch.float32 or v.dtype != torch.float32:
+            raise ValueError(f"tensor {i}: params/grads must be bfloat16, moments float32")
+        if not (p.is_contiguous() and g.is_contiguous() and m.is_contiguous() and v.is_contiguous()):
+            raise ValueError(f"tensor {i}: tensors must be contiguous")
+        if not (p.numel() == g.numel() == m.numel() == v.numel()) or any(t.device.type != "cuda" for t in (p, g, m, v)):
+            raise ValueError(f"tensor {i}: sizes differ or not on cuda")
+    numel = (ctypes.c_int64 * n)(*[p.numel() for p in params])
+    _check(lib().dmuon_adamw_step_noalloc(_ptr_array(params), _ptr_array(grads), _ptr_array(exp_avg),
+                                          _ptr_array(exp_avg_sq), numel, n, float(lr), float(beta1), float(beta2),
+                                          float(eps), float(wd), int(step), _stream(stream)))
 
 
 def measure_cost(shape: Sequence[int], batch: int, reps: int = 3, stream=None) -> float:

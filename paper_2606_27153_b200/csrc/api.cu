@@ -636,6 +636,42 @@ DMUON_API int dmuon_adamw_step(void* const* params, const void* const* grads, vo
   return launch_adamw(ac.d_recs, ac.d_prefix, count, ac.chunks, sc, stream);
 }
 
+// dmuon_adamw_step for callers that must not touch the CUDA allocator: same kernel, same arithmetic, the work table
+// in the library's static device array (elementwise.cu: launch_adamw_static).  No cudaMalloc / cudaFree / cudaMallocHost
+// and no event creation on this path (the profile option does not record it).
+DMUON_API int dmuon_adamw_step_noalloc(void* const* params, const void* const* grads, void* const* exp_avg,
+                                       void* const* exp_avg_sq, const int64_t* numel, int32_t count, float lr,
+                                       float beta1, float beta2, float eps, float wd, int32_t step,
+                                       dmuon_stream_t stream_) {
+  DMUON_LOCK;
+  static const char* const fn = "dmuon_adamw_step_noalloc";
+  if (count < 0) { set_error("%s: count < 0", fn); return DMUON_ERR_INVALID_ARG; }
+  if (count == 0) return DMUON_OK;
+  if (count > DMUON_ADAMW_NOALLOC_MAX_TENSORS) {
+    set_error("%s: %d tensors in one call, the built-in table holds DMUON_ADAMW_NOALLOC_MAX_TENSORS = %d (split the list, or use dmuon_adamw_step)",
+              fn, count, DMUON_ADAMW_NOALLOC_MAX_TENSORS);
+    return DMUON_ERR_INVALID_ARG;
+  }
+  if (!params || !grads || !exp_avg || !exp_avg_sq || !numel) { set_error("%s: null argument", fn); return DMUON_ERR_INVALID_ARG; }
+  if (step < 1) { set_error("%s: step counts from 1 (got %d)", fn, step); return DMUON_ERR_INVALID_ARG; }
+  if (!(beta1 >= 0.f && beta1 < 1.f) || !(beta2 >= 0.f && beta2 < 1.f) || !(eps >= 0.f)) { set_error("%s: beta1, beta2 must be in [0, 1), eps >= 0", fn); return DMUON_ERR_INVALID_ARG; }
+  for (int i = 0; i < count; ++i) {
+    if (numel[i] <= 0) { set_error("%s: tensor %d has %lld elements", fn, i, static_cast<long long>(numel[i])); return DMUON_ERR_INVALID_ARG; }
+    const void* ptrs[4] = {params[i], grads[i], exp_avg[i], exp_avg_sq[i]};
+    for (const void* p : ptrs) {
+      if (!p) { set_error("%s: tensor %d has a null pointer", fn, i); return DMUON_ERR_INVALID_ARG; }
+      if (reinterpret_cast<uintptr_t>(p) & 15) { set_error("%s: tensor %d pointer %p is not 16-byte aligned", fn, i, p); return DMUON_ERR_INVALID_ARG; }
+    }
+  }
+  int rc = check_device();
+  if (rc) return rc;
+  AdamScalars sc;
+  sc.lr = lr; sc.beta1 = beta1; sc.beta2 = beta2; sc.eps = eps; sc.wd = wd;
+  sc.inv_bc1 = static_cast<float>(1.0 / (1.0 - std::pow(static_cast<double>(beta1), step)));
+  sc.inv_sqrt_bc2 = static_cast<float>(1.0 / std::sqrt(1.0 - std::pow(static_cast<double>(beta2), step)));
+  return launch_adamw_static(params, grads, exp_avg, exp_avg_sq, numel, count, sc, reinterpret_cast<cudaStream_t>(stream_));
+}
+
 DMUON_API int dmuon_warmup(const int32_t* shapes, int32_t count, dmuon_stream_t stream) {
   DMUON_LOCK;
   if (count < 0 || (count > 0 && !shapes)) { set_error("dmuon_warmup: bad arguments"); return DMUON_ERR_INVALID_ARG; }

@@ -214,6 +214,11 @@ struct AdamScalars {
 };
 int launch_adamw(const AdamRec* d_recs, const int64_t* d_prefix, int count, int64_t total_chunks, const AdamScalars& sc,
                  cudaStream_t s);
+// The same kernel with its work table in a static device array instead of cudaMalloc'ed memory (elementwise.cu):
+// builds and uploads the table of this call, then launches.  At most kAdamStaticMaxTensors tensors per call.
+constexpr int kAdamStaticMaxTensors = DMUON_ADAMW_NOALLOC_MAX_TENSORS;       // dmuon.h
+int launch_adamw_static(void* const* params, const void* const* grads, void* const* exp_avg, void* const* exp_avg_sq,
+                        const int64_t* numel, int count, const AdamScalars& sc, cudaStream_t s);
 
 int launch_export(const void* O, float* out, int rows, int cols, int n_pad, bool transposed, bool fp32_internal,
                   float inv_xscale, cudaStream_t s);                                             // test hook

@@ -713,4 +713,58 @@ int launch_adamw(const AdamRec* d_recs, const int64_t* d_prefix, int count, int6
   return DMUON_OK;
 }
 
+// ---------------------------------------------------------------------------------------------- AdamW, no allocation
+// dmuon_adamw_step_noalloc (include/dmuon.h).  adamw_kernel reads a work table -- one AdamRec per tensor plus the chunk
+// prefix -- from global memory; dmuon_adamw_step cudaMallocs that table.  Here the table lives in device memory that
+// belongs to the library image itself, so a call needs nothing from the CUDA allocator.  The array is part of every
+// context that loads libdmuon (192 KiB per GPU, held until the process exits).
+struct AdamStaticTable {
+  AdamRec recs[kAdamStaticMaxTensors];
+  int64_t prefix[kAdamStaticMaxTensors + 1];
+};
+static __device__ __align__(256) unsigned char g_adam_static[sizeof(AdamStaticTable)];
+
+namespace {
+// On the host the name g_adam_static is only a handle for the runtime's symbol lookup, NOT the array's device address
+// (handing &g_adam_static to a kernel would make it read host memory or fault).  The real address differs per device
+// and is looked up once per device below.
+AdamStaticTable* g_adam_static_dev[kMaxDevices] = {};
+AdamStaticTable g_adam_static_host;        // where a call assembles its table (calls are serialised by the API lock)
+}  // namespace
+
+int launch_adamw_static(void* const* params, const void* const* grads, void* const* exp_avg, void* const* exp_avg_sq,
+                        const int64_t* numel, int count, const AdamScalars& sc, cudaStream_t s) {
+  if (count <= 0) return DMUON_OK;
+  if (count > kAdamStaticMaxTensors) {
+    set_error("dmuon_adamw_step_noalloc: %d tensors in one call, the built-in table holds %d (split the list)", count,
+              kAdamStaticMaxTensors);
+    return DMUON_ERR_INVALID_ARG;
+  }
+  int dev = 0;
+  DMUON_CUDA_CHECK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kMaxDevices) { set_error("dmuon_adamw_step_noalloc: device ordinal %d is not supported", dev); return DMUON_ERR_UNSUPPORTED_DEVICE; }
+  if (!g_adam_static_dev[dev]) {           // first call on this device (it is the current one): resolve the address
+    void* p = nullptr;
+    DMUON_CUDA_CHECK(cudaGetSymbolAddress(&p, g_adam_static));
+    g_adam_static_dev[dev] = static_cast<AdamStaticTable*>(p);
+  }
+  AdamStaticTable* const tab = g_adam_static_dev[dev];
+  AdamStaticTable& h = g_adam_static_host;
+  h.prefix[0] = 0;
+  for (int i = 0; i < count; ++i) {
+    h.recs[i] = AdamRec{params[i], grads[i], static_cast<float*>(exp_avg[i]), static_cast<float*>(exp_avg_sq[i]), numel[i]};
+    h.prefix[i + 1] = h.prefix[i] + (numel[i] + kFlatChunk - 1) / kFlatChunk;
+  }
+  // Every entry the kernel reads (recs[0..count), prefix[0..count]) is rewritten by these two copies, so nothing of an
+  // earlier call's table is used and nothing has to be cleared.  The source is ordinary (pageable) host memory: the
+  // runtime has taken its copy of it when cudaMemcpyAsync returns, and the transfer itself is ordered on `s` before
+  // the kernel.
+  DMUON_CUDA_CHECK(cudaMemcpyAsync(tab->recs, h.recs, sizeof(AdamRec) * count, cudaMemcpyHostToDevice, s));
+  DMUON_CUDA_CHECK(cudaMemcpyAsync(tab->prefix, h.prefix, sizeof(int64_t) * (count + 1), cudaMemcpyHostToDevice, s));
+  const int64_t total_chunks = h.prefix[count];
+  adamw_kernel<<<grid_for(total_chunks, 8), kThreads, 0, s>>>(tab->recs, tab->prefix, count, total_chunks, sc);
+  DMUON_CUDA_CHECK(cudaGetLastError());
+  return DMUON_OK;
+}
+
 }  // namespace dmuon
