@@ -53,7 +53,7 @@ def _load():
         lib.oracle_muon_step.restype = ctypes.c_int
         lib.oracle_muon_step.argtypes = [dp, dp, dp, ctypes.c_int, ctypes.c_int, ctypes.c_double,
                                          ctypes.c_double, ctypes.c_double, ctypes.c_int, dp, ctypes.c_int,
-                                         ctypes.c_double, ctypes.c_int, ctypes.c_int, dp, dp, dp, dp]
+                                         ctypes.c_double, ctypes.c_int, dp, dp, dp, dp]
         lib.oracle_adamw_step.restype = ctypes.c_int
         lib.oracle_adamw_step.argtypes = [dp, dp, dp, dp, ctypes.c_longlong, ctypes.c_double, ctypes.c_double,
                                           ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_int, dp, dp, dp]
@@ -102,10 +102,9 @@ def ns(X, steps: int = 5, coeffs=DEFAULT_COEFFS, eps: float = DEFAULT_EPS, norma
 
 
 def muon_step(W, G, M, lr: float, mu: float, wd: float, steps: int = 5, coeffs=DEFAULT_COEFFS,
-              eps: float = DEFAULT_EPS, u_cast: bool = True, momentum_fp32: bool = False):
+              eps: float = DEFAULT_EPS, u_cast: bool = True):
     """One Muon step (Eq. 1, Alg. 1 l.12-15).  Returns dict with M_new, U, O, W_new (float64,
-    unrounded except U when u_cast).  momentum_fp32: form M' and U in binary32 before they are quantised to bf16
-    (reading N16: quantisation decisions are taken in the kernel's precision on both sides)."""
+    unrounded except U when u_cast).  M' and U are formed in float64 (PAPER.md:49-51 defines them in real arithmetic)."""
     W = np.ascontiguousarray(W, dtype=np.float64)
     G = np.ascontiguousarray(G, dtype=np.float64)
     M = np.ascontiguousarray(M, dtype=np.float64)
@@ -115,7 +114,7 @@ def muon_step(W, G, M, lr: float, mu: float, wd: float, steps: int = 5, coeffs=D
     co, per = _coeff_array(coeffs, steps)
     Mo, U, O, Wo = (np.empty((r, c)) for _ in range(4))
     rc = _load().oracle_muon_step(_ptr(W), _ptr(G), _ptr(M), r, c, float(lr), float(mu), float(wd), int(steps),
-                                  _ptr(co), per, float(eps), int(bool(u_cast)), int(bool(momentum_fp32)), _ptr(Mo), _ptr(U),
+                                  _ptr(co), per, float(eps), int(bool(u_cast)), _ptr(Mo), _ptr(U),
                                   _ptr(O), _ptr(Wo))
     if rc != 0:
         raise RuntimeError("oracle_muon_step failed")

@@ -169,7 +169,6 @@ ORACLE_API int oracle_ns(double* X, int rows, int cols, int steps, const double*
 /* One Muon step for one rows x cols parameter (Eq. 1; Alg. 1 l.12-15 :232-238).
  * Inputs W, G, M: doubles holding the stored (bf16-exact) values.  lr, mu, wd: the values the
  * caller passes to the C ABI (floats widened to double).  u_cast != 0 applies reading N15.
- * momentum_fp32 != 0 forms M' and U in binary32 (reading N16, see below); 0 keeps them in fp64.
  * Outputs (each rows*cols doubles, any may be NULL):
  *   M_out   = mu M + G                       (unrounded)
  *   U_out   = G + mu M_out, after the cast if u_cast
@@ -178,7 +177,7 @@ ORACLE_API int oracle_ns(double* X, int rows, int cols, int steps, const double*
  * The caller rounds M_out / W_out with oracle_round_bf16 to get the stored values. */
 ORACLE_API int oracle_muon_step(const double* W, const double* G, const double* M, int rows, int cols,
                                 double lr, double mu, double wd, int steps, const double* coeffs,
-                                int per_step, double eps, int u_cast, int momentum_fp32, double* M_out,
+                                int per_step, double eps, int u_cast, double* M_out,
                                 double* U_out, double* O_out, double* W_out) {
   if (!W || !G || !M || rows <= 0 || cols <= 0) return -1;
   const size_t cnt = (size_t)rows * cols;
@@ -186,18 +185,8 @@ ORACLE_API int oracle_muon_step(const double* W, const double* G, const double* 
   double* U = dalloc(cnt);
   if (!Mn || !U) { free(Mn); free(U); return -1; }
   for (size_t i = 0; i < cnt; ++i) {
-    if (momentum_fp32) {
-      /* Reading N16: the two values that are then QUANTISED to bf16 (the stored M' and the cast U) are formed in
-       * binary32 with one rounding each (fused multiply-add), the precision the kernel uses, so that both sides
-       * take the rounding decision on the same number.  With mu = 0.95f about 1.5 % of the fp64 values sit within
-       * 2^-24 of a bf16 tie, and binary32 rounds those onto the tie first. */
-      const float mn = fmaf((float)mu, (float)M[i], (float)G[i]);
-      Mn[i] = (double)mn;                                   /* N3: M' = mu M + G */
-      U[i] = (double)fmaf((float)mu, mn, (float)G[i]);      /*     U  = G + mu M' (from the unrounded M') */
-    } else {
-      Mn[i] = mu * M[i] + G[i];               /* N3: M' = mu M + G */
-      U[i] = G[i] + mu * Mn[i];               /*     U  = G + mu M' (from the unrounded M') */
-    }
+    Mn[i] = mu * M[i] + G[i];                 /* N3: M' = mu M + G */
+    U[i] = G[i] + mu * Mn[i];                 /*     U  = G + mu M' (from the unrounded M') */
     if (u_cast) U[i] = oracle_round_bf16(U[i]); /* N15 */
   }
   if (U_out) memcpy(U_out, U, cnt * sizeof(double));

@@ -1,4 +1,5 @@
-"""Shared helpers for the parity tests (no method arithmetic here)."""
+"""Shared helpers for the parity tests (no method arithmetic here, apart from binary32_momentum, which documents the
+kernel's own precision and is never used as the expected value of a parity check)."""
 import numpy as np
 import torch
 
@@ -21,6 +22,16 @@ def rel_fro(a: np.ndarray, b: np.ndarray) -> float:
     """||a - b||_F / ||b||_F  (b = oracle)."""
     den = np.linalg.norm(b)
     return float(np.linalg.norm(a - b) / (den if den > 0 else 1.0))
+
+
+def binary32_momentum(M: np.ndarray, G: np.ndarray, mu: float):
+    """What the tensor-core path's a1 kernel is documented to form (N16): M' = fma(mu, M, G) and
+    U = fma(mu, M', G) in binary32, one rounding each.  mu*M + G is exact in float64 for a 24-bit mu and bf16 M, G of
+    comparable scale, so rounding it once to float32 is the fused result.  A statement about the KERNEL's precision kept
+    beside the tests; the oracle holds only the paper's real-arithmetic definition and knows nothing of this."""
+    mn = (mu * M + G).astype(np.float32)
+    u = (mu * mn.astype(np.float64) + G).astype(np.float32)
+    return mn.astype(np.float64), u.astype(np.float64)
 
 
 def bf16_ulp(x: np.ndarray) -> np.ndarray:

@@ -4,9 +4,10 @@ Bars (BASELINE.json north_star): relative Frobenius error of O = NS_5(.) <= 1e-2
 (16-bit operands, fp32 accumulation) and <= 1e-4 in the fp32-operand check mode.  M' is compared elementwise
 with the fp64 oracle's (<= 1 bf16 ulp: fp32 vs fp64 arithmetic before the same rounding; the share of elements
 that differ is printed), W' by the criterion of DESIGN.md ("error no worse than the output rounding plus 1 % of
-the update").  Every comparison is against oracle.muon_step(..., momentum_fp32=False), the definition
-north_star gives.  ADDITIONALLY M' is checked bit for bit against the oracle's binary32-momentum mode (reading
-N16, steps = 0 so no NS work is repeated): that check is extra, it replaces none of the fp64 ones.
+the update").  Every comparison is against oracle.muon_step, which holds only the paper's definition in float64
+(PAPER.md:49-51).  The elements of M' that differ from it (by one ulp) are additionally required to be explained
+by the binary32 rounding DESIGN.md N16 documents for the kernel (tests/helpers.py binary32_momentum: a numpy
+statement of the kernel's precision, kept out of oracle/).
 """
 import functools
 
@@ -17,7 +18,7 @@ import torch
 import oracle
 import paper_2606_27153_b200 as dm
 from paper_2606_27153_b200 import synth
-from helpers import LR, LR_F, MU, MU_F, TOL_CHECK, TOL_TC, WD, WD_F, bf16_ulp, rel_fro, to64
+from helpers import LR, LR_F, MU, MU_F, TOL_CHECK, TOL_TC, WD, WD_F, bf16_ulp, binary32_momentum, rel_fro, to64
 
 pytestmark = pytest.mark.gpu
 
@@ -48,9 +49,10 @@ def oracle_muon(config: int, index: int, random_momentum: bool):
 
 
 def oracle_both(w, g, m):
-    """The plain fp64 oracle step, plus (key "M_n16") the stored M' of the binary32-momentum mode (N16)."""
+    """The plain fp64 oracle step, plus (key "M_n16", NOT from the oracle) the binary32 M' that DESIGN.md N16 says the
+    tensor-core path forms (tests/helpers.py binary32_momentum): used only to report how the <= 1 ulp differences arise."""
     orc = oracle.muon_step(w, g, m, LR_F, MU_F, WD_F)
-    orc["M_n16"] = oracle.muon_step(w, g, m, LR_F, MU_F, WD_F, steps=0, momentum_fp32=True)["M_new"]
+    orc["M_n16"] = binary32_momentum(m, g, MU_F)[0]
     return orc
 
 
@@ -70,10 +72,12 @@ def check_muon_matrix(idx, shape, W0, Wg, Mg, Og, orc, tol, exact_momentum=False
     STATS["m_mismatch"].append(float((dm_ != 0).mean()))
     if exact_momentum:
         assert np.array_equal(mg, m_orc), f"matrix {idx}: check mode must reproduce the fp64 oracle's M' bit for bit"
-    # additional check (reading N16): formed in binary32 with one fused rounding on both sides -> identical bits
+    # not a parity check (the oracle is the fp64 definition above): every element that differs from the oracle is one
+    # where binary32 and binary64 arithmetic round to neighbouring bf16 values (N16), nothing else
     elif "M_n16" in orc:
         m16 = oracle.round_bf16(orc["M_n16"])
-        assert np.array_equal(mg, m16), f"matrix {idx}: M' differs from the binary32 mode ({(mg != m16).mean():.2e} of elements)"
+        unexplained = (mg != m_orc) & (mg != m16)
+        assert not unexplained.any(), f"matrix {idx}: {unexplained.mean():.2e} of M' differ from the oracle for another reason than the binary32 rounding"
     # W': no worse than the output rounding plus 1 % of the update (2 % slack on the rounding term: the two
     # roundings are different random draws of the same distribution)
     w_orc = orc["W_new"]
@@ -386,9 +390,10 @@ def test_master_weights_step():
     for i, s in enumerate(shapes):
         orc = oracle_both(W0[i], to64(G[i]), M0[i])
         assert torch.equal(W[i], W32[i].to(torch.bfloat16)), f"{s}: bf16 parameter is not the rounding of the master"
-        assert np.array_equal(to64(M[i]), oracle.round_bf16(orc["M_n16"])), f"{s}: M' differs from the binary32 mode"
         m_orc = oracle.round_bf16(orc["M_new"])
         assert (np.abs(to64(M[i]) - m_orc) <= bf16_ulp(m_orc)).all(), f"{s}: M' off the fp64 oracle by more than 1 bf16 ulp"
+        unexplained = (to64(M[i]) != m_orc) & (to64(M[i]) != oracle.round_bf16(orc["M_n16"]))
+        assert not unexplained.any(), f"{s}: M' differs from the oracle for another reason than the binary32 rounding (N16)"
         upd_orc = orc["W_new"] - W0[i]
         upd_gpu = to64(W32[i]) - W0[i]
         e = np.linalg.norm(upd_gpu - upd_orc) / np.linalg.norm(upd_orc)
