@@ -27,7 +27,20 @@
  *     autotunes tile configurations on scratch buffers (never on caller data) and synchronises the device.
  *   - errors: return value 0 = DMUON_OK, negative = error; dmuon_last_error() gives a message for the calling
  *     thread's last failure.  Nothing throws or aborts across this boundary.  Non-finite inputs propagate.
- *   - count == 0 is a valid no-op.  Not thread-safe: serialise calls from several host threads.
+ *   - count == 0 is a valid no-op.
+ *   - threads: every entry point takes one process-wide mutex for its whole host-side duration, so calls from several
+ *     host threads are safe and run one after another (the enqueued GPU work still overlaps only as its streams
+ *     allow, and the per-device workspace is shared: see "devices").  dmuon_last_error() is per thread.
+ *   - CUDA graphs: once a shape set's plan exists (first call, or dmuon_warmup) a step only enqueues kernels and one
+ *     pointer-table upload, and may be captured.  The captured graph keeps RAW POINTERS into that plan's device tables
+ *     and into the workspace, and its replay re-uploads the tensors it was captured with.  The library therefore
+ *     (a) records the upload in every capture and, after a plan has been captured once, uploads on every later eager
+ *     call too, so replays and eager calls with other tensors can be mixed in any order on one stream;
+ *     (b) never evicts a captured plan from its cache of 8 plans, and REFUSES (DMUON_ERR_INVALID_ARG) what would free
+ *     memory a graph may still use: dmuon_set_workspace, a new shape set that needs a larger shared workspace, a
+ *     ninth plan when all eight are captured.  Warm up the largest shape set before capturing.  After destroying
+ *     the graphs, dmuon_set_option("graphs_destroyed", "1") lifts (a) and (b); dmuon_shutdown frees everything
+ *     regardless, so destroy the graphs first.
  *   - devices: every call works on the CURRENT CUDA device (cudaSetDevice before the call); plans, workspaces and
  *     kernel attributes are kept per device.  Calls that share a device share that device's workspace: issue them
  *     on one stream, or order the streams yourself.
@@ -216,6 +229,8 @@ DMUON_API int dmuon_set_workspace(void* dev_ptr, size_t bytes);
  *   "small_fused" "1"/"0": matrices whose padded oriented shape is 256 x 256 run ALL their NS steps in one on-chip
  *                 kernel (X, G, B resident in the shared memory of a CTA pair; nothing stored between products), up to
  *                 16 steps (default "1"; "0" = the grouped per-product launches, as for every other shape)
+ *   "graphs_destroyed" "1": a statement, not a setting: every CUDA graph captured from calls of this library has been
+ *                 destroyed (see "CUDA graphs" at the top).
  *   "keep_ns_output" "1"/"0": keep every matrix's unrounded NS result readable after the call (dmuon_read_ns_output):
  *                 fused epilogues also store it and buckets get disjoint workspace regions (default "0")
  *   "chunk_mb"    workspace a bucket may use, MiB (default "12288"): a bucket whose matrices need more runs as

@@ -53,8 +53,15 @@ def build_library(force: bool = False, verbose: bool = False, extra_flags=()) ->
     for src in SOURCES:
         s = os.path.join(CSRC, src)
         o = os.path.join(OBJ, src.replace(".cu", ".o"))
+        carries_id = src == "planner.cu"
+        id_file = o + ".id"       # the id compiled into planner.o: ANY source change makes that object stale
+        if carries_id and os.path.exists(o) and (not os.path.exists(id_file) or open(id_file).read().strip() != bid):
+            os.remove(o)
         if force or _stale(o, [s] + headers):
-            defs = [f'-DDMUON_BUILD_ID="{bid}"'] if src == "planner.cu" else []
+            defs = [f'-DDMUON_BUILD_ID="{bid}"'] if carries_id else []
+            if carries_id:
+                with open(id_file, "w") as f:
+                    f.write(bid)
             jobs.append([nvcc] + NVCC_FLAGS + list(extra_flags) + defs + (["-Xptxas", "-v"] if verbose else []) + ["-c", s, "-o", o])
 
     def run(cmd):

@@ -158,7 +158,14 @@ int bind_pointers(Plan& plan, void* const* w, const void* const* g, void* const*
     if (r.O != o) dirty = true;
     r.O = o;
   }
-  if (dirty && count > 0) return upload_snapshot(plan.d_recs, plan.h_recs.data(), sizeof(MatRec) * count, stream);
+  // A graph replay rewrites d_recs from its own pinned snapshot WITHOUT touching the host mirror, so once a capture
+  // has recorded a call on this plan the mirror no longer says what the device holds: from then on every call uploads.
+  // A capture always records its upload, so that a replay never runs on what another call left in d_recs.
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  cudaStreamIsCapturing(stream, &cap);
+  if (cap != cudaStreamCaptureStatusNone) plan.captured = true;
+  if ((dirty || plan.captured) && count > 0)
+    return upload_snapshot(plan.d_recs, plan.h_recs.data(), sizeof(MatRec) * count, stream);
   return DMUON_OK;
 }
 
@@ -377,6 +384,15 @@ DMUON_API int dmuon_set_option(const char* key, const char* value) {
   if (k == "profile") { if (as_bool(&g_opt.profile)) return DMUON_OK; set_error("option profile: bad value '%s'", value); return DMUON_ERR_INVALID_ARG; }
   if (k == "fuse_epilogue") { if (as_bool(&g_opt.fuse)) return DMUON_OK; set_error("option fuse_epilogue: bad value '%s'", value); return DMUON_ERR_INVALID_ARG; }
   if (k == "small_fused") { if (as_bool(&g_opt.small_fused)) return DMUON_OK; set_error("option small_fused: bad value '%s'", value); return DMUON_ERR_INVALID_ARG; }
+  if (k == "graphs_destroyed") {
+    // the caller states that every CUDA graph captured from this library's calls has been destroyed: plans and the
+    // workspace may be evicted / moved again, and eager calls stop re-uploading their tables
+    bool yes = false;
+    if (!as_bool(&yes) || !yes) { set_error("option graphs_destroyed: the only value is 1"); return DMUON_ERR_INVALID_ARG; }
+    forget_captures();
+    for (PinnedBuf& b : g_pinned) b.permanent = false;      // the graphs' upload snapshots can be reused
+    return DMUON_OK;
+  }
   if (k == "keep_ns_output") { if (as_bool(&g_opt.keep_o)) return DMUON_OK; set_error("option keep_ns_output: bad value '%s'", value); return DMUON_ERR_INVALID_ARG; }
   if (k == "schedule") {
     if (v == "auto") g_opt.gram_blocks = true;
@@ -756,6 +772,11 @@ DMUON_API int dmuon_set_workspace(void* dev_ptr, size_t bytes) {
   DMUON_LOCK;
   if ((dev_ptr == nullptr) != (bytes == 0)) { set_error("dmuon_set_workspace: pointer and size must both be set or both be zero"); return DMUON_ERR_INVALID_ARG; }
   if (reinterpret_cast<uintptr_t>(dev_ptr) & 255) { set_error("dmuon_set_workspace: pointer must be 256-byte aligned"); return DMUON_ERR_INVALID_ARG; }
+  if (captured_plans() > 0) {
+    set_error("dmuon_set_workspace: a captured CUDA graph refers to the current plans and workspace; destroy the graphs "
+              "and set option graphs_destroyed=1 first");
+    return DMUON_ERR_INVALID_ARG;
+  }
   cudaDeviceSynchronize();
   cudaGetLastError();
   drop_plans();
@@ -983,6 +1004,7 @@ DMUON_API int dmuon_measure_cost(int32_t rows, int32_t cols, int32_t batch, int3
   if (e0) cudaEventDestroy(e0);
   if (e1) cudaEventDestroy(e1);
   cudaFree(buf);
+  g_last_plan = 0;      // the workspace now holds the NS results of noise: dmuon_read_ns_output must not hand them out
   return rc;
 }
 

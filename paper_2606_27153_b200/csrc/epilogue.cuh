@@ -28,16 +28,21 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
   return *reinterpret_cast<const uint32_t*>(&b);
 }
 
-// W words of one 32-column chunk of one row (EPI_APPLY), loaded one chunk ahead.  Through L1 (ld.global.nc): a lane
+// W words of one 32-column chunk of one row (EPI_APPLY), loaded one chunk ahead.  Through L1 (ld.global.ca): a lane
 // reads its row's 64 bytes as four 16-byte loads, the first brings the sectors in and the other three hit; a streaming
-// load (ld.global.cs) sent all four to L2/DRAM and halved the throughput of the fused X update.
+// load (ld.global.cs) sent all four to L2/DRAM and halved the throughput of the fused X update.  Not the read-only
+// path (ld.global.nc / __ldg): the same kernel overwrites W in final_store, and .nc is defined only for memory that
+// nobody writes while the kernel runs.
 struct WWords { uint4 w[4]; };
 template <int kEpi>
 __device__ __forceinline__ void load_w(WWords& a, const FinalCtx& x, int64_t grow, int64_t gcol) {
   if (kEpi == EPI_APPLY) {
     const uint4* wp = reinterpret_cast<const uint4*>(x.W + grow * x.ldw + gcol);
 #pragma unroll
-    for (int g = 0; g < 4; ++g) a.w[g] = __ldg(wp + g);
+    for (int g = 0; g < 4; ++g)
+      asm volatile("ld.global.ca.v4.u32 {%0, %1, %2, %3}, [%4];"
+                   : "=r"(a.w[g].x), "=r"(a.w[g].y), "=r"(a.w[g].z), "=r"(a.w[g].w)
+                   : "l"(wp + g));
   }
 }
 

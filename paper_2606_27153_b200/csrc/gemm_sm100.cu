@@ -283,12 +283,13 @@ __device__ __forceinline__ void red_release_gpu_add(uint32_t* p, uint32_t v) {
 // stores were bulk tensor stores (async proxy) completed before the release; the loads that follow are bulk tensor
 // loads: a proxy fence on each side.
 __device__ __forceinline__ void wait_done(const uint32_t* ctr, uint32_t need) {
+  // (the 20 s limit applies in a DMUON_WATCHDOG build only, see umma.cuh)
   if (ld_acquire_gpu(ctr) < need) {
     const uint64_t t0 = global_timer_ns();
     uint32_t polls = 0;
     while (ld_acquire_gpu(ctr) < need) {
       __nanosleep(100);
-      if ((++polls & 0x3FFu) == 0 && global_timer_ns() - t0 > 20000000000ull) __trap();
+      if ((++polls & 0x3FFu) == 0 && global_timer_ns() - t0 > 20000000000ull) DMUON_WATCHDOG_TRAP();
     }
   }
   asm volatile("fence.proxy.async;" ::: "memory");

@@ -540,6 +540,16 @@ size_t plan_workspace_bytes(const int32_t* shapes, int count, const Options& opt
 
 void drop_plans() { g_plans.clear(); }
 
+int captured_plans() {
+  int n = 0;
+  for (auto& up : g_plans) n += up->captured ? 1 : 0;
+  return n;
+}
+
+void forget_captures() {
+  for (auto& up : g_plans) up->captured = false;
+}
+
 Plan* find_plan(uint64_t id) {
   for (auto& up : g_plans)
     if (up->id == id) return up.get();
@@ -606,7 +616,15 @@ int get_plan(const int32_t* shapes, int count, const Options& opt, void* ext_ws,
   } else {
     DeviceWs& w = g_ws[dev];
     if (w.bytes < p.ws_bytes) {
-      // growing moves the region: plans that point into the old one are dropped (their tuned choices stay cached)
+      // growing moves the region: plans that point into the old one are dropped (their tuned choices stay cached).
+      // A captured graph holds raw pointers into the region and into those plans' tables: refuse rather than free them.
+      for (auto& q : g_plans)
+        if (q->device == dev && !q->ext_ws && q->captured) {
+          set_error("this shape set needs a %zu-byte workspace (the device's is %zu) but a captured CUDA graph refers to the "
+                    "current one: destroy the graphs and set option graphs_destroyed=1, or size the workspace first with "
+                    "dmuon_warmup on the largest shape set before capturing", p.ws_bytes, w.bytes);
+          return DMUON_ERR_INVALID_ARG;
+        }
       DMUON_CUDA_CHECK(cudaDeviceSynchronize());
       drop_plans_of_device(dev, true);
       if (w.ptr) cudaFree(w.ptr);
@@ -626,6 +644,10 @@ int get_plan(const int32_t* shapes, int count, const Options& opt, void* ext_ws,
   // check mode: padding of the fp32 buffers must be zero (the tensor-core path's padding is written by the normalise kernel
   // for generic matrices and does not exist for aligned ones)
   DMUON_CUDA_CHECK(cudaMemsetAsync(p.ws, 0, p.ws_bytes, stream));
+  // building a plan writes the region (this memset, the autotune's noise): NS results another plan left there are gone,
+  // whether or not a step follows (dmuon_warmup / dmuon_describe_plan build plans without running one)
+  for (auto& q : g_plans)
+    if (q->device == dev && q->ws == p.ws) q->o_valid = false;
 
   // ---- elementwise records and per-bucket work lists
   const size_t nrec = std::max(count, 1);
@@ -744,10 +766,16 @@ int get_plan(const int32_t* shapes, int count, const Options& opt, void* ext_ws,
   }
   DMUON_CUDA_CHECK(cudaDeviceSynchronize());
   // least-recently-used plans make room
+  // (never a plan that a captured CUDA graph refers to: its replay reads the plan's device tables)
   while (g_plans.size() >= kMaxPlans) {
-    size_t victim = 0;
-    for (size_t i = 1; i < g_plans.size(); ++i)
-      if (g_plans[i]->stamp < g_plans[victim]->stamp) victim = i;
+    size_t victim = g_plans.size();
+    for (size_t i = 0; i < g_plans.size(); ++i)
+      if (!g_plans[i]->captured && (victim == g_plans.size() || g_plans[i]->stamp < g_plans[victim]->stamp)) victim = i;
+    if (victim == g_plans.size()) {
+      set_error("all %zu cached plans are referred to by captured CUDA graphs: destroy the graphs and set option "
+                "graphs_destroyed=1", g_plans.size());
+      return DMUON_ERR_INVALID_ARG;
+    }
     g_plans.erase(g_plans.begin() + victim);
   }
   g_plans.push_back(std::move(up));

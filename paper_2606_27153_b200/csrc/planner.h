@@ -145,6 +145,7 @@ struct Plan {
   int device = 0;
   void* ext_ws = nullptr;
   uint64_t stamp = 0;                  // last use (LRU eviction)
+  bool captured = false;               // a CUDA graph recorded a call on this plan: tables re-uploaded at every call, plan and workspace pinned
   uint64_t id = 0;                     // unique; find_plan(id) tells whether the plan still exists
   bool o_valid = false;                // the last call left every matrix's NS result readable in the workspace
   std::vector<MatrixInfo> mats;
@@ -169,6 +170,8 @@ size_t plan_workspace_bytes(const int32_t* shapes, int count, const Options& opt
 int get_plan(const int32_t* shapes, int count, const Options& opt, void* ext_ws, size_t ext_bytes, cudaStream_t stream,
              Plan** out);
 void drop_plans();
+int captured_plans();                 // plans a CUDA graph refers to (all devices)
+void forget_captures();               // the caller states that every such graph has been destroyed
 Plan* find_plan(uint64_t id);
 void release_workspaces();
 int tune_cache_entries();

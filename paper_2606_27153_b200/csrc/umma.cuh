@@ -38,20 +38,28 @@ __device__ __forceinline__ uint32_t mbar_try_wait(uint32_t bar, uint32_t parity)
       : "memory");
   return done;
 }
+// Hang watchdog, OFF unless the library is built with -DDMUON_WATCHDOG (build.py extra_flags).  A wait of the program
+// kernel is bounded by other CTAs' progress, which compute-sanitizer, a debugger, MPS time-slicing or preemption by
+// another process can stretch past any fixed limit, and a trap destroys the CUDA context with the caller's tensors.
+#ifdef DMUON_WATCHDOG
+#define DMUON_WATCHDOG_TRAP() __trap()
+#else
+#define DMUON_WATCHDOG_TRAP() ((void)0)
+#endif
 __device__ __forceinline__ uint64_t global_timer_ns() {
   uint64_t t;
   asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
   return t;
 }
 // Wait for the phase with the given parity.  mbarrier.try_wait suspends the thread for a hardware-chosen time slice
-// before it returns false, so the loop is not a hot spin.  A protocol bug would hang the GPU: after 20 s of WALL time
-// (not a poll count: a time-sliced or profiled GPU may need many polls) the kernel traps instead.
+// before it returns false, so the loop is not a hot spin.  A protocol bug would hang the GPU: in a DMUON_WATCHDOG build
+// the kernel traps after 20 s of WALL time (not a poll count: a time-sliced or profiled GPU may need many polls).
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   if (mbar_try_wait(bar, parity)) return;
   const uint64_t t0 = global_timer_ns();
   uint32_t polls = 0;
   while (!mbar_try_wait(bar, parity)) {
-    if ((++polls & 0xFFFu) == 0 && global_timer_ns() - t0 > 20000000000ull) __trap();
+    if ((++polls & 0xFFFu) == 0 && global_timer_ns() - t0 > 20000000000ull) DMUON_WATCHDOG_TRAP();
   }
 }
 // Whole-warp wait of the epilogue warps: lane 0 polls, sleeping between polls (the accumulator of a 256-wide unit
@@ -64,7 +72,7 @@ __device__ __forceinline__ void mbar_wait_warp(uint32_t bar, uint32_t parity, ui
       uint32_t polls = 0;
       while (!mbar_try_wait(bar, parity)) {
         if (sleep_ns) __nanosleep(sleep_ns);
-        if ((++polls & 0xFFFu) == 0 && global_timer_ns() - t0 > 20000000000ull) __trap();
+        if ((++polls & 0xFFFu) == 0 && global_timer_ns() - t0 > 20000000000ull) DMUON_WATCHDOG_TRAP();
       }
     }
   }
@@ -90,7 +98,7 @@ __device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity)
   const uint64_t t0 = global_timer_ns();
   uint32_t polls = 0;
   while (!mbar_try_wait_cluster(bar, parity)) {
-    if ((++polls & 0xFFFu) == 0 && global_timer_ns() - t0 > 20000000000ull) __trap();
+    if ((++polls & 0xFFFu) == 0 && global_timer_ns() - t0 > 20000000000ull) DMUON_WATCHDOG_TRAP();
   }
 }
 // Latency-critical waits (the on-chip small-matrix kernel's product chain): mbarrier.test_wait never suspends the
@@ -111,7 +119,7 @@ __device__ __forceinline__ void mbar_spin_wait(uint32_t bar, uint32_t parity) {
     if ((++polls & 0xFFFFu) == 0) {
       const uint64_t t = global_timer_ns();
       if (t0 == 0) t0 = t;
-      else if (t - t0 > 20000000000ull) __trap();
+      else if (t - t0 > 20000000000ull) DMUON_WATCHDOG_TRAP();
     }
   }
 }

@@ -412,6 +412,63 @@ def test_master_weights_step():
     assert all(torch.equal(a, b) for a, b in zip(keep, W32))
 
 
+def test_graph_replays_and_eager_calls_do_not_inherit_each_others_tensors():
+    """A graph replay rewrites the plan's device pointer table from its own snapshot, behind the back of the host mirror
+    that eager calls compare against.  Two orders used to go wrong: (1) a capture that found "nothing changed" recorded
+    no upload, so its replay ran on whatever a later eager call had bound; (2) an eager call after a replay found its
+    own pointers in the host mirror, uploaded nothing and updated the GRAPH's tensors.  Both orders, with the tensors
+    that must NOT move checked too; then the pinning rules (a captured plan's workspace cannot be replaced until the
+    caller says the graphs are gone)."""
+    dm.set_option("keep_ns_output", 0)
+    idx = list(range(12))
+    _, WA, GA, MA = synth.muon_inputs(2, "cuda", True, indices=idx)
+    WB, GB, MB = [t.clone() for t in WA], [t.clone() for t in GA], [t.clone() for t in MA]
+    W0, M0 = [t.clone() for t in WA], [t.clone() for t in MA]
+
+    def restore(W, M):
+        for w, w0, m, m0 in zip(W, W0, M, M0):
+            w.copy_(w0)
+            m.copy_(m0)
+
+    def same(X, Y):
+        return all(torch.equal(a, b) for a, b in zip(X, Y))
+
+    dm.muon_step(WA, GA, MA, LR, MU, WD)                   # builds the plan, binds A; also the expected result
+    torch.cuda.synchronize()
+    W1, M1 = [t.clone() for t in WA], [t.clone() for t in MA]
+    assert not same(W1, W0)
+    restore(WA, MA)
+    side = torch.cuda.Stream()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(graph, stream=side):        # A is what the plan holds already: "nothing changed"
+            dm.muon_step(WA, GA, MA, LR, MU, WD)
+    dm.muon_step(WB, GB, MB, LR, MU, WD)                   # eager call binds B
+    torch.cuda.synchronize()
+    assert same(WB, W1) and same(MB, M1) and same(WA, W0) and same(MA, M0)
+    restore(WB, MB)
+    graph.replay()                                         # order (1): must step A, not B
+    torch.cuda.synchronize()
+    assert same(WA, W1) and same(MA, M1), "the replay did not update the tensors it was captured with"
+    assert same(WB, W0) and same(MB, M0), "the replay updated the tensors of a later eager call"
+    restore(WA, MA)
+    dm.muon_step(WB, GB, MB, LR, MU, WD)                   # order (2): must step B, not A
+    torch.cuda.synchronize()
+    assert same(WB, W1) and same(MB, M1), "the eager call after a replay did not update its own tensors"
+    assert same(WA, W0) and same(MA, M0), "the eager call after a replay updated the graph's tensors"
+    # the graph holds raw pointers into the plan's tables and the workspace: both stay until the caller releases them
+    buf = torch.empty(dm.workspace_bytes([tuple(w.shape) for w in WA]) + 256, dtype=torch.uint8, device="cuda")
+    with pytest.raises(dm.binding.DmuonError, match="graphs_destroyed"):
+        dm.set_workspace(buf)
+    graph.replay()
+    torch.cuda.synchronize()
+    assert same(WA, W1)
+    del graph
+    dm.set_option("graphs_destroyed", 1)
+    dm.set_workspace(buf)
+    dm.set_workspace(None)
+
+
 @pytest.mark.parametrize("rebind", [False, True])
 def test_step_is_cuda_graph_capturable(rebind):
     """After the first call for a shape set (plan, autotune) a step only enqueues kernels (and, when the tensors
