@@ -248,42 +248,66 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------------ oracle arm
-def oracle_sample(config: int, max_seconds: float = 30.0):
-    """Time the fp64 oracle, as it stands, on a bounded sample of the workload: whole Muon steps of single matrices,
-    smallest distinct shapes first, until ~max_seconds are used.  Returns (dense TFLOP/s, description, cores, seconds)."""
+def _oracle_inputs(config: int, shapes, s):
+    from paper_2606_27153_b200 import synth
+    i = shapes.index(s)
+    _, W, G, M = synth.muon_inputs(config, "cpu", False, indices=[i]) if config != 1 else (None, *([synth.ns_inputs("cpu")[1][:1]] * 3))
+    return tuple(t[0].to(torch.float64).numpy() for t in (W, G, M))
+
+
+def oracle_shape_seconds(config: int, s, shapes) -> tuple:
+    """Seconds of one full oracle Muon step (NS_STEPS steps) of one matrix of shape s, and how they were obtained.
+    Shapes whose full step fits ~3 s are timed whole.  Larger ones are timed at steps = 1 and steps = 0 and
+    EXTRAPOLATED: t(0) + NS_STEPS * (t(1) - t(0)); the oracle's NS steps are the same plain loops at every step."""
+    import oracle
+    w, g, m = _oracle_inputs(config, shapes, s)
+    if dense_flops([s]) / 4.5e10 <= 3.0:            # ~45 GFLOP/s plain loops on 16 cores
+        t0 = time.perf_counter()
+        oracle.muon_step(w, g, m, LR, MU, WD)
+        return time.perf_counter() - t0, "whole"
+    t0 = time.perf_counter()
+    oracle.muon_step(w, g, m, LR, MU, WD, steps=0)
+    t1 = time.perf_counter()
+    oracle.muon_step(w, g, m, LR, MU, WD, steps=1)
+    t2 = time.perf_counter()
+    e0, e1 = t1 - t0, t2 - t1
+    return e0 + NS_STEPS * (e1 - e0), "extrapolated from steps=0 and steps=1"
+
+
+def oracle_sample(config: int, per_shape: dict = None):
+    """Time the fp64 oracle, as it stands, on a bounded sample of the workload: one matrix of EVERY distinct shape (SURVEY
+    8(d)), scaled by the shape counts.  With per_shape (seconds per shape from an earlier call) only the smallest shape
+    is timed again and the others keep their seconds: the reference arm's repeated steps stay bounded.
+    Returns (dense TFLOP/s of the whole config, description, cores, seconds spent, per_shape)."""
     import oracle
     from paper_2606_27153_b200 import synth
     shapes = synth.config_shapes(config)
     distinct = sorted(set(shapes), key=lambda s: dense_flops([s]))
     oracle.ns(torch.zeros(8, 8).double().numpy())          # build + load outside the timed region
-    done, flops, secs = [], 0.0, 0.0
-    for s in distinct:
-        est = dense_flops([s]) / 4.5e10                     # ~45 GFLOP/s plain loops on 16 cores: skip what cannot fit the budget
-        if done and secs + est > max_seconds:
-            break
-        i = shapes.index(s)
-        _, W, G, M = synth.muon_inputs(config, "cpu", False, indices=[i]) if config != 1 else (None, *([synth.ns_inputs("cpu")[1][:1]] * 3))
-        w, g, m = (t[0].to(torch.float64).numpy() for t in (W, G, M))
-        t0 = time.perf_counter()
-        oracle.muon_step(w, g, m, LR, MU, WD)
-        secs += time.perf_counter() - t0
-        flops += dense_flops([s])
-        done.append(f"{s[0]}x{s[1]}")
-        if secs > max_seconds:
-            break
-    desc = f"one full Muon step (5 NS steps, fp64, dense) of one matrix each of shape {', '.join(done)} from {WORKLOADS[config].split(':')[0]}"
-    return flops / secs / 1e12, desc, oracle.num_threads(), secs
+    t_start = time.perf_counter()
+    fresh = per_shape is None
+    per_shape = {} if fresh else dict(per_shape)
+    how = {}
+    for s in (distinct if fresh else distinct[:1]):
+        per_shape[s], how[s] = oracle_shape_seconds(config, s, shapes)
+    spent = time.perf_counter() - t_start
+    total = sum(per_shape[s] * shapes.count(s) for s in distinct)
+    parts = ", ".join(f"{s[0]}x{s[1]} x{shapes.count(s)}: {per_shape[s]:.1f} s" + (f" ({how[s]})" if s in how else " (kept from the first step)")
+                      for s in distinct)
+    desc = (f"EXTRAPOLATED to {WORKLOADS[config].split(':')[0]}: one full Muon step ({NS_STEPS} NS steps, fp64, dense) of ONE matrix "
+            f"of every distinct shape, times the shape counts [{parts}]")
+    return dense_flops(shapes) / total / 1e12, desc, oracle.num_threads(), spent, per_shape
 
 
 def run_reference(args):
-    """--impl reference: the oracle on the host cores; each step is one bounded sample."""
+    """--impl reference: the oracle on the host cores.  The first step times one matrix of every distinct shape; every
+    later step re-times the smallest shape and keeps the others, so that K + W steps stay within a few minutes."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    budget = args.sample_seconds if args.sample_seconds > 0 else max(5.0, 60.0 / max(1, args.steps + args.warmup))
-    vals, secs, desc, cores = [], [], "", 0
+    vals, secs, desc, cores, per_shape = [], [], "", 0, None
     for it in range(args.warmup + args.steps):
-        v, desc, cores, s = oracle_sample(args.config, budget)
+        v, desc, cores, s, per_shape = oracle_sample(args.config, per_shape)
         if it >= args.warmup:
             vals.append(v)
             secs.append(s)
@@ -294,7 +318,7 @@ def run_reference(args):
         "warmup": args.warmup, "ms_per_step": 1e3 * dense_flops(shapes) / (value * 1e12), "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": WORKLOADS[args.config], "ns_steps": NS_STEPS, "coeffs": [3.4445, -4.7750, 2.0315], "lr": LR,
-                   "mu": MU, "wd": WD, "note": "ms_per_step extrapolated from the sample by FLOPs"},
+                   "mu": MU, "wd": WD, "note": "ms_per_step extrapolated from the sample by shape counts"},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
                          "seconds_per_sample": statistics.mean(secs)},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -499,7 +523,7 @@ def run_ours(args):
 
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        v, desc, cores, secs = oracle_sample(cfg, 32.0)
+        v, desc, cores, secs, _ = oracle_sample(cfg)
         cpu_baseline = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc, "seconds": secs}
 
     if rank == 0:
@@ -528,6 +552,10 @@ def run_ours(args):
             "tune_seconds": plan_desc.get("tune_seconds"),
             "paper_context": "DMuon reports 6.85x-163x optimizer-step and 1.48x-3.01x end-to-end speedups on 8-256 A800 "
                              "(PAPER.md:5, :274) and ~2x on one GPU (:329): other hardware, context only",
+            # last on purpose (a reader of the line's tail sees it): fraction of the measured HBM peak of the elementwise
+            # passes as they run INSIDE the step, and of the tensor peak of the dominant launch type
+            "in_step_frac": {k: round(v["frac"], 4) for k, v in kernels.items()
+                             if v.get("frac") is not None and (v.get("bound") == "hbm" or k == "ns_program_apply")},
         }
         print(json.dumps(line))
     if dist:
@@ -632,6 +660,16 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="configs[4]: NS-only shape sweep, one JSON line per shape")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and not args.sweep:
+        # `python bench.py --gpus N` without a launcher: start N ranks (one replica per GPU) the way the driver does
+        import socket
+        import subprocess
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr",
+               "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        raise SystemExit(subprocess.call(cmd))
     if args.sweep:
         run_sweep(args)
     elif args.impl == "reference":

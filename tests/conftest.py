@@ -25,3 +25,15 @@ def pytest_collection_modifyitems(config, items):
     for item in items:
         if "gpu" in item.keywords:
             item.add_marker(skip)
+
+
+@pytest.fixture(autouse=True)
+def _captured_graphs_released(request):
+    """Tests that capture a step into a CUDA graph drop the graph when they return.  The library pins a captured plan and
+    its workspace until it is told the graphs are gone (include/dmuon.h, "CUDA graphs"): tell it after every GPU test."""
+    yield
+    if "gpu" in request.node.keywords:
+        import gc
+        gc.collect()
+        import paper_2606_27153_b200 as dm
+        dm.set_option("graphs_destroyed", 1)

@@ -38,3 +38,20 @@ def bf16_ulp(x: np.ndarray) -> np.ndarray:
     """Spacing of bf16 at |x| (normal range)."""
     ax = np.maximum(np.abs(x), 2.0 ** -126)
     return 2.0 ** (np.floor(np.log2(ax)) - 7)
+
+
+W_USED = []      # (err - r) / (tol * upd) per checked matrix: the share of the update allowance a W' check used
+
+
+def w_bound(w_gpu: np.ndarray, w_orc: np.ndarray, w_before: np.ndarray, tol: float, round_bf16) -> tuple:
+    """(err, bound) of the stored parameter against the oracle's unrounded W' (DESIGN.md section 5 derives it):
+    err = ||W'_gpu - w_orc||, bound = (1 + s) r + tol ||w_orc - W||, r = ||RNE_bf16(w_orc) - w_orc|| the rounding the
+    oracle's own result takes when stored.  s = min(0.02, 4 / sqrt(N)): the GPU rounds ITS unrounded value, another
+    draw of the same rounding-error distribution, whose norm differs from r by a relative 0.63 / sqrt(N) (one sigma)."""
+    r = np.linalg.norm(round_bf16(w_orc) - w_orc)
+    upd = np.linalg.norm(w_orc - w_before)
+    err = np.linalg.norm(w_gpu - w_orc)
+    s = min(0.02, 4.0 / np.sqrt(w_orc.size))
+    if upd > 0:
+        W_USED.append(float((err - r) / (tol * upd)))
+    return err, (1.0 + s) * r + tol * upd

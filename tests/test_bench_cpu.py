@@ -114,3 +114,27 @@ def test_reference_arm_rank0_only_under_torchrun():
     assert line["impl"] == "reference" and line["n_gpus"] == 2 and line["value"] > 0
     assert line["cpu_baseline"]["kind"] == "oracle" and line["cpu_baseline"]["cores"] >= 1
     assert line["e2e"]["h2d_bytes_per_step"] == 0
+
+
+def test_gpus_flag_launches_the_ranks_itself():
+    """`python bench.py --gpus 2` with no launcher (WORLD_SIZE unset) starts 2 ranks under torch.distributed.run."""
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    cmd = [sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2", "--steps", "2", "--warmup", "1",
+           "--config", "1"]
+    r = subprocess.run(cmd, capture_output=True, text=True, timeout=300, cwd=ROOT, env=env)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [json.loads(l) for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1 and lines[0]["n_gpus"] == 2 and lines[0]["impl"] == "reference"
+
+
+def test_cpu_baseline_covers_every_distinct_shape():
+    """the oracle sample is one matrix of EVERY distinct shape scaled by the counts; a later step re-times
+    only the smallest shape and keeps the rest."""
+    import bench
+    from paper_2606_27153_b200 import synth
+    v, desc, cores, secs, per_shape = bench.oracle_sample(2)
+    assert set(per_shape) == set(synth.config_shapes(2)) and all(t > 0 for t in per_shape.values())
+    assert v > 0 and cores >= 1 and "EXTRAPOLATED" in desc and "768x768 x48" in desc and "3072x768 x12" in desc
+    v2, desc2, _, secs2, per2 = bench.oracle_sample(2, per_shape)
+    big = [s for s in per_shape if s != (768, 768)]
+    assert all(per2[s] == per_shape[s] for s in big) and "kept from the first step" in desc2 and v2 > 0

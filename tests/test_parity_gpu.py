@@ -18,7 +18,7 @@ import torch
 import oracle
 import paper_2606_27153_b200 as dm
 from paper_2606_27153_b200 import synth
-from helpers import LR, LR_F, MU, MU_F, TOL_CHECK, TOL_TC, WD, WD_F, bf16_ulp, binary32_momentum, rel_fro, to64
+from helpers import LR, LR_F, MU, MU_F, TOL_CHECK, TOL_TC, WD, WD_F, W_USED, bf16_ulp, binary32_momentum, rel_fro, to64, w_bound
 
 pytestmark = pytest.mark.gpu
 
@@ -78,13 +78,9 @@ def check_muon_matrix(idx, shape, W0, Wg, Mg, Og, orc, tol, exact_momentum=False
         m16 = oracle.round_bf16(orc["M_n16"])
         unexplained = (mg != m_orc) & (mg != m16)
         assert not unexplained.any(), f"matrix {idx}: {unexplained.mean():.2e} of M' differ from the oracle for another reason than the binary32 rounding"
-    # W': no worse than the output rounding plus 1 % of the update (2 % slack on the rounding term: the two
-    # roundings are different random draws of the same distribution)
-    w_orc = orc["W_new"]
-    r = np.linalg.norm(oracle.round_bf16(w_orc) - w_orc)
-    upd = np.linalg.norm(w_orc - W0)
-    err = np.linalg.norm(to64(Wg) - w_orc)
-    assert err <= 1.02 * r + tol * upd, f"matrix {idx}: W' err {err:.3e} > {1.02 * r + tol * upd:.3e}"
+    # W': no worse than the output rounding plus 1 % of the update (helpers.w_bound)
+    err, bound = w_bound(to64(Wg), orc["W_new"], W0, tol, oracle.round_bf16)
+    assert err <= bound, f"matrix {idx}: W' err {err:.3e} > {bound:.3e}"
     return e_o
 
 
@@ -283,21 +279,57 @@ def test_config3_full_launch_sampled_layers():
 
 @pytest.mark.slow
 def test_config4_full_size_sampled():
-    """Llama-3-8B-shaped set at full size (42 GB resident), in the launch configuration bench.py times.  The plain
-    fp64 oracle runs a whole Muon step of one matrix of EVERY distinct shape: k (1024x4096, layers 0 and 31),
-    q (4096x4096), gate (14336x4096, tall) and down (4096x14336) -- the three shapes that carry 99 % of the FLOPs
-    (>= one matrix per distinct shape).  O, M' and W' are compared as on the small configs."""
+    """Llama-3-8B-shaped set at full size (42 GB resident) with a momentum state, tied to the oracle in THREE layouts.
+
+    (1) keep_ns_output = 0, everything else default: the launch configuration bench.py times (one 12 GiB workspace
+        region reused by the five buckets, the 64-matrix tall bucket in chunks, program kernel, final epilogue writing
+        W' only).
+    (2) the same layout through dmuon_muon_step_master (fp32 masters), which shows the APPLIED UPDATE: bf16 weights hide
+        it under their own rounding.
+    (3) keep_ns_output = 1: disjoint per-matrix slots, O readable.
+    W' and M' of ALL 224 matrices must be bitwise equal between (1) and (3); M' and the bf16 parameter of (2) equal to
+    (1)'s where the oracle is sampled.  The plain fp64 oracle then runs a whole Muon step of one matrix of EVERY distinct
+    shape: k (1024x4096, layers 0 and 31), q (4096x4096), gate (14336x4096, tall) and down (4096x14336) (SURVEY 8(d):
+    >= one matrix per distinct shape), and O, M', W' of (3) and the update of (2) are held to it."""
     import time
     dm.set_option("mode", "tc")
-    shapes, W, G, M = synth.muon_inputs(4, "cuda", False)
+    shapes, W, G, M = synth.muon_inputs(4, "cuda", True)
     idx = [1, 218, 0, 4, 6]
     pre = {i: (to64(W[i]), to64(G[i]), to64(M[i])) for i in idx}
+    G0 = {i: G[i].clone() for i in idx}
+
+    # (2) masters, bench layout.  Masters start at the bf16 weights, so one oracle evaluation serves (2) and (3)
+    dm.set_option("keep_ns_output", 0)
+    W32 = [w.float() for w in W]
+    Wb = [torch.full_like(w, float("nan")) for w in W]
+    Mm = [m.clone() for m in M]
+    dm.muon_step_master(Wb, W32, G, Mm, LR, MU, WD)
+    torch.cuda.synchronize()
+    got_master = {i: (W32[i].clone(), Wb[i].clone(), Mm[i].clone()) for i in idx}
+    assert all(torch.equal(wb, w32.to(torch.bfloat16)) for wb, w32 in zip(Wb, W32)), "bf16 parameter != rounding of its master"
+    del W32, Wb, Mm
+    torch.cuda.empty_cache()
+
+    # (1) bf16 weights, bench layout
+    WA, MA = [w.clone() for w in W], [m.clone() for m in M]
+    dm.muon_step(WA, G, MA, LR, MU, WD)
+    torch.cuda.synchronize()
+    plan0 = dm.describe_plan(shapes, steps=5)
+
+    # (3) per-matrix slots, in place on the originals
+    dm.set_option("keep_ns_output", 1)
     dm.muon_step(W, G, M, LR, MU, WD)
     torch.cuda.synchronize()
+    bad = [i for i in range(len(shapes)) if not (torch.equal(W[i], WA[i]) and torch.equal(M[i], MA[i]))]
+    assert not bad, f"keep_ns_output=0 (the bench's layout) and =1 differ on matrices {bad[:10]} ({len(bad)} of {len(shapes)})"
+    for i in idx:
+        assert torch.equal(G[i], G0[i]), "grads must never be written"
+        assert torch.equal(got_master[i][2], MA[i]), f"matrix {i}: M' of the master step differs from the plain step's"
     got = {i: (W[i].clone(), M[i].clone(), dm.binding.read_ns_output(i, shapes[i]).cpu()) for i in idx}
     plan = dm.describe_plan(shapes, steps=5)
-    del W, G, M
+    del W, G, M, WA, MA, G0
     torch.cuda.empty_cache()
+    n_used = len(W_USED)
     for i in idx:
         w0, g0, m0 = pre.pop(i)
         t0 = time.perf_counter()
@@ -305,14 +337,21 @@ def test_config4_full_size_sampled():
         secs = time.perf_counter() - t0
         wg, mg, og = got.pop(i)
         e = check_muon_matrix(i, shapes[i], w0, wg, mg, og, orc, TOL_TC)
-        print(f"config4 matrix {i} {shapes[i]}: O rel err vs fp64 oracle {e:.3e}; M' mismatch share {STATS['m_mismatch'][-1]:.2e} "
+        w32, _, _ = got_master.pop(i)
+        upd_orc = orc["W_new"] - w0
+        e_upd = np.linalg.norm((to64(w32) - w0) - upd_orc) / np.linalg.norm(upd_orc)
+        assert e_upd <= TOL_TC + 1e-4, f"matrix {i}: relative error of the applied update (fp32 masters, bench layout) {e_upd:.3e}"
+        print(f"config4 matrix {i} {shapes[i]}: O rel err vs fp64 oracle {e:.3e}; applied update (masters, keep_ns_output=0) {e_upd:.3e}; "
+              f"M' mismatch share {STATS['m_mismatch'][-1]:.2e}; share of the W' update allowance used {W_USED[-1]:+.3f} "
               f"(oracle {secs:.0f} s on {oracle.num_threads()} threads)")
         del orc, w0, g0, m0
-    print("config4 plan:", plan["buckets"])
+    assert len(W_USED) == n_used + len(idx)
+    print("config4 plan (keep_ns_output=0):", plan0["buckets"])
+    print("config4 plan (keep_ns_output=1):", plan["buckets"])
     # X larger than the L2 (117 MB per matrix): the X update's unit order is the one that reads X once -- row blocks of Y
     # for the tall buckets (odd tile variant), column panels of X for the wide one (even); measured 51.8 GB -> 9.8 GB of
     # DRAM reads per launch of the tall update (profiles/r2_step_ncu.md)
-    for b in plan["buckets"]:
+    for b in plan["buckets"] + plan0["buckets"]:
         if b["n"] == 14336:
             assert b["variants"][2] % 2 == (1 if b["kind"] == "tall" else 0), b
 

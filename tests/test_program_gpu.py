@@ -12,7 +12,7 @@ import torch
 import oracle
 import paper_2606_27153_b200 as dm
 from paper_2606_27153_b200 import synth
-from helpers import LR, LR_F, MU, MU_F, TOL_TC, WD, WD_F, bf16_ulp, rel_fro, to64
+from helpers import LR, LR_F, MU, MU_F, TOL_TC, WD, WD_F, bf16_ulp, rel_fro, to64, w_bound
 
 pytestmark = pytest.mark.gpu
 
@@ -45,8 +45,7 @@ def _check_step(i, shape, W0, G0, M0, Wg, Mg, Og):
     m_orc = oracle.round_bf16(orc["M_new"])
     assert (np.abs(to64(Mg) - m_orc) <= bf16_ulp(np.maximum(np.abs(to64(Mg)), np.abs(m_orc)))).all()
     w_orc = orc["W_new"]
-    err = np.linalg.norm(to64(Wg) - w_orc)
-    bound = 1.02 * np.linalg.norm(oracle.round_bf16(w_orc) - w_orc) + TOL_TC * np.linalg.norm(w_orc - W0)
+    err, bound = w_bound(to64(Wg), w_orc, W0, TOL_TC, oracle.round_bf16)
     assert err <= bound, f"matrix {i}: W' err {err:.3e} > {bound:.3e}"
     return e
 
